@@ -1,0 +1,247 @@
+/*
+ * tpc_track.h — C ABI of the B200 TPC sector-tracking library (libtpctrack.so).
+ *
+ * What the library computes: the "sector tracking" phase of the ALICE Run 3 TPC
+ * tracking as summarised in PAPER.md:25-27 (§2): a time frame of TPC clusters
+ * (§1) goes in; for each of the 36 sectors the library builds the
+ * per-pad-row "fast cluster search grid" (§3), finds cellular-automaton
+ * neighbour links and seeds ("combinatorial seeding based on a cellular automaton",
+ * PAPER.md:27), follows every seed through the sector with a Kalman filter "picking
+ * up more clusters of the track", and runs the ambiguity solving that
+ * "identifies the best instance of each track, assigns all clusters to this instance
+ * and removes the clones", with "a configurable fraction of a track's clusters, by
+ * default 10%, ... allowed to be shared" and the Phase-I criterion
+ * (smaller global chi2 gets priority, shared clusters counted from the outermost pad
+ * row, §3).  Output: sector tracks with cluster lists, ready for the
+ * track-merging phase, which is outside this library.
+ *
+ * Every constant / window / tie-break the paper leaves open is fixed in DESIGN.md
+ * ("Readings") and is a field of tpc_params below.
+ *
+ * Conventions
+ *  - All structs are POD, little-endian, natural alignment.  No C++ or torch types.
+ *  - Pointers named d_* are DEVICE pointers (CUDA global memory on the current device);
+ *    all other pointers are HOST pointers.
+ *  - Every function returns TPC_OK (0) or a negative tpc_error; nothing throws or aborts.
+ *  - A context is not thread-safe; use one context per host thread / stream.
+ *  - The library allocates device memory only inside tpc_geom_init (a few KB of tables
+ *    and counters) and creates no streams.  All scratch and all outputs live in the
+ *    caller's workspace.
+ */
+#ifndef TPC_TRACK_H
+#define TPC_TRACK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ------------------------------------------------------------------ errors */
+typedef enum tpc_error {
+  TPC_OK = 0,
+  TPC_E_ARG = -1,       /* null / misaligned pointer, bad descriptor, n_clusters >= 2^31,
+                           or (reported by tpc_get_tracks) a cluster whose sector/row is
+                           outside the geometry                                         */
+  TPC_E_WORKSPACE = -2, /* workspace smaller than tpc_workspace_bytes(); nothing written */
+  TPC_E_OVERFLOW = -3,  /* a capacity bound was hit on the device (bin index, tracks);
+                           results are invalid, never silently truncated               */
+  TPC_E_CUDA = -4,      /* a CUDA runtime call failed; see tpc_last_cuda_error()         */
+  TPC_E_STATE = -5      /* call order violated (e.g. tpc_get_tracks before a run)       */
+} tpc_error;
+
+/* ------------------------------------------------------------------ input */
+/* One TPC cluster, 16 bytes (BASELINE.json config 4: "cluster struct 16 B").
+ * y, z are local sector coordinates in cm: y along the pad row, z along the drift
+ * ("time-z": with continuous readout the collision time is unknown, so z
+ * carries an unknown per-collision offset; the tracker never uses a vertex constraint).
+ * The pad row fixes the local x.  q (charge) and flags are carried but unused. */
+typedef struct tpc_cluster {
+  float y, z;
+  float q;
+  uint8_t sector; /* 0..n_sectors-1 (0..17 A side, 18..35 C side) */
+  uint8_t row;    /* 0..n_rows-1 */
+  uint16_t flags;
+} tpc_cluster;
+
+/* Geometry descriptor (2 halves x 18 trapezoidal sectors; row count, radii
+ * and pad pitches from BASELINE.json config 1).  Row r sits at local
+ * x_r = r_min + r*(r_max-r_min)/(n_rows-1); its half width is x_r*tan(half_angle). */
+typedef struct tpc_geom_desc {
+  int32_t n_sectors;    /* 36 */
+  int32_t n_rows;       /* 152 (max 255) */
+  int32_t n_inner_rows; /* 63; informational */
+  float r_min, r_max;   /* 85, 245 cm */
+  float pad_pitch_inner, pad_pitch_outer; /* 0.4, 0.6 cm; informational */
+  float z_max;          /* 250 cm drift length; only sizes the default bin capacity */
+  float bz_tesla;       /* 0.5 */
+  float sector_half_angle_deg; /* 10 */
+} tpc_geom_desc;
+
+/* Every tunable of the method.  Defaults (tpc_default_params) are DESIGN.md's readings. */
+typedef struct tpc_params {
+  float err_y, err_z;            /* measurement sigma, cm (0.1, 0.1)                    */
+  float nf_slope_y, nf_slope_z;  /* neighbour-finder window slopes (1.0, 1.6)           */
+  float nf_max_d2;               /* max 3-point straightness^2, cm^2 (0.70)             */
+  int32_t seed_min_len;          /* min clusters in a link chain to seed (4)            */
+  float init_var_sinphi, init_var_tanl, init_var_qpt; /* (0.25, 4, 100)                 */
+  float max_sinphi;              /* 0.95                                                */
+  float max_qpt;                 /* clamp on |q/pT|, c/GeV (20)                         */
+  float road_nsigma, road_min, road_max; /* search road (3.5, 0.3 cm, 2.0 cm)           */
+  float chi2_max_hit;            /* 2-dof chi2 cut for pick-up (12)                     */
+  int32_t max_gap_follow;        /* rows without hit before the follower stops (4)      */
+  int32_t min_hits_tracklet;     /* (10)                                                */
+  float sel_chi2_weight;         /* weight = nHits - w*chi2/ndf (2.0)                   */
+  int32_t shared_permille;       /* allowed shared-cluster fraction, permille (100)     */
+  int32_t max_gap_select;        /* rows; a larger hole splits the track (4)            */
+  int32_t min_hits_track;        /* (20)                                                */
+  float grid_dy, grid_dz;        /* bin size, cm (2, 2) — performance knob only         */
+  uint64_t max_bins;             /* bin-index capacity; 0 = default
+                                    8*n_clusters + n_sectors*n_rows*(ny_max*(z_max/grid_dz+2)) */
+  uint32_t reserved[4];
+} tpc_params;
+
+/* ------------------------------------------------------------------ output */
+#define TPC_TRACK_PARAMS_STALE 1u /* segment does not contain the row the parameters refer to */
+
+/* One sector track (108 bytes).  Parameters are (y, z, sin(phi), tan(lambda), q/pT) at
+ * local x of the tracklet's innermost row, c[] the lower-triangular covariance
+ * (c00,c10,c11,c20,...,c44). */
+typedef struct tpc_track {
+  float x;
+  float p[5];
+  float c[15];
+  float chi2;            /* of the inward refit pass                                   */
+  uint32_t cluster_ofs;  /* first entry in cluster_ids / cluster_shared                */
+  uint32_t seed_id;      /* ORIGINAL input index of the seed's start cluster           */
+  uint16_t n_clusters, n_shared;
+  uint8_t sector, row_first, row_last, flags;
+  uint16_t n_hits_tracklet; /* hits of the whole tracklet (ndf = 2*n-5)                */
+  uint8_t segment;          /* 0 = outermost segment of this tracklet                  */
+  uint8_t pad_;
+} tpc_track;
+
+typedef struct tpc_track_view {
+  uint64_t n_tracks;
+  uint64_t n_cluster_ids;
+  const tpc_track* d_tracks;        /* [n_tracks]                                      */
+  const uint32_t* d_cluster_ids;    /* [n_cluster_ids] original input indices, per track
+                                       ascending in pad row                            */
+  const uint8_t* d_cluster_shared;  /* [n_cluster_ids] 1 = attached as shared          */
+  /* diagnostics */
+  uint64_t n_ignored;               /* NaN/Inf clusters ignored                         */
+  uint64_t n_dropped;               /* |y| beyond the row's half width + 2 cm          */
+  uint64_t n_seeds;
+  uint64_t n_tracklets;
+  uint64_t n_bins;
+} tpc_track_view;
+
+/* One row of the search grid. */
+typedef struct tpc_row_desc {
+  float y0, z0;        /* lower edges                                                  */
+  int32_t ny, nz;      /* bins; bin = bz*ny + by (z-major)                             */
+  uint32_t bin_ofs;    /* index of this row's first bin in d_bin_start                 */
+  uint32_t clu_ofs;    /* sorted index of this row's first cluster                     */
+  uint32_t count;      /* clusters in the row                                          */
+  uint32_t pad_;
+} tpc_row_desc;
+
+/* One tracklet (follower output, before ambiguity solving), 112 bytes. */
+typedef struct tpc_tracklet {
+  float x;
+  float p[5];
+  float c[15];
+  float chi2;
+  uint32_t seed_sorted;  /* sorted index of the start cluster                          */
+  uint32_t seed_id;      /* original index of the start cluster                        */
+  int16_t n_hits;        /* 0 = rejected (below min_hits_tracklet)                     */
+  uint8_t row_first, row_last;
+  uint8_t sector;
+  uint8_t seed_len;      /* length of the seed's link chain                            */
+  uint16_t pad_;
+  uint32_t pad2_[2];
+} tpc_tracklet;
+
+/* Intermediates, valid after a run with TPC_KEEP_INTERMEDIATES.  Index spaces:
+ * "sorted index" = position in the grid-sorted cluster array; d_orig_id maps it to the
+ * original input index.  Links are in sorted-index space, -1 = none. */
+typedef struct tpc_debug_view {
+  uint64_t n_clusters;           /* input clusters                                     */
+  uint64_t n_sorted;             /* clusters in the grid (input - ignored - dropped)   */
+  uint64_t n_rows_total;         /* n_sectors*n_rows                                   */
+  uint64_t n_bins;
+  uint64_t n_seeds;
+  uint64_t tracklet_stride;      /* row_hit is [row][tracklet_stride]                  */
+  const tpc_row_desc* d_row_desc;/* [n_rows_total]                                     */
+  const uint32_t* d_bin_start;   /* [n_bins + 1] global sorted positions               */
+  const float* d_yz_sorted;      /* [n_sorted][2]                                      */
+  const uint32_t* d_orig_id;     /* [n_sorted]                                         */
+  const int32_t* d_link_up;      /* [n_sorted] after neighbour finding                 */
+  const int32_t* d_link_dn;
+  const int32_t* d_link_up2;     /* [n_sorted] after cleanup                           */
+  const int32_t* d_link_dn2;
+  const uint32_t* d_seeds;       /* [n_seeds] sorted index of each start cluster       */
+  const tpc_tracklet* d_tracklets; /* [n_seeds]                                        */
+  const int32_t* d_row_hit;      /* [n_rows][tracklet_stride] sorted index or -1; only
+                                    rows row_first..row_last of a tracklet are defined */
+} tpc_debug_view;
+
+/* ------------------------------------------------------------------ flags */
+#define TPC_DETERMINISTIC 1u      /* bit-reproducible mode: no FMA contraction,
+                                     stable grid order, scans instead of atomics         */
+#define TPC_KEEP_INTERMEDIATES 2u /* keep the buffers tpc_get_intermediates exposes      */
+#define TPC_STAGE_TIMERS 4u       /* record CUDA events per stage (tpc_get_stage_ms)     */
+
+#define TPC_N_STAGES 6            /* grid, neighbours, cleanup+seeds, follower, selector, total */
+
+typedef struct tpc_ctx tpc_ctx;   /* opaque, owned by the library */
+
+/* ------------------------------------------------------------------ calls */
+
+/* Fill *out with the default parameters. HOST pointer. */
+void tpc_default_params(tpc_params* out);
+
+/* Create a context for one geometry + parameter set (params == NULL: defaults).
+ * Computes the row tables in double, rounds once to fp32 (DESIGN.md rule D5) and uploads
+ * them.  HOST pointers.  *out is owned by the library; release with tpc_destroy. */
+int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx** out);
+
+/* Upper bound of the workspace tpc_sector_track needs for n_clusters input clusters. */
+size_t tpc_workspace_bytes(const tpc_ctx* ctx, uint64_t n_clusters);
+
+/* Track one time frame.  d_clusters: DEVICE, [n_clusters], 16-byte
+ * aligned, read-only, any order, must stay valid until tpc_get_tracks returns.
+ * d_workspace: DEVICE, 256-byte aligned, >= tpc_workspace_bytes(); the library carves all
+ * scratch and outputs from it.  cuda_stream: a cudaStream_t (NULL = legacy default stream).
+ * All work is enqueued asynchronously on that stream; the call does not block. */
+int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters,
+                     void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                     uint32_t flags);
+
+/* Synchronise the stream of the last run, read the counters back and fill *out (HOST)
+ * with device pointers into the workspace.  They stay valid until the next
+ * tpc_sector_track on this context or until the caller frees the workspace.
+ * Returns TPC_E_OVERFLOW / TPC_E_ARG if the device flagged an error during the run. */
+int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out);
+
+/* As above for the intermediates; requires TPC_KEEP_INTERMEDIATES in the last run. */
+int tpc_get_intermediates(tpc_ctx* ctx, tpc_debug_view* out);
+
+/* Per-stage device times in ms of the last run (needs TPC_STAGE_TIMERS):
+ * out_ms[0..5] = grid, neighbours, cleanup+seeds, follower, selector, total. HOST pointer.
+ * Syncs the stream. */
+int tpc_get_stage_ms(tpc_ctx* ctx, float* out_ms);
+
+/* Number of kernel launches the last tpc_sector_track enqueued. */
+int tpc_last_launch_count(const tpc_ctx* ctx);
+
+void tpc_destroy(tpc_ctx* ctx);
+const char* tpc_strerror(int err);
+/* Text of the last failing CUDA call of this context ("" if none). */
+const char* tpc_last_cuda_error(const tpc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_TRACK_H */

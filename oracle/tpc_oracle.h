@@ -1,0 +1,135 @@
+/*
+ * tpc_oracle.h — C interface of the CPU ORACLE of the TPC sector tracking.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may load it.  It shares no code, header,
+ * table or constant generator with the CUDA path under paper_2601_20569_b200/csrc: the
+ * structs below are the oracle's own definitions (the parameter list of the method is the
+ * same list on both sides because it IS the method's parameter list).
+ *
+ * What it computes: the sector tracking of PAPER.md:25-27 (section 2) with the Phase-I
+ * ambiguity criterion of PAPER.md:57 (section 3) and the search grid of PAPER.md:59,
+ * step by step in the order of DESIGN.md "Readings" R0..R6:
+ *   R0 geometry tables, R1 grid, R2 neighbour finder, R3 link cleanup, R4 seeds,
+ *   R5 Kalman track following, R6 ambiguity solving.
+ * Plain single-threaded loops per sector (sectors may be spread over threads for the timed
+ * baseline; the result does not depend on that).  fp32 arithmetic, only + - * / sqrt, built
+ * with -ffp-contract=off (rule D1).  All results are expressed in ORIGINAL input indices
+ * (rule D3).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form geometry, exact-helix
+ * propagation, finite-difference Jacobian, Kalman update == weighted least squares,
+ * unit-width pulls, brute-force neighbour search, grid invariants + brute-force window
+ * queries, link/seed invariants, selector invariants and constructed cases.
+ * Parity unpinned: absolute efficiency / clone / fake values (the paper's Fig. 2 is an
+ * image that is not in PAPER.md and is ALICE MC); only sanity floors are tested.
+ */
+#ifndef TPC_ORACLE_H
+#define TPC_ORACLE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_cluster { /* 16 bytes, the input record (BASELINE.json config 4) */
+  float y, z, q;
+  uint8_t sector, row;
+  uint16_t flags;
+} orc_cluster;
+
+typedef struct orc_geom {
+  int32_t n_sectors, n_rows, n_inner_rows;
+  float r_min, r_max, pad_pitch_inner, pad_pitch_outer, z_max, bz_tesla, sector_half_angle_deg;
+} orc_geom;
+
+typedef struct orc_params {
+  float err_y, err_z;
+  float nf_slope_y, nf_slope_z, nf_max_d2;
+  int32_t seed_min_len;
+  float init_var_sinphi, init_var_tanl, init_var_qpt;
+  float max_sinphi, max_qpt;
+  float road_nsigma, road_min, road_max;
+  float chi2_max_hit;
+  int32_t max_gap_follow, min_hits_tracklet;
+  float sel_chi2_weight;
+  int32_t shared_permille, max_gap_select, min_hits_track;
+  float grid_dy, grid_dz;
+} orc_params;
+
+typedef struct orc_row_desc {
+  float y0, z0;
+  int32_t ny, nz;
+  uint32_t bin_ofs, clu_ofs, count, pad_;
+} orc_row_desc;
+
+typedef struct orc_seed {
+  uint32_t start_id; /* original index of the start hit */
+  int32_t len;       /* clusters in the link chain */
+  int32_t sector, row;
+} orc_seed;
+
+typedef struct orc_tracklet {
+  float x, p[5], c[15], chi2;
+  uint32_t seed_id;
+  int32_t n_hits; /* 0 = rejected (below min_hits_tracklet or broken) */
+  int32_t row_first, row_last, sector, seed_len;
+} orc_tracklet;
+
+typedef struct orc_track {
+  float x, p[5], c[15], chi2;
+  uint32_t cluster_ofs, seed_id;
+  int32_t n_clusters, n_shared;
+  int32_t sector, row_first, row_last, flags; /* flags bit0 = PARAMS_STALE */
+  int32_t n_hits_tracklet, segment;
+} orc_track;
+
+typedef struct orc_result orc_result;
+
+void orc_default_params(orc_params* p);
+
+/* Run the whole path on sectors [sector_lo, sector_hi) of the frame.  n_threads > 1 spreads
+ * sectors over std::threads (same result).  Returns NULL on a bad argument. */
+orc_result* orc_run(const orc_cluster* clusters, uint64_t n, const orc_geom* g, const orc_params* p,
+                    int sector_lo, int sector_hi, int n_threads);
+void orc_free(orc_result* r);
+
+/* sizes: out[0]=n_rows_total out[1]=n_bins out[2]=n_sorted out[3]=n_seeds out[4]=n_tracks
+ * out[5]=n_cluster_ids out[6]=n_ignored out[7]=n_dropped out[8]=n_bad (sector/row outside geometry)
+ * out[9]=n_tracklets (n_hits>0) */
+void orc_sizes(const orc_result* r, uint64_t out[10]);
+/* stage wall times in seconds: grid, neighbours, cleanup+seeds, follower, selector */
+void orc_stage_seconds(const orc_result* r, double out[5]);
+/* copy-out; any pointer may be NULL.  Links are indexed by ORIGINAL cluster index and hold
+ * original indices (-1 none); entries of clusters outside [sector_lo,sector_hi) are -1. */
+void orc_fetch_grid(const orc_result* r, orc_row_desc* rows, uint32_t* bin_start, uint32_t* sorted_ids);
+void orc_fetch_links(const orc_result* r, int32_t* up, int32_t* dn, int32_t* up2, int32_t* dn2);
+void orc_fetch_seeds(const orc_result* r, orc_seed* seeds);
+void orc_fetch_tracklets(const orc_result* r, orc_tracklet* t, int32_t* row_hit /*[n_seeds][n_rows]*/);
+void orc_fetch_tracks(const orc_result* r, orc_track* t, uint32_t* cluster_ids, uint8_t* shared);
+
+/* ---- single-step entry points for the pins (float = the path's type, double = same
+ * statements instantiated in double) ---- */
+/* tables: x[n_rows], ymax[n_rows]; consts[0]=dx_row consts[1]=cfield (curvature per q/pT) */
+void orc_geom_tables(const orc_geom* g, float* x, float* ymax, float* consts);
+/* state = y,z,s,t,q,c[15] (20 values). returns 1 if propagated, 0 if the leg ends */
+int orc_propagate_f(float* state, float dx, float cfield, float max_sinphi, float* jac6);
+int orc_propagate_d(double* state, double dx, double cfield, double max_sinphi, double* jac6);
+/* returns chi2 of the hit; *stop = 1 if |sin phi| left the range */
+float orc_update_f(float* state, float ym, float zm, float vy, float vz, float max_sinphi, float max_qpt, int* stop);
+double orc_update_d(double* state, double ym, double zm, double vy, double vz, double max_sinphi, double max_qpt, int* stop);
+/* Kalman fit of a given hit list (truth association) exactly as steps R5.1/R5.2/R5.4/R5.5 do
+ * (up pass over the hits, turn, refit down).  rows[] ascending, consecutive or with gaps.
+ * out_state = 20 floats at rows[0]; returns chi2 of the down pass or -1 if the leg stopped. */
+float orc_fit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows, const float* y,
+                   const float* z, int n, float* out_state);
+/* selector on hand-made tracklets: row_hit[n_tracklets][n_rows] (cluster ids or -1),
+ * n_hits/chi2/seed_id per tracklet.  Results via orc_fetch_tracks. */
+orc_result* orc_select_only(const orc_geom* g, const orc_params* p, uint64_t n_clusters, int n_tracklets,
+                            const int32_t* row_hit, const int32_t* n_hits, const float* chi2,
+                            const uint32_t* seed_id);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
