@@ -41,7 +41,7 @@ extern "C" {
 /* ------------------------------------------------------------------ errors */
 typedef enum tpc_error {
   TPC_OK = 0,
-  TPC_E_ARG = -1,       /* null / misaligned pointer, bad descriptor, n_clusters >= 2^31,
+  TPC_E_ARG = -1,       /* null / misaligned pointer, bad descriptor, n_clusters >= 2^30,
                            or (reported by tpc_get_tracks) a cluster whose sector/row is
                            outside the geometry                                         */
   TPC_E_WORKSPACE = -2, /* workspace smaller than tpc_workspace_bytes(); nothing written */
@@ -98,8 +98,9 @@ typedef struct tpc_params {
   int32_t min_hits_track;        /* (20)                                                */
   float grid_dy, grid_dz;        /* bin size, cm (2, 2) — performance knob only         */
   uint64_t max_bins;             /* bin-index capacity; 0 = default
-                                    8*n_clusters + n_sectors*n_rows*(ny_max*(z_max/grid_dz+2)) */
-  uint32_t reserved[4];
+                                    4*n_clusters + n_sectors*n_rows*ny_max*(z_max/grid_dz+2)   */
+  uint32_t max_seeds;            /* seed/tracklet capacity; 0 = default n_clusters/8 + 4096     */
+  uint32_t reserved[3];
 } tpc_params;
 
 /* ------------------------------------------------------------------ output */

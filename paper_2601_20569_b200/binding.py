@@ -1,0 +1,309 @@
+"""Thin ctypes binding of the C-ABI library libtpctrack.so (include/tpc_track.h).
+
+Argument marshalling only: every step of the path (grid, neighbour finder, link cleanup,
+seeds, Kalman follower, ambiguity solving) runs in the CUDA kernels of csrc/.  PyTorch is used
+for device memory and streams, nothing else.  There is NO CPU fallback: importing this module
+without the built library, or calling it without a CUDA device, raises.
+
+Low level: the functions ``tpc_*`` have the names and arguments of the header.
+High level: ``SectorTracker`` owns a context and a workspace and returns results as arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import LIB_PATH
+
+TPC_OK, TPC_E_ARG, TPC_E_WORKSPACE, TPC_E_OVERFLOW, TPC_E_CUDA, TPC_E_STATE = 0, -1, -2, -3, -4, -5
+TPC_DETERMINISTIC, TPC_KEEP_INTERMEDIATES, TPC_STAGE_TIMERS = 1, 2, 4
+TPC_N_STAGES = 6
+STAGE_NAMES = ("grid", "neighbours", "cleanup_seeds", "follower", "selector", "total")
+
+CLUSTER_DTYPE = np.dtype(
+    [("y", "<f4"), ("z", "<f4"), ("q", "<f4"), ("sector", "u1"), ("row", "u1"), ("flags", "<u2")])
+TRACK_DTYPE = np.dtype(
+    [("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"), ("cluster_ofs", "<u4"),
+     ("seed_id", "<u4"), ("n_clusters", "<u2"), ("n_shared", "<u2"), ("sector", "u1"),
+     ("row_first", "u1"), ("row_last", "u1"), ("flags", "u1"), ("n_hits_tracklet", "<u2"),
+     ("segment", "u1"), ("pad_", "u1")])
+TRACKLET_DTYPE = np.dtype(
+    [("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"), ("seed_sorted", "<u4"),
+     ("seed_id", "<u4"), ("n_hits", "<i2"), ("row_first", "u1"), ("row_last", "u1"), ("sector", "u1"),
+     ("seed_len", "u1"), ("pad_", "<u2"), ("pad2_", "<u4", (2,))])
+ROW_DESC_DTYPE = np.dtype(
+    [("y0", "<f4"), ("z0", "<f4"), ("ny", "<i4"), ("nz", "<i4"), ("bin_ofs", "<u4"),
+     ("clu_ofs", "<u4"), ("count", "<u4"), ("pad_", "<u4")])
+assert TRACK_DTYPE.itemsize == 108 and TRACKLET_DTYPE.itemsize == 112 and ROW_DESC_DTYPE.itemsize == 32
+
+
+class GeomDesc(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("n_inner_rows", C.c_int32),
+                ("r_min", C.c_float), ("r_max", C.c_float), ("pad_pitch_inner", C.c_float),
+                ("pad_pitch_outer", C.c_float), ("z_max", C.c_float), ("bz_tesla", C.c_float),
+                ("sector_half_angle_deg", C.c_float)]
+
+
+class Params(C.Structure):
+    _fields_ = [("err_y", C.c_float), ("err_z", C.c_float),
+                ("nf_slope_y", C.c_float), ("nf_slope_z", C.c_float), ("nf_max_d2", C.c_float),
+                ("seed_min_len", C.c_int32),
+                ("init_var_sinphi", C.c_float), ("init_var_tanl", C.c_float), ("init_var_qpt", C.c_float),
+                ("max_sinphi", C.c_float), ("max_qpt", C.c_float),
+                ("road_nsigma", C.c_float), ("road_min", C.c_float), ("road_max", C.c_float),
+                ("chi2_max_hit", C.c_float),
+                ("max_gap_follow", C.c_int32), ("min_hits_tracklet", C.c_int32),
+                ("sel_chi2_weight", C.c_float),
+                ("shared_permille", C.c_int32), ("max_gap_select", C.c_int32), ("min_hits_track", C.c_int32),
+                ("grid_dy", C.c_float), ("grid_dz", C.c_float),
+                ("max_bins", C.c_uint64), ("max_seeds", C.c_uint32), ("reserved", C.c_uint32 * 3)]
+
+
+class TrackView(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint64), ("n_cluster_ids", C.c_uint64),
+                ("d_tracks", C.c_void_p), ("d_cluster_ids", C.c_void_p), ("d_cluster_shared", C.c_void_p),
+                ("n_ignored", C.c_uint64), ("n_dropped", C.c_uint64), ("n_seeds", C.c_uint64),
+                ("n_tracklets", C.c_uint64), ("n_bins", C.c_uint64)]
+
+
+class DebugView(C.Structure):
+    _fields_ = [("n_clusters", C.c_uint64), ("n_sorted", C.c_uint64), ("n_rows_total", C.c_uint64),
+                ("n_bins", C.c_uint64), ("n_seeds", C.c_uint64), ("tracklet_stride", C.c_uint64),
+                ("d_row_desc", C.c_void_p), ("d_bin_start", C.c_void_p), ("d_yz_sorted", C.c_void_p),
+                ("d_orig_id", C.c_void_p), ("d_link_up", C.c_void_p), ("d_link_dn", C.c_void_p),
+                ("d_link_up2", C.c_void_p), ("d_link_dn2", C.c_void_p), ("d_seeds", C.c_void_p),
+                ("d_tracklets", C.c_void_p), ("d_row_hit", C.c_void_p)]
+
+
+EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
+           "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_last_launch_count",
+           "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtpctrack.so and declare the prototypes of include/tpc_track.h.  Raises if
+    the library has not been built (python -m paper_2601_20569_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2601_20569_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp = C.c_void_p
+    L.tpc_default_params.restype = None
+    L.tpc_default_params.argtypes = [C.POINTER(Params)]
+    L.tpc_geom_init.restype = C.c_int
+    L.tpc_geom_init.argtypes = [C.POINTER(GeomDesc), C.POINTER(Params), C.POINTER(vp)]
+    L.tpc_workspace_bytes.restype = C.c_size_t
+    L.tpc_workspace_bytes.argtypes = [vp, C.c_uint64]
+    L.tpc_sector_track.restype = C.c_int
+    L.tpc_sector_track.argtypes = [vp, vp, C.c_uint64, vp, C.c_size_t, vp, C.c_uint32]
+    L.tpc_get_tracks.restype = C.c_int
+    L.tpc_get_tracks.argtypes = [vp, C.POINTER(TrackView)]
+    L.tpc_get_intermediates.restype = C.c_int
+    L.tpc_get_intermediates.argtypes = [vp, C.POINTER(DebugView)]
+    L.tpc_get_stage_ms.restype = C.c_int
+    L.tpc_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.tpc_last_launch_count.restype = C.c_int
+    L.tpc_last_launch_count.argtypes = [vp]
+    L.tpc_destroy.restype = None
+    L.tpc_destroy.argtypes = [vp]
+    L.tpc_strerror.restype = C.c_char_p
+    L.tpc_strerror.argtypes = [C.c_int]
+    L.tpc_last_cuda_error.restype = C.c_char_p
+    L.tpc_last_cuda_error.argtypes = [vp]
+    _lib = L
+    return L
+
+
+# ---------------------------------------------------------------- header-named thin wrappers
+def tpc_default_params(**overrides) -> Params:
+    p = Params()
+    load_library().tpc_default_params(C.byref(p))
+    for k, v in overrides.items():
+        setattr(p, k, v)
+    return p
+
+
+def default_geom(**overrides) -> GeomDesc:
+    """The TPC of BASELINE.json config 1: 36 sectors x 152 rows, 85-245 cm, 0.5 T."""
+    g = GeomDesc(36, 152, 63, 85.0, 245.0, 0.4, 0.6, 250.0, 0.5, 10.0)
+    for k, v in overrides.items():
+        setattr(g, k, v)
+    return g
+
+
+class TpcError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        self.code = code
+        msg = load_library().tpc_strerror(code).decode()
+        super().__init__(f"{where}: {msg} ({code}) {detail}".strip())
+
+
+def tpc_geom_init(geom: GeomDesc, params: Params | None) -> int:
+    ctx = C.c_void_p()
+    rc = load_library().tpc_geom_init(C.byref(geom), C.byref(params) if params is not None else None, C.byref(ctx))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpc_geom_init")
+    return ctx.value
+
+
+def tpc_workspace_bytes(ctx: int, n_clusters: int) -> int:
+    return int(load_library().tpc_workspace_bytes(ctx, n_clusters))
+
+
+def tpc_sector_track(ctx: int, d_clusters: int, n_clusters: int, d_workspace: int, workspace_bytes: int,
+                     cuda_stream: int, flags: int) -> int:
+    return load_library().tpc_sector_track(ctx, d_clusters, n_clusters, d_workspace, workspace_bytes,
+                                           cuda_stream, flags)
+
+
+def tpc_get_tracks(ctx: int):
+    v = TrackView()
+    rc = load_library().tpc_get_tracks(ctx, C.byref(v))
+    return rc, v
+
+
+def tpc_get_intermediates(ctx: int):
+    v = DebugView()
+    rc = load_library().tpc_get_intermediates(ctx, C.byref(v))
+    return rc, v
+
+
+def tpc_get_stage_ms(ctx: int):
+    out = (C.c_float * TPC_N_STAGES)()
+    rc = load_library().tpc_get_stage_ms(ctx, out)
+    return rc, [float(x) for x in out]
+
+
+def tpc_last_launch_count(ctx: int) -> int:
+    return load_library().tpc_last_launch_count(ctx)
+
+
+def tpc_destroy(ctx: int) -> None:
+    load_library().tpc_destroy(ctx)
+
+
+def tpc_last_cuda_error(ctx: int) -> str:
+    return load_library().tpc_last_cuda_error(ctx).decode()
+
+
+# ---------------------------------------------------------------- convenience class
+class SectorTracker:
+    """One context + one workspace.  ``track(d_clusters)`` enqueues the path on a stream;
+    ``tracks()`` / ``intermediates()`` synchronise and return arrays."""
+
+    def __init__(self, geom: GeomDesc | None = None, params: Params | None = None, device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("SectorTracker needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        self.geom = geom or default_geom()
+        self.params = params
+        self.ctx = tpc_geom_init(self.geom, params)
+        self.workspace = None
+        self._clusters = None
+        self.n = 0
+
+    def close(self):
+        if self.ctx:
+            tpc_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def upload(self, clusters: np.ndarray):
+        """Host structured array (16-byte records) -> device uint8 tensor."""
+        assert clusters.dtype.itemsize == 16
+        t = self.torch.from_numpy(np.ascontiguousarray(clusters).view(np.uint8).reshape(-1))
+        return t.to(self.device)
+
+    def ensure_workspace(self, n: int):
+        need = tpc_workspace_bytes(self.ctx, n)
+        if need == 0 and n:
+            raise TpcError(TPC_E_ARG, "tpc_workspace_bytes")
+        if self.workspace is None or self.workspace.numel() < need:
+            self.workspace = None
+            self.workspace = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        return need
+
+    def track(self, d_clusters, flags: int = 0, stream=None) -> None:
+        """d_clusters: device uint8 tensor holding n 16-byte cluster records."""
+        n = d_clusters.numel() // 16
+        need = self.ensure_workspace(n)
+        ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc = tpc_sector_track(self.ctx, d_clusters.data_ptr(), n, ws_ptr, need, st.cuda_stream, flags)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_sector_track", tpc_last_cuda_error(self.ctx))
+        self._clusters = d_clusters  # keep alive until the results are read
+        self.n = n
+
+    def _view(self, ptr: int, nbytes: int):
+        off = ptr - self.workspace.data_ptr()
+        assert 0 <= off and off + nbytes <= self.workspace.numel()
+        return self.workspace[off:off + nbytes]
+
+    def _to_numpy(self, ptr: int, count: int, dtype) -> np.ndarray:
+        dtype = np.dtype(dtype)
+        if count == 0:
+            return np.zeros(0, dtype=dtype)
+        return self._view(ptr, count * dtype.itemsize).cpu().numpy().view(dtype).copy()
+
+    def counts(self, check: bool = True):
+        rc, v = tpc_get_tracks(self.ctx)
+        if check and rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_tracks", tpc_last_cuda_error(self.ctx))
+        return rc, v
+
+    def tracks(self):
+        """Synchronise and copy out (tracks, cluster_ids, cluster_shared, view)."""
+        rc, v = self.counts()
+        tr = self._to_numpy(v.d_tracks, v.n_tracks, TRACK_DTYPE)
+        ids = self._to_numpy(v.d_cluster_ids, v.n_cluster_ids, np.uint32)
+        sh = self._to_numpy(v.d_cluster_shared, v.n_cluster_ids, np.uint8)
+        return tr, ids, sh, v
+
+    def stage_ms(self) -> dict:
+        rc, ms = tpc_get_stage_ms(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_stage_ms")
+        return dict(zip(STAGE_NAMES, ms))
+
+    def launch_count(self) -> int:
+        return tpc_last_launch_count(self.ctx)
+
+    def intermediates(self) -> dict:
+        """Everything tpc_get_intermediates exposes, as numpy arrays (needs the run to have
+        been made with TPC_KEEP_INTERMEDIATES)."""
+        rc, v = tpc_get_intermediates(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_intermediates", tpc_last_cuda_error(self.ctx))
+        ns, nb, nseeds, stride = v.n_sorted, v.n_bins, v.n_seeds, v.tracklet_stride
+        out = dict(n_sorted=ns, n_bins=nb, n_seeds=nseeds)
+        out["row_desc"] = self._to_numpy(v.d_row_desc, v.n_rows_total, ROW_DESC_DTYPE)
+        out["bin_start"] = self._to_numpy(v.d_bin_start, nb + 1, np.uint32)
+        out["yz_sorted"] = self._to_numpy(v.d_yz_sorted, 2 * ns, np.float32).reshape(-1, 2)
+        out["orig_id"] = self._to_numpy(v.d_orig_id, ns, np.uint32)
+        for k in ("link_up", "link_dn", "link_up2", "link_dn2"):
+            out[k] = self._to_numpy(getattr(v, "d_" + k), ns, np.int32)
+        out["seeds"] = self._to_numpy(v.d_seeds, nseeds, np.uint32)
+        out["tracklets"] = self._to_numpy(v.d_tracklets, nseeds, TRACKLET_DTYPE)
+        n_rows = self.geom.n_rows
+        if nseeds:
+            rh = self._view(v.d_row_hit, 4 * n_rows * stride).view(self.torch.int32).reshape(n_rows, stride)
+            out["row_hit"] = rh[:, :nseeds].t().contiguous().cpu().numpy()
+        else:
+            out["row_hit"] = np.zeros((0, n_rows), dtype=np.int32)
+        return out

@@ -1,0 +1,344 @@
+// tpc_api.cu — the C ABI of include/tpc_track.h: context, workspace carving, stream handling.
+// Host code only; all arithmetic of the method runs in the kernels of tpc_kernels.cu.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "tpc_internal.h"
+
+struct tpc_ctx {
+  tpc_geom_desc geom;
+  tpc_params params;
+  TpcConst hconst;
+  TpcConst* d_const = nullptr;
+  TpcCounters* d_cnt = nullptr;
+  TpcRowStat* d_row_stat = nullptr;
+  TpcCounters* h_cnt = nullptr;  // pinned
+  TpcStageEvents events;
+  int n_sm = 148;
+  int device = 0;
+  // last run
+  bool ran = false;
+  bool synced = false;
+  TpcBuffers buf;
+  cudaStream_t stream = nullptr;
+  uint32_t flags = 0;
+  int launches = 0;
+  uint64_t n_bins_cap = 0;
+  char cuda_err[256] = {0};
+};
+
+namespace {
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int set_cuda_err(tpc_ctx* c, cudaError_t e, const char* what) {
+  if (c) std::snprintf(c->cuda_err, sizeof(c->cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  return TPC_E_CUDA;
+}
+
+struct Capacities {
+  uint64_t max_bins;
+  uint32_t max_seeds, max_tracks, max_ids, scan_blocks;
+};
+
+Capacities capacities(const tpc_ctx* c, uint64_t n) {
+  Capacities k;
+  const tpc_params& P = c->params;
+  int ny_max = 1;
+  for (int r = 0; r < c->geom.n_rows; ++r) ny_max = c->hconst.ny[r] > ny_max ? c->hconst.ny[r] : ny_max;
+  uint64_t bins = P.max_bins;
+  if (bins == 0)
+    bins = 4 * n + (uint64_t)c->geom.n_sectors * c->geom.n_rows * ny_max *
+                       ((uint64_t)std::ceil(c->geom.z_max / P.grid_dz) + 2);
+  if (bins > 0xFFFFFFF0ull) bins = 0xFFFFFFF0ull;
+  k.max_bins = bins;
+  uint64_t seeds = P.max_seeds ? P.max_seeds : n / 8 + 4096;
+  seeds = align_up(seeds, 64);
+  k.max_seeds = (uint32_t)seeds;
+  const uint64_t ids = n * 1000 / (1000 - (uint64_t)P.shared_permille) + 64;
+  k.max_ids = (uint32_t)(ids > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : ids);
+  k.max_tracks = (uint32_t)(k.max_ids / (uint32_t)(P.min_hits_track > 0 ? P.min_hits_track : 1) + 1);
+  const uint64_t b1 = (n + 1023) / 1024 + 2, b2 = 2 * ((seeds + 255) / 256 + 2);
+  k.scan_blocks = (uint32_t)(b1 > b2 ? b1 : b2);
+  return k;
+}
+
+// Carve the workspace.  base == nullptr: only the size is computed.
+size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
+  const Capacities k = capacities(c, n);
+  const uint32_t n_sr = (uint32_t)(c->geom.n_sectors * c->geom.n_rows);
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  TpcBuffers b;
+  std::memset(&b, 0, sizeof(b));
+  b.n = (uint32_t)n;
+  b.n_sr = n_sr;
+  b.max_bins = k.max_bins;
+  b.max_seeds = k.max_seeds;
+  b.max_tracks = k.max_tracks;
+  b.max_ids = k.max_ids;
+  b.scan_blocks = k.scan_blocks;
+  b.row_desc = (tpc_row_desc*)take(sizeof(tpc_row_desc) * n_sr);
+  b.tile_ofs = (uint32_t*)take(4 * (size_t)(n_sr + 1));
+  b.slot = (uint32_t*)take(4 * n);
+  b.bin_start = (uint32_t*)take(4 * (k.max_bins + 4));
+  b.yz = (float2*)take(8 * n);
+  b.orig_id = (uint32_t*)take(4 * n);
+  b.link_up = (int32_t*)take(4 * n);
+  b.link_dn = (int32_t*)take(4 * n);
+  b.link_up2 = (int32_t*)take(4 * n);
+  b.link_dn2 = (int32_t*)take(4 * n);
+  b.seed_len = (uint8_t*)take(n);
+  b.scan_partials = (uint32_t*)take(4 * (size_t)(k.scan_blocks + 2));
+  b.seeds = (uint32_t*)take(4 * (size_t)k.max_seeds);
+  b.tracklets = (tpc_tracklet*)take(sizeof(tpc_tracklet) * (size_t)k.max_seeds);
+  b.row_hit = (int32_t*)take(4 * (size_t)c->geom.n_rows * k.max_seeds);
+  b.owner = (unsigned long long*)take(8 * n);
+  b.tl_key = (unsigned long long*)take(8 * (size_t)k.max_seeds);
+  b.seg_cnt = (uint32_t*)take(4 * (size_t)(k.max_seeds + 1));
+  b.id_cnt = (uint32_t*)take(4 * (size_t)(k.max_seeds + 1));
+  b.tracks = (tpc_track*)take(sizeof(tpc_track) * (size_t)k.max_tracks);
+  b.cluster_ids = (uint32_t*)take(4 * (size_t)k.max_ids);
+  b.cluster_shared = (uint8_t*)take((size_t)k.max_ids);
+  if (B) *B = b;
+  return off;
+}
+
+}  // namespace
+
+extern "C" {
+
+void tpc_default_params(tpc_params* p) {
+  std::memset(p, 0, sizeof(*p));
+  p->err_y = 0.1f; p->err_z = 0.1f;
+  p->nf_slope_y = 1.0f; p->nf_slope_z = 1.6f; p->nf_max_d2 = 0.70f;
+  p->seed_min_len = 4;
+  p->init_var_sinphi = 0.25f; p->init_var_tanl = 4.0f; p->init_var_qpt = 100.0f;
+  p->max_sinphi = 0.95f; p->max_qpt = 20.0f;
+  p->road_nsigma = 3.5f; p->road_min = 0.3f; p->road_max = 2.0f;
+  p->chi2_max_hit = 12.0f;
+  p->max_gap_follow = 4; p->min_hits_tracklet = 10;
+  p->sel_chi2_weight = 2.0f;
+  p->shared_permille = 100; p->max_gap_select = 4; p->min_hits_track = 20;
+  p->grid_dy = 2.0f; p->grid_dz = 2.0f;
+  p->max_bins = 0; p->max_seeds = 0;
+}
+
+int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx** out) {
+  if (!geom || !out) return TPC_E_ARG;
+  *out = nullptr;
+  if (geom->n_sectors < 1 || geom->n_sectors > 256 || geom->n_rows < 3 || geom->n_rows > 255 ||
+      !(geom->r_max > geom->r_min) || !(geom->r_min > 0.f) || !(geom->sector_half_angle_deg > 0.f) ||
+      !(geom->sector_half_angle_deg < 90.f) || !(geom->z_max > 0.f))
+    return TPC_E_ARG;
+  tpc_params P;
+  if (params) P = *params; else tpc_default_params(&P);
+  if (!(P.grid_dy > 0.f) || !(P.grid_dz > 0.f) || P.shared_permille < 0 || P.shared_permille > 500 ||
+      P.seed_min_len < 2 || P.seed_min_len > 255 || P.min_hits_track < 1 || P.min_hits_tracklet < 2 ||
+      !(P.err_y > 0.f) || !(P.err_z > 0.f) || !(P.max_sinphi > 0.f) || !(P.max_sinphi < 1.f) ||
+      P.max_gap_follow < 0 || P.max_gap_select < 0)
+    return TPC_E_ARG;
+  tpc_ctx* c = new (std::nothrow) tpc_ctx();
+  if (!c) return TPC_E_ARG;
+  c->geom = *geom;
+  c->params = P;
+  // R0 tables in double, rounded once to fp32 (rule D5)
+  TpcConst& K = c->hconst;
+  std::memset(&K, 0, sizeof(K));
+  K.n_sectors = geom->n_sectors;
+  K.n_rows = geom->n_rows;
+  const double pitch = ((double)geom->r_max - (double)geom->r_min) / (double)(geom->n_rows - 1);
+  const double th = std::tan((double)geom->sector_half_angle_deg * (3.14159265358979323846 / 180.0));
+  for (int r = 0; r < geom->n_rows; ++r) {
+    const double xr = (double)geom->r_min + r * pitch;
+    const double ym = xr * th;
+    K.x[r] = (float)xr;
+    K.ylim[r] = (float)(ym + 2.0);
+    const int ny = (int)std::ceil(2.0 * (ym + 2.0) / (double)P.grid_dy);
+    K.ny[r] = ny < 1 ? 1 : ny;
+  }
+  K.dx_row = (float)pitch;
+  K.cfield = (float)(-0.00299792458 * (double)geom->bz_tesla);
+  K.inv_dy = 1.0f / P.grid_dy;
+  K.inv_dz = 1.0f / P.grid_dz;
+  K.vy = P.err_y * P.err_y;
+  K.vz = P.err_z * P.err_z;
+  K.wy = P.nf_slope_y * K.dx_row;
+  K.wz = P.nf_slope_z * K.dx_row;
+  K.P = P;
+  cudaError_t e;
+  const uint32_t n_sr = (uint32_t)(geom->n_sectors * geom->n_rows);
+  if ((e = cudaGetDevice(&c->device)) != cudaSuccess ||
+      (e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device)) != cudaSuccess ||
+      (e = cudaMalloc(&c->d_const, sizeof(TpcConst))) != cudaSuccess ||
+      (e = cudaMalloc(&c->d_cnt, sizeof(TpcCounters))) != cudaSuccess ||
+      (e = cudaMalloc(&c->d_row_stat, sizeof(TpcRowStat) * n_sr)) != cudaSuccess ||
+      (e = cudaMallocHost(&c->h_cnt, sizeof(TpcCounters))) != cudaSuccess ||
+      (e = cudaMemcpy(c->d_const, &K, sizeof(TpcConst), cudaMemcpyHostToDevice)) != cudaSuccess) {
+    std::fprintf(stderr, "tpc_geom_init: %s\n", cudaGetErrorString(e));
+    tpc_destroy(c);
+    return TPC_E_CUDA;
+  }
+  c->events.enabled = false;
+  for (int i = 0; i < TPC_N_STAGES; ++i) {
+    c->events.ev[i] = nullptr;
+    if ((e = cudaEventCreate(&c->events.ev[i])) != cudaSuccess) {
+      tpc_destroy(c);
+      return TPC_E_CUDA;
+    }
+  }
+  *out = c;
+  return TPC_OK;
+}
+
+size_t tpc_workspace_bytes(const tpc_ctx* ctx, uint64_t n_clusters) {
+  if (!ctx || n_clusters >= (1ull << 30)) return 0;
+  return carve(ctx, n_clusters, nullptr, nullptr);
+}
+
+int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream, uint32_t flags) {
+  if (!ctx || !d_workspace || (!d_clusters && n_clusters) || n_clusters >= (1ull << 30)) return TPC_E_ARG;
+  if (((uintptr_t)d_clusters & 15u) || ((uintptr_t)d_workspace & 255u)) return TPC_E_ARG;
+  TpcBuffers B;
+  const size_t need = carve(ctx, n_clusters, (char*)d_workspace, &B);
+  if (workspace_bytes < need) return TPC_E_WORKSPACE;
+  B.clusters = d_clusters;
+  B.K = ctx->d_const;
+  B.cnt = ctx->d_cnt;
+  B.row_stat = ctx->d_row_stat;
+  ctx->buf = B;
+  ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->flags = flags;
+  ctx->ran = false;
+  ctx->synced = false;
+  ctx->events.enabled = (flags & TPC_STAGE_TIMERS) != 0;
+  (void)cudaGetLastError();
+  const int launches = (flags & TPC_DETERMINISTIC)
+                           ? tpc_det::run_pipeline(B, ctx->stream, flags, ctx->events, ctx->n_sm)
+                           : tpc_fast::run_pipeline(B, ctx->stream, flags, ctx->events, ctx->n_sm);
+  if (launches < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch");
+  cudaError_t e = cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(TpcCounters), cudaMemcpyDeviceToHost, ctx->stream);
+  if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(counters)");
+  ctx->launches = launches;
+  ctx->ran = true;
+  return TPC_OK;
+}
+
+static int sync_run(tpc_ctx* ctx) {
+  if (!ctx) return TPC_E_ARG;
+  if (!ctx->ran) return TPC_E_STATE;
+  if (!ctx->synced) {
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize");
+    ctx->synced = true;
+  }
+  return TPC_OK;
+}
+
+static int device_status(const tpc_ctx* ctx) {
+  const uint32_t err = ctx->h_cnt->error;
+  if (err & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return TPC_E_OVERFLOW;
+  if (err & TPC_DEVERR_BAD_CLUSTER) return TPC_E_ARG;
+  return TPC_OK;
+}
+
+int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out) {
+  if (!out) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  const TpcCounters& c = *ctx->h_cnt;
+  std::memset(out, 0, sizeof(*out));
+  rc = device_status(ctx);
+  const bool valid = rc != TPC_E_OVERFLOW;
+  out->n_tracks = valid ? c.n_tracks : 0;
+  out->n_cluster_ids = valid ? c.n_ids : 0;
+  out->d_tracks = ctx->buf.tracks;
+  out->d_cluster_ids = ctx->buf.cluster_ids;
+  out->d_cluster_shared = ctx->buf.cluster_shared;
+  out->n_ignored = c.n_ignored;
+  out->n_dropped = c.n_dropped;
+  out->n_seeds = c.n_seeds;
+  out->n_tracklets = c.n_tracklets;
+  out->n_bins = c.n_bins;
+  return rc;
+}
+
+int tpc_get_intermediates(tpc_ctx* ctx, tpc_debug_view* out) {
+  if (!out) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!(ctx->flags & TPC_KEEP_INTERMEDIATES)) return TPC_E_STATE;
+  const TpcCounters& c = *ctx->h_cnt;
+  const TpcBuffers& B = ctx->buf;
+  std::memset(out, 0, sizeof(*out));
+  out->n_clusters = B.n;
+  out->n_sorted = c.n_sorted;
+  out->n_rows_total = B.n_sr;
+  out->n_bins = c.n_bins;
+  out->n_seeds = c.n_seeds;
+  out->tracklet_stride = B.max_seeds;
+  out->d_row_desc = B.row_desc;
+  out->d_bin_start = B.bin_start;
+  out->d_yz_sorted = (const float*)B.yz;
+  out->d_orig_id = B.orig_id;
+  out->d_link_up = B.link_up;
+  out->d_link_dn = B.link_dn;
+  out->d_link_up2 = B.link_up2;
+  out->d_link_dn2 = B.link_dn2;
+  out->d_seeds = B.seeds;
+  out->d_tracklets = B.tracklets;
+  out->d_row_hit = B.row_hit;
+  return device_status(ctx);
+}
+
+int tpc_get_stage_ms(tpc_ctx* ctx, float* out_ms) {
+  if (!out_ms) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!(ctx->flags & TPC_STAGE_TIMERS)) return TPC_E_STATE;
+  for (int i = 0; i < TPC_N_STAGES - 1; ++i) {
+    cudaError_t e = cudaEventElapsedTime(&out_ms[i], ctx->events.ev[i], ctx->events.ev[i + 1]);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaEventElapsedTime");
+  }
+  cudaError_t e = cudaEventElapsedTime(&out_ms[TPC_N_STAGES - 1], ctx->events.ev[0], ctx->events.ev[TPC_N_STAGES - 1]);
+  if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaEventElapsedTime");
+  return TPC_OK;
+}
+
+int tpc_last_launch_count(const tpc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+void tpc_destroy(tpc_ctx* c) {
+  if (!c) return;
+  for (int i = 0; i < TPC_N_STAGES; ++i)
+    if (c->events.ev[i]) cudaEventDestroy(c->events.ev[i]);
+  if (c->d_const) cudaFree(c->d_const);
+  if (c->d_cnt) cudaFree(c->d_cnt);
+  if (c->d_row_stat) cudaFree(c->d_row_stat);
+  if (c->h_cnt) cudaFreeHost(c->h_cnt);
+  delete c;
+}
+
+const char* tpc_strerror(int err) {
+  switch (err) {
+    case TPC_OK: return "ok";
+    case TPC_E_ARG: return "bad argument (null/misaligned pointer, bad descriptor, or a cluster outside the geometry)";
+    case TPC_E_WORKSPACE: return "workspace too small";
+    case TPC_E_OVERFLOW: return "device capacity exceeded (bins, seeds or tracks); results invalid";
+    case TPC_E_CUDA: return "CUDA runtime error";
+    case TPC_E_STATE: return "call order violated";
+    default: return "unknown error";
+  }
+}
+
+const char* tpc_last_cuda_error(const tpc_ctx* ctx) { return ctx ? ctx->cuda_err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,97 @@
+// tpc_internal.h — internal types shared by the host API (tpc_api.cu) and the two builds of
+// the kernel translation unit (tpc_kernels.cu compiled once with -DTPC_DET=1 --fmad=false as
+// namespace tpc_det, once with -DTPC_DET=0 --fmad=true as namespace tpc_fast).
+// Product code: nothing here is used by, or uses, the oracle.
+#ifndef TPC_INTERNAL_H
+#define TPC_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tpc_track.h"
+
+#define TPC_MAX_ROWS 256
+
+// Per-context constants, resident in device global memory (DESIGN.md rule D5: tables are
+// computed in double on the host and rounded once to fp32).
+struct TpcConst {
+  int32_t n_sectors, n_rows;
+  float dx_row;   // row pitch (r_max-r_min)/(n_rows-1)
+  float cfield;   // signed curvature per unit q/pT: -0.00299792458*Bz
+  float inv_dy, inv_dz;
+  float vy, vz;   // err_y^2, err_z^2
+  float wy, wz;   // neighbour windows nf_slope_*dx_row
+  tpc_params P;
+  float x[TPC_MAX_ROWS];
+  float ylim[TPC_MAX_ROWS];  // ymax_r + 2 cm
+  int32_t ny[TPC_MAX_ROWS];
+};
+
+// error bits raised on the device
+#define TPC_DEVERR_BAD_CLUSTER 1u   // sector/row outside the geometry -> TPC_E_ARG
+#define TPC_DEVERR_BINS 2u          // bin index capacity            -> TPC_E_OVERFLOW
+#define TPC_DEVERR_SEEDS 4u         // seed capacity                 -> TPC_E_OVERFLOW
+#define TPC_DEVERR_TRACKS 8u        // track / cluster-id capacity   -> TPC_E_OVERFLOW
+
+struct TpcCounters {
+  uint32_t n_sorted, n_ignored, n_dropped, n_bad;
+  uint32_t n_bins, n_tiles, n_seeds, n_tracklets;
+  uint32_t n_tracks, n_ids, error, pad_;
+};
+
+// per (sector,row) statistics of pass 1
+struct TpcRowStat {
+  uint32_t zmin_key, zmax_key;  // order-preserving uint image of the float
+  uint32_t count, pad_;
+};
+
+#define TPC_NF_TILE 256  // clusters per neighbour-finder tile (one CTA)
+
+// All device buffers of one run (pointers into the caller's workspace, or ctx-owned).
+struct TpcBuffers {
+  const tpc_cluster* clusters;
+  uint32_t n;            // input clusters
+  uint32_t n_sr;         // n_sectors*n_rows
+  uint64_t max_bins;
+  uint32_t max_seeds, max_tracks, max_ids;
+  uint32_t scan_blocks;  // capacity of scan_partials
+  const TpcConst* K;
+  TpcCounters* cnt;
+  TpcRowStat* row_stat;   // [n_sr]
+  tpc_row_desc* row_desc; // [n_sr]
+  uint32_t* tile_ofs;     // [n_sr+1] first neighbour-finder tile of each row
+  uint32_t* slot;         // [n] rank of the cluster inside its bin, 0xFFFFFFFF = not in the grid
+  uint32_t* bin_start;    // [max_bins+1]
+  float2* yz;             // [n] sorted
+  uint32_t* orig_id;      // [n] sorted
+  int32_t* link_up;       // [n]
+  int32_t* link_dn;
+  int32_t* link_up2;
+  int32_t* link_dn2;
+  uint8_t* seed_len;      // [n] chain length if the cluster is a start hit of a seed, else 0
+  uint32_t* scan_partials;// [scan_blocks+1]
+  uint32_t* seeds;        // [max_seeds] sorted index of start hits
+  tpc_tracklet* tracklets;// [max_seeds]
+  int32_t* row_hit;       // [n_rows][max_seeds]
+  unsigned long long* owner;     // [n]
+  unsigned long long* tl_key;    // [max_seeds]
+  uint32_t* seg_cnt;      // [max_seeds+1] tracks per tracklet -> exclusive scan
+  uint32_t* id_cnt;       // [max_seeds+1] cluster ids per tracklet -> exclusive scan
+  tpc_track* tracks;      // [max_tracks]
+  uint32_t* cluster_ids;  // [max_ids]
+  uint8_t* cluster_shared;// [max_ids]
+};
+
+struct TpcStageEvents {
+  cudaEvent_t ev[TPC_N_STAGES];  // boundaries: start, after grid, nf, seeds, follower, selector
+  bool enabled;
+};
+
+namespace tpc_det {
+int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, const TpcStageEvents& E, int n_sm);
+}
+namespace tpc_fast {
+int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, const TpcStageEvents& E, int n_sm);
+}
+
+#endif

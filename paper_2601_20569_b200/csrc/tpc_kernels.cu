@@ -1,0 +1,1075 @@
+// tpc_kernels.cu — sm_100a CUDA kernels of the TPC sector tracking (section 2,
+// PAPER.md:57,59 section 3; readings R0..R6 of DESIGN.md).
+//
+// This translation unit is compiled TWICE:
+//   -DTPC_DET=1 --fmad=false  -> namespace tpc_det  : deterministic mode: no FMA
+//                                contraction, stable grid order; bit-comparable to the CPU oracle
+//   -DTPC_DET=0 --fmad=true   -> namespace tpc_fast : FMA contraction allowed, no in-bin sort
+// Both use only + - * / sqrt on the decision path; every argmin carries an integer tie-break on
+// the ORIGINAL cluster index (rule D2), so atomics / thread order never change a result.
+//
+// Kernel groups:  K1 grid (row stats -> row descriptors -> histogram -> per-row scan -> scatter
+//                 [-> in-bin sort]),  K2 neighbour finder,  K3 link cleanup + seeds,
+//                 K4 Kalman track follower,  K5 ambiguity solving.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "tpc_internal.h"
+
+#ifndef TPC_DET
+#error "compile with -DTPC_DET=0 or 1"
+#endif
+#if TPC_DET
+#define TPC_NS tpc_det
+#else
+#define TPC_NS tpc_fast
+#endif
+
+namespace TPC_NS {
+
+// ------------------------------------------------------------------ small device helpers
+__device__ __forceinline__ uint32_t f2key(float f) {  // order-preserving float -> uint
+  uint32_t b = __float_as_uint(f);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float key2f(uint32_t k) {
+  return __uint_as_float((k & 0x80000000u) ? (k & 0x7FFFFFFFu) : ~k);
+}
+__device__ __forceinline__ int bin_coord(float v, float v0, float inv_d, int n) {
+  int b = (int)floorf((v - v0) * inv_d);
+  b = b < 0 ? 0 : b;
+  return b > n - 1 ? n - 1 : b;
+}
+__device__ __forceinline__ bool finite2(float a, float b) {
+  return (fabsf(a) <= 3.402823466e38f) && (fabsf(b) <= 3.402823466e38f);  // false for NaN/Inf
+}
+__device__ __forceinline__ uint4 ld_stream16(const void* p) {  // streaming 16-byte load
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+// Classify one input cluster. Returns: 0 in grid, 1 ignored (NaN/Inf), 2 dropped (|y| beyond
+// the row + 2 cm), 3 bad (sector/row outside the geometry).  R1 of DESIGN.md.
+__device__ __forceinline__ int classify(const uint4& raw, const TpcConst* __restrict__ K, int& sr, float& y,
+                                        float& z, int& row) {
+  y = __uint_as_float(raw.x);
+  z = __uint_as_float(raw.y);
+  const int sector = raw.w & 0xFF;
+  row = (raw.w >> 8) & 0xFF;
+  sr = sector * K->n_rows + row;
+  if (sector >= K->n_sectors || row >= K->n_rows) return 3;
+  if (!finite2(y, z)) return 1;
+  if (!(fabsf(y) <= K->ylim[row])) return 2;
+  return 0;
+}
+
+// ================================================================== K1 grid
+// K1a: per (sector,row) min/max z and cluster count.  One coalesced 16-byte load per cluster.
+// Inputs usually arrive grouped by (sector,row) (clusteriser order), so a warp whose lanes
+// all hit the same row does 3 atomics instead of 96.
+__global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
+  const TpcConst* __restrict__ K = B.K;
+  uint32_t n_ign = 0, n_drop = 0, n_bad = 0;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < ((B.n + 31u) & ~31u);
+       i += gridDim.x * blockDim.x) {
+    int cls = 4, sr = -1, row;
+    float y, z = 0.f;
+    if (i < B.n) {
+      const uint4 raw = ld_stream16(B.clusters + i);
+      cls = classify(raw, K, sr, y, z, row);
+    }
+    n_ign += cls == 1;
+    n_drop += cls == 2;
+    n_bad += cls == 3;
+    const bool ok = cls == 0;
+    const unsigned okmask = __ballot_sync(0xffffffffu, ok);
+    if (okmask == 0) continue;
+    const int leader = __ffs(okmask) - 1;
+    const int sr0 = __shfl_sync(0xffffffffu, sr, leader);
+    const bool uniform = __all_sync(0xffffffffu, !ok || sr == sr0);
+    const uint32_t zk = f2key(z);
+    if (uniform) {
+      const uint32_t mn = __reduce_min_sync(0xffffffffu, ok ? zk : 0xFFFFFFFFu);
+      const uint32_t mx = __reduce_max_sync(0xffffffffu, ok ? zk : 0u);
+      if ((int)(threadIdx.x & 31) == leader) {
+        atomicMin(&B.row_stat[sr0].zmin_key, mn);
+        atomicMax(&B.row_stat[sr0].zmax_key, mx);
+        atomicAdd(&B.row_stat[sr0].count, (uint32_t)__popc(okmask));
+      }
+    } else if (ok) {
+      atomicMin(&B.row_stat[sr].zmin_key, zk);
+      atomicMax(&B.row_stat[sr].zmax_key, zk);
+      atomicAdd(&B.row_stat[sr].count, 1u);
+    }
+  }
+  n_ign = __reduce_add_sync(0xffffffffu, n_ign);
+  n_drop = __reduce_add_sync(0xffffffffu, n_drop);
+  n_bad = __reduce_add_sync(0xffffffffu, n_bad);
+  if ((threadIdx.x & 31) == 0) {
+    if (n_ign) atomicAdd(&B.cnt->n_ignored, n_ign);
+    if (n_drop) atomicAdd(&B.cnt->n_dropped, n_drop);
+    if (n_bad) {
+      atomicAdd(&B.cnt->n_bad, n_bad);
+      atomicOr(&B.cnt->error, TPC_DEVERR_BAD_CLUSTER);
+    }
+  }
+}
+
+// Block-wide exclusive scan of one value per thread (blockDim.x <= 1024); returns the
+// exclusive prefix, *total = block sum.  Warp-level scans with shuffles + one smem hop.
+__device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* total, uint32_t* smem33) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += t;
+  }
+  __syncthreads();  // smem33 may still be in use from a previous call
+  if (lane == 31) smem33[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    uint32_t s = lane < nw ? smem33[lane] : 0u;
+    uint32_t si = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, si, d);
+      if (lane >= d) si += t;
+    }
+    smem33[lane] = si - s;
+    if (lane == 31) smem33[32] = si;
+  }
+  __syncthreads();
+  *total = smem33[32];
+  return smem33[w] + inc - v;
+}
+
+// K1b: row descriptors (one CTA).  nz from the z range, exclusive scans over the (sector,row)
+// list for the first bin, first sorted cluster and first neighbour-finder tile of each row.
+__global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  const TpcConst* __restrict__ K = B.K;
+  uint32_t base_bin = 0, base_clu = 0, base_tile = 0;
+  unsigned long long bins64 = 0;
+  bool overflow = false;
+  for (uint32_t s0 = 0; s0 < B.n_sr; s0 += blockDim.x) {
+    const uint32_t sr = s0 + threadIdx.x;
+    uint32_t cnt = 0, nb = 0, nt = 0;
+    int nz = 0, ny = 0;
+    float z0 = 0.f, y0 = 0.f;
+    if (sr < B.n_sr) {
+      const int row = sr % K->n_rows;
+      cnt = B.row_stat[sr].count;
+      ny = K->ny[row];
+      y0 = -K->ylim[row];
+      if (cnt) {
+        z0 = key2f(B.row_stat[sr].zmin_key);
+        const float zhi = key2f(B.row_stat[sr].zmax_key);
+        const float fz = floorf((zhi - z0) * K->inv_dz);
+        // bound nz so that ny*nz cannot wrap; a frame this sparse overflows max_bins anyway
+        nz = fz >= 16777216.f ? 16777216 : (int)fz + 1;
+        nz = nz < 1 ? 1 : nz;
+        const unsigned long long nb64 = (unsigned long long)ny * (unsigned long long)nz;
+        if (nb64 > B.max_bins) { overflow = true; nb = 0; nz = 0; }
+        else nb = (uint32_t)nb64;
+        nt = (cnt + TPC_NF_TILE - 1) / TPC_NF_TILE;
+      }
+    }
+    uint32_t tot_b, tot_c, tot_t;
+    const uint32_t pb = block_excl_scan(nb, &tot_b, sm);
+    const uint32_t pc = block_excl_scan(cnt, &tot_c, sm);
+    const uint32_t pt = block_excl_scan(nt, &tot_t, sm);
+    if (sr < B.n_sr) {
+      tpc_row_desc d;
+      d.y0 = y0; d.z0 = z0; d.ny = ny; d.nz = nz;
+      d.bin_ofs = base_bin + pb;
+      d.clu_ofs = base_clu + pc;
+      d.count = cnt;
+      d.pad_ = 0;
+      B.row_desc[sr] = d;
+      B.tile_ofs[sr] = base_tile + pt;
+    }
+    bins64 += tot_b;
+    base_bin += tot_b; base_clu += tot_c; base_tile += tot_t;
+  }
+  overflow = __syncthreads_or(overflow || bins64 > B.max_bins);
+  if (threadIdx.x == 0) {
+    B.tile_ofs[B.n_sr] = base_tile;
+    B.cnt->n_sorted = base_clu;
+    B.cnt->n_tiles = base_tile;
+    if (overflow) {
+      atomicOr(&B.cnt->error, TPC_DEVERR_BINS);
+      B.cnt->n_bins = 0;
+    } else {
+      B.cnt->n_bins = base_bin;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_zero_bins(TpcBuffers B) {
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  const uint32_t n = B.cnt->n_bins + 1;
+  uint4* p4 = reinterpret_cast<uint4*>(B.bin_start);
+  const uint32_t n4 = n / 4;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x)
+    p4[i] = make_uint4(0, 0, 0, 0);
+  if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) B.bin_start[n4 * 4 + threadIdx.x] = 0;
+}
+
+__device__ __forceinline__ uint32_t bin_of(const tpc_row_desc& d, const TpcConst* __restrict__ K, float y, float z) {
+  const int by = bin_coord(y, d.y0, K->inv_dy, d.ny);
+  const int bz = bin_coord(z, d.z0, K->inv_dz, d.nz);
+  return d.bin_ofs + (uint32_t)bz * (uint32_t)d.ny + (uint32_t)by;
+}
+
+// K1c: histogram.  slot[i] = rank of cluster i inside its bin (the value the atomic returns),
+// so the scatter needs no second atomic.
+__global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
+  const TpcConst* __restrict__ K = B.K;
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
+    const uint4 raw = ld_stream16(B.clusters + i);
+    int sr, row;
+    float y, z;
+    uint32_t s = 0xFFFFFFFFu;
+    if (classify(raw, K, sr, y, z, row) == 0) {
+      const tpc_row_desc d = B.row_desc[sr];
+      s = atomicAdd(&B.bin_start[bin_of(d, K, y, z)], 1u);
+    }
+    B.slot[i] = s;
+  }
+}
+
+// K1d: per-row exclusive scan of the bin counts -> bin_start (global sorted positions).
+// One CTA per (sector,row); warp-level shuffles scan 8 bins per thread per step
+// (north star: "a per-row bin index built by a warp-level scan").
+__global__ void __launch_bounds__(512) k_bin_scan(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
+    const tpc_row_desc d = B.row_desc[sr];
+    const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
+    uint32_t* p = B.bin_start + d.bin_ofs;
+    uint32_t carry = d.clu_ofs;
+    for (uint32_t b0 = 0; b0 < nb; b0 += blockDim.x * 8) {
+      const uint32_t b = b0 + threadIdx.x * 8;
+      uint32_t v[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) v[k] = (b + k < nb) ? p[b + k] : 0u;
+      uint32_t s = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) s += v[k];
+      uint32_t tot;
+      uint32_t pre = carry + block_excl_scan(s, &tot, sm);
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        if (b + k < nb) p[b + k] = pre;
+        pre += v[k];
+      }
+      carry += tot;
+    }
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) B.bin_start[B.cnt->n_bins] = B.cnt->n_sorted;
+}
+
+// K1e: scatter into bin order: sorted (y,z) pairs + original index.
+__global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
+  const TpcConst* __restrict__ K = B.K;
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
+    const uint32_t s = B.slot[i];
+    if (s == 0xFFFFFFFFu) continue;
+    const uint4 raw = ld_stream16(B.clusters + i);
+    int sr, row;
+    float y, z;
+    classify(raw, K, sr, y, z, row);
+    const tpc_row_desc d = B.row_desc[sr];
+    const uint32_t pos = B.bin_start[bin_of(d, K, y, z)] + s;
+    B.yz[pos] = make_float2(y, z);
+    B.orig_id[pos] = i;
+  }
+}
+
+#if TPC_DET
+// K1f (deterministic mode only): order the clusters of every bin by ascending original index,
+// so that the sorted order is a function of the input alone (stable sort).
+__global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  const uint32_t nb = B.cnt->n_bins;
+  for (uint32_t b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
+    const uint32_t lo = B.bin_start[b], hi = B.bin_start[b + 1];
+    for (uint32_t i = lo + 1; i < hi; ++i) {  // insertion sort, bins hold a few clusters
+      const uint32_t id = B.orig_id[i];
+      const float2 v = B.yz[i];
+      uint32_t j = i;
+      while (j > lo && B.orig_id[j - 1] > id) {
+        B.orig_id[j] = B.orig_id[j - 1];
+        B.yz[j] = B.yz[j - 1];
+        --j;
+      }
+      B.orig_id[j] = id;
+      B.yz[j] = v;
+    }
+  }
+}
+#endif
+
+// ================================================================== window queries
+// Visit the sorted clusters of one row whose bin intersects [ylo,yhi]x[zlo,zhi].  The margins
+// make sure rounding can never hide a cluster that satisfies a window inequality; membership
+// is always decided by the caller on the inequality itself (rule D3: results do not depend
+// on the bin size).
+struct BinWindow {
+  uint32_t base;  // bin_ofs + by0 of z-row 0
+  int ny, by_span, bz0, bz1;
+};
+__device__ __forceinline__ BinWindow make_window(const tpc_row_desc& d, const TpcConst* __restrict__ K, float ylo,
+                                                 float yhi, float zlo, float zhi) {
+  const float my = 1e-3f;
+  const float mz = 1e-3f + 4e-7f * fmaxf(fabsf(zlo), fabsf(zhi));
+  const int by0 = bin_coord(ylo - my, d.y0, K->inv_dy, d.ny);
+  const int by1 = bin_coord(yhi + my, d.y0, K->inv_dy, d.ny);
+  BinWindow w;
+  w.ny = d.ny;
+  w.base = d.bin_ofs + (uint32_t)by0;
+  w.by_span = by1 - by0 + 1;
+  w.bz0 = bin_coord(zlo - mz, d.z0, K->inv_dz, d.nz);
+  w.bz1 = bin_coord(zhi + mz, d.z0, K->inv_dz, d.nz);
+  return w;
+}
+
+// ================================================================== K2 neighbour finder
+// PAPER.md:27 "combinatorial seeding based on a cellular automaton"; R2.
+// One CTA per tile of TPC_NF_TILE consecutive sorted clusters of one row (bins are z-major,
+// so a tile is a compact z-slab and its windows on rows r+-1 overlap heavily -> L1 reuse).
+// One thread per cluster; the best (up,down) pair is the lexicographic minimum of
+// (d2, original id of up, original id of down).
+__global__ void __launch_bounds__(TPC_NF_TILE) k_neighbours(TpcBuffers B) {
+  const TpcConst* __restrict__ K = B.K;
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  const uint32_t n_tiles = B.cnt->n_tiles;
+  const int R = K->n_rows;
+  const float wy = K->wy, wz = K->wz, max_d2 = K->P.nf_max_d2;
+  const uint32_t* __restrict__ bin_start = B.bin_start;
+  const float2* __restrict__ yz = B.yz;
+  const uint32_t* __restrict__ orig = B.orig_id;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    // row of this tile: last sr with tile_ofs[sr] <= tile
+    uint32_t lo = 0, hi = B.n_sr;
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (B.tile_ofs[mid] <= tile) lo = mid; else hi = mid;
+    }
+    const uint32_t sr = lo;
+    const int r = (int)(sr % (uint32_t)R);
+    const tpc_row_desc d = B.row_desc[sr];
+    const uint32_t local = (tile - B.tile_ofs[sr]) * TPC_NF_TILE + threadIdx.x;
+    if (local >= d.count) continue;
+    const uint32_t i = d.clu_ofs + local;
+    int32_t bj = -1, bk = -1;
+    if (r >= 1 && r <= R - 2) {
+      const tpc_row_desc du = B.row_desc[sr + 1], dd = B.row_desc[sr - 1];
+      if (du.count && dd.count) {
+        const float2 ci = yz[i];
+        const float yi = ci.x, zi = ci.y;
+        const float ti = yi / K->x[r];
+        const float ty = ti * K->dx_row;
+        const BinWindow wu = make_window(du, K, (yi + ty) - wy, (yi + ty) + wy, zi - wz, zi + wz);
+        const BinWindow wd = make_window(dd, K, (yi - ty) - wy, (yi - ty) + wy, zi - wz, zi + wz);
+        float best = 0.f;
+        uint32_t bjid = 0, bkid = 0;
+        for (int bzu = wu.bz0; bzu <= wu.bz1; ++bzu) {
+          const uint32_t bu = wu.base + (uint32_t)bzu * (uint32_t)wu.ny;
+          const uint32_t ju1 = bin_start[bu + wu.by_span];
+          for (uint32_t j = bin_start[bu]; j < ju1; ++j) {
+            const float2 cj = yz[j];
+            if (!(fabsf((cj.x - yi) - ty) <= wy && fabsf(cj.y - zi) <= wz)) continue;
+            const float dyu = cj.x - yi, dzu = cj.y - zi;
+            uint32_t jid = 0xFFFFFFFFu;  // fetched lazily
+            for (int bzd = wd.bz0; bzd <= wd.bz1; ++bzd) {
+              const uint32_t bd = wd.base + (uint32_t)bzd * (uint32_t)wd.ny;
+              const uint32_t k1 = bin_start[bd + wd.by_span];
+              for (uint32_t k = bin_start[bd]; k < k1; ++k) {
+                const float2 ck = yz[k];
+                if (!(fabsf((yi - ck.x) - ty) <= wy && fabsf(zi - ck.y) <= wz)) continue;
+                const float dy = dyu + (ck.x - yi);
+                const float dz = dzu + (ck.y - zi);
+                const float d2 = dy * dy + dz * dz;
+                if (!(d2 <= max_d2)) continue;
+                bool better = bj < 0 || d2 < best;
+                if (!better && d2 == best) {
+                  if (jid == 0xFFFFFFFFu) jid = orig[j];
+                  const uint32_t kid = orig[k];
+                  better = jid < bjid || (jid == bjid && kid < bkid);
+                }
+                if (better) {
+                  if (jid == 0xFFFFFFFFu) jid = orig[j];
+                  best = d2; bj = (int32_t)j; bk = (int32_t)k; bjid = jid; bkid = orig[k];
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+    B.link_up[i] = bj;
+    B.link_dn[i] = bk;
+  }
+}
+
+// ================================================================== K3 cleanup + seeds
+// R3: one evolution step of the automaton — keep reciprocal links only.
+__global__ void __launch_bounds__(256) k_link_cleanup(TpcBuffers B) {
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  const uint32_t n = B.cnt->n_sorted;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const int32_t u = B.link_up[i], d = B.link_dn[i];
+    B.link_up2[i] = (u >= 0 && B.link_dn[u] == (int32_t)i) ? u : -1;
+    B.link_dn2[i] = (d >= 0 && B.link_up[d] == (int32_t)i) ? d : -1;
+  }
+}
+
+// R4 pass A: start hits (no down link, an up link, chain >= seed_min_len); per-block counts.
+__global__ void __launch_bounds__(1024) k_seed_flags(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  const uint32_t n = B.cnt->n_sorted;
+  const int min_len = B.K->P.seed_min_len;
+  const uint32_t n_blocks = (n + blockDim.x - 1) / blockDim.x;
+  for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+    const uint32_t i = blk * blockDim.x + threadIdx.x;
+    uint32_t len = 0;
+    if (i < n && B.link_dn2[i] < 0 && B.link_up2[i] >= 0) {
+      len = 1;
+      for (int32_t c = B.link_up2[i]; c >= 0; c = B.link_up2[c]) ++len;
+      if ((int)len < min_len) len = 0;
+    }
+    if (i < n) B.seed_len[i] = (uint8_t)len;
+    uint32_t tot;
+    block_excl_scan(len ? 1u : 0u, &tot, sm);
+    if (threadIdx.x == 0) B.scan_partials[blk] = tot;
+  }
+}
+
+// Exclusive scan of up to scan_blocks partial sums by one CTA; writes the grand total to
+// *total_out (clamped to cap, raising err_bit when it does not fit).
+__global__ void __launch_bounds__(1024) k_scan_partials(uint32_t* p, const uint32_t* n_items_ptr,
+                                                        uint32_t items_per_block, uint32_t* total_out, uint32_t cap,
+                                                        uint32_t* error, uint32_t err_bit) {
+  __shared__ uint32_t sm[33];
+  const uint32_t n = (*n_items_ptr + items_per_block - 1) / items_per_block;
+  uint32_t carry = 0;
+  for (uint32_t b0 = 0; b0 < n; b0 += blockDim.x) {
+    const uint32_t b = b0 + threadIdx.x;
+    const uint32_t v = b < n ? p[b] : 0u;
+    uint32_t tot;
+    const uint32_t pre = block_excl_scan(v, &tot, sm);
+    if (b < n) p[b] = carry + pre;
+    carry += tot;
+  }
+  if (threadIdx.x == 0) {
+    if (carry > cap) {
+      atomicOr(error, err_bit);
+      carry = 0;  // later stages see an empty list; the error is reported by tpc_get_tracks
+    }
+    *total_out = carry;
+  }
+}
+
+// R4 pass B: write the seed list in ascending sorted index (deterministic order).
+__global__ void __launch_bounds__(1024) k_seed_write(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const uint32_t n = B.cnt->n_sorted;
+  const uint32_t n_blocks = (n + blockDim.x - 1) / blockDim.x;
+  for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+    const uint32_t i = blk * blockDim.x + threadIdx.x;
+    const uint32_t f = (i < n && B.seed_len[i]) ? 1u : 0u;
+    uint32_t tot;
+    const uint32_t pre = block_excl_scan(f, &tot, sm);
+    if (f) B.seeds[B.scan_partials[blk] + pre] = i;
+  }
+}
+
+// ================================================================== K4 track follower
+// "the track following fits all seeds and propagates them through the TPC volume
+// using the Kalman filter picking up more clusters of the track".  DESIGN.md R5.
+// One seed per thread; the 5-parameter state and the 15 covariance entries live in
+// registers, fp32 (north star item 4).  Expression order follows DESIGN.md "Formulas" so
+// that the deterministic build (no FMA) is bit-comparable with the CPU oracle.
+struct KF {
+  float y, z, s, t, q;
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+};
+
+struct FollowConst {
+  float dx, cfield, max_sinphi, max_qpt, vy, vz;
+  float road_nsigma, road_min, road_max, chi2_max;
+  float ivs, ivt, ivq;
+  int max_gap, min_hits, R;
+};
+
+__device__ __forceinline__ void kf_init_cov(KF& k, const FollowConst& F) {
+  k.c00 = F.vy; k.c10 = 0.f; k.c11 = F.vz;
+  k.c20 = 0.f; k.c21 = 0.f; k.c22 = F.ivs;
+  k.c30 = 0.f; k.c31 = 0.f; k.c32 = 0.f; k.c33 = F.ivt;
+  k.c40 = 0.f; k.c41 = 0.f; k.c42 = 0.f; k.c43 = 0.f; k.c44 = F.ivq;
+}
+
+// Formulas P: exact circle in xy, z advances with tan(lambda) times the arc length.
+__device__ __forceinline__ bool kf_propagate(KF& k, float dx, const FollowConst& F) {
+  const float s = k.s, t = k.t;
+  const float cf = F.cfield;
+  const float kap = cf * k.q;
+  const float ex = sqrtf(1.f - s * s);
+  const float s1 = s + kap * dx;
+  if (!(fabsf(s1) <= F.max_sinphi)) return false;
+  const float ex1 = sqrtf(1.f - s1 * s1);
+  const float h = 1.f / (ex + ex1);
+  const float ss = s + s1;
+  const float tt = ss * h;
+  const float dy = dx * tt;
+  const float dl = dx * sqrtf(1.f + tt * tt);
+  const float a = (0.5f * kap) * dl;
+  const float a2 = a * a;
+  const float dS = dl * (1.f + a2 * ((1.f / 6.f) + a2 * (3.f / 40.f)));
+  const float hh = h * h;
+  const float g = s / ex + s1 / ex1;
+  const float f02 = dx * (2.f * h + (ss * hh) * g);
+  const float f04 = ((dx * dx) * cf) * (h + (ss * hh) * (s1 / ex1));
+  const float f12 = ((t * dx) * tt) / (ex * ex1);
+  const float f13 = dS;
+  const float sm = 0.5f * ss;
+  const float exm = 0.5f * (ex + ex1);
+  const float f14 = (((t * cf) * (0.5f * (dx * dx))) * sm) / ((exm * exm) * exm);
+  const float f24 = cf * dx;
+  k.y = k.y + dy;
+  k.z = k.z + t * dS;
+  k.s = s1;
+  const float c00 = k.c00, c10 = k.c10, c11 = k.c11, c20 = k.c20, c21 = k.c21, c22 = k.c22;
+  const float c30 = k.c30, c31 = k.c31, c32 = k.c32, c33 = k.c33;
+  const float c40 = k.c40, c41 = k.c41, c42 = k.c42, c43 = k.c43, c44 = k.c44;
+  const float m00 = (c00 + f02 * c20) + f04 * c40;
+  const float m02 = (c20 + f02 * c22) + f04 * c42;
+  const float m04 = (c40 + f02 * c42) + f04 * c44;
+  const float m10 = ((c10 + f12 * c20) + f13 * c30) + f14 * c40;
+  const float m11 = ((c11 + f12 * c21) + f13 * c31) + f14 * c41;
+  const float m12 = ((c21 + f12 * c22) + f13 * c32) + f14 * c42;
+  const float m13 = ((c31 + f12 * c32) + f13 * c33) + f14 * c43;
+  const float m14 = ((c41 + f12 * c42) + f13 * c43) + f14 * c44;
+  const float m20 = c20 + f24 * c40;
+  const float m21 = c21 + f24 * c41;
+  const float m22 = c22 + f24 * c42;
+  const float m23 = c32 + f24 * c43;
+  const float m24 = c42 + f24 * c44;
+  k.c00 = (m00 + f02 * m02) + f04 * m04;
+  k.c10 = (m10 + f02 * m12) + f04 * m14;
+  k.c11 = ((m11 + f12 * m12) + f13 * m13) + f14 * m14;
+  k.c20 = (m20 + f02 * m22) + f04 * m24;
+  k.c21 = ((m21 + f12 * m22) + f13 * m23) + f14 * m24;
+  k.c22 = m22 + f24 * m24;
+  k.c30 = (c30 + f02 * c32) + f04 * c43;
+  k.c31 = ((c31 + f12 * c32) + f13 * c33) + f14 * c43;
+  k.c32 = c32 + f24 * c43;
+  k.c40 = (c40 + f02 * c42) + f04 * c44;
+  k.c41 = ((c41 + f12 * c42) + f13 * c43) + f14 * c44;
+  k.c42 = c42 + f24 * c44;
+  return true;
+}
+
+struct Gain { float si00, si01, si11; };
+
+// Formulas U: innovation covariance inverse by the 2x2 determinant.
+__device__ __forceinline__ Gain kf_gain(const KF& k, const FollowConst& F) {
+  const float s00 = k.c00 + F.vy, s01 = k.c10, s11 = k.c11 + F.vz;
+  const float det = s00 * s11 - s01 * s01;
+  const float inv = 1.f / det;
+  Gain g;
+  g.si00 = s11 * inv;
+  g.si01 = -(s01 * inv);
+  g.si11 = s00 * inv;
+  return g;
+}
+__device__ __forceinline__ float kf_chi2(const KF& k, const Gain& g, float ym, float zm) {
+  const float r0 = ym - k.y, r1 = zm - k.z;
+  return ((r0 * r0) * g.si00 + (2.f * (r0 * r1)) * g.si01) + (r1 * r1) * g.si11;
+}
+// Kalman update; returns true if the leg must stop (|sin phi| left the range).
+__device__ __forceinline__ bool kf_update(KF& k, const Gain& g, float ym, float zm, const FollowConst& F) {
+  const float r0 = ym - k.y, r1 = zm - k.z;
+  const float a00 = k.c00, a01 = k.c10, a02 = k.c20, a03 = k.c30, a04 = k.c40;  // C_i0
+  const float a10 = k.c10, a11 = k.c11, a12 = k.c21, a13 = k.c31, a14 = k.c41;  // C_i1
+  const float k00 = a00 * g.si00 + a10 * g.si01, k10 = a00 * g.si01 + a10 * g.si11;
+  const float k01 = a01 * g.si00 + a11 * g.si01, k11 = a01 * g.si01 + a11 * g.si11;
+  const float k02 = a02 * g.si00 + a12 * g.si01, k12 = a02 * g.si01 + a12 * g.si11;
+  const float k03 = a03 * g.si00 + a13 * g.si01, k13 = a03 * g.si01 + a13 * g.si11;
+  const float k04 = a04 * g.si00 + a14 * g.si01, k14 = a04 * g.si01 + a14 * g.si11;
+  k.y = k.y + (k00 * r0 + k10 * r1);
+  k.z = k.z + (k01 * r0 + k11 * r1);
+  k.s = k.s + (k02 * r0 + k12 * r1);
+  k.t = k.t + (k03 * r0 + k13 * r1);
+  k.q = k.q + (k04 * r0 + k14 * r1);
+  k.c00 = k.c00 - (k00 * a00 + k10 * a10);
+  k.c10 = k.c10 - (k01 * a00 + k11 * a10);
+  k.c11 = k.c11 - (k01 * a01 + k11 * a11);
+  k.c20 = k.c20 - (k02 * a00 + k12 * a10);
+  k.c21 = k.c21 - (k02 * a01 + k12 * a11);
+  k.c22 = k.c22 - (k02 * a02 + k12 * a12);
+  k.c30 = k.c30 - (k03 * a00 + k13 * a10);
+  k.c31 = k.c31 - (k03 * a01 + k13 * a11);
+  k.c32 = k.c32 - (k03 * a02 + k13 * a12);
+  k.c33 = k.c33 - (k03 * a03 + k13 * a13);
+  k.c40 = k.c40 - (k04 * a00 + k14 * a10);
+  k.c41 = k.c41 - (k04 * a01 + k14 * a11);
+  k.c42 = k.c42 - (k04 * a02 + k14 * a12);
+  k.c43 = k.c43 - (k04 * a03 + k14 * a13);
+  k.c44 = k.c44 - (k04 * a04 + k14 * a14);
+  if (k.q > F.max_qpt) k.q = F.max_qpt;
+  if (k.q < -F.max_qpt) k.q = -F.max_qpt;
+  if (!(fabsf(k.s) <= F.max_sinphi)) {
+    k.s = (k.s < 0.f) ? -F.max_sinphi : F.max_sinphi;
+    return true;
+  }
+  return false;
+}
+
+__device__ __forceinline__ float clampf(float v, float lo, float hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+// R5.3: best cluster of row sr inside the road around the predicted state: minimum of
+// (chi2, original id).  Returns the sorted index or -1.
+__device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcConst* __restrict__ K, uint32_t sr,
+                                                const KF& k, const Gain& g, const FollowConst& F, float* chi2_out) {
+  const tpc_row_desc d = B.row_desc[sr];
+  if (d.count == 0) return -1;
+  const float ry = clampf(F.road_nsigma * sqrtf(k.c00 + F.vy), F.road_min, F.road_max);
+  const float rz = clampf(F.road_nsigma * sqrtf(k.c11 + F.vz), F.road_min, F.road_max);
+  const BinWindow w = make_window(d, K, k.y - ry, k.y + ry, k.z - rz, k.z + rz);
+  int32_t best = -1;
+  float best_chi2 = 0.f;
+  uint32_t best_id = 0;
+  for (int bz = w.bz0; bz <= w.bz1; ++bz) {
+    const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
+    const uint32_t c1 = B.bin_start[b + w.by_span];
+    for (uint32_t c = B.bin_start[b]; c < c1; ++c) {
+      const float2 m = B.yz[c];
+      if (!(fabsf(m.x - k.y) <= ry && fabsf(m.y - k.z) <= rz)) continue;
+      const float chi2 = kf_chi2(k, g, m.x, m.y);
+      bool better = best < 0 || chi2 < best_chi2;
+      if (!better && chi2 == best_chi2) better = B.orig_id[c] < best_id;
+      if (better) { best = (int32_t)c; best_chi2 = chi2; best_id = B.orig_id[c]; }
+    }
+  }
+  *chi2_out = best_chi2;
+  return best;
+}
+
+// Extrapolate from row r_from (exclusive) in direction dir, picking up clusters (R5.3/R5.6).
+// Rows visited without an accepted cluster get row_hit = -1.  On return *r_edge is the last
+// row with an accepted hit; SAVE(k) is applied after every accepted update.
+template <class SaveFn>
+__device__ __forceinline__ void extrapolate(const TpcBuffers& B, const TpcConst* __restrict__ K, const float* s_ylim,
+                                            const FollowConst& F, KF& k, uint32_t sr_base, int r_from, int dir,
+                                            int32_t* __restrict__ hit_col, uint32_t stride, float& chi2_acc, int& n_acc,
+                                            int& r_edge, SaveFn save) {
+  const float dx = dir > 0 ? F.dx : -F.dx;
+  int gap = 0;
+  for (int r = r_from + dir; r >= 0 && r < F.R; r += dir) {
+    if (!kf_propagate(k, dx, F)) break;
+    bool got = false;
+    if (fabsf(k.y) <= s_ylim[r]) {
+      const Gain g = kf_gain(k, F);
+      float chi2 = 0.f;
+      const int32_t c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2);
+      if (c >= 0 && chi2 <= F.chi2_max) {
+        const float2 m = B.yz[c];
+        const bool stop = kf_update(k, g, m.x, m.y, F);
+        hit_col[(size_t)r * stride] = c;
+        chi2_acc = chi2_acc + chi2;
+        n_acc = n_acc + 1;
+        r_edge = r;
+        save(k);
+        got = true;
+        gap = 0;
+        if (stop) break;
+      }
+    }
+    if (!got) {
+      hit_col[(size_t)r * stride] = -1;
+      ++gap;
+      if (gap > F.max_gap) break;
+    }
+  }
+}
+
+__global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
+  __shared__ float s_ylim[TPC_MAX_ROWS];
+  const TpcConst* __restrict__ K = B.K;
+  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_ylim[r] = K->ylim[r];
+  __syncthreads();
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  FollowConst F;
+  F.dx = K->dx_row; F.cfield = K->cfield; F.max_sinphi = K->P.max_sinphi; F.max_qpt = K->P.max_qpt;
+  F.vy = K->vy; F.vz = K->vz;
+  F.road_nsigma = K->P.road_nsigma; F.road_min = K->P.road_min; F.road_max = K->P.road_max;
+  F.chi2_max = K->P.chi2_max_hit;
+  F.ivs = K->P.init_var_sinphi; F.ivt = K->P.init_var_tanl; F.ivq = K->P.init_var_qpt;
+  F.max_gap = K->P.max_gap_follow; F.min_hits = K->P.min_hits_tracklet; F.R = K->n_rows;
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const uint32_t stride = B.max_seeds;
+  const int32_t* __restrict__ up2 = B.link_up2;
+
+  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
+    const uint32_t start = B.seeds[sd];
+    // (sector,row) of the start hit: last sr with clu_ofs <= start among non-empty rows
+    uint32_t lo = 0, hi = B.n_sr;
+    while (hi - lo > 1) {
+      const uint32_t mid = (lo + hi) >> 1;
+      if (B.row_desc[mid].clu_ofs <= start) lo = mid; else hi = mid;
+    }
+    // empty rows share clu_ofs with the next non-empty one: the search lands on the LAST
+    // row with clu_ofs <= start, which is the non-empty one
+    const uint32_t sr0 = lo;
+    const int r0 = (int)(sr0 % (uint32_t)F.R);
+    const uint32_t sr_base = sr0 - (uint32_t)r0;
+    int32_t* __restrict__ hit_col = B.row_hit + sd;
+
+    // R5.1 init from the first two chain clusters
+    const int32_t c1 = up2[start];
+    KF k;
+    const float2 m0 = B.yz[start];
+    {
+      const float2 m1 = B.yz[c1];
+      const float dy = m1.x - m0.x;
+      const float dl = sqrtf(F.dx * F.dx + dy * dy);
+      k.y = m0.x; k.z = m0.y;
+      k.s = dy / dl;
+      k.t = (m1.y - m0.y) / dl;
+      k.q = 0.f;
+      kf_init_cov(k, F);
+    }
+    hit_col[(size_t)r0 * stride] = (int32_t)start;
+    int r_out = r0;
+    float snap_s = k.s, snap_t = k.t, snap_q = k.q;
+    float chi2_up = 0.f;
+    int n_up = 1;
+    bool stopped = false;
+    // R5.2 chain fit (up), no chi2 cut
+    {
+      int r = r0;
+      for (int32_t c = c1; c >= 0; c = up2[c]) {
+        ++r;
+        if (!kf_propagate(k, F.dx, F)) { stopped = true; break; }
+        const Gain g = kf_gain(k, F);
+        const float2 m = B.yz[c];
+        const bool stop = kf_update(k, g, m.x, m.y, F);
+        hit_col[(size_t)r * stride] = c;
+        r_out = r;
+        ++n_up;
+        snap_s = k.s; snap_t = k.t; snap_q = k.q;
+        if (stop) { stopped = true; break; }
+      }
+    }
+    // R5.3 extrapolate up
+    if (!stopped)
+      extrapolate(B, K, s_ylim, F, k, sr_base, r_out, +1, hit_col, stride, chi2_up, n_up, r_out,
+                  [&](const KF& kk) { snap_s = kk.s; snap_t = kk.t; snap_q = kk.q; });
+    // R5.4 turn at the outermost accepted hit
+    {
+      const float2 mo = B.yz[hit_col[(size_t)r_out * stride]];
+      k.y = mo.x; k.z = mo.y;
+      k.s = snap_s; k.t = snap_t; k.q = snap_q;
+      kf_init_cov(k, F);
+    }
+    float chi2 = 0.f;
+    int nh = 1;
+    int r_in = r_out;
+    KF k_in = k;
+    stopped = false;
+    // R5.5 refit down through the recorded hits
+    for (int r = r_out - 1; r >= r0; --r) {
+      if (!kf_propagate(k, -F.dx, F)) { stopped = true; break; }
+      const int32_t c = hit_col[(size_t)r * stride];
+      if (c < 0) continue;
+      const Gain g = kf_gain(k, F);
+      const float2 m = B.yz[c];
+      const float c2 = kf_chi2(k, g, m.x, m.y);
+      const bool stop = kf_update(k, g, m.x, m.y, F);
+      chi2 = chi2 + c2;
+      ++nh;
+      r_in = r;
+      k_in = k;
+      if (stop) { stopped = true; break; }
+    }
+    // R5.6 extrapolate down (hits below r_in of a refit that ended early are outside
+    // [row_first,row_last] and thereby not part of the tracklet)
+    if (!stopped)
+      extrapolate(B, K, s_ylim, F, k, sr_base, r_in, -1, hit_col, stride, chi2, nh, r_in,
+                  [&](const KF& kk) { k_in = kk; });
+    // R5.7 output
+    tpc_tracklet t;
+    t.x = K->x[r_in];
+    t.p[0] = k_in.y; t.p[1] = k_in.z; t.p[2] = k_in.s; t.p[3] = k_in.t; t.p[4] = k_in.q;
+    t.c[0] = k_in.c00; t.c[1] = k_in.c10; t.c[2] = k_in.c11; t.c[3] = k_in.c20; t.c[4] = k_in.c21;
+    t.c[5] = k_in.c22; t.c[6] = k_in.c30; t.c[7] = k_in.c31; t.c[8] = k_in.c32; t.c[9] = k_in.c33;
+    t.c[10] = k_in.c40; t.c[11] = k_in.c41; t.c[12] = k_in.c42; t.c[13] = k_in.c43; t.c[14] = k_in.c44;
+    t.chi2 = chi2;
+    t.seed_sorted = start;
+    t.seed_id = B.orig_id[start];
+    const bool keep = nh >= F.min_hits;
+    t.n_hits = keep ? (int16_t)nh : (int16_t)0;
+    t.row_first = (uint8_t)r_in;
+    t.row_last = (uint8_t)r_out;
+    t.sector = (uint8_t)(sr_base / (uint32_t)F.R);
+    t.seed_len = B.seed_len[start];
+    t.pad_ = 0; t.pad2_[0] = 0; t.pad2_[1] = 0;
+    B.tracklets[sd] = t;
+    if (keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+  }
+}
+
+// ================================================================== K5 ambiguity solving
+// PAPER.md:27 ("identifies the best instance of each track, assigns all clusters to this
+// instance and removes the clones"; 10 % shared by default) with the Phase-I criterion of
+// PAPER.md:57 (chi2 priority; shared clusters counted from the outermost pad row).  R6.
+// K5a: weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
+__global__ void __launch_bounds__(128) k_sel_owner(TpcBuffers B) {
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const uint32_t stride = B.max_seeds;
+  const float w = B.K->P.sel_chi2_weight;
+  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
+    const int nh = B.tracklets[sd].n_hits;
+    unsigned long long key = 0ull;
+    if (nh > 0) {
+      const int ndf = 2 * nh - 5;
+      const float Q = (float)nh - w * (B.tracklets[sd].chi2 / (float)ndf);
+      key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - B.tracklets[sd].seed_id);
+      const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
+      for (int r = r0; r <= r1; ++r) {
+        const int32_t c = B.row_hit[(size_t)r * stride + sd];
+        if (c >= 0) atomicMax(&B.owner[c], key);
+      }
+    }
+    B.tl_key[sd] = key;
+  }
+}
+
+// The walk of R6.3: from the outermost row inward with the running shared budget; segments
+// split at holes > max_gap_select; EMIT=false counts, EMIT=true writes tracks and cluster ids.
+template <bool EMIT>
+__device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, uint32_t& n_seg_out, uint32_t& n_id_out,
+                                              uint32_t trk_ofs, uint32_t id_ofs) {
+  const tpc_params& P = B.K->P;
+  const uint32_t stride = B.max_seeds;
+  const unsigned long long key = B.tl_key[sd];
+  const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
+  const int min_hits = P.min_hits_track, max_gap = P.max_gap_select;
+  const long long permille = P.shared_permille;
+  int n_acc = 0, n_sh = 0, gap = 0, seg_last = -1, seg_first = -1;
+  uint32_t n_seg = 0, n_id = 0;
+  // decisions of the current segment, one bit per row (the ids are written in ascending row
+  // order only once the segment is known to survive)
+  uint32_t acc_bits[TPC_MAX_ROWS / 32], sh_bits[TPC_MAX_ROWS / 32];
+  if (EMIT) {
+#pragma unroll
+    for (int i = 0; i < TPC_MAX_ROWS / 32; ++i) { acc_bits[i] = 0u; sh_bits[i] = 0u; }
+  }
+  auto close = [&]() {
+    if (n_acc >= min_hits) {
+      if (EMIT) {
+        uint32_t o = id_ofs + n_id;
+        for (int r = seg_first; r <= seg_last; ++r) {
+          if (!((acc_bits[r >> 5] >> (r & 31)) & 1u)) continue;
+          B.cluster_ids[o] = B.orig_id[B.row_hit[(size_t)r * stride + sd]];
+          B.cluster_shared[o] = (uint8_t)((sh_bits[r >> 5] >> (r & 31)) & 1u);
+          ++o;
+        }
+        const tpc_tracklet& tl = B.tracklets[sd];
+        tpc_track t;
+        t.x = tl.x;
+#pragma unroll
+        for (int i = 0; i < 5; ++i) t.p[i] = tl.p[i];
+#pragma unroll
+        for (int i = 0; i < 15; ++i) t.c[i] = tl.c[i];
+        t.chi2 = tl.chi2;
+        t.cluster_ofs = id_ofs + n_id;
+        t.seed_id = tl.seed_id;
+        t.n_clusters = (uint16_t)n_acc;
+        t.n_shared = (uint16_t)n_sh;
+        t.sector = tl.sector;
+        t.row_first = (uint8_t)seg_first;
+        t.row_last = (uint8_t)seg_last;
+        t.flags = (seg_first == r0) ? 0 : TPC_TRACK_PARAMS_STALE;
+        t.n_hits_tracklet = (uint16_t)tl.n_hits;
+        t.segment = (uint8_t)n_seg;
+        t.pad_ = 0;
+        B.tracks[trk_ofs + n_seg] = t;
+      }
+      ++n_seg;
+      n_id += (uint32_t)n_acc;
+    }
+    if (EMIT && n_acc > 0) {
+      for (int w = seg_first >> 5; w <= seg_last >> 5; ++w) { acc_bits[w] = 0u; sh_bits[w] = 0u; }
+    }
+    n_acc = 0; n_sh = 0; seg_last = -1; seg_first = -1;
+  };
+  for (int r = r1; r >= r0; --r) {
+    int32_t c = B.row_hit[(size_t)r * stride + sd];
+    bool sh = false;
+    if (c >= 0 && B.owner[c] != key) {
+      if ((long long)(n_sh + 1) * 1000 <= permille * (long long)(n_acc + 1)) sh = true;
+      else c = -1;
+    }
+    if (c >= 0) {
+      if (n_acc == 0) seg_last = r;
+      seg_first = r;
+      if (EMIT) {
+        acc_bits[r >> 5] |= 1u << (r & 31);
+        if (sh) sh_bits[r >> 5] |= 1u << (r & 31);
+      }
+      ++n_acc;
+      if (sh) ++n_sh;
+      gap = 0;
+    } else {
+      ++gap;
+      if (gap > max_gap && n_acc > 0) close();
+    }
+  }
+  close();
+  n_seg_out = n_seg;
+  n_id_out = n_id;
+}
+
+// K5b: count tracks / cluster ids per tracklet + per-block partial sums (for the scans).
+__global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const uint32_t n_blocks = (n_seeds + blockDim.x - 1) / blockDim.x;
+  uint32_t* part_seg = B.scan_partials;
+  uint32_t* part_id = B.scan_partials + (B.scan_blocks + 1) / 2;
+  for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
+    const uint32_t sd = blk * blockDim.x + threadIdx.x;
+    uint32_t ns = 0, ni = 0;
+    if (sd < n_seeds && B.tracklets[sd].n_hits > 0) walk_tracklet<false>(B, sd, ns, ni, 0, 0);
+    uint32_t tot_s, tot_i;
+    const uint32_t ps = block_excl_scan(ns, &tot_s, sm);
+    const uint32_t pi = block_excl_scan(ni, &tot_i, sm);
+    if (sd < n_seeds) { B.seg_cnt[sd] = ps; B.id_cnt[sd] = pi; }  // block-local exclusive prefix
+    if (threadIdx.x == 0) { part_seg[blk] = tot_s; part_id[blk] = tot_i; }
+  }
+}
+
+// K5c: emit tracks + cluster lists at their scanned offsets (order = seed order).
+__global__ void __launch_bounds__(256) k_sel_emit(TpcBuffers B) {
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return;
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const uint32_t* part_seg = B.scan_partials;
+  const uint32_t* part_id = B.scan_partials + (B.scan_blocks + 1) / 2;
+  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
+    if (B.tracklets[sd].n_hits <= 0) continue;
+    const uint32_t blk = sd / blockDim.x;
+    uint32_t ns, ni;
+    walk_tracklet<true>(B, sd, ns, ni, part_seg[blk] + B.seg_cnt[sd], part_id[blk] + B.id_cnt[sd]);
+  }
+}
+
+__global__ void k_init(TpcBuffers B) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < B.n_sr) {
+    TpcRowStat s;
+    s.zmin_key = 0xFFFFFFFFu; s.zmax_key = 0u; s.count = 0u; s.pad_ = 0u;
+    B.row_stat[i] = s;
+  }
+  if (i == 0) {
+    TpcCounters c;
+    c.n_sorted = c.n_ignored = c.n_dropped = c.n_bad = 0;
+    c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
+    c.n_tracks = c.n_ids = c.error = c.pad_ = 0;
+    *B.cnt = c;
+  }
+}
+
+// ================================================================== host: enqueue the path
+#define TPC_LAUNCH_CHECK()                          \
+  do {                                              \
+    if (cudaPeekAtLastError() != cudaSuccess) return -1; \
+    ++launches;                                     \
+  } while (0)
+
+static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
+  uint64_t g = (n + block - 1) / block;
+  const uint64_t cap = (uint64_t)n_sm * ctas_per_sm;
+  if (g > cap) g = cap;
+  return g < 1 ? 1 : (int)g;
+}
+
+// Returns the number of kernels launched, or -1 on a launch error.
+int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, const TpcStageEvents& E, int n_sm) {
+  int launches = 0;
+  const bool timers = E.enabled;
+  k_init<<<(B.n_sr + 255) / 256, 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  if (timers) cudaEventRecord(E.ev[0], st);
+  // ---- K1 grid
+  k_row_stats<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_row_desc<<<1, 1024, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_bin_hist<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_bin_scan<<<grid_for((uint64_t)B.n_sr * 512, 512, n_sm, 4), 512, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_scatter<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+#if TPC_DET
+  k_bin_sort<<<grid_for(B.max_bins, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+#endif
+  if (timers) cudaEventRecord(E.ev[1], st);
+  // ---- K2 neighbour finder
+  k_neighbours<<<grid_for((uint64_t)(B.n / TPC_NF_TILE + B.n_sr) * TPC_NF_TILE, TPC_NF_TILE, n_sm, 8), TPC_NF_TILE, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  if (timers) cudaEventRecord(E.ev[2], st);
+  // ---- K3 cleanup + seeds
+  k_link_cleanup<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_seed_flags<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_sorted, 1024u, &B.cnt->n_seeds, B.max_seeds,
+                                      &B.cnt->error, TPC_DEVERR_SEEDS);
+  TPC_LAUNCH_CHECK();
+  k_seed_write<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  if (timers) cudaEventRecord(E.ev[3], st);
+  // ---- K4 follower
+  k_follow<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  if (timers) cudaEventRecord(E.ev[4], st);
+  // ---- K5 ambiguity solving
+  if (cudaMemsetAsync(B.owner, 0, (size_t)B.n * sizeof(unsigned long long), st) != cudaSuccess) return -1;
+  k_sel_owner<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  const uint32_t half = (B.scan_blocks + 1) / 2;
+  k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_seeds, 256u, &B.cnt->n_tracks, B.max_tracks,
+                                      &B.cnt->error, TPC_DEVERR_TRACKS);
+  TPC_LAUNCH_CHECK();
+  k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials + half, &B.cnt->n_seeds, 256u, &B.cnt->n_ids, B.max_ids,
+                                      &B.cnt->error, TPC_DEVERR_TRACKS);
+  TPC_LAUNCH_CHECK();
+  k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK();
+  if (timers) cudaEventRecord(E.ev[5], st);
+  (void)flags;
+  return launches;
+}
+
+}  // namespace TPC_NS

@@ -1,0 +1,220 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle — the tests proper.
+
+Deterministic mode: grid, links, seeds, tracklets, track cluster lists, counts and track
+parameters BIT-EXACT (north star; rule D1-D5 of DESIGN.md).  Fast mode: parameters within
+1e-3 relative, efficiency / clone rate within 0.2 % absolute.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import parity
+from paper_2601_20569_b200 import datagen as dg
+from paper_2601_20569_b200.metrics import track_quality
+
+pytestmark = pytest.mark.gpu
+
+DET = 1 | 2      # TPC_DETERMINISTIC | TPC_KEEP_INTERMEDIATES
+FAST = 2
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_20569_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def params_pair(B, **kw):
+    return B.tpc_default_params(**kw), oracle.default_params(**kw)
+
+
+def run_gpu(B, clusters, gparams=None, flags=DET, geom=None):
+    trk = B.SectorTracker(geom=geom, params=gparams)
+    try:
+        trk.track(trk.upload(clusters), flags=flags)
+        tracks, ids, shared, view = trk.tracks()
+        inter = trk.intermediates() if flags & 2 else None
+        return tracks, ids, shared, view, inter
+    finally:
+        trk.close()
+
+
+def assert_det_parity(B, clusters, **pkw):
+    gp, op = params_pair(B, **pkw)
+    tracks, ids, shared, view, gi = run_gpu(B, clusters, gp, DET)
+    o = oracle.run(clusters, params=op, n_threads=8)
+    n = len(clusters)
+    for name, bad in (("grid", parity.compare_grid(gi, o)),
+                      ("links", parity.compare_links(gi, o, n)),
+                      ("tracklets", parity.compare_tracklets(gi, o)),
+                      ("tracks", parity.compare_tracks(tracks, ids, shared, o))):
+        assert parity.all_zero(bad), (name, bad)
+    assert view.n_seeds == o.n_seeds and view.n_tracklets == o.n_tracklets
+    assert view.n_tracks == o.n_tracks and view.n_cluster_ids == o.n_cluster_ids
+    assert view.n_ignored == o.n_ignored and view.n_dropped == o.n_dropped
+    return o, tracks
+
+
+def test_det_parity_c1(B):
+    cl, _, _ = dg.generate(dg.preset("C1"))
+    o, _ = assert_det_parity(B, cl)
+    assert o.n_tracks > 50
+
+
+def test_det_parity_c2_reduced_all_sectors(B):
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=1500))
+    o, _ = assert_det_parity(B, cl)
+    assert o.n_tracks > 1500 and len(np.unique(o.tracks["sector"])) == 36
+
+
+def test_det_parity_c3_reduced_overlapping_events(B):
+    cl, _, _ = dg.generate(dg.preset("C3", tracks_per_event=500))
+    o, _ = assert_det_parity(B, cl)
+    assert o.n_tracks > 1500
+
+
+def test_det_parity_c4_reduced_long_frame_with_distortion(B):
+    """2.8 ms frame shape: z extent ~7500 cm (fp32 ulp 4.9e-4 cm), distortion on."""
+    cl, _, _ = dg.generate(dg.preset("C4", n_events=8, tracks_per_event=500))
+    assert cl["z"].max() - cl["z"].min() > 6000
+    o, _ = assert_det_parity(B, cl, grid_dz=8.0)
+    assert o.n_tracks > 2000
+
+
+def test_det_parity_c5_reduced_dense_shared(B):
+    cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+    o, tracks = assert_det_parity(B, cl, err_y=0.15, err_z=0.15, nf_max_d2=1.6, shared_permille=200)
+    assert o.cluster_shared.sum() > 0
+
+
+def test_det_parity_shuffled_input_and_ragged_sizes(B):
+    """Input in any order (not grouped by row), sizes that are not multiples of any tile."""
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=700, seed=31))
+    rng = np.random.default_rng(0)
+    cl = cl[rng.permutation(len(cl))][: len(cl) - 37]
+    assert_det_parity(B, cl)
+
+
+def test_det_parity_other_bin_sizes(B):
+    cl, _, _ = dg.generate(dg.preset("C1"))
+    ref = oracle.run(cl)
+    for dy, dz in ((4.0, 4.0), (1.0, 3.0)):
+        gp = B.tpc_default_params(grid_dy=dy, grid_dz=dz)
+        tracks, ids, shared, view, gi = run_gpu(B, cl, gp, DET)
+        # rule D3: results do not depend on the bin size -> compare with the 2x2 oracle
+        assert parity.all_zero(parity.compare_tracks(tracks, ids, shared, ref))
+        assert parity.all_zero(parity.compare_links(gi, ref, len(cl)))
+
+
+def test_edge_cases(B):
+    geom = B.default_geom()
+    # empty input
+    tracks, ids, shared, view, gi = run_gpu(B, np.zeros(0, dtype=B.CLUSTER_DTYPE))
+    assert view.n_tracks == 0 and view.n_seeds == 0 and gi["n_sorted"] == 0
+    # a single cluster; NaN / Inf / out-of-acceptance clusters are ignored / dropped
+    c = np.zeros(5, dtype=B.CLUSTER_DTYPE)
+    c["row"] = [10, 10, 10, 10, 11]
+    c["y"] = [0.0, 17.4 + 1.9, 17.4 + 2.6, np.nan, 0.0]
+    c["z"] = [1.0, 2.0, 3.0, 4.0, np.inf]
+    tracks, ids, shared, view, gi = run_gpu(B, c)
+    o = oracle.run(c)
+    assert (gi["n_sorted"], view.n_dropped, view.n_ignored) == (o.n_sorted, o.n_dropped, o.n_ignored) == (2, 1, 2)
+    assert view.n_tracks == 0
+    # a cluster outside the geometry is reported as TPC_E_ARG by tpc_get_tracks
+    bad = np.zeros(3, dtype=B.CLUSTER_DTYPE)
+    bad["sector"] = [0, 36, 0]
+    bad["row"] = [1, 1, 152]
+    trk = B.SectorTracker()
+    trk.track(trk.upload(bad), flags=DET)
+    rc, view = trk.counts(check=False)
+    assert rc == B.TPC_E_ARG
+    trk.close()
+
+
+def test_error_codes(B):
+    import torch
+    cl, _, _ = dg.generate(dg.preset("C1"))
+    trk = B.SectorTracker()
+    d = trk.upload(cl)
+    n = len(cl)
+    need = B.tpc_workspace_bytes(trk.ctx, n)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    assert B.tpc_sector_track(trk.ctx, d.data_ptr(), n, ws.data_ptr(), need - 1, st, 0) == B.TPC_E_WORKSPACE
+    assert B.tpc_sector_track(trk.ctx, d.data_ptr(), n, 0, need, st, 0) == B.TPC_E_ARG
+    assert B.tpc_sector_track(trk.ctx, d.data_ptr() + 4, n - 1, ws.data_ptr(), need, st, 0) == B.TPC_E_ARG
+    rc, _ = B.tpc_get_tracks(trk.ctx)
+    assert rc == B.TPC_E_STATE
+    trk.close()
+    # capacity overflow is reported, never silently truncated
+    trk = B.SectorTracker(params=B.tpc_default_params(max_seeds=64))
+    trk.track(trk.upload(cl), flags=0)
+    rc, view = trk.counts(check=False)
+    assert rc == B.TPC_E_OVERFLOW and view.n_tracks == 0
+    trk.close()
+    trk = B.SectorTracker(params=B.tpc_default_params(max_bins=1000))
+    trk.track(trk.upload(cl), flags=0)
+    rc, view = trk.counts(check=False)
+    assert rc == B.TPC_E_OVERFLOW
+    trk.close()
+
+
+def test_repeated_runs_same_context_identical(B):
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=800, seed=3))
+    trk = B.SectorTracker()
+    d = trk.upload(cl)
+    outs = []
+    for _ in range(3):
+        trk.track(d, flags=1)
+        tracks, ids, shared, _ = trk.tracks()
+        outs.append((tracks.tobytes(), ids.tobytes(), shared.tobytes()))
+    trk.close()
+    assert outs[0] == outs[1] == outs[2]
+
+
+def quality(tracks, ids, labels):
+    return track_quality(tracks["n_clusters"], tracks["cluster_ofs"], ids, tracks["sector"], labels)
+
+
+def test_fast_mode_tolerances(B):
+    """North star: fast mode parameters <= 1e-3 relative, efficiency and clone rate within
+    0.2 % absolute of the oracle."""
+    cl, lab, _ = dg.generate(dg.preset("C2", tracks_per_event=4000))
+    tracks, ids, shared, view, _ = run_gpu(B, cl, None, 0)
+    o = oracle.run(cl, n_threads=8, want=("tracks",))
+    st = parity.compare_tracks_fast(tracks, ids, shared, o)
+    assert st["n_paired"] >= 0.995 * st["n_oracle"], st
+    assert st["n_param_bad"] <= 0.002 * st["n_paired"], st
+    assert st["n_list_diff"] <= 0.01 * st["n_paired"], st
+    qg, qo = quality(tracks, ids, lab), quality(o.tracks, o.cluster_ids, lab)
+    assert abs(qg["efficiency"] - qo["efficiency"]) <= 0.002, (qg, qo)
+    assert abs(qg["clone_rate"] - qo["clone_rate"]) <= 0.002, (qg, qo)
+    assert qo["efficiency"] > 0.95
+
+
+def test_det_parity_full_c2_bench_configuration(B):
+    """BASELINE.json configs[1] at full size (~1.8 M clusters, 36 sectors)."""
+    cl, lab, _ = dg.generate(dg.preset("C2"))
+    gp, op = params_pair(B)
+    tracks, ids, shared, view, _ = run_gpu(B, cl, gp, 1)
+    o = oracle.run(cl, params=op, n_threads=8, want=("tracks",))
+    assert parity.all_zero(parity.compare_tracks(tracks, ids, shared, o))
+    q = quality(tracks, ids, lab)
+    assert q["efficiency"] >= 0.95 and q["clone_rate"] <= 0.10 and q["fake_rate"] <= 0.02
+
+
+def test_det_parity_full_c4_sampled_sectors(B):
+    """BASELINE.json configs[3], the headline workload, at a size the oracle can still check:
+    the whole 2.8 ms frame shape (140 events) at 1/4 of the track multiplicity is tracked in
+    the launch configuration bench.py times; two sampled sectors are compared bit by bit with
+    the oracle (sectors are independent, tests/test_oracle_path.py::test_sectors_are_independent)."""
+    cl, lab, _ = dg.generate(dg.preset("C4", tracks_per_event=3000))
+    gp = B.tpc_default_params(grid_dy=4.0, grid_dz=4.0)
+    tracks, ids, shared, view, _ = run_gpu(B, cl, gp, 1)
+    for s in (5, 23):
+        o = oracle.run(cl, params=oracle.default_params(grid_dy=4.0, grid_dz=4.0), sector_lo=s, sector_hi=s + 1,
+                       want=("tracks",))
+        bad = parity.compare_tracks(tracks, ids, shared, o, sector=s)
+        assert parity.all_zero(bad), (s, bad)
+        assert o.n_tracks > 1000
