@@ -26,7 +26,8 @@ def B():
 
 
 def params_pair(B, **kw):
-    return B.tpc_default_params(**kw), oracle.default_params(**kw)
+    okw = {k: v for k, v in kw.items() if k not in ("max_bins", "max_seeds")}   # capacities: library only
+    return B.tpc_default_params(**kw), oracle.default_params(**okw)
 
 
 def run_gpu(B, clusters, gparams=None, flags=DET, geom=None):
@@ -78,7 +79,7 @@ def test_det_parity_c4_reduced_long_frame_with_distortion(B):
     """2.8 ms frame shape: z extent ~7500 cm (fp32 ulp 4.9e-4 cm), distortion on."""
     cl, _, _ = dg.generate(dg.preset("C4", n_events=8, tracks_per_event=500))
     assert cl["z"].max() - cl["z"].min() > 6000
-    o, _ = assert_det_parity(B, cl, grid_dz=8.0)
+    o, _ = assert_det_parity(B, cl, grid_dz=8.0, max_bins=200_000_000)   # long frame, few clusters
     assert o.n_tracks > 2000
 
 
