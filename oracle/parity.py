@@ -68,7 +68,8 @@ def canonical_tracklets(gi):
     if len(tl):
         rows = np.arange(n_rows)[None, :]
         inside = (rows >= tl["row_first"][:, None]) & (rows <= tl["row_last"][:, None]) & (tl["n_hits"][:, None] > 0)
-        rh = np.where(inside & (rh >= 0), gi["orig_id"][np.maximum(rh, 0)].astype(np.int64), -1).astype(np.int32)
+        valid = inside & (rh >= 0)          # entries outside the row range are undefined (stale workspace)
+        rh = np.where(valid, gi["orig_id"][np.where(valid, rh, 0)].astype(np.int64), -1).astype(np.int32)
     order = np.lexsort((tl["seed_id"], tl["sector"]))
     return tl[order], rh[order]
 
@@ -128,30 +129,74 @@ def compare_tracks(g_tracks, g_ids, g_shared, o, sector=None):
     return bad
 
 
+def _overlap_pairs(tr, ids, otr, oids, un_g, un_o, n_clusters_total, frac=0.9):
+    """Pair leftover tracks by cluster overlap: a GPU track and an oracle track are the same
+    physical track if they share >= frac of the larger cluster list.  (Clone instances of one
+    track collect the same clusters from different seeds; which instance wins the ambiguity
+    solving is decided by a weight difference at rounding level, so in fast mode the winner's
+    seed id may differ from the oracle's while the track is the same.)"""
+    if len(un_g) == 0 or len(un_o) == 0:
+        return np.zeros(0, dtype=np.int64), np.zeros(0, dtype=np.int64)
+    og_ofs = np.cumsum(tr["n_clusters"].astype(np.int64)) - tr["n_clusters"].astype(np.int64)
+    oo_ofs = np.cumsum(otr["n_clusters"].astype(np.int64)) - otr["n_clusters"].astype(np.int64)
+    owner = np.full(n_clusters_total, -1, dtype=np.int64)      # cluster -> leftover oracle track
+    for j in un_o:
+        owner[oids[oo_ofs[j]:oo_ofs[j] + int(otr["n_clusters"][j])]] = j
+    pg, po, used = [], [], set()
+    for i in un_g:
+        n = int(tr["n_clusters"][i])
+        cand = owner[ids[og_ofs[i]:og_ofs[i] + n]]
+        cand = cand[cand >= 0]
+        if len(cand) == 0:
+            continue
+        vals, cnt = np.unique(cand, return_counts=True)
+        j = int(vals[np.argmax(cnt)])
+        if j in used or tr["sector"][i] != otr["sector"][j]:
+            continue
+        if cnt.max() >= frac * max(n, int(otr["n_clusters"][j])):
+            pg.append(i); po.append(j); used.add(j)
+    return np.asarray(pg, dtype=np.int64), np.asarray(po, dtype=np.int64)
+
+
 def compare_tracks_fast(g_tracks, g_ids, g_shared, o, rel=1e-3):
-    """Fast-mode comparison (north star): tracks paired by (sector, seed id, segment); on the
-    pairs, |dp_i| <= rel*max(|p_i|, scale_i), scales (1 cm, 1 cm, 0.1, 0.1, 0.1 c/GeV), z taken
-    relative to the oracle track's z.  Returns a dict of statistics."""
+    """Fast-mode comparison (north star): tracks paired by (sector, seed id, segment), falling
+    back to >= 90 % cluster overlap; on the key pairs |dp_i| <= rel*max(|p_i|, scale_i), scales
+    (1 cm, 1 cm, 0.1, 0.1, 0.1 c/GeV), z taken relative to the oracle track's z.  Returns a dict
+    of statistics (n_paired = key pairs + overlap pairs)."""
     def keyof(t):
         return (t["sector"].astype(np.int64) << 40) | (t["seed_id"].astype(np.int64) << 8) | t["segment"].astype(np.int64)
     tr, ids, sh = canonical_tracks(g_tracks, g_ids, g_shared)
     otr, oids, osh = canonical_tracks(o.tracks, o.cluster_ids, o.cluster_shared)
     kg, ko = keyof(tr), keyof(otr)
     common, ig, io = np.intersect1d(kg, ko, return_indices=True)
-    out = {"n_gpu": len(tr), "n_oracle": len(otr), "n_paired": len(common)}
-    if len(common) == 0:
-        out.update(n_param_bad=0, n_list_diff=0, max_rel=0.0)
-        return out
-    a, b = tr[ig], otr[io]
-    pa, pb = a["p"].astype(np.float64), b["p"].astype(np.float64)
+    out = {"n_gpu": len(tr), "n_oracle": len(otr), "n_paired_key": len(common)}
+    un_g = np.setdiff1d(np.arange(len(tr)), ig)
+    un_o = np.setdiff1d(np.arange(len(otr)), io)
+    pg, po = _overlap_pairs(tr, ids, otr, oids, un_g, un_o, o.n_clusters)
+    out["n_paired_overlap"] = len(pg)
+    out["n_paired"] = len(common) + len(pg)
     scale = np.array([1.0, 1.0, 0.1, 0.1, 0.1])
-    denom = np.maximum(np.abs(pb), scale)
-    denom[:, 1] = 1.0  # z: relative to the track's own z (offset-free), scale 1 cm
-    relerr = np.abs(pa - pb) / denom
-    same_list = (a["n_clusters"] == b["n_clusters"]) & (a["n_shared"] == b["n_shared"])
-    out["n_list_diff"] = int((~same_list).sum())
-    out["n_param_bad"] = int(((relerr > rel).any(axis=1) & same_list).sum())
-    out["max_rel"] = float(relerr[same_list].max()) if same_list.any() else 0.0
+
+    def relerr_of(a, b):
+        pa, pb = a["p"].astype(np.float64), b["p"].astype(np.float64)
+        denom = np.maximum(np.abs(pb), scale)
+        denom[:, 1] = 1.0  # z: relative to the track's own z (offset-free), scale 1 cm
+        return np.abs(pa - pb) / denom
+    out.update(n_param_bad=0, n_list_diff=0, max_rel=0.0, n_param_bad_overlap=0, max_rel_overlap=0.0)
+    if len(common):
+        a, b = tr[ig], otr[io]
+        relerr = relerr_of(a, b)
+        same_list = (a["n_clusters"] == b["n_clusters"]) & (a["n_shared"] == b["n_shared"])
+        out["n_list_diff"] = int((~same_list).sum())
+        out["n_param_bad"] = int(((relerr > rel).any(axis=1) & same_list).sum())
+        out["max_rel"] = float(relerr[same_list].max()) if same_list.any() else 0.0
+    if len(pg):
+        a, b = tr[pg], otr[po]
+        ok = (a["row_first"] == b["row_first"]) & (a["flags"] == 0) & (b["flags"] == 0)   # parameters at the same x
+        if ok.any():
+            relerr = relerr_of(a[ok], b[ok])
+            out["n_param_bad_overlap"] = int((relerr > rel).any(axis=1).sum())
+            out["max_rel_overlap"] = float(relerr.max())
     return out
 
 

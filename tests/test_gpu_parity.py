@@ -116,7 +116,8 @@ def test_edge_cases(B):
     # a single cluster; NaN / Inf / out-of-acceptance clusters are ignored / dropped
     c = np.zeros(5, dtype=B.CLUSTER_DTYPE)
     c["row"] = [10, 10, 10, 10, 11]
-    c["y"] = [0.0, 17.4 + 1.9, 17.4 + 2.6, np.nan, 0.0]
+    ymax10 = float(oracle.geom_tables()[1][10])            # 16.856 cm (closed form pinned in test_oracle_math)
+    c["y"] = [0.0, ymax10 + 1.9, ymax10 + 2.1, np.nan, 0.0]   # the acceptance is ymax + 2 cm (R1)
     c["z"] = [1.0, 2.0, 3.0, 4.0, np.inf]
     tracks, ids, shared, view, gi = run_gpu(B, c)
     o = oracle.run(c)
