@@ -1,0 +1,436 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the TPC sector-tracking hot path on B200 (BASELINE.json metric).
+
+    python bench.py --gpus 1 --steps K --warmup W            # the CUDA path (this repo)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands
+
+One "step" = one pass of the whole hot path (grid -> neighbour finder -> link cleanup ->
+seeds -> Kalman follower -> ambiguity solving) over one
+synthetic time frame.  Default workload: BASELINE.json configs[3] (C4), the 2.8 ms Pb-Pb
+time frame the metric is quoted on (~2.4e8 clusters, 3.8 GB, fits one B200).
+
+N > 1 (torchrun, one rank per GPU): time frames are independent units (the
+farm processes independent time frames), so every rank tracks its own frame (seed + rank),
+no data-path collective; scaling = weak; value = all ranks' clusters / max-over-ranks time.
+
+Prints ONE JSON line on rank 0 (contract in the task statement).
+states the algorithmic bytes / flops behind the "roofline" object.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "TPC clusters/sec tracked per B200 (2.8 ms Pb-Pb time frame)"
+UNIT = "clusters/s"
+
+# ---- tracker parameters per workload (grid_* are performance knobs)
+WORKLOAD_PARAMS = {
+    "C1": dict(),
+    "C2": dict(),
+    "C3": dict(),
+    "C4": dict(grid_dy=4.0, grid_dz=4.0),
+    "C5": dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6),
+}
+
+# ---- algorithmic work per kernel launch.
+# HBM kernels: bytes as a function of (N input clusters, Ns clusters in the grid, NB bins,
+# NSD seeds).  k_follow: fp32 flops from the work counters the kernel keeps.
+FLOPS_PROPAGATE, FLOPS_UPDATE, FLOPS_GAIN_ROAD, FLOPS_CAND = 163, 112, 16, 13
+
+
+def algorithmic_work(name: str, st: dict):
+    N, Ns, NB, NSD, R = st["n"], st["n_sorted"], st["n_bins"], st["n_seeds"], st["n_rows"]
+    hbm = {
+        "k_row_stats": 16 * N,
+        "k_zero_bins": 4 * NB,
+        "k_bin_hist": 16 * N + 4 * N + 8 * Ns,          # cluster in, slot out, counter RMW
+        "k_bin_scan": 8 * NB,
+        "k_scatter": 16 * N + 4 * N + 4 * Ns + 12 * Ns,  # cluster+slot in, bin_start in, yz+id out
+        "k_bin_sort": 4 * NB + 24 * Ns,
+        "k_neighbours": 8 * Ns + 8 * Ns + 4 * NB,        # yz in (ideal reuse), links out, bin index
+        "k_link_cleanup": 8 * Ns + 8 * Ns + 8 * Ns,      # links in, 2 gathers, links out
+        "k_seed_flags": 8 * Ns + 1 * Ns,
+        "k_seed_write": 1 * Ns + 4 * NSD,
+        "k_zero_owner": 8 * Ns,
+        "k_sel_owner": 112 * NSD + 12 * st["follow_updates"] // 2,
+        "k_sel_count": 12 * st["follow_updates"] // 2,
+        "k_sel_emit": 12 * st["follow_updates"] // 2,
+    }
+    if name in hbm:
+        return "hbm", float(hbm[name])
+    if name == "k_follow":
+        fl = (FLOPS_PROPAGATE * st["follow_steps"] + FLOPS_UPDATE * st["follow_updates"]
+              + FLOPS_GAIN_ROAD * st["follow_steps"] + FLOPS_CAND * st["follow_cands"])
+        return "alu", float(fl)
+    return "hbm", 0.0
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+# ------------------------------------------------------------------ clocks sampler
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, reasons, smax, pw = [], set(), None, []
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        try:
+            for ln in open(self.path):
+                f = [x.strip() for x in ln.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    sm.append(float(f[0]))
+                    smax = float(f[1])
+                    pw.append(float(f[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=smax, reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw) if pw else None)
+        return out
+
+
+# ------------------------------------------------------------------ workload
+def make_frame(workload: str, rank: int, events: int | None, tracks: int | None):
+    from paper_2601_20569_b200 import datagen as dg
+    base = dg.preset(workload)
+    kw = dict(seed=base.seed + 1000 * rank)
+    if events is not None:
+        kw["n_events"] = events
+    if tracks is not None:
+        kw["tracks_per_event"] = tracks
+    cfg = dg.preset(workload, **kw)
+    t0 = time.time()
+    clusters, labels, truth = dg.generate(cfg)
+    return cfg, clusters, labels, time.time() - t0
+
+
+def oracle_params(workload: str):
+    import oracle
+    return oracle.default_params(**WORKLOAD_PARAMS[workload])
+
+
+def oracle_sample(clusters: np.ndarray, budget_clusters: int):
+    """A bounded sample of the same workload for the CPU oracle: whole sectors (sectors are
+    independent units), starting at sector 0, until ~budget_clusters clusters."""
+    per_sector = np.bincount(clusters["sector"], minlength=36)
+    present = [s for s in range(len(per_sector)) if per_sector[s]]
+    lo = present[0]
+    hi, tot = lo, 0
+    for s in present:
+        if tot and tot + per_sector[s] > budget_clusters:
+            break
+        tot += int(per_sector[s])
+        hi = s + 1
+    return lo, hi, tot
+
+
+def time_oracle(clusters, workload, lo, hi, n_threads=1):
+    import oracle
+    t0 = time.perf_counter()
+    o = oracle.run(clusters, params=oracle_params(workload), sector_lo=lo, sector_hi=hi, n_threads=n_threads,
+                   want=("tracks",))
+    return time.perf_counter() - t0, o
+
+
+# ------------------------------------------------------------------ the reference arm
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle as it stands, on the box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    cfg, clusters, labels, gen_s = make_frame(args.workload, 0, args.events, args.tracks)
+    lo, hi, n_sample = oracle_sample(clusters, args.oracle_budget)
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(clusters, args.workload, lo, hi)
+    times = []
+    for _ in range(args.steps):
+        dt, o = time_oracle(clusters, args.workload, lo, hi)
+        times.append(dt)
+    total = sum(times)
+    value = n_sample * args.steps / total
+    sample = f"sectors [{lo},{hi}) of the {args.workload} frame: {n_sample} of {len(clusters)} clusters per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload} (BASELINE.json configs[{int(args.workload[1]) - 1}])",
+                   "n_clusters": int(len(clusters)), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ the CUDA arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2601_20569_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback; use --impl reference "
+                         "for the CPU oracle)")
+    B.load_library()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    cfg, clusters, labels, gen_s = make_frame(args.workload, rank, args.events, args.tracks)
+    n = len(clusters)
+    flags = B.TPC_STAGE_TIMERS | (B.TPC_DETERMINISTIC if args.mode == "det" else 0)
+    pkw = dict(WORKLOAD_PARAMS[args.workload])
+    if args.grid_dy:
+        pkw["grid_dy"] = args.grid_dy
+    if args.grid_dz:
+        pkw["grid_dz"] = args.grid_dz
+    trk = B.SectorTracker(params=B.tpc_default_params(**pkw), device=local_rank)
+    stream = torch.cuda.Stream(device=dev)
+
+    # pinned host copy of the frame (e2e leg) and the device-resident copy (kernel leg)
+    h_clusters = torch.empty(n * 16, dtype=torch.uint8).pin_memory()
+    h_clusters.numpy()[:] = clusters.view(np.uint8).reshape(-1)
+    d_clusters = torch.empty(n * 16, dtype=torch.uint8, device=dev)
+    d_clusters.copy_(h_clusters)
+    ws_bytes = trk.ensure_workspace(n)
+    torch.cuda.synchronize()
+
+    def step():
+        trk.track(d_clusters, flags=flags, stream=stream)
+        rc, v = trk.counts()          # tpc_get_tracks: syncs the stream, reads the counters
+        return v
+
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            v = step()
+    kernel_ms: dict = {}
+    order: list = []
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        for _ in range(args.steps):
+            v = step()
+            for name, ms in trk.kernel_ms():
+                if name not in kernel_ms:
+                    kernel_ms[name] = [0.0, 0]
+                    order.append(name)
+                kernel_ms[name][0] += ms
+                kernel_ms[name][1] += 1
+        ev1.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+    n_all = sum_over_ranks(float(n))
+    launches = trk.launch_count() * args.steps
+    stage_ms = trk.stage_ms()
+    value = n_all * args.steps / (ms_total * 1e-3)
+
+    # ---- end-to-end: HOST buffers through the C ABI, copies inside the timed region
+    cap_tracks = int(v.n_tracks * 1.05) + 1024
+    cap_ids = int(v.n_cluster_ids * 1.05) + 1024
+    h_tracks = torch.empty(cap_tracks * B.TRACK_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    h_ids = torch.empty(cap_ids * 4, dtype=torch.uint8).pin_memory()
+    h_shared = torch.empty(cap_ids, dtype=torch.uint8).pin_memory()
+    e2e_flags = flags & ~B.TPC_STAGE_TIMERS
+    with torch.cuda.stream(stream):
+        for _ in range(min(args.warmup, 2)):
+            ve = trk.track_host(h_clusters, d_clusters, h_tracks, h_ids, h_shared, flags=e2e_flags, stream=stream)
+    barrier()
+    with torch.cuda.stream(stream):
+        ev0.record(stream)
+        for _ in range(args.steps):
+            ve = trk.track_host(h_clusters, d_clusters, h_tracks, h_ids, h_shared, flags=e2e_flags, stream=stream)
+        ev1.record(stream)
+    barrier()
+    e2e_ms = max_over_ranks(ev0.elapsed_time(ev1))
+    h2d = n * 16
+    d2h = int(ve.n_tracks) * B.TRACK_DTYPE.itemsize + int(ve.n_cluster_ids) * 5 + 48
+    e2e = {"value": n_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+
+    if rank != 0:
+        trk.close()
+        return
+
+    # ---- roofline of the dominant kernel (live CUDA-event times over the timed region)
+    hbm_peak, peak_src, sm_max_mhz = load_peaks()
+    rc, iv = B.tpc_get_tracks(trk.ctx)
+    st = dict(n=n, n_sorted=n - int(v.n_ignored) - int(v.n_dropped), n_bins=int(v.n_bins), n_seeds=int(v.n_seeds),
+              n_rows=trk.geom.n_rows, follow_steps=int(v.n_follow_steps), follow_updates=int(v.n_follow_updates),
+              follow_cands=int(v.n_follow_candidates))
+    per_kernel = []
+    for name in order:
+        tot, cnt = kernel_ms[name]
+        per_step = tot / args.steps            # all launches of that name in one step
+        bound, work = algorithmic_work(name, st)
+        launches_per_step = cnt // args.steps
+        per_kernel.append(dict(name=name, ms_per_step=per_step, launches_per_step=launches_per_step, bound=bound,
+                               work_per_step=work * (1 if launches_per_step <= 1 else 1)))
+    ksum = sum(k["ms_per_step"] for k in per_kernel)
+    dom = max(per_kernel, key=lambda k: k["ms_per_step"])
+    alu_peak_tflops = 148 * 128 * sm_max_mhz * 1e6 * (1 if args.mode == "det" else 2) / 1e12
+    if dom["bound"] == "hbm":
+        achieved = dom["work_per_step"] / (dom["ms_per_step"] * 1e-3) / 1e9
+        roof = {"kernel": dom["name"], "bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                "frac": achieved / hbm_peak, "traffic": None, "peak_source": peak_src}
+    else:
+        achieved = dom["work_per_step"] / (dom["ms_per_step"] * 1e-3) / 1e12
+        roof = {"kernel": dom["name"], "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": None,
+                "peak_source": "148 SM x 128 fp32 lanes x sm_max_mhz x (2 if FMA) — DESIGN.md"}
+    roof["share_of_step"] = dom["ms_per_step"] / ksum if ksum else None
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # written from an ncu --set full capture
+    if os.path.exists(traffic_file):
+        try:
+            roof["traffic"] = json.load(open(traffic_file)).get(dom["name"])
+        except Exception:
+            pass
+    # north star: HBM fraction of the grid and neighbour stages
+    stages = {}
+    grid_names = ("k_row_stats", "k_row_desc", "k_zero_bins", "k_bin_hist", "k_bin_scan", "k_scatter", "k_bin_sort")
+    gb = sum(k["work_per_step"] for k in per_kernel if k["name"] in grid_names)
+    gms = sum(k["ms_per_step"] for k in per_kernel if k["name"] in grid_names)
+    nb = next((k for k in per_kernel if k["name"] == "k_neighbours"), None)
+    if gms:
+        stages["grid"] = {"ms": gms, "GB/s": gb / gms / 1e6, "frac_hbm": gb / gms / 1e6 / hbm_peak}
+    if nb and nb["ms_per_step"]:
+        stages["neighbours"] = {"ms": nb["ms_per_step"], "GB/s": nb["work_per_step"] / nb["ms_per_step"] / 1e6,
+                                "frac_hbm": nb["work_per_step"] / nb["ms_per_step"] / 1e6 / hbm_peak}
+
+    # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N=1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        lo, hi, n_sample = oracle_sample(clusters, args.oracle_budget)
+        dt, o = time_oracle(clusters, args.workload, lo, hi)
+        cpu = {"value": n_sample / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": f"sectors [{lo},{hi}) of the same {args.workload} frame: {n_sample} of {n} clusters, "
+                         "single thread"}
+
+    idx = int(args.workload[1]) - 1
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload} (BASELINE.json configs[{idx}])", "n_clusters_per_gpu": n,
+                   "n_events": cfg.n_events, "tracks_per_event": cfg.tracks_per_event, "mode": args.mode,
+                   "tracker_params": pkw, "parallelism": f"independent time frames x{world}",
+                   "l2": "inputs larger than L2 (frame %.2f GB + workspace %.1f GB)" % (n * 16 / 1e9, ws_bytes / 1e9),
+                   "n_seeds": int(v.n_seeds), "n_tracklets": int(v.n_tracklets), "n_tracks": int(v.n_tracks),
+                   "n_bins": int(v.n_bins), "generator_s": gen_s},
+        "time_frames_per_s": world * args.steps / (ms_total * 1e-3),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "roofline": roof, "stages_hbm": stages,
+        "stage_ms": {k: round(x, 4) for k, x in stage_ms.items()},
+        "kernels_ms_per_step": {k["name"]: round(k["ms_per_step"], 4) for k in per_kernel},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    trk.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--workload", default="C4", choices=tuple(WORKLOAD_PARAMS))
+    ap.add_argument("--mode", default="fast", choices=("fast", "det"))
+    ap.add_argument("--events", type=int, default=None, help="override the preset's n_events (smaller frame)")
+    ap.add_argument("--tracks", type=int, default=None, help="override tracks_per_event")
+    ap.add_argument("--grid-dy", type=float, default=0.0)
+    ap.add_argument("--grid-dz", type=float, default=0.0)
+    ap.add_argument("--oracle-budget", type=int, default=7_000_000,
+                    help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -136,6 +136,9 @@ typedef struct tpc_track_view {
   uint64_t n_seeds;
   uint64_t n_tracklets;
   uint64_t n_bins;
+  uint64_t n_follow_steps;          /* follower work: one-row propagations ...           */
+  uint64_t n_follow_updates;        /* ... Kalman updates ...                            */
+  uint64_t n_follow_candidates;     /* ... and chi2 evaluations of road candidates       */
 } tpc_track_view;
 
 /* One row of the search grid. */
@@ -233,6 +236,25 @@ int tpc_get_intermediates(tpc_ctx* ctx, tpc_debug_view* out);
  * out_ms[0..5] = grid, neighbours, cleanup+seeds, follower, selector, total. HOST pointer.
  * Syncs the stream. */
 int tpc_get_stage_ms(tpc_ctx* ctx, float* out_ms);
+
+/* Per-kernel device times of the last run (needs TPC_STAGE_TIMERS): fills names_out[i]
+ * (static strings owned by the library) and ms_out[i] for the first min(launched, max_kernels)
+ * kernels in launch order and returns that count (>= 0), or a negative tpc_error.  HOST
+ * pointers.  Syncs the stream.  Each time is the span between CUDA events recorded around
+ * the launch on the caller's stream. */
+int tpc_get_kernel_ms(tpc_ctx* ctx, int max_kernels, const char** names_out, float* ms_out);
+
+/* The whole path with HOST buffers (the end-to-end call): copies h_clusters (HOST, pinned
+ * for full speed) into d_staging (DEVICE, >= n_clusters*16 bytes, 16-byte aligned, caller
+ * owned), runs tpc_sector_track on it, synchronises, and copies the tracks, the cluster ids
+ * and the shared flags back into the caller's HOST buffers (each may be NULL = not wanted).
+ * *out (HOST) receives the counts; its d_* pointers stay valid as for tpc_get_tracks.
+ * Returns TPC_E_OVERFLOW if the results do not fit cap_tracks / cap_ids (nothing copied). */
+int tpc_sector_track_host(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t n_clusters,
+                          void* d_staging, void* d_workspace, size_t workspace_bytes,
+                          void* cuda_stream, uint32_t flags, tpc_track* h_tracks,
+                          uint64_t cap_tracks, uint32_t* h_cluster_ids, uint8_t* h_cluster_shared,
+                          uint64_t cap_ids, tpc_track_view* out);
 
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);

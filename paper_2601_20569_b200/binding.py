@@ -65,7 +65,9 @@ class TrackView(C.Structure):
     _fields_ = [("n_tracks", C.c_uint64), ("n_cluster_ids", C.c_uint64),
                 ("d_tracks", C.c_void_p), ("d_cluster_ids", C.c_void_p), ("d_cluster_shared", C.c_void_p),
                 ("n_ignored", C.c_uint64), ("n_dropped", C.c_uint64), ("n_seeds", C.c_uint64),
-                ("n_tracklets", C.c_uint64), ("n_bins", C.c_uint64)]
+                ("n_tracklets", C.c_uint64), ("n_bins", C.c_uint64),
+                ("n_follow_steps", C.c_uint64), ("n_follow_updates", C.c_uint64),
+                ("n_follow_candidates", C.c_uint64)]
 
 
 class DebugView(C.Structure):
@@ -78,7 +80,8 @@ class DebugView(C.Structure):
 
 
 EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
-           "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_last_launch_count",
+           "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
+           "tpc_sector_track_host", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -109,6 +112,11 @@ def load_library():
     L.tpc_get_intermediates.argtypes = [vp, C.POINTER(DebugView)]
     L.tpc_get_stage_ms.restype = C.c_int
     L.tpc_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.tpc_get_kernel_ms.restype = C.c_int
+    L.tpc_get_kernel_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    L.tpc_sector_track_host.restype = C.c_int
+    L.tpc_sector_track_host.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_size_t, vp, C.c_uint32, vp, C.c_uint64,
+                                        vp, vp, C.c_uint64, C.POINTER(TrackView)]
     L.tpc_last_launch_count.restype = C.c_int
     L.tpc_last_launch_count.argtypes = [vp]
     L.tpc_destroy.restype = None
@@ -179,6 +187,25 @@ def tpc_get_stage_ms(ctx: int):
     out = (C.c_float * TPC_N_STAGES)()
     rc = load_library().tpc_get_stage_ms(ctx, out)
     return rc, [float(x) for x in out]
+
+
+def tpc_get_kernel_ms(ctx: int, max_kernels: int = 32):
+    names = (C.c_char_p * max_kernels)()
+    ms = (C.c_float * max_kernels)()
+    rc = load_library().tpc_get_kernel_ms(ctx, max_kernels, names, ms)
+    if rc < 0:
+        return rc, []
+    return rc, [(names[i].decode(), float(ms[i])) for i in range(rc)]
+
+
+def tpc_sector_track_host(ctx: int, h_clusters: int, n_clusters: int, d_staging: int, d_workspace: int,
+                          workspace_bytes: int, cuda_stream: int, flags: int, h_tracks: int, cap_tracks: int,
+                          h_cluster_ids: int, h_cluster_shared: int, cap_ids: int):
+    v = TrackView()
+    rc = load_library().tpc_sector_track_host(ctx, h_clusters, n_clusters, d_staging, d_workspace, workspace_bytes,
+                                              cuda_stream, flags, h_tracks, cap_tracks, h_cluster_ids,
+                                              h_cluster_shared, cap_ids, C.byref(v))
+    return rc, v
 
 
 def tpc_last_launch_count(ctx: int) -> int:
@@ -280,6 +307,28 @@ class SectorTracker:
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_get_stage_ms")
         return dict(zip(STAGE_NAMES, ms))
+
+    def kernel_ms(self) -> list:
+        rc, out = tpc_get_kernel_ms(self.ctx)
+        if rc < 0:
+            raise TpcError(rc, "tpc_get_kernel_ms")
+        return out
+
+    def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
+        """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the
+        clusters in, tracks, copies tracks / cluster ids / shared flags out.  Returns the view."""
+        n = h_clusters.numel() // 16
+        need = self.ensure_workspace(n)
+        ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc, v = tpc_sector_track_host(self.ctx, h_clusters.data_ptr(), n, d_staging.data_ptr(), ws_ptr, need,
+                                      st.cuda_stream, flags, h_tracks.data_ptr(),
+                                      h_tracks.numel() // TRACK_DTYPE.itemsize, h_ids.data_ptr(),
+                                      h_shared.data_ptr(), min(h_ids.numel() // 4, h_shared.numel()))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_sector_track_host", tpc_last_cuda_error(self.ctx))
+        self.n = n
+        return v
 
     def launch_count(self) -> int:
         return tpc_last_launch_count(self.ctx)

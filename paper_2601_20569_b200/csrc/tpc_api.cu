@@ -188,9 +188,17 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
     return TPC_E_CUDA;
   }
   c->events.enabled = false;
+  c->events.n_kernels = 0;
+  for (int i = 0; i < TPC_N_STAGES; ++i) c->events.ev[i] = nullptr;
+  for (int i = 0; i <= TPC_MAX_KERNELS; ++i) c->events.kev[i] = nullptr;
   for (int i = 0; i < TPC_N_STAGES; ++i) {
-    c->events.ev[i] = nullptr;
     if ((e = cudaEventCreate(&c->events.ev[i])) != cudaSuccess) {
+      tpc_destroy(c);
+      return TPC_E_CUDA;
+    }
+  }
+  for (int i = 0; i <= TPC_MAX_KERNELS; ++i) {
+    if ((e = cudaEventCreate(&c->events.kev[i])) != cudaSuccess) {
       tpc_destroy(c);
       return TPC_E_CUDA;
     }
@@ -269,6 +277,9 @@ int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out) {
   out->n_seeds = c.n_seeds;
   out->n_tracklets = c.n_tracklets;
   out->n_bins = c.n_bins;
+  out->n_follow_steps = c.follow_steps;
+  out->n_follow_updates = c.follow_updates;
+  out->n_follow_candidates = c.follow_cands;
   return rc;
 }
 
@@ -314,12 +325,62 @@ int tpc_get_stage_ms(tpc_ctx* ctx, float* out_ms) {
   return TPC_OK;
 }
 
+int tpc_get_kernel_ms(tpc_ctx* ctx, int max_kernels, const char** names_out, float* ms_out) {
+  if (!names_out || !ms_out || max_kernels < 0) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!(ctx->flags & TPC_STAGE_TIMERS)) return TPC_E_STATE;
+  const int n = ctx->events.n_kernels < max_kernels ? ctx->events.n_kernels : max_kernels;
+  for (int i = 0; i < n; ++i) {
+    names_out[i] = ctx->events.kname[i];
+    cudaError_t e = cudaEventElapsedTime(&ms_out[i], ctx->events.kev[i], ctx->events.kev[i + 1]);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaEventElapsedTime");
+  }
+  return n;
+}
+
+int tpc_sector_track_host(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t n_clusters, void* d_staging,
+                          void* d_workspace, size_t workspace_bytes, void* cuda_stream, uint32_t flags,
+                          tpc_track* h_tracks, uint64_t cap_tracks, uint32_t* h_cluster_ids,
+                          uint8_t* h_cluster_shared, uint64_t cap_ids, tpc_track_view* out) {
+  if (!ctx || !out || (!h_clusters && n_clusters) || (!d_staging && n_clusters)) return TPC_E_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t e;
+  if (n_clusters) {
+    e = cudaMemcpyAsync(d_staging, h_clusters, n_clusters * sizeof(tpc_cluster), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(clusters)");
+  }
+  int rc = tpc_sector_track(ctx, (const tpc_cluster*)d_staging, n_clusters, d_workspace, workspace_bytes,
+                            cuda_stream, flags);
+  if (rc != TPC_OK) return rc;
+  rc = tpc_get_tracks(ctx, out);  // syncs; counts are needed to size the copies back
+  if (rc != TPC_OK) return rc;
+  if (out->n_tracks > cap_tracks || out->n_cluster_ids > cap_ids) return TPC_E_OVERFLOW;
+  if (h_tracks && out->n_tracks) {
+    e = cudaMemcpyAsync(h_tracks, out->d_tracks, out->n_tracks * sizeof(tpc_track), cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(tracks)");
+  }
+  if (h_cluster_ids && out->n_cluster_ids) {
+    e = cudaMemcpyAsync(h_cluster_ids, out->d_cluster_ids, out->n_cluster_ids * 4, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(cluster ids)");
+  }
+  if (h_cluster_shared && out->n_cluster_ids) {
+    e = cudaMemcpyAsync(h_cluster_shared, out->d_cluster_shared, out->n_cluster_ids, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(shared flags)");
+  }
+  e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize");
+  return TPC_OK;
+}
+
 int tpc_last_launch_count(const tpc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 void tpc_destroy(tpc_ctx* c) {
   if (!c) return;
   for (int i = 0; i < TPC_N_STAGES; ++i)
     if (c->events.ev[i]) cudaEventDestroy(c->events.ev[i]);
+  for (int i = 0; i <= TPC_MAX_KERNELS; ++i)
+    if (c->events.kev[i]) cudaEventDestroy(c->events.kev[i]);
   if (c->d_const) cudaFree(c->d_const);
   if (c->d_cnt) cudaFree(c->d_cnt);
   if (c->d_row_stat) cudaFree(c->d_row_stat);

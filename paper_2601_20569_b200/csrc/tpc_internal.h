@@ -37,6 +37,9 @@ struct TpcCounters {
   uint32_t n_sorted, n_ignored, n_dropped, n_bad;
   uint32_t n_bins, n_tiles, n_seeds, n_tracklets;
   uint32_t n_tracks, n_ids, error, pad_;
+  // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
+  // chi2 evaluations of road candidates
+  unsigned long long follow_steps, follow_updates, follow_cands;
 };
 
 // per (sector,row) statistics of pass 1
@@ -82,16 +85,20 @@ struct TpcBuffers {
   uint8_t* cluster_shared;// [max_ids]
 };
 
+#define TPC_MAX_KERNELS 32
 struct TpcStageEvents {
   cudaEvent_t ev[TPC_N_STAGES];  // boundaries: start, after grid, nf, seeds, follower, selector
+  cudaEvent_t kev[TPC_MAX_KERNELS + 1];  // kev[0] before the first kernel, kev[i+1] after kernel i
+  const char* kname[TPC_MAX_KERNELS];
+  int n_kernels;
   bool enabled;
 };
 
 namespace tpc_det {
-int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, const TpcStageEvents& E, int n_sm);
+int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
-int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, const TpcStageEvents& E, int n_sm);
+int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 
 #endif

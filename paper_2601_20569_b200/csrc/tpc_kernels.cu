@@ -642,7 +642,8 @@ __device__ __forceinline__ float clampf(float v, float lo, float hi) { return v 
 // R5.3: best cluster of row sr inside the road around the predicted state: minimum of
 // (chi2, original id).  Returns the sorted index or -1.
 __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcConst* __restrict__ K, uint32_t sr,
-                                                const KF& k, const Gain& g, const FollowConst& F, float* chi2_out) {
+                                                const KF& k, const Gain& g, const FollowConst& F, float* chi2_out,
+                                                uint32_t& n_cand) {
   const tpc_row_desc d = B.row_desc[sr];
   if (d.count == 0) return -1;
   const float ry = clampf(F.road_nsigma * sqrtf(k.c00 + F.vy), F.road_min, F.road_max);
@@ -658,6 +659,7 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
       const float2 m = B.yz[c];
       if (!(fabsf(m.x - k.y) <= ry && fabsf(m.y - k.z) <= rz)) continue;
       const float chi2 = kf_chi2(k, g, m.x, m.y);
+      ++n_cand;
       bool better = best < 0 || chi2 < best_chi2;
       if (!better && chi2 == best_chi2) better = B.orig_id[c] < best_id;
       if (better) { best = (int32_t)c; best_chi2 = chi2; best_id = B.orig_id[c]; }
@@ -674,16 +676,17 @@ template <class SaveFn>
 __device__ __forceinline__ void extrapolate(const TpcBuffers& B, const TpcConst* __restrict__ K, const float* s_ylim,
                                             const FollowConst& F, KF& k, uint32_t sr_base, int r_from, int dir,
                                             int32_t* __restrict__ hit_col, uint32_t stride, float& chi2_acc, int& n_acc,
-                                            int& r_edge, SaveFn save) {
+                                            int& r_edge, uint32_t& n_step, uint32_t& n_cand, SaveFn save) {
   const float dx = dir > 0 ? F.dx : -F.dx;
   int gap = 0;
   for (int r = r_from + dir; r >= 0 && r < F.R; r += dir) {
+    ++n_step;
     if (!kf_propagate(k, dx, F)) break;
     bool got = false;
     if (fabsf(k.y) <= s_ylim[r]) {
       const Gain g = kf_gain(k, F);
       float chi2 = 0.f;
-      const int32_t c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2);
+      const int32_t c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2, n_cand);
       if (c >= 0 && chi2 <= F.chi2_max) {
         const float2 m = B.yz[c];
         const bool stop = kf_update(k, g, m.x, m.y, F);
@@ -721,6 +724,7 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
   const uint32_t n_seeds = B.cnt->n_seeds;
   const uint32_t stride = B.max_seeds;
   const int32_t* __restrict__ up2 = B.link_up2;
+  uint32_t w_step = 0, w_cand = 0, w_upd = 0;  // work counters (diagnostics only)
 
   for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
     const uint32_t start = B.seeds[sd];
@@ -762,6 +766,7 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
       int r = r0;
       for (int32_t c = c1; c >= 0; c = up2[c]) {
         ++r;
+        ++w_step;
         if (!kf_propagate(k, F.dx, F)) { stopped = true; break; }
         const Gain g = kf_gain(k, F);
         const float2 m = B.yz[c];
@@ -775,7 +780,7 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
     }
     // R5.3 extrapolate up
     if (!stopped)
-      extrapolate(B, K, s_ylim, F, k, sr_base, r_out, +1, hit_col, stride, chi2_up, n_up, r_out,
+      extrapolate(B, K, s_ylim, F, k, sr_base, r_out, +1, hit_col, stride, chi2_up, n_up, r_out, w_step, w_cand,
                   [&](const KF& kk) { snap_s = kk.s; snap_t = kk.t; snap_q = kk.q; });
     // R5.4 turn at the outermost accepted hit
     {
@@ -791,6 +796,7 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
     stopped = false;
     // R5.5 refit down through the recorded hits
     for (int r = r_out - 1; r >= r0; --r) {
+      ++w_step;
       if (!kf_propagate(k, -F.dx, F)) { stopped = true; break; }
       const int32_t c = hit_col[(size_t)r * stride];
       if (c < 0) continue;
@@ -807,7 +813,7 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
     // R5.6 extrapolate down (hits below r_in of a refit that ended early are outside
     // [row_first,row_last] and thereby not part of the tracklet)
     if (!stopped)
-      extrapolate(B, K, s_ylim, F, k, sr_base, r_in, -1, hit_col, stride, chi2, nh, r_in,
+      extrapolate(B, K, s_ylim, F, k, sr_base, r_in, -1, hit_col, stride, chi2, nh, r_in, w_step, w_cand,
                   [&](const KF& kk) { k_in = kk; });
     // R5.7 output
     tpc_tracklet t;
@@ -828,6 +834,15 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
     t.pad_ = 0; t.pad2_[0] = 0; t.pad2_[1] = 0;
     B.tracklets[sd] = t;
     if (keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+    w_upd += (uint32_t)(n_up - 1) + (uint32_t)(nh - 1);
+  }
+  w_step = __reduce_add_sync(0xffffffffu, w_step);
+  w_cand = __reduce_add_sync(0xffffffffu, w_cand);
+  w_upd = __reduce_add_sync(0xffffffffu, w_upd);
+  if ((threadIdx.x & 31) == 0 && w_step) {
+    atomicAdd(&B.cnt->follow_steps, (unsigned long long)w_step);
+    atomicAdd(&B.cnt->follow_updates, (unsigned long long)w_upd);
+    atomicAdd(&B.cnt->follow_cands, (unsigned long long)w_cand);
   }
 }
 
@@ -835,6 +850,14 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
 // PAPER.md:27 ("identifies the best instance of each track, assigns all clusters to this
 // instance and removes the clones"; 10 % shared by default) with the Phase-I criterion of
 // PAPER.md:57 (chi2 priority; shared clusters counted from the outermost pad row).  R6.
+__global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
+  const uint32_t n = B.cnt->n_sorted;  // owner[] is indexed by sorted position
+  uint4* p4 = reinterpret_cast<uint4*>(B.owner);
+  const uint32_t n2 = (n + 1) / 2;      // the buffer is padded to 256 bytes
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += gridDim.x * blockDim.x)
+    p4[i] = make_uint4(0, 0, 0, 0);
+}
+
 // K5a: weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
 __global__ void __launch_bounds__(128) k_sel_owner(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
@@ -990,15 +1013,20 @@ __global__ void k_init(TpcBuffers B) {
     c.n_sorted = c.n_ignored = c.n_dropped = c.n_bad = 0;
     c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
     c.n_tracks = c.n_ids = c.error = c.pad_ = 0;
+    c.follow_steps = c.follow_updates = c.follow_cands = 0ull;
     *B.cnt = c;
   }
 }
 
 // ================================================================== host: enqueue the path
-#define TPC_LAUNCH_CHECK()                          \
-  do {                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return -1; \
-    ++launches;                                     \
+#define TPC_LAUNCH_CHECK(name)                                      \
+  do {                                                              \
+    if (cudaPeekAtLastError() != cudaSuccess) return -1;            \
+    if (timers && launches < TPC_MAX_KERNELS) {                     \
+      E.kname[launches] = name;                                     \
+      cudaEventRecord(E.kev[launches + 1], st);                     \
+    }                                                               \
+    ++launches;                                                     \
   } while (0)
 
 static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
@@ -1009,66 +1037,69 @@ static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.
-int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, const TpcStageEvents& E, int n_sm) {
+int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageEvents& E, int n_sm) {
   int launches = 0;
   const bool timers = E.enabled;
+  if (timers) cudaEventRecord(E.kev[0], st);
   k_init<<<(B.n_sr + 255) / 256, 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_init");
   if (timers) cudaEventRecord(E.ev[0], st);
   // ---- K1 grid
   k_row_stats<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_row_stats");
   k_row_desc<<<1, 1024, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_row_desc");
   k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_zero_bins");
   k_bin_hist<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_bin_hist");
   k_bin_scan<<<grid_for((uint64_t)B.n_sr * 512, 512, n_sm, 4), 512, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_bin_scan");
   k_scatter<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_scatter");
 #if TPC_DET
   k_bin_sort<<<grid_for(B.max_bins, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_bin_sort");
 #endif
   if (timers) cudaEventRecord(E.ev[1], st);
   // ---- K2 neighbour finder
   k_neighbours<<<grid_for((uint64_t)(B.n / TPC_NF_TILE + B.n_sr) * TPC_NF_TILE, TPC_NF_TILE, n_sm, 8), TPC_NF_TILE, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_neighbours");
   if (timers) cudaEventRecord(E.ev[2], st);
   // ---- K3 cleanup + seeds
   k_link_cleanup<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_link_cleanup");
   k_seed_flags<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_seed_flags");
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_sorted, 1024u, &B.cnt->n_seeds, B.max_seeds,
                                       &B.cnt->error, TPC_DEVERR_SEEDS);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_scan_partials");
   k_seed_write<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
   k_follow<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_follow");
   if (timers) cudaEventRecord(E.ev[4], st);
   // ---- K5 ambiguity solving
-  if (cudaMemsetAsync(B.owner, 0, (size_t)B.n * sizeof(unsigned long long), st) != cudaSuccess) return -1;
+  k_zero_owner<<<grid_for(B.n / 2 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_zero_owner");
   k_sel_owner<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_sel_owner");
   k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_sel_count");
   const uint32_t half = (B.scan_blocks + 1) / 2;
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_seeds, 256u, &B.cnt->n_tracks, B.max_tracks,
                                       &B.cnt->error, TPC_DEVERR_TRACKS);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_scan_partials");
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials + half, &B.cnt->n_seeds, 256u, &B.cnt->n_ids, B.max_ids,
                                       &B.cnt->error, TPC_DEVERR_TRACKS);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_scan_partials");
   k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
-  TPC_LAUNCH_CHECK();
+  TPC_LAUNCH_CHECK("k_sel_emit");
   if (timers) cudaEventRecord(E.ev[5], st);
   (void)flags;
+  E.n_kernels = launches < TPC_MAX_KERNELS ? launches : TPC_MAX_KERNELS;
   return launches;
 }
 
