@@ -256,6 +256,8 @@ def run_ours(args, rank, world, local_rank):
         pkw["grid_dy"] = args.grid_dy
     if args.grid_dz:
         pkw["grid_dz"] = args.grid_dz
+    if args.max_bins:
+        pkw["max_bins"] = args.max_bins
     trk = B.SectorTracker(params=B.tpc_default_params(**pkw), device=local_rank)
     stream = torch.cuda.Stream(device=dev)
 
@@ -393,7 +395,9 @@ def run_ours(args, rank, world, local_rank):
                    "tracker_params": pkw, "parallelism": f"independent time frames x{world}",
                    "l2": "inputs larger than L2 (frame %.2f GB + workspace %.1f GB)" % (n * 16 / 1e9, ws_bytes / 1e9),
                    "n_seeds": int(v.n_seeds), "n_tracklets": int(v.n_tracklets), "n_tracks": int(v.n_tracks),
-                   "n_bins": int(v.n_bins), "generator_s": gen_s},
+                   "n_bins": int(v.n_bins), "follow_steps": st["follow_steps"],
+                   "follow_updates": st["follow_updates"], "follow_cands": st["follow_cands"],
+                   "generator_s": gen_s},
         "time_frames_per_s": world * args.steps / (ms_total * 1e-3),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "roofline": roof, "stages_hbm": stages,
@@ -419,6 +423,7 @@ def main():
     ap.add_argument("--tracks", type=int, default=None, help="override tracks_per_event")
     ap.add_argument("--grid-dy", type=float, default=0.0)
     ap.add_argument("--grid-dz", type=float, default=0.0)
+    ap.add_argument("--max-bins", type=int, default=0, help="bin-index capacity (0 = library default)")
     ap.add_argument("--oracle-budget", type=int, default=7_000_000,
                     help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -176,7 +176,7 @@ typedef struct tpc_debug_view {
   uint64_t n_rows_total;         /* n_sectors*n_rows                                   */
   uint64_t n_bins;
   uint64_t n_seeds;
-  uint64_t tracklet_stride;      /* row_hit is [row][tracklet_stride]                  */
+  uint64_t tracklet_stride;      /* row_hit is [tracklet][tracklet_stride], = n_rows   */
   const tpc_row_desc* d_row_desc;/* [n_rows_total]                                     */
   const uint32_t* d_bin_start;   /* [n_bins + 1] global sorted positions               */
   const float* d_yz_sorted;      /* [n_sorted][2]                                      */
@@ -187,7 +187,7 @@ typedef struct tpc_debug_view {
   const int32_t* d_link_dn2;
   const uint32_t* d_seeds;       /* [n_seeds] sorted index of each start cluster       */
   const tpc_tracklet* d_tracklets; /* [n_seeds]                                        */
-  const int32_t* d_row_hit;      /* [n_rows][tracklet_stride] sorted index or -1; only
+  const int32_t* d_row_hit;      /* [n_seeds][tracklet_stride] sorted index or -1; only
                                     rows row_first..row_last of a tracklet are defined */
 } tpc_debug_view;
 

@@ -351,8 +351,8 @@ class SectorTracker:
         out["tracklets"] = self._to_numpy(v.d_tracklets, nseeds, TRACKLET_DTYPE)
         n_rows = self.geom.n_rows
         if nseeds:
-            rh = self._view(v.d_row_hit, 4 * n_rows * stride).view(self.torch.int32).reshape(n_rows, stride)
-            out["row_hit"] = rh[:, :nseeds].t().contiguous().cpu().numpy()
+            rh = self._view(v.d_row_hit, 4 * nseeds * stride).view(self.torch.int32).reshape(nseeds, stride)
+            out["row_hit"] = rh[:, :n_rows].contiguous().cpu().numpy()
         else:
             out["row_hit"] = np.zeros((0, n_rows), dtype=np.int32)
         return out

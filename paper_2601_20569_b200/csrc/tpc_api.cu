@@ -296,7 +296,7 @@ int tpc_get_intermediates(tpc_ctx* ctx, tpc_debug_view* out) {
   out->n_rows_total = B.n_sr;
   out->n_bins = c.n_bins;
   out->n_seeds = c.n_seeds;
-  out->tracklet_stride = B.max_seeds;
+  out->tracklet_stride = (uint64_t)ctx->geom.n_rows;
   out->d_row_desc = B.row_desc;
   out->d_bin_start = B.bin_start;
   out->d_yz_sorted = (const float*)B.yz;

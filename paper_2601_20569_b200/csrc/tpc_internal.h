@@ -40,6 +40,7 @@ struct TpcCounters {
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
   unsigned long long follow_steps, follow_updates, follow_cands;
+  uint32_t follow_next, pad2_;  // next unclaimed seed of the follower's work queue
 };
 
 // per (sector,row) statistics of pass 1
@@ -75,7 +76,7 @@ struct TpcBuffers {
   uint32_t* scan_partials;// [scan_blocks+1]
   uint32_t* seeds;        // [max_seeds] sorted index of start hits
   tpc_tracklet* tracklets;// [max_seeds]
-  int32_t* row_hit;       // [n_rows][max_seeds]
+  int32_t* row_hit;       // [max_seeds][n_rows]
   unsigned long long* owner;     // [n]
   unsigned long long* tl_key;    // [max_seeds]
   uint32_t* seg_cnt;      // [max_seeds+1] tracks per tracklet -> exclusive scan

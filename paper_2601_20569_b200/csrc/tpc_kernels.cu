@@ -669,49 +669,22 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
   return best;
 }
 
-// Extrapolate from row r_from (exclusive) in direction dir, picking up clusters (R5.3/R5.6).
-// Rows visited without an accepted cluster get row_hit = -1.  On return *r_edge is the last
-// row with an accepted hit; SAVE(k) is applied after every accepted update.
-template <class SaveFn>
-__device__ __forceinline__ void extrapolate(const TpcBuffers& B, const TpcConst* __restrict__ K, const float* s_ylim,
-                                            const FollowConst& F, KF& k, uint32_t sr_base, int r_from, int dir,
-                                            int32_t* __restrict__ hit_col, uint32_t stride, float& chi2_acc, int& n_acc,
-                                            int& r_edge, uint32_t& n_step, uint32_t& n_cand, SaveFn save) {
-  const float dx = dir > 0 ? F.dx : -F.dx;
-  int gap = 0;
-  for (int r = r_from + dir; r >= 0 && r < F.R; r += dir) {
-    ++n_step;
-    if (!kf_propagate(k, dx, F)) break;
-    bool got = false;
-    if (fabsf(k.y) <= s_ylim[r]) {
-      const Gain g = kf_gain(k, F);
-      float chi2 = 0.f;
-      const int32_t c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2, n_cand);
-      if (c >= 0 && chi2 <= F.chi2_max) {
-        const float2 m = B.yz[c];
-        const bool stop = kf_update(k, g, m.x, m.y, F);
-        hit_col[(size_t)r * stride] = c;
-        chi2_acc = chi2_acc + chi2;
-        n_acc = n_acc + 1;
-        r_edge = r;
-        save(k);
-        got = true;
-        gap = 0;
-        if (stop) break;
-      }
-    }
-    if (!got) {
-      hit_col[(size_t)r * stride] = -1;
-      ++gap;
-      if (gap > F.max_gap) break;
-    }
-  }
-}
+// The follower is written as ONE uniform loop per thread ("one row step per iteration") so
+// that all lanes of a warp execute the same instructions whatever part of R5 their seed is
+// in; a lane whose seed is finished fetches the next seed at once (seeds are claimed in
+// chunks from a global counter).  The arithmetic per seed, and its order, are exactly those
+// of R5.1-R5.7, so the assignment of seeds to lanes never changes a result.
+enum FollowPhase { PH_CHAIN = 0, PH_UP = 1, PH_REFIT = 2, PH_DOWN = 3, PH_IDLE = 4 };
 
-__global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
+#define TPC_FOLLOW_BLOCK 128
+#define TPC_FOLLOW_CHUNK 64
+
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
+  __shared__ float s_x[TPC_MAX_ROWS];
+  __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];  // state at the innermost accepted hit (R5.7)
   const TpcConst* __restrict__ K = B.K;
-  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_ylim[r] = K->ylim[r];
+  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) { s_ylim[r] = K->ylim[r]; s_x[r] = K->x[r]; }
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   FollowConst F;
@@ -722,124 +695,185 @@ __global__ void __launch_bounds__(128) k_follow(TpcBuffers B) {
   F.ivs = K->P.init_var_sinphi; F.ivt = K->P.init_var_tanl; F.ivq = K->P.init_var_qpt;
   F.max_gap = K->P.max_gap_follow; F.min_hits = K->P.min_hits_tracklet; F.R = K->n_rows;
   const uint32_t n_seeds = B.cnt->n_seeds;
-  const uint32_t stride = B.max_seeds;
   const int32_t* __restrict__ up2 = B.link_up2;
+  const float2* __restrict__ yz = B.yz;
+  const int lane = threadIdx.x & 31;
+  const int tx = threadIdx.x;
   uint32_t w_step = 0, w_cand = 0, w_upd = 0;  // work counters (diagnostics only)
 
-  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
-    const uint32_t start = B.seeds[sd];
-    // (sector,row) of the start hit: last sr with clu_ofs <= start among non-empty rows
-    uint32_t lo = 0, hi = B.n_sr;
-    while (hi - lo > 1) {
-      const uint32_t mid = (lo + hi) >> 1;
-      if (B.row_desc[mid].clu_ofs <= start) lo = mid; else hi = mid;
-    }
-    // empty rows share clu_ofs with the next non-empty one: the search lands on the LAST
-    // row with clu_ofs <= start, which is the non-empty one
-    const uint32_t sr0 = lo;
-    const int r0 = (int)(sr0 % (uint32_t)F.R);
-    const uint32_t sr_base = sr0 - (uint32_t)r0;
-    int32_t* __restrict__ hit_col = B.row_hit + sd;
+  // warp-uniform: the chunk of seeds this warp currently draws from
+  uint32_t chunk_next = 0, chunk_end = 0;
+  bool exhausted = false;
 
-    // R5.1 init from the first two chain clusters
-    const int32_t c1 = up2[start];
-    KF k;
-    const float2 m0 = B.yz[start];
-    {
-      const float2 m1 = B.yz[c1];
-      const float dy = m1.x - m0.x;
-      const float dl = sqrtf(F.dx * F.dx + dy * dy);
-      k.y = m0.x; k.z = m0.y;
-      k.s = dy / dl;
-      k.t = (m1.y - m0.y) / dl;
-      k.q = 0.f;
-      kf_init_cov(k, F);
+  // per-lane state of the seed being followed
+  int phase = PH_IDLE;
+  KF k;
+  k.y = k.z = k.s = k.t = k.q = 0.f;
+  kf_init_cov(k, F);
+  uint32_t sd = 0, start = 0, sr_base = 0;
+  int32_t* __restrict__ hit_row = B.row_hit;  // this seed's row -> sorted index table
+  int32_t c_next = -1;
+  int r = 0, r0 = 0, r_out = 0, r_in = 0, gap = 0, nh = 0, n_up = 0;
+  float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, chi2 = 0.f;
+
+  for (;;) {
+    // ---------------------------------------------------------------- refill idle lanes
+    unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
+    if (idle) {
+      bool need = phase == PH_IDLE;
+      while (!exhausted) {
+        const unsigned want = __ballot_sync(0xffffffffu, need);
+        if (!want) break;
+        if (chunk_next >= chunk_end) {
+          uint32_t base = 0;
+          if (lane == 0) base = atomicAdd(&B.cnt->follow_next, (uint32_t)TPC_FOLLOW_CHUNK);
+          base = __shfl_sync(0xffffffffu, base, 0);
+          if (base >= n_seeds) { exhausted = true; break; }
+          chunk_next = base;
+          chunk_end = min(base + (uint32_t)TPC_FOLLOW_CHUNK, n_seeds);
+        }
+        const uint32_t rank = (uint32_t)__popc(want & ((1u << lane) - 1u));
+        const uint32_t avail = chunk_end - chunk_next;
+        if (need && rank < avail) {
+          sd = chunk_next + rank;
+          need = false;
+          // ---- R5.1 init from the first two chain clusters
+          start = B.seeds[sd];
+          // (sector,row) of the start hit: last sr with clu_ofs <= start (empty rows share
+          // clu_ofs with the next non-empty one, so the search lands on the non-empty row)
+          uint32_t lo = 0, hi = B.n_sr;
+          while (hi - lo > 1) {
+            const uint32_t mid = (lo + hi) >> 1;
+            if (B.row_desc[mid].clu_ofs <= start) lo = mid; else hi = mid;
+          }
+          r0 = (int)(lo % (uint32_t)F.R);
+          sr_base = lo - (uint32_t)r0;
+          hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
+          const int32_t c1 = up2[start];
+          const float2 m0 = yz[start];
+          const float2 m1 = yz[c1];
+          const float dy = m1.x - m0.x;
+          const float dl = sqrtf(F.dx * F.dx + dy * dy);
+          k.y = m0.x; k.z = m0.y;
+          k.s = dy / dl;
+          k.t = (m1.y - m0.y) / dl;
+          k.q = 0.f;
+          kf_init_cov(k, F);
+          hit_row[r0] = (int32_t)start;
+          r = r0; r_out = r0; r_in = r0;
+          snap_s = k.s; snap_t = k.t; snap_q = k.q;
+          n_up = 1; nh = 0; chi2 = 0.f; gap = 0;
+          c_next = c1;
+          phase = PH_CHAIN;
+        }
+        const uint32_t taken = min((uint32_t)__popc(want), avail);
+        chunk_next += taken;
+      }
+      if (__all_sync(0xffffffffu, phase == PH_IDLE)) break;  // nothing left for this warp
     }
-    hit_col[(size_t)r0 * stride] = (int32_t)start;
-    int r_out = r0;
-    float snap_s = k.s, snap_t = k.t, snap_q = k.q;
-    float chi2_up = 0.f;
-    int n_up = 1;
-    bool stopped = false;
-    // R5.2 chain fit (up), no chi2 cut
-    {
-      int r = r0;
-      for (int32_t c = c1; c >= 0; c = up2[c]) {
-        ++r;
+
+    // ---------------------------------------------------------------- one row step
+    if (phase != PH_IDLE) {
+      const bool extrap = (phase == PH_UP) || (phase == PH_DOWN);
+      const int dir = (phase <= PH_UP) ? 1 : -1;
+      const int rn = r + dir;
+      bool fin = false;    // this direction ends here
+      bool stop = false;   // ... because the leg left the |sin phi| range
+      if (rn < 0 || rn >= F.R) {
+        fin = true;        // only an extrapolation can run off the pad plane
+      } else {
         ++w_step;
-        if (!kf_propagate(k, F.dx, F)) { stopped = true; break; }
-        const Gain g = kf_gain(k, F);
-        const float2 m = B.yz[c];
-        const bool stop = kf_update(k, g, m.x, m.y, F);
-        hit_col[(size_t)r * stride] = c;
-        r_out = r;
-        ++n_up;
-        snap_s = k.s; snap_t = k.t; snap_q = k.q;
-        if (stop) { stopped = true; break; }
+        if (!kf_propagate(k, dir > 0 ? F.dx : -F.dx, F)) {
+          fin = true; stop = true;
+        } else {
+          r = rn;
+          const Gain g = kf_gain(k, F);
+          int32_t c = -1;
+          float chi2h = 0.f;
+          if (phase == PH_CHAIN) {
+            c = c_next;                                   // R5.2: no chi2 cut
+          } else if (phase == PH_REFIT) {
+            c = hit_row[r];                               // R5.5: recorded hit or hole
+          } else if (fabsf(k.y) <= s_ylim[r]) {           // R5.3 / R5.6: road search
+            c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2h, w_cand);
+            if (!(c >= 0 && chi2h <= F.chi2_max)) c = -1;
+          }
+          if (c >= 0) {
+            const float2 m = yz[c];
+            if (phase == PH_REFIT) chi2h = kf_chi2(k, g, m.x, m.y);
+            stop = kf_update(k, g, m.x, m.y, F);
+            ++w_upd;
+            if (phase <= PH_UP) {                         // outward: record, remember the turn state
+              hit_row[r] = c;
+              r_out = r;
+              ++n_up;
+              snap_s = k.s; snap_t = k.t; snap_q = k.q;
+              if (phase == PH_CHAIN) c_next = up2[c];
+            } else {                                      // inward: accumulate chi2, remember the state
+              if (phase == PH_DOWN) hit_row[r] = c;
+              chi2 = chi2 + chi2h;
+              ++nh;
+              r_in = r;
+              s_kin[0][tx] = k.y; s_kin[1][tx] = k.z; s_kin[2][tx] = k.s; s_kin[3][tx] = k.t; s_kin[4][tx] = k.q;
+              s_kin[5][tx] = k.c00; s_kin[6][tx] = k.c10; s_kin[7][tx] = k.c11; s_kin[8][tx] = k.c20;
+              s_kin[9][tx] = k.c21; s_kin[10][tx] = k.c22; s_kin[11][tx] = k.c30; s_kin[12][tx] = k.c31;
+              s_kin[13][tx] = k.c32; s_kin[14][tx] = k.c33; s_kin[15][tx] = k.c40; s_kin[16][tx] = k.c41;
+              s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;
+            }
+            gap = 0;
+            if (stop) fin = true;
+          } else if (extrap) {
+            hit_row[r] = -1;
+            ++gap;
+            if (gap > F.max_gap) fin = true;
+          }
+        }
+      }
+      // ---- phase transitions
+      if (phase == PH_CHAIN && !fin && c_next < 0) { phase = PH_UP; gap = 0; }   // chain fitted: extrapolate up
+      else if (phase == PH_REFIT && !fin && r == r0) { phase = PH_DOWN; gap = 0; }  // refit done: extrapolate down
+      else if (fin && phase <= PH_UP) {
+        // R5.4 turn at the outermost accepted hit
+        const float2 mo = yz[hit_row[r_out]];
+        k.y = mo.x; k.z = mo.y;
+        k.s = snap_s; k.t = snap_t; k.q = snap_q;
+        kf_init_cov(k, F);
+        chi2 = 0.f; nh = 1; r_in = r_out; r = r_out; gap = 0;
+        s_kin[0][tx] = k.y; s_kin[1][tx] = k.z; s_kin[2][tx] = k.s; s_kin[3][tx] = k.t; s_kin[4][tx] = k.q;
+        s_kin[5][tx] = k.c00; s_kin[6][tx] = k.c10; s_kin[7][tx] = k.c11; s_kin[8][tx] = k.c20;
+        s_kin[9][tx] = k.c21; s_kin[10][tx] = k.c22; s_kin[11][tx] = k.c30; s_kin[12][tx] = k.c31;
+        s_kin[13][tx] = k.c32; s_kin[14][tx] = k.c33; s_kin[15][tx] = k.c40; s_kin[16][tx] = k.c41;
+        s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;
+        phase = (r_out > r0) ? PH_REFIT : PH_DOWN;
+      } else if (fin) {
+        // R5.7 output (hits below r_in of a refit that ended early are outside
+        // [row_first,row_last] and thereby not part of the tracklet)
+        tpc_tracklet t;
+        t.x = s_x[r_in];
+#pragma unroll
+        for (int i = 0; i < 5; ++i) t.p[i] = s_kin[i][tx];
+#pragma unroll
+        for (int i = 0; i < 15; ++i) t.c[i] = s_kin[5 + i][tx];
+        t.chi2 = chi2;
+        t.seed_sorted = start;
+        t.seed_id = B.orig_id[start];
+        const bool keep = nh >= F.min_hits;
+        t.n_hits = keep ? (int16_t)nh : (int16_t)0;
+        t.row_first = (uint8_t)r_in;
+        t.row_last = (uint8_t)r_out;
+        t.sector = (uint8_t)(sr_base / (uint32_t)F.R);
+        t.seed_len = B.seed_len[start];
+        t.pad_ = 0; t.pad2_[0] = 0; t.pad2_[1] = 0;
+        B.tracklets[sd] = t;
+        if (keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+        phase = PH_IDLE;
       }
     }
-    // R5.3 extrapolate up
-    if (!stopped)
-      extrapolate(B, K, s_ylim, F, k, sr_base, r_out, +1, hit_col, stride, chi2_up, n_up, r_out, w_step, w_cand,
-                  [&](const KF& kk) { snap_s = kk.s; snap_t = kk.t; snap_q = kk.q; });
-    // R5.4 turn at the outermost accepted hit
-    {
-      const float2 mo = B.yz[hit_col[(size_t)r_out * stride]];
-      k.y = mo.x; k.z = mo.y;
-      k.s = snap_s; k.t = snap_t; k.q = snap_q;
-      kf_init_cov(k, F);
-    }
-    float chi2 = 0.f;
-    int nh = 1;
-    int r_in = r_out;
-    KF k_in = k;
-    stopped = false;
-    // R5.5 refit down through the recorded hits
-    for (int r = r_out - 1; r >= r0; --r) {
-      ++w_step;
-      if (!kf_propagate(k, -F.dx, F)) { stopped = true; break; }
-      const int32_t c = hit_col[(size_t)r * stride];
-      if (c < 0) continue;
-      const Gain g = kf_gain(k, F);
-      const float2 m = B.yz[c];
-      const float c2 = kf_chi2(k, g, m.x, m.y);
-      const bool stop = kf_update(k, g, m.x, m.y, F);
-      chi2 = chi2 + c2;
-      ++nh;
-      r_in = r;
-      k_in = k;
-      if (stop) { stopped = true; break; }
-    }
-    // R5.6 extrapolate down (hits below r_in of a refit that ended early are outside
-    // [row_first,row_last] and thereby not part of the tracklet)
-    if (!stopped)
-      extrapolate(B, K, s_ylim, F, k, sr_base, r_in, -1, hit_col, stride, chi2, nh, r_in, w_step, w_cand,
-                  [&](const KF& kk) { k_in = kk; });
-    // R5.7 output
-    tpc_tracklet t;
-    t.x = K->x[r_in];
-    t.p[0] = k_in.y; t.p[1] = k_in.z; t.p[2] = k_in.s; t.p[3] = k_in.t; t.p[4] = k_in.q;
-    t.c[0] = k_in.c00; t.c[1] = k_in.c10; t.c[2] = k_in.c11; t.c[3] = k_in.c20; t.c[4] = k_in.c21;
-    t.c[5] = k_in.c22; t.c[6] = k_in.c30; t.c[7] = k_in.c31; t.c[8] = k_in.c32; t.c[9] = k_in.c33;
-    t.c[10] = k_in.c40; t.c[11] = k_in.c41; t.c[12] = k_in.c42; t.c[13] = k_in.c43; t.c[14] = k_in.c44;
-    t.chi2 = chi2;
-    t.seed_sorted = start;
-    t.seed_id = B.orig_id[start];
-    const bool keep = nh >= F.min_hits;
-    t.n_hits = keep ? (int16_t)nh : (int16_t)0;
-    t.row_first = (uint8_t)r_in;
-    t.row_last = (uint8_t)r_out;
-    t.sector = (uint8_t)(sr_base / (uint32_t)F.R);
-    t.seed_len = B.seed_len[start];
-    t.pad_ = 0; t.pad2_[0] = 0; t.pad2_[1] = 0;
-    B.tracklets[sd] = t;
-    if (keep) atomicAdd(&B.cnt->n_tracklets, 1u);
-    w_upd += (uint32_t)(n_up - 1) + (uint32_t)(nh - 1);
   }
   w_step = __reduce_add_sync(0xffffffffu, w_step);
   w_cand = __reduce_add_sync(0xffffffffu, w_cand);
   w_upd = __reduce_add_sync(0xffffffffu, w_upd);
-  if ((threadIdx.x & 31) == 0 && w_step) {
+  if (lane == 0 && w_step) {
     atomicAdd(&B.cnt->follow_steps, (unsigned long long)w_step);
     atomicAdd(&B.cnt->follow_updates, (unsigned long long)w_upd);
     atomicAdd(&B.cnt->follow_cands, (unsigned long long)w_cand);
@@ -862,7 +896,7 @@ __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
 __global__ void __launch_bounds__(128) k_sel_owner(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
-  const uint32_t stride = B.max_seeds;
+  const uint32_t stride = (uint32_t)B.K->n_rows;
   const float w = B.K->P.sel_chi2_weight;
   for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
     const int nh = B.tracklets[sd].n_hits;
@@ -873,7 +907,7 @@ __global__ void __launch_bounds__(128) k_sel_owner(TpcBuffers B) {
       key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - B.tracklets[sd].seed_id);
       const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
       for (int r = r0; r <= r1; ++r) {
-        const int32_t c = B.row_hit[(size_t)r * stride + sd];
+        const int32_t c = B.row_hit[(size_t)sd * stride + r];
         if (c >= 0) atomicMax(&B.owner[c], key);
       }
     }
@@ -887,7 +921,7 @@ template <bool EMIT>
 __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, uint32_t& n_seg_out, uint32_t& n_id_out,
                                               uint32_t trk_ofs, uint32_t id_ofs) {
   const tpc_params& P = B.K->P;
-  const uint32_t stride = B.max_seeds;
+  const uint32_t stride = (uint32_t)B.K->n_rows;
   const unsigned long long key = B.tl_key[sd];
   const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
   const int min_hits = P.min_hits_track, max_gap = P.max_gap_select;
@@ -907,7 +941,7 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
         uint32_t o = id_ofs + n_id;
         for (int r = seg_first; r <= seg_last; ++r) {
           if (!((acc_bits[r >> 5] >> (r & 31)) & 1u)) continue;
-          B.cluster_ids[o] = B.orig_id[B.row_hit[(size_t)r * stride + sd]];
+          B.cluster_ids[o] = B.orig_id[B.row_hit[(size_t)sd * stride + r]];
           B.cluster_shared[o] = (uint8_t)((sh_bits[r >> 5] >> (r & 31)) & 1u);
           ++o;
         }
@@ -941,7 +975,7 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
     n_acc = 0; n_sh = 0; seg_last = -1; seg_first = -1;
   };
   for (int r = r1; r >= r0; --r) {
-    int32_t c = B.row_hit[(size_t)r * stride + sd];
+    int32_t c = B.row_hit[(size_t)sd * stride + r];
     bool sh = false;
     if (c >= 0 && B.owner[c] != key) {
       if ((long long)(n_sh + 1) * 1000 <= permille * (long long)(n_acc + 1)) sh = true;
@@ -1014,6 +1048,7 @@ __global__ void k_init(TpcBuffers B) {
     c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
     c.n_tracks = c.n_ids = c.error = c.pad_ = 0;
     c.follow_steps = c.follow_updates = c.follow_cands = 0ull;
+    c.follow_next = 0u; c.pad2_ = 0u;
     *B.cnt = c;
   }
 }
