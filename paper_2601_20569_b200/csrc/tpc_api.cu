@@ -99,6 +99,7 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.seed_len = (uint8_t*)take(n);
   b.scan_partials = (uint32_t*)take(4 * (size_t)(k.scan_blocks + 2));
   b.seeds = (uint32_t*)take(4 * (size_t)k.max_seeds);
+  b.seed_sr = (uint16_t*)take(2 * (size_t)k.max_seeds);
   b.tracklets = (tpc_tracklet*)take(sizeof(tpc_tracklet) * (size_t)k.max_seeds);
   b.row_hit = (int32_t*)take(4 * (size_t)c->geom.n_rows * k.max_seeds);
   b.owner = (unsigned long long*)take(8 * n);

@@ -75,6 +75,7 @@ struct TpcBuffers {
   uint8_t* seed_len;      // [n] chain length if the cluster is a start hit of a seed, else 0
   uint32_t* scan_partials;// [scan_blocks+1]
   uint32_t* seeds;        // [max_seeds] sorted index of start hits
+  uint16_t* seed_sr;      // [max_seeds] sector*n_rows+row of each start hit
   tpc_tracklet* tracklets;// [max_seeds]
   int32_t* row_hit;       // [max_seeds][n_rows]
   unsigned long long* owner;     // [n]

@@ -491,7 +491,17 @@ __global__ void __launch_bounds__(1024) k_seed_write(TpcBuffers B) {
     const uint32_t f = (i < n && B.seed_len[i]) ? 1u : 0u;
     uint32_t tot;
     const uint32_t pre = block_excl_scan(f, &tot, sm);
-    if (f) B.seeds[B.scan_partials[blk] + pre] = i;
+    if (f) {
+      // (sector,row) of the start hit: last sr with clu_ofs <= i (empty rows share clu_ofs
+      // with the next non-empty one, so the search lands on the non-empty row)
+      uint32_t lo = 0, hi = B.n_sr;
+      while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (B.row_desc[mid].clu_ofs <= i) lo = mid; else hi = mid;
+      }
+      B.seeds[B.scan_partials[blk] + pre] = i;
+      B.seed_sr[B.scan_partials[blk] + pre] = (uint16_t)lo;
+    }
   }
 }
 
@@ -639,11 +649,13 @@ __device__ __forceinline__ bool kf_update(KF& k, const Gain& g, float ym, float 
 
 __device__ __forceinline__ float clampf(float v, float lo, float hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // R5.3: best cluster of row sr inside the road around the predicted state: minimum of
-// (chi2, original id).  Returns the sorted index or -1.
+// (chi2, original id).  Returns the sorted index or -1; *m_out = its (y,z).
 __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcConst* __restrict__ K, uint32_t sr,
                                                 const KF& k, const Gain& g, const FollowConst& F, float* chi2_out,
-                                                uint32_t& n_cand) {
+                                                float2* m_out, uint32_t& n_cand) {
   const tpc_row_desc d = B.row_desc[sr];
   if (d.count == 0) return -1;
   const float ry = clampf(F.road_nsigma * sqrtf(k.c00 + F.vy), F.road_min, F.road_max);
@@ -651,35 +663,59 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
   const BinWindow w = make_window(d, K, k.y - ry, k.y + ry, k.z - rz, k.z + rz);
   int32_t best = -1;
   float best_chi2 = 0.f;
-  uint32_t best_id = 0;
+  float2 best_m = make_float2(0.f, 0.f);
+  const float2* __restrict__ yz = B.yz;
+  auto eval = [&](uint32_t c, const float2 m) {
+    if (!(fabsf(m.x - k.y) <= ry && fabsf(m.y - k.z) <= rz)) return;
+    const float chi2 = kf_chi2(k, g, m.x, m.y);
+    ++n_cand;
+    bool better = best < 0 || chi2 < best_chi2;
+    if (!better && chi2 == best_chi2) better = B.orig_id[c] < B.orig_id[best];  // rule D2, rare
+    if (better) { best = (int32_t)c; best_chi2 = chi2; best_m = m; }
+  };
   for (int bz = w.bz0; bz <= w.bz1; ++bz) {
     const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
-    const uint32_t c1 = B.bin_start[b + w.by_span];
-    for (uint32_t c = B.bin_start[b]; c < c1; ++c) {
-      const float2 m = B.yz[c];
-      if (!(fabsf(m.x - k.y) <= ry && fabsf(m.y - k.z) <= rz)) continue;
-      const float chi2 = kf_chi2(k, g, m.x, m.y);
-      ++n_cand;
-      bool better = best < 0 || chi2 < best_chi2;
-      if (!better && chi2 == best_chi2) better = B.orig_id[c] < best_id;
-      if (better) { best = (int32_t)c; best_chi2 = chi2; best_id = B.orig_id[c]; }
+    const uint32_t c0 = B.bin_start[b], c1 = B.bin_start[b + w.by_span];
+    for (uint32_t c = c0; c < c1; c += 2) {   // two loads in flight
+      const bool two = c + 1 < c1;
+      const float2 ma = yz[c];
+      const float2 mb = two ? yz[c + 1] : ma;
+      eval(c, ma);
+      if (two) eval(c + 1, mb);
     }
   }
   *chi2_out = best_chi2;
+  *m_out = best_m;
   return best;
 }
 
 // The follower is written as ONE uniform loop per thread ("one row step per iteration") so
 // that all lanes of a warp execute the same instructions whatever part of R5 their seed is
 // in; a lane whose seed is finished fetches the next seed at once (seeds are claimed in
-// chunks from a global counter).  The arithmetic per seed, and its order, are exactly those
-// of R5.1-R5.7, so the assignment of seeds to lanes never changes a result.
+// chunks from a global counter).  Loads are software-pipelined one row ahead: the chain /
+// recorded hit of the next row and, during extrapolation, the bin of the predicted next-row
+// position are requested while the current row is computed.  The arithmetic per seed, and
+// its order, are exactly those of R5.1-R5.7, so neither the assignment of seeds to lanes
+// nor the prefetching changes a result.
 enum FollowPhase { PH_CHAIN = 0, PH_UP = 1, PH_REFIT = 2, PH_DOWN = 3, PH_IDLE = 4 };
 
 #define TPC_FOLLOW_BLOCK 128
 #define TPC_FOLLOW_CHUNK 64
+#ifndef TPC_FOLLOW_MINBLOCKS
+#define TPC_FOLLOW_MINBLOCKS 6   // resident CTAs per SM the register budget is sized for
+#endif
+#define TPC_NO_BIN 0xFFFFFFFFu
 
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
+#define TPC_SAVE_KIN()                                                                                         \
+  do {                                                                                                         \
+    s_kin[0][tx] = k.y; s_kin[1][tx] = k.z; s_kin[2][tx] = k.s; s_kin[3][tx] = k.t; s_kin[4][tx] = k.q;        \
+    s_kin[5][tx] = k.c00; s_kin[6][tx] = k.c10; s_kin[7][tx] = k.c11; s_kin[8][tx] = k.c20;                    \
+    s_kin[9][tx] = k.c21; s_kin[10][tx] = k.c22; s_kin[11][tx] = k.c30; s_kin[12][tx] = k.c31;                 \
+    s_kin[13][tx] = k.c32; s_kin[14][tx] = k.c33; s_kin[15][tx] = k.c40; s_kin[16][tx] = k.c41;                \
+    s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;                                       \
+  } while (0)
+
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_MINBLOCKS) k_follow(TpcBuffers B) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
   __shared__ float s_x[TPC_MAX_ROWS];
   __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];  // state at the innermost accepted hit (R5.7)
@@ -694,9 +730,11 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
   F.chi2_max = K->P.chi2_max_hit;
   F.ivs = K->P.init_var_sinphi; F.ivt = K->P.init_var_tanl; F.ivq = K->P.init_var_qpt;
   F.max_gap = K->P.max_gap_follow; F.min_hits = K->P.min_hits_tracklet; F.R = K->n_rows;
+  const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const int32_t* __restrict__ up2 = B.link_up2;
   const float2* __restrict__ yz = B.yz;
+  const uint32_t* __restrict__ bin_start = B.bin_start;
   const int lane = threadIdx.x & 31;
   const int tx = threadIdx.x;
   uint32_t w_step = 0, w_cand = 0, w_upd = 0;  // work counters (diagnostics only)
@@ -712,13 +750,16 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
   kf_init_cov(k, F);
   uint32_t sd = 0, start = 0, sr_base = 0;
   int32_t* __restrict__ hit_row = B.row_hit;  // this seed's row -> sorted index table
-  int32_t c_next = -1;
-  int r = 0, r0 = 0, r_out = 0, r_in = 0, gap = 0, nh = 0, n_up = 0;
-  float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, chi2 = 0.f;
+  int r = 0, r0 = 0, r_out = 0, r_in = 0, gap = 0, nh = 0;
+  float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, snap_y = 0.f, snap_z = 0.f, chi2 = 0.f;
+  // load pipeline: the hit of the coming row (chain fit / refit) and the one after it
+  int32_t c_cur = -1, c_nxt = -1;
+  float2 m_cur = make_float2(0.f, 0.f);
+  uint32_t pb = TPC_NO_BIN;  // extrapolation: first cluster of the predicted bin on the coming row
 
   for (;;) {
     // ---------------------------------------------------------------- refill idle lanes
-    unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
+    const unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
     if (idle) {
       bool need = phase == PH_IDLE;
       while (!exhausted) {
@@ -739,19 +780,14 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
           need = false;
           // ---- R5.1 init from the first two chain clusters
           start = B.seeds[sd];
-          // (sector,row) of the start hit: last sr with clu_ofs <= start (empty rows share
-          // clu_ofs with the next non-empty one, so the search lands on the non-empty row)
-          uint32_t lo = 0, hi = B.n_sr;
-          while (hi - lo > 1) {
-            const uint32_t mid = (lo + hi) >> 1;
-            if (B.row_desc[mid].clu_ofs <= start) lo = mid; else hi = mid;
-          }
-          r0 = (int)(lo % (uint32_t)F.R);
-          sr_base = lo - (uint32_t)r0;
+          const uint32_t sr0 = B.seed_sr[sd];
+          r0 = (int)(sr0 % (uint32_t)F.R);
+          sr_base = sr0 - (uint32_t)r0;
           hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
           const int32_t c1 = up2[start];
           const float2 m0 = yz[start];
           const float2 m1 = yz[c1];
+          c_nxt = up2[c1];
           const float dy = m1.x - m0.x;
           const float dl = sqrtf(F.dx * F.dx + dy * dy);
           k.y = m0.x; k.z = m0.y;
@@ -761,9 +797,10 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
           kf_init_cov(k, F);
           hit_row[r0] = (int32_t)start;
           r = r0; r_out = r0; r_in = r0;
-          snap_s = k.s; snap_t = k.t; snap_q = k.q;
-          n_up = 1; nh = 0; chi2 = 0.f; gap = 0;
-          c_next = c1;
+          snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m0.x; snap_z = m0.y;
+          nh = 0; chi2 = 0.f; gap = 0;
+          c_cur = c1; m_cur = m1;
+          pb = TPC_NO_BIN;
           phase = PH_CHAIN;
         }
         const uint32_t taken = min((uint32_t)__popc(want), avail);
@@ -779,46 +816,59 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
       const int rn = r + dir;
       bool fin = false;    // this direction ends here
       bool stop = false;   // ... because the leg left the |sin phi| range
+      if (extrap && pb != TPC_NO_BIN) prefetch_l1(yz + pb);
       if (rn < 0 || rn >= F.R) {
         fin = true;        // only an extrapolation can run off the pad plane
       } else {
         ++w_step;
+        const float y_prev = k.y, z_prev = k.z;
         if (!kf_propagate(k, dir > 0 ? F.dx : -F.dx, F)) {
           fin = true; stop = true;
         } else {
           r = rn;
+          // ---- request the next row's data while this row is computed
+          int32_t c_nxt2 = -1;
+          float2 m_nxt = make_float2(0.f, 0.f);
+          if (extrap) {
+            pb = TPC_NO_BIN;
+            const int rp = r + dir;
+            if (rp >= 0 && rp < F.R) {
+              const tpc_row_desc dn = B.row_desc[sr_base + (uint32_t)rp];
+              if (dn.count) {  // linear continuation of this step
+                const int by = bin_coord(k.y + (k.y - y_prev), dn.y0, inv_dy, dn.ny);
+                const int bz = bin_coord(k.z + (k.z - z_prev), dn.z0, inv_dz, dn.nz);
+                pb = bin_start[dn.bin_ofs + (uint32_t)bz * (uint32_t)dn.ny + (uint32_t)by];
+              }
+            }
+          } else {
+            if (c_nxt >= 0) m_nxt = yz[c_nxt];
+            if (phase == PH_CHAIN) { if (c_nxt >= 0) c_nxt2 = up2[c_nxt]; }
+            else if (r - 2 >= r0) c_nxt2 = hit_row[r - 2];
+          }
           const Gain g = kf_gain(k, F);
           int32_t c = -1;
           float chi2h = 0.f;
-          if (phase == PH_CHAIN) {
-            c = c_next;                                   // R5.2: no chi2 cut
-          } else if (phase == PH_REFIT) {
-            c = hit_row[r];                               // R5.5: recorded hit or hole
+          float2 m = m_cur;
+          if (!extrap) {
+            c = c_cur;                                    // R5.2 (no chi2 cut) / R5.5 (recorded hit or hole)
           } else if (fabsf(k.y) <= s_ylim[r]) {           // R5.3 / R5.6: road search
-            c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2h, w_cand);
+            c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2h, &m, w_cand);
             if (!(c >= 0 && chi2h <= F.chi2_max)) c = -1;
           }
           if (c >= 0) {
-            const float2 m = yz[c];
             if (phase == PH_REFIT) chi2h = kf_chi2(k, g, m.x, m.y);
             stop = kf_update(k, g, m.x, m.y, F);
             ++w_upd;
             if (phase <= PH_UP) {                         // outward: record, remember the turn state
               hit_row[r] = c;
               r_out = r;
-              ++n_up;
-              snap_s = k.s; snap_t = k.t; snap_q = k.q;
-              if (phase == PH_CHAIN) c_next = up2[c];
+              snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m.x; snap_z = m.y;
             } else {                                      // inward: accumulate chi2, remember the state
               if (phase == PH_DOWN) hit_row[r] = c;
               chi2 = chi2 + chi2h;
               ++nh;
               r_in = r;
-              s_kin[0][tx] = k.y; s_kin[1][tx] = k.z; s_kin[2][tx] = k.s; s_kin[3][tx] = k.t; s_kin[4][tx] = k.q;
-              s_kin[5][tx] = k.c00; s_kin[6][tx] = k.c10; s_kin[7][tx] = k.c11; s_kin[8][tx] = k.c20;
-              s_kin[9][tx] = k.c21; s_kin[10][tx] = k.c22; s_kin[11][tx] = k.c30; s_kin[12][tx] = k.c31;
-              s_kin[13][tx] = k.c32; s_kin[14][tx] = k.c33; s_kin[15][tx] = k.c40; s_kin[16][tx] = k.c41;
-              s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;
+              TPC_SAVE_KIN();
             }
             gap = 0;
             if (stop) fin = true;
@@ -827,24 +877,28 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK) k_follow(TpcBuffers B) {
             ++gap;
             if (gap > F.max_gap) fin = true;
           }
+          if (!extrap) { c_cur = c_nxt; m_cur = m_nxt; c_nxt = c_nxt2; }
         }
       }
       // ---- phase transitions
-      if (phase == PH_CHAIN && !fin && c_next < 0) { phase = PH_UP; gap = 0; }   // chain fitted: extrapolate up
-      else if (phase == PH_REFIT && !fin && r == r0) { phase = PH_DOWN; gap = 0; }  // refit done: extrapolate down
+      if (phase == PH_CHAIN && !fin && c_cur < 0) { phase = PH_UP; gap = 0; pb = TPC_NO_BIN; }  // chain fitted
+      else if (phase == PH_REFIT && !fin && r == r0) { phase = PH_DOWN; gap = 0; pb = TPC_NO_BIN; }  // refit done
       else if (fin && phase <= PH_UP) {
         // R5.4 turn at the outermost accepted hit
-        const float2 mo = yz[hit_row[r_out]];
-        k.y = mo.x; k.z = mo.y;
+        k.y = snap_y; k.z = snap_z;
         k.s = snap_s; k.t = snap_t; k.q = snap_q;
         kf_init_cov(k, F);
         chi2 = 0.f; nh = 1; r_in = r_out; r = r_out; gap = 0;
-        s_kin[0][tx] = k.y; s_kin[1][tx] = k.z; s_kin[2][tx] = k.s; s_kin[3][tx] = k.t; s_kin[4][tx] = k.q;
-        s_kin[5][tx] = k.c00; s_kin[6][tx] = k.c10; s_kin[7][tx] = k.c11; s_kin[8][tx] = k.c20;
-        s_kin[9][tx] = k.c21; s_kin[10][tx] = k.c22; s_kin[11][tx] = k.c30; s_kin[12][tx] = k.c31;
-        s_kin[13][tx] = k.c32; s_kin[14][tx] = k.c33; s_kin[15][tx] = k.c40; s_kin[16][tx] = k.c41;
-        s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;
-        phase = (r_out > r0) ? PH_REFIT : PH_DOWN;
+        TPC_SAVE_KIN();
+        pb = TPC_NO_BIN;
+        if (r_out > r0) {
+          phase = PH_REFIT;
+          c_cur = hit_row[r_out - 1];
+          c_nxt = (r_out - 2 >= r0) ? hit_row[r_out - 2] : -1;
+          if (c_cur >= 0) m_cur = yz[c_cur];
+        } else {
+          phase = PH_DOWN;
+        }
       } else if (fin) {
         // R5.7 output (hits below r_in of a refit that ended early are outside
         // [row_first,row_last] and thereby not part of the tracklet)
@@ -1113,7 +1167,7 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
-  k_follow<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
+  k_follow<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_follow");
   if (timers) cudaEventRecord(E.ev[4], st);
   // ---- K5 ambiguity solving
