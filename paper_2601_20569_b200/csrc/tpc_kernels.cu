@@ -649,6 +649,19 @@ __device__ __forceinline__ bool kf_update(KF& k, const Gain& g, float ym, float 
 
 __device__ __forceinline__ float clampf(float v, float lo, float hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+// Row descriptors are read at every row step of every seed: keep their lines in L1/L2.
+__device__ __forceinline__ tpc_row_desc ld_row_desc(const tpc_row_desc* p) {
+  uint4 a, b;
+  asm volatile("ld.global.nc.L1::evict_last.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "l"(p));
+  asm volatile("ld.global.nc.L1::evict_last.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(reinterpret_cast<const char*>(p) + 16));
+  tpc_row_desc d;
+  d.y0 = __uint_as_float(a.x); d.z0 = __uint_as_float(a.y); d.ny = (int)a.z; d.nz = (int)a.w;
+  d.bin_ofs = b.x; d.clu_ofs = b.y; d.count = b.z; d.pad_ = b.w;
+  return d;
+}
+
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // R5.3: best cluster of row sr inside the road around the predicted state: minimum of
@@ -656,7 +669,7 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcConst* __restrict__ K, uint32_t sr,
                                                 const KF& k, const Gain& g, const FollowConst& F, float* chi2_out,
                                                 float2* m_out, uint32_t& n_cand) {
-  const tpc_row_desc d = B.row_desc[sr];
+  const tpc_row_desc d = ld_row_desc(B.row_desc + sr);
   if (d.count == 0) return -1;
   const float ry = clampf(F.road_nsigma * sqrtf(k.c00 + F.vy), F.road_min, F.road_max);
   const float rz = clampf(F.road_nsigma * sqrtf(k.c11 + F.vz), F.road_min, F.road_max);
@@ -665,6 +678,7 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
   float best_chi2 = 0.f;
   float2 best_m = make_float2(0.f, 0.f);
   const float2* __restrict__ yz = B.yz;
+  const uint32_t* __restrict__ bin_start = B.bin_start;
   auto eval = [&](uint32_t c, const float2 m) {
     if (!(fabsf(m.x - k.y) <= ry && fabsf(m.y - k.z) <= rz)) return;
     const float chi2 = kf_chi2(k, g, m.x, m.y);
@@ -673,16 +687,31 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
     if (!better && chi2 == best_chi2) better = B.orig_id[c] < B.orig_id[best];  // rule D2, rare
     if (better) { best = (int32_t)c; best_chi2 = chi2; best_m = m; }
   };
-  for (int bz = w.bz0; bz <= w.bz1; ++bz) {
+  // Fast path: the road is small against the bins, so the window covers one or two z-rows of
+  // bins with a few clusters each.  All index loads, then all candidate loads, are issued
+  // together (two memory round trips in total); leftovers take the generic loops below.
+  const bool two_rows = w.bz1 > w.bz0;
+  const uint32_t bA = w.base + (uint32_t)w.bz0 * (uint32_t)w.ny;
+  const uint32_t bB = bA + (uint32_t)w.ny;
+  const uint32_t a0 = bin_start[bA], a1 = bin_start[bA + w.by_span];
+  uint32_t b0 = 0, b1 = 0;
+  if (two_rows) { b0 = bin_start[bB]; b1 = bin_start[bB + w.by_span]; }
+  const bool ha0 = a0 < a1, ha1 = a0 + 1 < a1, hb0 = b0 < b1, hb1 = b0 + 1 < b1;
+  float2 ma0 = best_m, ma1 = best_m, mb0 = best_m, mb1 = best_m;
+  if (ha0) ma0 = yz[a0];
+  if (ha1) ma1 = yz[a0 + 1];
+  if (hb0) mb0 = yz[b0];
+  if (hb1) mb1 = yz[b0 + 1];
+  if (ha0) eval(a0, ma0);
+  if (ha1) eval(a0 + 1, ma1);
+  if (hb0) eval(b0, mb0);
+  if (hb1) eval(b0 + 1, mb1);
+  for (uint32_t c = a0 + 2; c < a1; ++c) eval(c, yz[c]);
+  for (uint32_t c = b0 + 2; c < b1; ++c) eval(c, yz[c]);
+  for (int bz = w.bz0 + 2; bz <= w.bz1; ++bz) {
     const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
-    const uint32_t c0 = B.bin_start[b], c1 = B.bin_start[b + w.by_span];
-    for (uint32_t c = c0; c < c1; c += 2) {   // two loads in flight
-      const bool two = c + 1 < c1;
-      const float2 ma = yz[c];
-      const float2 mb = two ? yz[c + 1] : ma;
-      eval(c, ma);
-      if (two) eval(c + 1, mb);
-    }
+    const uint32_t c1 = bin_start[b + w.by_span];
+    for (uint32_t c = bin_start[b]; c < c1; ++c) eval(c, yz[c]);
   }
   *chi2_out = best_chi2;
   *m_out = best_m;
@@ -833,7 +862,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_MINBLOCKS) k_foll
             pb = TPC_NO_BIN;
             const int rp = r + dir;
             if (rp >= 0 && rp < F.R) {
-              const tpc_row_desc dn = B.row_desc[sr_base + (uint32_t)rp];
+              const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)rp);
               if (dn.count) {  // linear continuation of this step
                 const int by = bin_coord(k.y + (k.y - y_prev), dn.y0, inv_dy, dn.ny);
                 const int bz = bin_coord(k.z + (k.z - z_prev), dn.z0, inv_dz, dn.nz);
