@@ -149,6 +149,8 @@ def make_frame(workload: str, rank: int, events: int | None, tracks: int | None)
     kw = dict(seed=base.seed + 1000 * rank)
     if events is not None:
         kw["n_events"] = events
+        # a shorter frame at the SAME interaction rate (same cluster density per cm of drift)
+        kw["t_window_us"] = base.t_window_us * events / base.n_events
     if tracks is not None:
         kw["tracks_per_event"] = tracks
     cfg = dg.preset(workload, **kw)
