@@ -88,6 +88,7 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.scan_blocks = k.scan_blocks;
   b.row_desc = (tpc_row_desc*)take(sizeof(tpc_row_desc) * n_sr);
   b.tile_ofs = (uint32_t*)take(4 * (size_t)(n_sr + 1));
+  b.tile_sr = (uint16_t*)take(2 * (size_t)(n / TPC_NF_TILE + n_sr + 1));
   b.slot = (uint32_t*)take(4 * n);
   b.bin_start = (uint32_t*)take(4 * (k.max_bins + 4));
   b.yz = (float2*)take(8 * n);

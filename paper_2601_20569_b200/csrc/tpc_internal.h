@@ -64,6 +64,7 @@ struct TpcBuffers {
   TpcRowStat* row_stat;   // [n_sr]
   tpc_row_desc* row_desc; // [n_sr]
   uint32_t* tile_ofs;     // [n_sr+1] first neighbour-finder tile of each row
+  uint16_t* tile_sr;      // [n/TPC_NF_TILE + n_sr + 1] (sector,row) of each neighbour-finder tile
   uint32_t* slot;         // [n] rank of the cluster inside its bin, 0xFFFFFFFF = not in the grid
   uint32_t* bin_start;    // [max_bins+1]
   float2* yz;             // [n] sorted

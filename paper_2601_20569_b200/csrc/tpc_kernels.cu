@@ -210,6 +210,14 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
   }
 }
 
+// (sector,row) of every neighbour-finder tile, so that K2 needs no search.
+__global__ void __launch_bounds__(128) k_tile_rows(TpcBuffers B) {
+  for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
+    const uint32_t t0 = B.tile_ofs[sr], t1 = B.tile_ofs[sr + 1];
+    for (uint32_t t = t0 + threadIdx.x; t < t1; t += blockDim.x) B.tile_sr[t] = (uint16_t)sr;
+  }
+}
+
 __global__ void __launch_bounds__(256) k_zero_bins(TpcBuffers B) {
   if (B.cnt->error & TPC_DEVERR_BINS) return;
   const uint32_t n = B.cnt->n_bins + 1;
@@ -344,11 +352,95 @@ __device__ __forceinline__ BinWindow make_window(const tpc_row_desc& d, const Tp
 
 // ================================================================== K2 neighbour finder
 // PAPER.md:27 "combinatorial seeding based on a cellular automaton"; R2.
-// One CTA per tile of TPC_NF_TILE consecutive sorted clusters of one row (bins are z-major,
-// so a tile is a compact z-slab and its windows on rows r+-1 overlap heavily -> L1 reuse).
-// One thread per cluster; the best (up,down) pair is the lexicographic minimum of
-// (d2, original id of up, original id of down).
-__global__ void __launch_bounds__(TPC_NF_TILE) k_neighbours(TpcBuffers B) {
+// One CTA per tile of TPC_NF_TILE consecutive sorted clusters of one row, one thread per
+// cluster.  Bins are z-major, so a tile is a compact z-slab of its row and everything its
+// threads can see on rows r+1 / r-1 is ONE contiguous range of the sorted arrays (all y-bins
+// of the z-rows the windows touch).  That range (the (y,z) pairs and the slice of the bin
+// index) is staged in shared memory with coalesced loads; the candidate search then runs on
+// shared memory in two flat loops (window members -> per-thread lists) and one flat pair
+// loop, so the lanes of a warp stay converged.  The best (up,down) pair is the lexicographic
+// minimum of (d2, original id of up, original id of down) (rule D2), which makes the result
+// independent of the visiting order.  Tiles whose slab does not fit (very sparse or very
+// dense rows) take the same search on global memory (nf_generic).
+#define TPC_NF_SLAB 1024   // clusters staged per neighbour row
+#define TPC_NF_BINS 1023   // bins staged per neighbour row (+1 end marker)
+#define TPC_NF_LIST 12     // window members kept per thread and side
+
+// The search of one cluster directly on global memory.
+__device__ __forceinline__ void nf_generic(const TpcBuffers& B, const BinWindow& wu, const BinWindow& wd, float yi,
+                                           float zi, float ty, float wy, float wz, float max_d2, int32_t& bj,
+                                           int32_t& bk) {
+  const uint32_t* __restrict__ bin_start = B.bin_start;
+  const float2* __restrict__ yz = B.yz;
+  const uint32_t* __restrict__ orig = B.orig_id;
+  float best = 0.f;
+  for (int bzu = wu.bz0; bzu <= wu.bz1; ++bzu) {
+    const uint32_t bu = wu.base + (uint32_t)bzu * (uint32_t)wu.ny;
+    const uint32_t ju1 = bin_start[bu + wu.by_span];
+    for (uint32_t j = bin_start[bu]; j < ju1; ++j) {
+      const float2 cj = yz[j];
+      if (!(fabsf((cj.x - yi) - ty) <= wy && fabsf(cj.y - zi) <= wz)) continue;
+      const float dyu = cj.x - yi, dzu = cj.y - zi;
+      for (int bzd = wd.bz0; bzd <= wd.bz1; ++bzd) {
+        const uint32_t bd = wd.base + (uint32_t)bzd * (uint32_t)wd.ny;
+        const uint32_t k1 = bin_start[bd + wd.by_span];
+        for (uint32_t k = bin_start[bd]; k < k1; ++k) {
+          const float2 ck = yz[k];
+          if (!(fabsf((yi - ck.x) - ty) <= wy && fabsf(zi - ck.y) <= wz)) continue;
+          const float dy = dyu + (ck.x - yi);
+          const float dz = dzu + (ck.y - zi);
+          const float d2 = dy * dy + dz * dz;
+          if (!(d2 <= max_d2)) continue;
+          bool better = bj < 0 || d2 < best;
+          if (!better && d2 == best) {  // exact tie: rule D2 (rare, ids fetched only here)
+            const uint32_t jid = orig[j], bjid = orig[bj];
+            better = jid < bjid || (jid == bjid && orig[k] < orig[bk]);
+          }
+          if (better) { best = d2; bj = (int32_t)j; bk = (int32_t)k; }
+        }
+      }
+    }
+  }
+}
+
+// Collect the window members of one side from the staged slab into the thread's list.
+// The window touches at most three z-rows of bins (the caller checks), each a contiguous
+// range of the slab; their bounds are fetched together and ONE flat loop then tests every
+// cluster of the three ranges.  UP: window inequality of the up row, else of the down row.
+// Returns the member count (members beyond TPC_NF_LIST are not stored: the caller then takes
+// the nested fallback).
+template <bool UP>
+__device__ __forceinline__ int nf_collect(const BinWindow& w, int bz_lo, uint32_t bin_ofs, uint32_t c0,
+                                          const uint32_t* __restrict__ s_bin, const float2* __restrict__ s_yz,
+                                          uint16_t* __restrict__ s_list, float yi, float zi, float ty, float wy,
+                                          float wz) {
+  const int nzr = w.bz1 - w.bz0;  // 0..2 extra z-rows
+  const uint32_t b = (w.base - bin_ofs) + (uint32_t)(w.bz0 - bz_lo) * (uint32_t)w.ny;
+  const uint32_t a0 = s_bin[b] - c0, l0 = (s_bin[b + w.by_span] - c0) - a0;
+  uint32_t a1 = 0, l1 = 0, a2 = 0, l2 = 0;
+  if (nzr >= 1) { a1 = s_bin[b + w.ny] - c0; l1 = (s_bin[b + w.ny + w.by_span] - c0) - a1; }
+  if (nzr >= 2) { a2 = s_bin[b + 2 * w.ny] - c0; l2 = (s_bin[b + 2 * w.ny + w.by_span] - c0) - a2; }
+  const uint32_t l01 = l0 + l1, total = l01 + l2;
+  const uint32_t o1 = a1 - l0, o2 = a2 - l01;
+  int n = 0;
+  for (uint32_t t = 0; t < total; ++t) {
+    const uint32_t j = t + (t < l0 ? a0 : (t < l01 ? o1 : o2));
+    const float2 c = s_yz[j];
+    const bool in = UP ? (fabsf((c.x - yi) - ty) <= wy && fabsf(c.y - zi) <= wz)
+                       : (fabsf((yi - c.x) - ty) <= wy && fabsf(zi - c.y) <= wz);
+    if (in) {
+      if (n < TPC_NF_LIST) s_list[n * TPC_NF_TILE] = (uint16_t)j;
+      ++n;
+    }
+  }
+  return n;
+}
+
+__global__ void __launch_bounds__(TPC_NF_TILE, 6) k_neighbours(TpcBuffers B) {
+  __shared__ float2 s_yz[2][TPC_NF_SLAB];
+  __shared__ uint32_t s_bin[2][TPC_NF_BINS + 1];
+  __shared__ uint16_t s_list[2][TPC_NF_LIST * TPC_NF_TILE];
+  __shared__ int s_red[4];
   const TpcConst* __restrict__ K = B.K;
   if (B.cnt->error & TPC_DEVERR_BINS) return;
   const uint32_t n_tiles = B.cnt->n_tiles;
@@ -357,67 +449,104 @@ __global__ void __launch_bounds__(TPC_NF_TILE) k_neighbours(TpcBuffers B) {
   const uint32_t* __restrict__ bin_start = B.bin_start;
   const float2* __restrict__ yz = B.yz;
   const uint32_t* __restrict__ orig = B.orig_id;
+  const int tx = threadIdx.x;
   for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    // row of this tile: last sr with tile_ofs[sr] <= tile
-    uint32_t lo = 0, hi = B.n_sr;
-    while (hi - lo > 1) {
-      const uint32_t mid = (lo + hi) >> 1;
-      if (B.tile_ofs[mid] <= tile) lo = mid; else hi = mid;
-    }
-    const uint32_t sr = lo;
+    const uint32_t sr = B.tile_sr[tile];
     const int r = (int)(sr % (uint32_t)R);
     const tpc_row_desc d = B.row_desc[sr];
-    const uint32_t local = (tile - B.tile_ofs[sr]) * TPC_NF_TILE + threadIdx.x;
-    if (local >= d.count) continue;
+    const uint32_t local = (tile - B.tile_ofs[sr]) * TPC_NF_TILE + (uint32_t)tx;
+    const bool have = local < d.count;
     const uint32_t i = d.clu_ofs + local;
+    tpc_row_desc du, dd;
+    du.count = 0; dd.count = 0;
+    if (r >= 1 && r <= R - 2) { du = B.row_desc[sr + 1]; dd = B.row_desc[sr - 1]; }
+    if (du.count == 0 || dd.count == 0) {  // uniform over the CTA: no links on this row
+      if (have) { B.link_up[i] = -1; B.link_dn[i] = -1; }
+      continue;
+    }
+    float yi = 0.f, zi = 0.f, ty = 0.f;
+    BinWindow wu, wd;
+    wu.bz0 = wd.bz0 = 0x7fffffff; wu.bz1 = wd.bz1 = -1;
+    wu.base = wd.base = 0; wu.ny = wd.ny = 1; wu.by_span = wd.by_span = 1;
+    if (have) {
+      const float2 ci = yz[i];
+      yi = ci.x; zi = ci.y;
+      const float ti = yi / K->x[r];
+      ty = ti * K->dx_row;
+      wu = make_window(du, K, (yi + ty) - wy, (yi + ty) + wy, zi - wz, zi + wz);
+      wd = make_window(dd, K, (yi - ty) - wy, (yi - ty) + wy, zi - wz, zi + wz);
+    }
+    // ---- the z-rows of bins this tile's windows touch on either side (block min / max)
+    __syncthreads();  // s_red, s_yz, s_bin, s_list of the previous tile are no longer read
+    if (tx == 0) { s_red[0] = 0x7fffffff; s_red[1] = -1; s_red[2] = 0x7fffffff; s_red[3] = -1; }
+    __syncthreads();
+    {
+      const int m0 = __reduce_min_sync(0xffffffffu, wu.bz0), m1 = __reduce_max_sync(0xffffffffu, wu.bz1);
+      const int m2 = __reduce_min_sync(0xffffffffu, wd.bz0), m3 = __reduce_max_sync(0xffffffffu, wd.bz1);
+      if ((tx & 31) == 0) {
+        atomicMin(&s_red[0], m0); atomicMax(&s_red[1], m1);
+        atomicMin(&s_red[2], m2); atomicMax(&s_red[3], m3);
+      }
+    }
+    __syncthreads();
+    const int ulo = s_red[0], uhi = s_red[1], dlo = s_red[2], dhi = s_red[3];
+    const uint32_t ub0 = du.bin_ofs + (uint32_t)ulo * (uint32_t)du.ny;
+    const uint32_t unb = (uint32_t)(uhi - ulo + 1) * (uint32_t)du.ny;
+    const uint32_t db0 = dd.bin_ofs + (uint32_t)dlo * (uint32_t)dd.ny;
+    const uint32_t dnb = (uint32_t)(dhi - dlo + 1) * (uint32_t)dd.ny;
+    const uint32_t cu0 = bin_start[ub0], cu1 = bin_start[ub0 + unb];
+    const uint32_t cd0 = bin_start[db0], cd1 = bin_start[db0 + dnb];
     int32_t bj = -1, bk = -1;
-    if (r >= 1 && r <= R - 2) {
-      const tpc_row_desc du = B.row_desc[sr + 1], dd = B.row_desc[sr - 1];
-      if (du.count && dd.count) {
-        const float2 ci = yz[i];
-        const float yi = ci.x, zi = ci.y;
-        const float ti = yi / K->x[r];
-        const float ty = ti * K->dx_row;
-        const BinWindow wu = make_window(du, K, (yi + ty) - wy, (yi + ty) + wy, zi - wz, zi + wz);
-        const BinWindow wd = make_window(dd, K, (yi - ty) - wy, (yi - ty) + wy, zi - wz, zi + wz);
-        float best = 0.f;
-        uint32_t bjid = 0, bkid = 0;
-        for (int bzu = wu.bz0; bzu <= wu.bz1; ++bzu) {
-          const uint32_t bu = wu.base + (uint32_t)bzu * (uint32_t)wu.ny;
-          const uint32_t ju1 = bin_start[bu + wu.by_span];
-          for (uint32_t j = bin_start[bu]; j < ju1; ++j) {
-            const float2 cj = yz[j];
-            if (!(fabsf((cj.x - yi) - ty) <= wy && fabsf(cj.y - zi) <= wz)) continue;
-            const float dyu = cj.x - yi, dzu = cj.y - zi;
-            uint32_t jid = 0xFFFFFFFFu;  // fetched lazily
-            for (int bzd = wd.bz0; bzd <= wd.bz1; ++bzd) {
-              const uint32_t bd = wd.base + (uint32_t)bzd * (uint32_t)wd.ny;
-              const uint32_t k1 = bin_start[bd + wd.by_span];
-              for (uint32_t k = bin_start[bd]; k < k1; ++k) {
-                const float2 ck = yz[k];
-                if (!(fabsf((yi - ck.x) - ty) <= wy && fabsf(zi - ck.y) <= wz)) continue;
-                const float dy = dyu + (ck.x - yi);
-                const float dz = dzu + (ck.y - zi);
-                const float d2 = dy * dy + dz * dz;
-                if (!(d2 <= max_d2)) continue;
-                bool better = bj < 0 || d2 < best;
-                if (!better && d2 == best) {
-                  if (jid == 0xFFFFFFFFu) jid = orig[j];
-                  const uint32_t kid = orig[k];
-                  better = jid < bjid || (jid == bjid && kid < bkid);
-                }
-                if (better) {
-                  if (jid == 0xFFFFFFFFu) jid = orig[j];
-                  best = d2; bj = (int32_t)j; bk = (int32_t)k; bjid = jid; bkid = orig[k];
-                }
+    const bool staged = unb <= TPC_NF_BINS && dnb <= TPC_NF_BINS && cu1 - cu0 <= TPC_NF_SLAB &&
+                        cd1 - cd0 <= TPC_NF_SLAB;
+    if (!staged) {
+      if (have) nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);
+    } else {
+      for (uint32_t t = tx; t <= unb; t += TPC_NF_TILE) s_bin[0][t] = bin_start[ub0 + t];
+      for (uint32_t t = tx; t <= dnb; t += TPC_NF_TILE) s_bin[1][t] = bin_start[db0 + t];
+      for (uint32_t t = tx; t < cu1 - cu0; t += TPC_NF_TILE) s_yz[0][t] = yz[cu0 + t];
+      for (uint32_t t = tx; t < cd1 - cd0; t += TPC_NF_TILE) s_yz[1][t] = yz[cd0 + t];
+      __syncthreads();
+      if (have && (wu.bz1 - wu.bz0 > 2 || wd.bz1 - wd.bz0 > 2)) {
+        nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);     // bins much smaller than the window
+      } else if (have) {
+        const int nU = nf_collect<true>(wu, ulo, du.bin_ofs, cu0, s_bin[0], s_yz[0], &s_list[0][tx], yi, zi, ty, wy, wz);
+        const int nD = nU ? nf_collect<false>(wd, dlo, dd.bin_ofs, cd0, s_bin[1], s_yz[1], &s_list[1][tx], yi, zi, ty,
+                                              wy, wz)
+                          : 0;
+        if (nU > TPC_NF_LIST || nD > TPC_NF_LIST) {
+          nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);   // rare: crowded windows
+        } else if (nU && nD) {
+          // flat pair loop over the two lists
+          float best = 0.f;
+          int a = 0, b = 0;
+          uint32_t ju = s_list[0][tx];
+          float2 cj = s_yz[0][ju];
+          const int total = nU * nD;
+          for (int t = 0; t < total; ++t) {
+            const uint32_t kd = s_list[1][b * TPC_NF_TILE + tx];
+            const float2 ck = s_yz[1][kd];
+            const float dy = (cj.x - yi) + (ck.x - yi);
+            const float dz = (cj.y - zi) + (ck.y - zi);
+            const float d2 = dy * dy + dz * dz;
+            if (d2 <= max_d2) {
+              bool better = bj < 0 || d2 < best;
+              if (!better && d2 == best) {  // exact tie: rule D2 (rare, ids fetched only here)
+                const uint32_t jid = orig[cu0 + ju], bjid = orig[cu0 + (uint32_t)bj];
+                better = jid < bjid || (jid == bjid && orig[cd0 + kd] < orig[cd0 + (uint32_t)bk]);
               }
+              if (better) { best = d2; bj = (int32_t)ju; bk = (int32_t)kd; }
+            }
+            if (++b == nD) {
+              b = 0;
+              if (++a < nU) { ju = s_list[0][a * TPC_NF_TILE + tx]; cj = s_yz[0][ju]; }
             }
           }
+          if (bj >= 0) { bj += (int32_t)cu0; bk += (int32_t)cd0; }
         }
       }
     }
-    B.link_up[i] = bj;
-    B.link_dn[i] = bk;
+    if (have) { B.link_up[i] = bj; B.link_dn[i] = bk; }
   }
 }
 
@@ -1167,6 +1296,8 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   TPC_LAUNCH_CHECK("k_row_stats");
   k_row_desc<<<1, 1024, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_row_desc");
+  k_tile_rows<<<grid_for((uint64_t)B.n_sr * 128, 128, n_sm, 8), 128, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_tile_rows");
   k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_bins");
   k_bin_hist<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
