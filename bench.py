@@ -48,6 +48,7 @@ WORKLOAD_PARAMS = {
 # HBM kernels: bytes as a function of (N input clusters, Ns clusters in the grid, NB bins,
 # NSD seeds).  k_follow: fp32 flops from the work counters the kernel keeps.
 FLOPS_PROPAGATE, FLOPS_UPDATE, FLOPS_GAIN_ROAD, FLOPS_CAND = 163, 112, 16, 13
+FOLLOW_KERNELS = ("k_follow_up", "k_follow_refit", "k_follow_down")
 
 
 def algorithmic_work(name: str, st: dict):
@@ -70,9 +71,9 @@ def algorithmic_work(name: str, st: dict):
     }
     if name in hbm:
         return "hbm", float(hbm[name])
-    if name == "k_follow":
-        fl = (FLOPS_PROPAGATE * st["follow_steps"] + FLOPS_UPDATE * st["follow_updates"]
-              + FLOPS_GAIN_ROAD * st["follow_steps"] + FLOPS_CAND * st["follow_cands"])
+    if name in FOLLOW_KERNELS:
+        steps, upd, cands = st["follow_work"][FOLLOW_KERNELS.index(name)]
+        fl = (FLOPS_PROPAGATE * steps + FLOPS_UPDATE * upd + FLOPS_GAIN_ROAD * steps + FLOPS_CAND * cands)
         return "alu", float(fl)
     return "hbm", 0.0
 
@@ -338,7 +339,8 @@ def run_ours(args, rank, world, local_rank):
     rc, iv = B.tpc_get_tracks(trk.ctx)
     st = dict(n=n, n_sorted=n - int(v.n_ignored) - int(v.n_dropped), n_bins=int(v.n_bins), n_seeds=int(v.n_seeds),
               n_rows=trk.geom.n_rows, follow_steps=int(v.n_follow_steps), follow_updates=int(v.n_follow_updates),
-              follow_cands=int(v.n_follow_candidates))
+              follow_cands=int(v.n_follow_candidates),
+              follow_work=[[int(v.follow_work[a][b]) for b in range(3)] for a in range(3)])
     per_kernel = []
     for name in order:
         tot, cnt = kernel_ms[name]

@@ -139,6 +139,8 @@ typedef struct tpc_track_view {
   uint64_t n_follow_steps;          /* follower work: one-row propagations ...           */
   uint64_t n_follow_updates;        /* ... Kalman updates ...                            */
   uint64_t n_follow_candidates;     /* ... and chi2 evaluations of road candidates       */
+  uint64_t follow_work[3][3];       /* the same three counters per follower kernel:
+                                       [outward | refit | inward][steps, updates, candidates] */
 } tpc_track_view;
 
 /* One row of the search grid. */

@@ -101,6 +101,8 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.scan_partials = (uint32_t*)take(4 * (size_t)(k.scan_blocks + 2));
   b.seeds = (uint32_t*)take(4 * (size_t)k.max_seeds);
   b.seed_sr = (uint16_t*)take(2 * (size_t)k.max_seeds);
+  b.turn = (uint4*)take(32 * (size_t)k.max_seeds);
+  b.down_list = (uint32_t*)take(4 * (size_t)k.max_seeds);
   b.tracklets = (tpc_tracklet*)take(sizeof(tpc_tracklet) * (size_t)k.max_seeds);
   b.row_hit = (int32_t*)take(4 * (size_t)c->geom.n_rows * k.max_seeds);
   b.owner = (unsigned long long*)take(8 * n);
@@ -279,9 +281,12 @@ int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out) {
   out->n_seeds = c.n_seeds;
   out->n_tracklets = c.n_tracklets;
   out->n_bins = c.n_bins;
-  out->n_follow_steps = c.follow_steps;
-  out->n_follow_updates = c.follow_updates;
-  out->n_follow_candidates = c.follow_cands;
+  for (int a = 0; a < 3; ++a) {
+    out->n_follow_steps += c.follow_work[a][0];
+    out->n_follow_updates += c.follow_work[a][1];
+    out->n_follow_candidates += c.follow_work[a][2];
+    for (int b = 0; b < 3; ++b) out->follow_work[a][b] = c.follow_work[a][b];
+  }
   return rc;
 }
 

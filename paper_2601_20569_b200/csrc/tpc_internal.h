@@ -39,8 +39,10 @@ struct TpcCounters {
   uint32_t n_tracks, n_ids, error, pad_;
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
-  unsigned long long follow_steps, follow_updates, follow_cands;
-  uint32_t follow_next, pad2_;  // next unclaimed seed of the follower's work queue
+  unsigned long long follow_work[3][3];  // [kernel up/refit/down][steps, updates, candidates]
+  // work queues of the three follower kernels (next unclaimed item) and the number of seeds
+  // handed from the refit to the inward extrapolation
+  uint32_t follow_next[3], n_down;
 };
 
 // per (sector,row) statistics of pass 1
@@ -77,6 +79,8 @@ struct TpcBuffers {
   uint32_t* scan_partials;// [scan_blocks+1]
   uint32_t* seeds;        // [max_seeds] sorted index of start hits
   uint16_t* seed_sr;      // [max_seeds] sector*n_rows+row of each start hit
+  uint4* turn;            // [max_seeds][2] state at the outermost hit (y,z,sin phi,tan lambda | q/pT,row,-,-)
+  uint32_t* down_list;    // [max_seeds] seeds whose refit reached the start row (inward extrapolation pending)
   tpc_tracklet* tracklets;// [max_seeds]
   int32_t* row_hit;       // [max_seeds][n_rows]
   unsigned long long* owner;     // [n]

@@ -795,6 +795,10 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 
 // R5.3: best cluster of row sr inside the road around the predicted state: minimum of
 // (chi2, original id).  Returns the sorted index or -1; *m_out = its (y,z).
+// The road is small against the bins, so the window covers one or two z-rows of bins, each a
+// contiguous range of the sorted clusters.  The two ranges are walked as ONE flat sequence in
+// batches of four: the four loads of a batch are issued together, so a search costs one
+// memory round trip for the index and one per batch instead of one per candidate.
 __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcConst* __restrict__ K, uint32_t sr,
                                                 const KF& k, const Gain& g, const FollowConst& F, float* chi2_out,
                                                 float2* m_out, uint32_t& n_cand) {
@@ -816,28 +820,30 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
     if (!better && chi2 == best_chi2) better = B.orig_id[c] < B.orig_id[best];  // rule D2, rare
     if (better) { best = (int32_t)c; best_chi2 = chi2; best_m = m; }
   };
-  // Fast path: the road is small against the bins, so the window covers one or two z-rows of
-  // bins with a few clusters each.  All index loads, then all candidate loads, are issued
-  // together (two memory round trips in total); leftovers take the generic loops below.
   const bool two_rows = w.bz1 > w.bz0;
   const uint32_t bA = w.base + (uint32_t)w.bz0 * (uint32_t)w.ny;
   const uint32_t bB = bA + (uint32_t)w.ny;
   const uint32_t a0 = bin_start[bA], a1 = bin_start[bA + w.by_span];
   uint32_t b0 = 0, b1 = 0;
   if (two_rows) { b0 = bin_start[bB]; b1 = bin_start[bB + w.by_span]; }
-  const bool ha0 = a0 < a1, ha1 = a0 + 1 < a1, hb0 = b0 < b1, hb1 = b0 + 1 < b1;
-  float2 ma0 = best_m, ma1 = best_m, mb0 = best_m, mb1 = best_m;
-  if (ha0) ma0 = yz[a0];
-  if (ha1) ma1 = yz[a0 + 1];
-  if (hb0) mb0 = yz[b0];
-  if (hb1) mb1 = yz[b0 + 1];
-  if (ha0) eval(a0, ma0);
-  if (ha1) eval(a0 + 1, ma1);
-  if (hb0) eval(b0, mb0);
-  if (hb1) eval(b0 + 1, mb1);
-  for (uint32_t c = a0 + 2; c < a1; ++c) eval(c, yz[c]);
-  for (uint32_t c = b0 + 2; c < b1; ++c) eval(c, yz[c]);
-  for (int bz = w.bz0 + 2; bz <= w.bz1; ++bz) {
+  const uint32_t la = a1 - a0, total = la + (b1 - b0), ob = b0 - la;
+  for (uint32_t t = 0; t < total; t += 4) {
+    const uint32_t c0 = t + (t < la ? a0 : ob);
+    const uint32_t c1 = (t + 1) + (t + 1 < la ? a0 : ob);
+    const uint32_t c2 = (t + 2) + (t + 2 < la ? a0 : ob);
+    const uint32_t c3 = (t + 3) + (t + 3 < la ? a0 : ob);
+    const bool h1 = t + 1 < total, h2 = t + 2 < total, h3 = t + 3 < total;
+    float2 m0, m1 = best_m, m2 = best_m, m3 = best_m;
+    m0 = yz[c0];
+    if (h1) m1 = yz[c1];
+    if (h2) m2 = yz[c2];
+    if (h3) m3 = yz[c3];
+    eval(c0, m0);
+    if (h1) eval(c1, m1);
+    if (h2) eval(c2, m2);
+    if (h3) eval(c3, m3);
+  }
+  for (int bz = w.bz0 + 2; bz <= w.bz1; ++bz) {  // roads taller than two bins (small grid_dz)
     const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
     const uint32_t c1 = bin_start[b + w.by_span];
     for (uint32_t c = bin_start[b]; c < c1; ++c) eval(c, yz[c]);
@@ -847,22 +853,71 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
   return best;
 }
 
-// The follower is written as ONE uniform loop per thread ("one row step per iteration") so
-// that all lanes of a warp execute the same instructions whatever part of R5 their seed is
-// in; a lane whose seed is finished fetches the next seed at once (seeds are claimed in
-// chunks from a global counter).  Loads are software-pipelined one row ahead: the chain /
-// recorded hit of the next row and, during extrapolation, the bin of the predicted next-row
-// position are requested while the current row is computed.  The arithmetic per seed, and
-// its order, are exactly those of R5.1-R5.7, so neither the assignment of seeds to lanes
-// nor the prefetching changes a result.
-enum FollowPhase { PH_CHAIN = 0, PH_UP = 1, PH_REFIT = 2, PH_DOWN = 3, PH_IDLE = 4 };
-
+// ------------------------------------------------------------------ follower kernels
+// R5 runs as THREE kernels, one per part of the procedure, so that the lanes of a warp are in
+// the same part (a lane searching a road next to lanes that only refit recorded hits would
+// leave those idle during the search and vice versa):
+//   k_follow_up    R5.1 init, R5.2 chain fit, R5.3 outward extrapolation -> row_hit, turn state
+//   k_follow_refit R5.4 turn, R5.5 inward refit through the recorded hits -> tracklet, or
+//                  hand-over (state in the tracklet record) when the start row is reached
+//   k_follow_down  R5.6 inward extrapolation below the start row, R5.7 output
+// Each is ONE uniform loop per thread ("one row step per iteration"); a lane whose seed is
+// finished claims the next one at once (chunks from a global counter).  Loads are software-
+// pipelined one row ahead.  The arithmetic per seed, and its order, are exactly those of
+// R5.1-R5.7, so neither the assignment of seeds to lanes nor the split changes a result.
 #define TPC_FOLLOW_BLOCK 128
 #define TPC_FOLLOW_CHUNK 64
-#ifndef TPC_FOLLOW_MINBLOCKS
-#define TPC_FOLLOW_MINBLOCKS 6   // resident CTAs per SM the register budget is sized for
-#endif
 #define TPC_NO_BIN 0xFFFFFFFFu
+#define TPC_TL_PENDING 1u   // tracklet.pad_: handed from the refit to the inward extrapolation
+
+// Claim work items for the idle lanes of a warp (need = this lane is idle).  Returns true
+// and the item index if this lane got one.  chunk_next / chunk_end / exhausted are
+// warp-uniform.
+__device__ __forceinline__ bool queue_claim(uint32_t* counter, uint32_t n_items, int lane, bool need,
+                                            uint32_t& chunk_next, uint32_t& chunk_end, bool& exhausted,
+                                            uint32_t& item) {
+  bool got = false;
+  while (!exhausted) {
+    const unsigned want = __ballot_sync(0xffffffffu, need && !got);
+    if (!want) break;
+    if (chunk_next >= chunk_end) {
+      uint32_t base = 0;
+      if (lane == 0) base = atomicAdd(counter, (uint32_t)TPC_FOLLOW_CHUNK);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (base >= n_items) { exhausted = true; break; }
+      chunk_next = base;
+      chunk_end = min(base + (uint32_t)TPC_FOLLOW_CHUNK, n_items);
+    }
+    const uint32_t rank = (uint32_t)__popc(want & ((1u << lane) - 1u));
+    const uint32_t avail = chunk_end - chunk_next;
+    if (need && !got && rank < avail) { item = chunk_next + rank; got = true; }
+    chunk_next += min((uint32_t)__popc(want), avail);
+  }
+  return got;
+}
+
+__device__ __forceinline__ FollowConst follow_const(const TpcConst* __restrict__ K) {
+  FollowConst F;
+  F.dx = K->dx_row; F.cfield = K->cfield; F.max_sinphi = K->P.max_sinphi; F.max_qpt = K->P.max_qpt;
+  F.vy = K->vy; F.vz = K->vz;
+  F.road_nsigma = K->P.road_nsigma; F.road_min = K->P.road_min; F.road_max = K->P.road_max;
+  F.chi2_max = K->P.chi2_max_hit;
+  F.ivs = K->P.init_var_sinphi; F.ivt = K->P.init_var_tanl; F.ivq = K->P.init_var_qpt;
+  F.max_gap = K->P.max_gap_follow; F.min_hits = K->P.min_hits_tracklet; F.R = K->n_rows;
+  return F;
+}
+
+__device__ __forceinline__ void follow_count_work(const TpcBuffers& B, int which, int lane, uint32_t w_step,
+                                                  uint32_t w_upd, uint32_t w_cand) {
+  w_step = __reduce_add_sync(0xffffffffu, w_step);
+  w_cand = __reduce_add_sync(0xffffffffu, w_cand);
+  w_upd = __reduce_add_sync(0xffffffffu, w_upd);
+  if (lane == 0 && w_step) {
+    atomicAdd(&B.cnt->follow_work[which][0], (unsigned long long)w_step);
+    atomicAdd(&B.cnt->follow_work[which][1], (unsigned long long)w_upd);
+    atomicAdd(&B.cnt->follow_work[which][2], (unsigned long long)w_cand);
+  }
+}
 
 #define TPC_SAVE_KIN()                                                                                         \
   do {                                                                                                         \
@@ -873,115 +928,115 @@ enum FollowPhase { PH_CHAIN = 0, PH_UP = 1, PH_REFIT = 2, PH_DOWN = 3, PH_IDLE =
     s_kin[17][tx] = k.c42; s_kin[18][tx] = k.c43; s_kin[19][tx] = k.c44;                                       \
   } while (0)
 
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_MINBLOCKS) k_follow(TpcBuffers B) {
+// R5.7: write the tracklet of seed sd from the state saved at its innermost accepted hit.
+// pending: the record is a hand-over to k_follow_down (n_hits is then the raw count).
+__device__ __forceinline__ void write_tracklet(const TpcBuffers& B, uint32_t sd, const float (*s_kin)[TPC_FOLLOW_BLOCK],
+                                               int tx, float x, float chi2, int nh, int r_in, int r_out, uint32_t start,
+                                               uint32_t sector, int min_hits, bool pending) {
+  tpc_tracklet t;
+  t.x = x;
+#pragma unroll
+  for (int i = 0; i < 5; ++i) t.p[i] = s_kin[i][tx];
+#pragma unroll
+  for (int i = 0; i < 15; ++i) t.c[i] = s_kin[5 + i][tx];
+  t.chi2 = chi2;
+  t.seed_sorted = start;
+  t.seed_id = B.orig_id[start];
+  const bool keep = nh >= min_hits;
+  t.n_hits = (pending || keep) ? (int16_t)nh : (int16_t)0;
+  t.row_first = (uint8_t)r_in;
+  t.row_last = (uint8_t)r_out;
+  t.sector = (uint8_t)sector;
+  t.seed_len = B.seed_len[start];
+  t.pad_ = pending ? (uint16_t)TPC_TL_PENDING : (uint16_t)0;
+  t.pad2_[0] = 0; t.pad2_[1] = 0;
+  B.tracklets[sd] = t;
+  if (!pending && keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+}
+
+#ifndef TPC_FOLLOW_UP_MINBLOCKS
+#define TPC_FOLLOW_UP_MINBLOCKS 6   // resident CTAs per SM the register budget is sized for
+#endif
+#ifndef TPC_FOLLOW_REFIT_MINBLOCKS
+#define TPC_FOLLOW_REFIT_MINBLOCKS 8
+#endif
+
+// ---- R5.1-R5.3: init, chain fit, outward extrapolation
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_up(TpcBuffers B) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
-  __shared__ float s_x[TPC_MAX_ROWS];
-  __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];  // state at the innermost accepted hit (R5.7)
   const TpcConst* __restrict__ K = B.K;
-  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) { s_ylim[r] = K->ylim[r]; s_x[r] = K->x[r]; }
+  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_ylim[r] = K->ylim[r];
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
-  FollowConst F;
-  F.dx = K->dx_row; F.cfield = K->cfield; F.max_sinphi = K->P.max_sinphi; F.max_qpt = K->P.max_qpt;
-  F.vy = K->vy; F.vz = K->vz;
-  F.road_nsigma = K->P.road_nsigma; F.road_min = K->P.road_min; F.road_max = K->P.road_max;
-  F.chi2_max = K->P.chi2_max_hit;
-  F.ivs = K->P.init_var_sinphi; F.ivt = K->P.init_var_tanl; F.ivq = K->P.init_var_qpt;
-  F.max_gap = K->P.max_gap_follow; F.min_hits = K->P.min_hits_tracklet; F.R = K->n_rows;
+  const FollowConst F = follow_const(K);
   const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const int32_t* __restrict__ up2 = B.link_up2;
   const float2* __restrict__ yz = B.yz;
   const uint32_t* __restrict__ bin_start = B.bin_start;
   const int lane = threadIdx.x & 31;
-  const int tx = threadIdx.x;
   uint32_t w_step = 0, w_cand = 0, w_upd = 0;  // work counters (diagnostics only)
-
-  // warp-uniform: the chunk of seeds this warp currently draws from
-  uint32_t chunk_next = 0, chunk_end = 0;
+  uint32_t chunk_next = 0, chunk_end = 0;      // warp-uniform: the chunk of seeds this warp draws from
   bool exhausted = false;
 
-  // per-lane state of the seed being followed
+  enum { PH_CHAIN = 0, PH_UP = 1, PH_IDLE = 2 };
   int phase = PH_IDLE;
   KF k;
   k.y = k.z = k.s = k.t = k.q = 0.f;
   kf_init_cov(k, F);
-  uint32_t sd = 0, start = 0, sr_base = 0;
+  uint32_t sd = 0, sr_base = 0;
   int32_t* __restrict__ hit_row = B.row_hit;  // this seed's row -> sorted index table
-  int r = 0, r0 = 0, r_out = 0, r_in = 0, gap = 0, nh = 0;
-  float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, snap_y = 0.f, snap_z = 0.f, chi2 = 0.f;
-  // load pipeline: the hit of the coming row (chain fit / refit) and the one after it
-  int32_t c_cur = -1, c_nxt = -1;
+  int r = 0, r_out = 0, gap = 0;
+  float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, snap_y = 0.f, snap_z = 0.f;
+  int32_t c_cur = -1, c_nxt = -1;   // chain hit of the coming row and the one after it
   float2 m_cur = make_float2(0.f, 0.f);
-  uint32_t pb = TPC_NO_BIN;  // extrapolation: first cluster of the predicted bin on the coming row
+  uint32_t pb = TPC_NO_BIN;         // first cluster of the predicted bin on the coming row
 
   for (;;) {
-    // ---------------------------------------------------------------- refill idle lanes
-    const unsigned idle = __ballot_sync(0xffffffffu, phase == PH_IDLE);
-    if (idle) {
-      bool need = phase == PH_IDLE;
-      while (!exhausted) {
-        const unsigned want = __ballot_sync(0xffffffffu, need);
-        if (!want) break;
-        if (chunk_next >= chunk_end) {
-          uint32_t base = 0;
-          if (lane == 0) base = atomicAdd(&B.cnt->follow_next, (uint32_t)TPC_FOLLOW_CHUNK);
-          base = __shfl_sync(0xffffffffu, base, 0);
-          if (base >= n_seeds) { exhausted = true; break; }
-          chunk_next = base;
-          chunk_end = min(base + (uint32_t)TPC_FOLLOW_CHUNK, n_seeds);
-        }
-        const uint32_t rank = (uint32_t)__popc(want & ((1u << lane) - 1u));
-        const uint32_t avail = chunk_end - chunk_next;
-        if (need && rank < avail) {
-          sd = chunk_next + rank;
-          need = false;
-          // ---- R5.1 init from the first two chain clusters
-          start = B.seeds[sd];
-          const uint32_t sr0 = B.seed_sr[sd];
-          r0 = (int)(sr0 % (uint32_t)F.R);
-          sr_base = sr0 - (uint32_t)r0;
-          hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
-          const int32_t c1 = up2[start];
-          const float2 m0 = yz[start];
-          const float2 m1 = yz[c1];
-          c_nxt = up2[c1];
-          const float dy = m1.x - m0.x;
-          const float dl = sqrtf(F.dx * F.dx + dy * dy);
-          k.y = m0.x; k.z = m0.y;
-          k.s = dy / dl;
-          k.t = (m1.y - m0.y) / dl;
-          k.q = 0.f;
-          kf_init_cov(k, F);
-          hit_row[r0] = (int32_t)start;
-          r = r0; r_out = r0; r_in = r0;
-          snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m0.x; snap_z = m0.y;
-          nh = 0; chi2 = 0.f; gap = 0;
-          c_cur = c1; m_cur = m1;
-          pb = TPC_NO_BIN;
-          phase = PH_CHAIN;
-        }
-        const uint32_t taken = min((uint32_t)__popc(want), avail);
-        chunk_next += taken;
+    if (__ballot_sync(0xffffffffu, phase == PH_IDLE)) {
+      uint32_t item = 0;
+      if (queue_claim(&B.cnt->follow_next[0], n_seeds, lane, phase == PH_IDLE, chunk_next, chunk_end, exhausted,
+                      item)) {
+        // ---- R5.1 init from the first two chain clusters
+        sd = item;
+        const uint32_t start = B.seeds[sd];
+        const uint32_t sr0 = B.seed_sr[sd];
+        const int r0 = (int)(sr0 % (uint32_t)F.R);
+        sr_base = sr0 - (uint32_t)r0;
+        hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
+        const int32_t c1 = up2[start];
+        const float2 m0 = yz[start];
+        const float2 m1 = yz[c1];
+        c_nxt = up2[c1];
+        const float dy = m1.x - m0.x;
+        const float dl = sqrtf(F.dx * F.dx + dy * dy);
+        k.y = m0.x; k.z = m0.y;
+        k.s = dy / dl;
+        k.t = (m1.y - m0.y) / dl;
+        k.q = 0.f;
+        kf_init_cov(k, F);
+        hit_row[r0] = (int32_t)start;
+        r = r0; r_out = r0;
+        snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m0.x; snap_z = m0.y;
+        gap = 0;
+        c_cur = c1; m_cur = m1;
+        pb = TPC_NO_BIN;
+        phase = PH_CHAIN;
       }
       if (__all_sync(0xffffffffu, phase == PH_IDLE)) break;  // nothing left for this warp
     }
-
-    // ---------------------------------------------------------------- one row step
     if (phase != PH_IDLE) {
-      const bool extrap = (phase == PH_UP) || (phase == PH_DOWN);
-      const int dir = (phase <= PH_UP) ? 1 : -1;
-      const int rn = r + dir;
-      bool fin = false;    // this direction ends here
-      bool stop = false;   // ... because the leg left the |sin phi| range
+      const bool extrap = phase == PH_UP;
+      const int rn = r + 1;
+      bool fin = false;
       if (extrap && pb != TPC_NO_BIN) prefetch_l1(yz + pb);
-      if (rn < 0 || rn >= F.R) {
-        fin = true;        // only an extrapolation can run off the pad plane
+      if (rn >= F.R) {
+        fin = true;  // ran off the pad plane
       } else {
         ++w_step;
         const float y_prev = k.y, z_prev = k.z;
-        if (!kf_propagate(k, dir > 0 ? F.dx : -F.dx, F)) {
-          fin = true; stop = true;
+        if (!kf_propagate(k, F.dx, F)) {
+          fin = true;  // the leg left the |sin phi| range
         } else {
           r = rn;
           // ---- request the next row's data while this row is computed
@@ -989,45 +1044,34 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_MINBLOCKS) k_foll
           float2 m_nxt = make_float2(0.f, 0.f);
           if (extrap) {
             pb = TPC_NO_BIN;
-            const int rp = r + dir;
-            if (rp >= 0 && rp < F.R) {
-              const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)rp);
+            if (r + 1 < F.R) {
+              const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)(r + 1));
               if (dn.count) {  // linear continuation of this step
                 const int by = bin_coord(k.y + (k.y - y_prev), dn.y0, inv_dy, dn.ny);
                 const int bz = bin_coord(k.z + (k.z - z_prev), dn.z0, inv_dz, dn.nz);
                 pb = bin_start[dn.bin_ofs + (uint32_t)bz * (uint32_t)dn.ny + (uint32_t)by];
               }
             }
-          } else {
-            if (c_nxt >= 0) m_nxt = yz[c_nxt];
-            if (phase == PH_CHAIN) { if (c_nxt >= 0) c_nxt2 = up2[c_nxt]; }
-            else if (r - 2 >= r0) c_nxt2 = hit_row[r - 2];
+          } else if (c_nxt >= 0) {
+            m_nxt = yz[c_nxt];
+            c_nxt2 = up2[c_nxt];
           }
           const Gain g = kf_gain(k, F);
           int32_t c = -1;
           float chi2h = 0.f;
           float2 m = m_cur;
           if (!extrap) {
-            c = c_cur;                                    // R5.2 (no chi2 cut) / R5.5 (recorded hit or hole)
-          } else if (fabsf(k.y) <= s_ylim[r]) {           // R5.3 / R5.6: road search
+            c = c_cur;                                    // R5.2: chain hit, no chi2 cut
+          } else if (fabsf(k.y) <= s_ylim[r]) {           // R5.3: road search
             c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2h, &m, w_cand);
             if (!(c >= 0 && chi2h <= F.chi2_max)) c = -1;
           }
           if (c >= 0) {
-            if (phase == PH_REFIT) chi2h = kf_chi2(k, g, m.x, m.y);
-            stop = kf_update(k, g, m.x, m.y, F);
+            const bool stop = kf_update(k, g, m.x, m.y, F);
             ++w_upd;
-            if (phase <= PH_UP) {                         // outward: record, remember the turn state
-              hit_row[r] = c;
-              r_out = r;
-              snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m.x; snap_z = m.y;
-            } else {                                      // inward: accumulate chi2, remember the state
-              if (phase == PH_DOWN) hit_row[r] = c;
-              chi2 = chi2 + chi2h;
-              ++nh;
-              r_in = r;
-              TPC_SAVE_KIN();
-            }
+            hit_row[r] = c;
+            r_out = r;
+            snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m.x; snap_z = m.y;
             gap = 0;
             if (stop) fin = true;
           } else if (extrap) {
@@ -1038,58 +1082,225 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_MINBLOCKS) k_foll
           if (!extrap) { c_cur = c_nxt; m_cur = m_nxt; c_nxt = c_nxt2; }
         }
       }
-      // ---- phase transitions
-      if (phase == PH_CHAIN && !fin && c_cur < 0) { phase = PH_UP; gap = 0; pb = TPC_NO_BIN; }  // chain fitted
-      else if (phase == PH_REFIT && !fin && r == r0) { phase = PH_DOWN; gap = 0; pb = TPC_NO_BIN; }  // refit done
-      else if (fin && phase <= PH_UP) {
-        // R5.4 turn at the outermost accepted hit
-        k.y = snap_y; k.z = snap_z;
-        k.s = snap_s; k.t = snap_t; k.q = snap_q;
-        kf_init_cov(k, F);
-        chi2 = 0.f; nh = 1; r_in = r_out; r = r_out; gap = 0;
-        TPC_SAVE_KIN();
-        pb = TPC_NO_BIN;
-        if (r_out > r0) {
-          phase = PH_REFIT;
-          c_cur = hit_row[r_out - 1];
-          c_nxt = (r_out - 2 >= r0) ? hit_row[r_out - 2] : -1;
-          if (c_cur >= 0) m_cur = yz[c_cur];
-        } else {
-          phase = PH_DOWN;
-        }
-      } else if (fin) {
-        // R5.7 output (hits below r_in of a refit that ended early are outside
-        // [row_first,row_last] and thereby not part of the tracklet)
-        tpc_tracklet t;
-        t.x = s_x[r_in];
-#pragma unroll
-        for (int i = 0; i < 5; ++i) t.p[i] = s_kin[i][tx];
-#pragma unroll
-        for (int i = 0; i < 15; ++i) t.c[i] = s_kin[5 + i][tx];
-        t.chi2 = chi2;
-        t.seed_sorted = start;
-        t.seed_id = B.orig_id[start];
-        const bool keep = nh >= F.min_hits;
-        t.n_hits = keep ? (int16_t)nh : (int16_t)0;
-        t.row_first = (uint8_t)r_in;
-        t.row_last = (uint8_t)r_out;
-        t.sector = (uint8_t)(sr_base / (uint32_t)F.R);
-        t.seed_len = B.seed_len[start];
-        t.pad_ = 0; t.pad2_[0] = 0; t.pad2_[1] = 0;
-        B.tracklets[sd] = t;
-        if (keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+      if (fin) {
+        // state for R5.4 (turn at the outermost accepted hit)
+        B.turn[2 * (size_t)sd] = make_uint4(__float_as_uint(snap_y), __float_as_uint(snap_z), __float_as_uint(snap_s),
+                                            __float_as_uint(snap_t));
+        B.turn[2 * (size_t)sd + 1] = make_uint4(__float_as_uint(snap_q), (uint32_t)r_out, 0u, 0u);
         phase = PH_IDLE;
+      } else if (phase == PH_CHAIN && c_cur < 0) {
+        phase = PH_UP; gap = 0; pb = TPC_NO_BIN;  // chain fitted
       }
     }
   }
-  w_step = __reduce_add_sync(0xffffffffu, w_step);
-  w_cand = __reduce_add_sync(0xffffffffu, w_cand);
-  w_upd = __reduce_add_sync(0xffffffffu, w_upd);
-  if (lane == 0 && w_step) {
-    atomicAdd(&B.cnt->follow_steps, (unsigned long long)w_step);
-    atomicAdd(&B.cnt->follow_updates, (unsigned long long)w_upd);
-    atomicAdd(&B.cnt->follow_cands, (unsigned long long)w_cand);
+  follow_count_work(B, 0, lane, w_step, w_upd, w_cand);
+}
+
+// ---- R5.4-R5.5: turn at the outermost accepted hit, refit inward through the recorded hits
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) k_follow_refit(TpcBuffers B) {
+  __shared__ float s_x[TPC_MAX_ROWS];
+  __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];  // state at the innermost accepted hit (R5.7)
+  const TpcConst* __restrict__ K = B.K;
+  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_x[r] = K->x[r];
+  __syncthreads();
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const FollowConst F = follow_const(K);
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const float2* __restrict__ yz = B.yz;
+  const int lane = threadIdx.x & 31;
+  const int tx = threadIdx.x;
+  uint32_t w_step = 0, w_upd = 0;
+  uint32_t chunk_next = 0, chunk_end = 0;
+  bool exhausted = false;
+
+  bool active = false;
+  KF k;
+  k.y = k.z = k.s = k.t = k.q = 0.f;
+  kf_init_cov(k, F);
+  uint32_t sd = 0, start = 0, sector = 0;
+  const int32_t* __restrict__ hit_row = B.row_hit;
+  int r = 0, r0 = 0, r_out = 0, r_in = 0, nh = 0;
+  float chi2 = 0.f;
+  int32_t c_cur = -1, c_nxt = -1;   // recorded hit of the coming row and of the one after it
+  float2 m_cur = make_float2(0.f, 0.f);
+
+  for (;;) {
+    if (__ballot_sync(0xffffffffu, !active)) {
+      uint32_t item = 0;
+      if (queue_claim(&B.cnt->follow_next[1], n_seeds, lane, !active, chunk_next, chunk_end, exhausted, item)) {
+        // ---- R5.4 turn: (y,z) of the outermost hit, (s,t,q) as they were after its update,
+        // covariance back to the initial diagonal
+        sd = item;
+        start = B.seeds[sd];
+        const uint32_t sr0 = B.seed_sr[sd];
+        r0 = (int)(sr0 % (uint32_t)F.R);
+        sector = sr0 / (uint32_t)F.R;
+        hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
+        const uint4 t0 = B.turn[2 * (size_t)sd], t1 = B.turn[2 * (size_t)sd + 1];
+        k.y = __uint_as_float(t0.x); k.z = __uint_as_float(t0.y);
+        k.s = __uint_as_float(t0.z); k.t = __uint_as_float(t0.w); k.q = __uint_as_float(t1.x);
+        r_out = (int)t1.y;
+        kf_init_cov(k, F);
+        chi2 = 0.f; nh = 1; r_in = r_out; r = r_out;
+        TPC_SAVE_KIN();
+        c_cur = -1; c_nxt = -1;
+        if (r_out > r0) {
+          c_cur = hit_row[r_out - 1];
+          c_nxt = (r_out - 2 >= r0) ? hit_row[r_out - 2] : -1;
+          if (c_cur >= 0) m_cur = yz[c_cur];
+        }
+        active = true;
+      }
+      if (__all_sync(0xffffffffu, !active)) break;
+    }
+    if (active) {
+      bool fin = false;      // the leg ended inside the refit: the tracklet is complete
+      if (r > r0) {
+        ++w_step;
+        if (!kf_propagate(k, -F.dx, F)) {
+          fin = true;
+        } else {
+          --r;
+          int32_t c_nxt2 = -1;
+          float2 m_nxt = make_float2(0.f, 0.f);
+          if (c_nxt >= 0) m_nxt = yz[c_nxt];
+          if (r - 2 >= r0) c_nxt2 = hit_row[r - 2];
+          if (c_cur >= 0) {     // R5.5: recorded hit (rows without one are pure propagation)
+            const Gain g = kf_gain(k, F);
+            const float chi2h = kf_chi2(k, g, m_cur.x, m_cur.y);
+            const bool stop = kf_update(k, g, m_cur.x, m_cur.y, F);
+            ++w_upd;
+            chi2 = chi2 + chi2h;
+            ++nh;
+            r_in = r;
+            TPC_SAVE_KIN();
+            if (stop) fin = true;
+          }
+          c_cur = c_nxt; m_cur = m_nxt; c_nxt = c_nxt2;
+        }
+      }
+      if (fin) {
+        // (hits below r_in are outside [row_first,row_last] and thereby not part of the tracklet)
+        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, false);
+        active = false;
+      } else if (r == r0) {
+        // the start row is reached (its hit is always present, so the saved state is the live one)
+        const bool pending = r0 > 0;   // rows below to extrapolate into
+        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, pending);
+        if (pending) B.down_list[atomicAdd(&B.cnt->n_down, 1u)] = sd;
+        active = false;
+      }
+    }
   }
+  follow_count_work(B, 1, lane, w_step, w_upd, 0u);
+}
+
+// ---- R5.6-R5.7: inward extrapolation below the start row, output
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_down(TpcBuffers B) {
+  __shared__ float s_ylim[TPC_MAX_ROWS];
+  __shared__ float s_x[TPC_MAX_ROWS];
+  __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];
+  const TpcConst* __restrict__ K = B.K;
+  for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) { s_ylim[r] = K->ylim[r]; s_x[r] = K->x[r]; }
+  __syncthreads();
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const FollowConst F = follow_const(K);
+  const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
+  const uint32_t n_down = B.cnt->n_down;
+  const float2* __restrict__ yz = B.yz;
+  const uint32_t* __restrict__ bin_start = B.bin_start;
+  const int lane = threadIdx.x & 31;
+  const int tx = threadIdx.x;
+  uint32_t w_step = 0, w_cand = 0, w_upd = 0;
+  uint32_t chunk_next = 0, chunk_end = 0;
+  bool exhausted = false;
+
+  bool active = false;
+  KF k;
+  k.y = k.z = k.s = k.t = k.q = 0.f;
+  kf_init_cov(k, F);
+  uint32_t sd = 0, start = 0, sr_base = 0;
+  int32_t* __restrict__ hit_row = B.row_hit;
+  int r = 0, r_out = 0, r_in = 0, gap = 0, nh = 0;
+  float chi2 = 0.f;
+  uint32_t pb = TPC_NO_BIN;
+
+  for (;;) {
+    if (__ballot_sync(0xffffffffu, !active)) {
+      uint32_t item = 0;
+      if (queue_claim(&B.cnt->follow_next[2], n_down, lane, !active, chunk_next, chunk_end, exhausted, item)) {
+        sd = B.down_list[item];
+        const tpc_tracklet* __restrict__ t = B.tracklets + sd;
+        k.y = t->p[0]; k.z = t->p[1]; k.s = t->p[2]; k.t = t->p[3]; k.q = t->p[4];
+        k.c00 = t->c[0]; k.c10 = t->c[1]; k.c11 = t->c[2]; k.c20 = t->c[3]; k.c21 = t->c[4]; k.c22 = t->c[5];
+        k.c30 = t->c[6]; k.c31 = t->c[7]; k.c32 = t->c[8]; k.c33 = t->c[9];
+        k.c40 = t->c[10]; k.c41 = t->c[11]; k.c42 = t->c[12]; k.c43 = t->c[13]; k.c44 = t->c[14];
+        chi2 = t->chi2; nh = t->n_hits; start = t->seed_sorted;
+        r = r_in = t->row_first; r_out = t->row_last;
+        sr_base = (uint32_t)t->sector * (uint32_t)F.R;
+        hit_row = B.row_hit + (size_t)sd * (size_t)F.R;
+        TPC_SAVE_KIN();
+        gap = 0;
+        pb = TPC_NO_BIN;
+        active = true;
+      }
+      if (__all_sync(0xffffffffu, !active)) break;
+    }
+    if (active) {
+      const int rn = r - 1;
+      bool fin = false;
+      if (pb != TPC_NO_BIN) prefetch_l1(yz + pb);
+      if (rn < 0) {
+        fin = true;
+      } else {
+        ++w_step;
+        const float y_prev = k.y, z_prev = k.z;
+        if (!kf_propagate(k, -F.dx, F)) {
+          fin = true;
+        } else {
+          r = rn;
+          pb = TPC_NO_BIN;
+          if (r - 1 >= 0) {
+            const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)(r - 1));
+            if (dn.count) {
+              const int by = bin_coord(k.y + (k.y - y_prev), dn.y0, inv_dy, dn.ny);
+              const int bz = bin_coord(k.z + (k.z - z_prev), dn.z0, inv_dz, dn.nz);
+              pb = bin_start[dn.bin_ofs + (uint32_t)bz * (uint32_t)dn.ny + (uint32_t)by];
+            }
+          }
+          int32_t c = -1;
+          float chi2h = 0.f;
+          float2 m = make_float2(0.f, 0.f);
+          const Gain g = kf_gain(k, F);
+          if (fabsf(k.y) <= s_ylim[r]) {                  // R5.6: road search
+            c = pick_cluster(B, K, sr_base + (uint32_t)r, k, g, F, &chi2h, &m, w_cand);
+            if (!(c >= 0 && chi2h <= F.chi2_max)) c = -1;
+          }
+          if (c >= 0) {
+            const bool stop = kf_update(k, g, m.x, m.y, F);
+            ++w_upd;
+            hit_row[r] = c;
+            chi2 = chi2 + chi2h;
+            ++nh;
+            r_in = r;
+            TPC_SAVE_KIN();
+            gap = 0;
+            if (stop) fin = true;
+          } else {
+            hit_row[r] = -1;
+            ++gap;
+            if (gap > F.max_gap) fin = true;
+          }
+        }
+      }
+      if (fin) {
+        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sr_base / (uint32_t)F.R, F.min_hits,
+                       false);
+        active = false;
+      }
+    }
+  }
+  follow_count_work(B, 2, lane, w_step, w_upd, w_cand);
 }
 
 // ================================================================== K5 ambiguity solving
@@ -1259,8 +1470,9 @@ __global__ void k_init(TpcBuffers B) {
     c.n_sorted = c.n_ignored = c.n_dropped = c.n_bad = 0;
     c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
     c.n_tracks = c.n_ids = c.error = c.pad_ = 0;
-    c.follow_steps = c.follow_updates = c.follow_cands = 0ull;
-    c.follow_next = 0u; c.pad2_ = 0u;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) c.follow_work[a][b] = 0ull;
+    c.follow_next[0] = c.follow_next[1] = c.follow_next[2] = 0u; c.n_down = 0u;
     *B.cnt = c;
   }
 }
@@ -1327,8 +1539,12 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
-  k_follow<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
-  TPC_LAUNCH_CHECK("k_follow");
+  k_follow_up<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_follow_up");
+  k_follow_refit<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_REFIT_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_follow_refit");
+  k_follow_down<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_follow_down");
   if (timers) cudaEventRecord(E.ev[4], st);
   // ---- K5 ambiguity solving
   k_zero_owner<<<grid_for(B.n / 2 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
