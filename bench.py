@@ -53,6 +53,8 @@ FOLLOW_KERNELS = ("k_follow_up", "k_follow_refit", "k_follow_down")
 
 def algorithmic_work(name: str, st: dict):
     N, Ns, NB, NSD, R = st["n"], st["n_sorted"], st["n_bins"], st["n_seeds"], st["n_rows"]
+    H = st["follow_work"][0][1] + st["follow_work"][2][1] + NSD   # hits recorded in row_hit
+    W, NT, NI = (R + 31) // 32, st["n_tracks"], st["n_ids"]
     hbm = {
         "k_row_stats": 16 * N,
         "k_zero_bins": 4 * NB,
@@ -65,9 +67,11 @@ def algorithmic_work(name: str, st: dict):
         "k_seed_flags": 8 * Ns + 1 * Ns,
         "k_seed_write": 1 * Ns + 4 * NSD,
         "k_zero_owner": 8 * Ns,
-        "k_sel_owner": 112 * NSD + 12 * st["follow_updates"] // 2,
-        "k_sel_count": 12 * st["follow_updates"] // 2,
-        "k_sel_emit": 12 * st["follow_updates"] // 2,
+        "k_sel_owner": 32 * NSD + 12 * H,                # tracklet head, row_hit in, 8-byte atomic
+        "k_sel_masks": 40 * NSD + 12 * H + 8 * W * NSD,  # key+head, row_hit + owner gather in, masks out
+        "k_sel_count": 8 * W * NSD + 8 * NSD,            # masks in, counts out
+        "k_sel_emit": 8 * NSD + (8 * W + 112 + 108 + 8 * W + 4) * NT,
+        "k_sel_ids": (8 * W + 16) * NT + 13 * NI,        # masks, row_hit + orig_id gather in, ids + flags out
     }
     if name in hbm:
         return "hbm", float(hbm[name])
@@ -339,7 +343,7 @@ def run_ours(args, rank, world, local_rank):
     rc, iv = B.tpc_get_tracks(trk.ctx)
     st = dict(n=n, n_sorted=n - int(v.n_ignored) - int(v.n_dropped), n_bins=int(v.n_bins), n_seeds=int(v.n_seeds),
               n_rows=trk.geom.n_rows, follow_steps=int(v.n_follow_steps), follow_updates=int(v.n_follow_updates),
-              follow_cands=int(v.n_follow_candidates),
+              follow_cands=int(v.n_follow_candidates), n_tracks=int(v.n_tracks), n_ids=int(v.n_cluster_ids),
               follow_work=[[int(v.follow_work[a][b]) for b in range(3)] for a in range(3)])
     per_kernel = []
     for name in order:

@@ -107,6 +107,9 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.row_hit = (int32_t*)take(4 * (size_t)c->geom.n_rows * k.max_seeds);
   b.owner = (unsigned long long*)take(8 * n);
   b.tl_key = (unsigned long long*)take(8 * (size_t)k.max_seeds);
+  b.tl_mask = (uint32_t*)take(4 * (size_t)(2 * (TPC_MAX_ROWS / 32)) * k.max_seeds);
+  b.trk_mask = (uint32_t*)take(4 * (size_t)(2 * (TPC_MAX_ROWS / 32)) * k.max_tracks);
+  b.trk_sd = (uint32_t*)take(4 * (size_t)k.max_tracks);
   b.seg_cnt = (uint32_t*)take(4 * (size_t)(k.max_seeds + 1));
   b.id_cnt = (uint32_t*)take(4 * (size_t)(k.max_seeds + 1));
   b.tracks = (tpc_track*)take(sizeof(tpc_track) * (size_t)k.max_tracks);

@@ -85,6 +85,9 @@ struct TpcBuffers {
   int32_t* row_hit;       // [max_seeds][n_rows]
   unsigned long long* owner;     // [n]
   unsigned long long* tl_key;    // [max_seeds]
+  uint32_t* tl_mask;      // [max_seeds][2][TPC_MAX_ROWS/32] rows with a hit | rows whose hit is owned
+  uint32_t* trk_mask;     // [max_tracks][2][TPC_MAX_ROWS/32] accepted rows | shared rows of each track
+  uint32_t* trk_sd;       // [max_tracks] tracklet of each track
   uint32_t* seg_cnt;      // [max_seeds+1] tracks per tracklet -> exclusive scan
   uint32_t* id_cnt;       // [max_seeds+1] cluster ids per tracklet -> exclusive scan
   tpc_track* tracks;      // [max_tracks]

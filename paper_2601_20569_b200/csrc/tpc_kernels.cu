@@ -51,6 +51,32 @@ __device__ __forceinline__ uint4 ld_stream16(const void* p) {  // streaming 16-b
   return r;
 }
 
+// L2 residency control (createpolicy + .L2::cache_hint): streams that are read once are marked
+// evict_first so that they do not push out the randomly accessed tables marked evict_last.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ int32_t ld_i32_hint(const int32_t* p, uint64_t pol) {  // streaming, not kept in L1
+  int32_t v;
+  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ unsigned long long ld_u64_hint(const unsigned long long* p, uint64_t pol) {
+  unsigned long long v;
+  asm volatile("ld.global.L2::cache_hint.b64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ void red_max_u64_hint(unsigned long long* p, unsigned long long v, uint64_t pol) {
+  asm volatile("red.global.max.L2::cache_hint.u64 [%0], %1, %2;" ::"l"(p), "l"(v), "l"(pol) : "memory");
+}
+
 // Classify one input cluster. Returns: 0 in grid, 1 ignored (NaN/Inf), 2 dropped (|y| beyond
 // the row + 2 cm), 3 bad (sector/row outside the geometry).  R1 of DESIGN.md.
 __device__ __forceinline__ int classify(const uint4& raw, const TpcConst* __restrict__ K, int& sr, float& y,
@@ -1307,6 +1333,13 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
 // PAPER.md:27 ("identifies the best instance of each track, assigns all clusters to this
 // instance and removes the clones"; 10 % shared by default) with the Phase-I criterion of
 // PAPER.md:57 (chi2 priority; shared clusters counted from the outermost pad row).  R6.
+// Layout of the work: everything that touches memory per (tracklet,row) runs with one WARP
+// per tracklet and the lanes across its rows (coalesced row_hit reads, 32 independent
+// gathers / atomics in flight per warp); the sequential walk of R6.3 runs with one THREAD per
+// tracklet on two bit masks in registers (row has a hit / the hit is owned) and touches no
+// memory inside its loop.
+#define TPC_MASK_WORDS (TPC_MAX_ROWS / 32)   // mask stride per tracklet / track, in words
+
 __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
   const uint32_t n = B.cnt->n_sorted;  // owner[] is indexed by sorted position
   uint4* p4 = reinterpret_cast<uint4*>(B.owner);
@@ -1315,60 +1348,102 @@ __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
     p4[i] = make_uint4(0, 0, 0, 0);
 }
 
-// K5a: weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
-__global__ void __launch_bounds__(128) k_sel_owner(TpcBuffers B) {
+// K5a (R6.1, R6.2): weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
+__global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
-  const uint32_t stride = (uint32_t)B.K->n_rows;
+  const uint32_t R = (uint32_t)B.K->n_rows;
   const float w = B.K->P.sel_chi2_weight;
-  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
-    const int nh = B.tracklets[sd].n_hits;
+  const int lane = threadIdx.x & 31;
+  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+  const uint64_t pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
+  for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
+    const tpc_tracklet* __restrict__ t = B.tracklets + sd;
+    const int nh = t->n_hits;
     unsigned long long key = 0ull;
     if (nh > 0) {
       const int ndf = 2 * nh - 5;
-      const float Q = (float)nh - w * (B.tracklets[sd].chi2 / (float)ndf);
-      key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - B.tracklets[sd].seed_id);
-      const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
-      for (int r = r0; r <= r1; ++r) {
-        const int32_t c = B.row_hit[(size_t)sd * stride + r];
-        if (c >= 0) atomicMax(&B.owner[c], key);
+      const float Q = (float)nh - w * (t->chi2 / (float)ndf);
+      key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - t->seed_id);
+      const int r0 = t->row_first, r1 = t->row_last;
+      const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
+      for (int r = r0 + lane; r <= r1; r += 32) {
+        const int32_t c = ld_i32_hint(hits + r, pol_stream);
+        if (c >= 0) red_max_u64_hint(&B.owner[c], key, pol_keep);
       }
     }
-    B.tl_key[sd] = key;
+    if (lane == 0) B.tl_key[sd] = key;
   }
 }
 
-// The walk of R6.3: from the outermost row inward with the running shared budget; segments
-// split at holes > max_gap_select; EMIT=false counts, EMIT=true writes tracks and cluster ids.
+// K5b: per tracklet the two row masks of R6.3: "row has a hit" and "the hit is owned".
+__global__ void __launch_bounds__(256) k_sel_masks(TpcBuffers B) {
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
+  const uint32_t n_seeds = B.cnt->n_seeds;
+  const uint32_t R = (uint32_t)B.K->n_rows;
+  const int W = (int)((R + 31u) >> 5);
+  const int lane = threadIdx.x & 31;
+  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+  const uint64_t pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
+  for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
+    const unsigned long long key = B.tl_key[sd];
+    if (key == 0ull) continue;   // rejected tracklet (uniform over the warp)
+    const tpc_tracklet* __restrict__ t = B.tracklets + sd;
+    const int r0 = t->row_first, r1 = t->row_last;
+    const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
+    uint32_t my_has = 0u, my_own = 0u;
+    for (int wd = r0 >> 5; wd <= (r1 >> 5); ++wd) {
+      const int r = wd * 32 + lane;
+      int32_t c = -1;
+      if (r >= r0 && r <= r1) c = ld_i32_hint(hits + r, pol_stream);
+      const bool own = c >= 0 && ld_u64_hint(&B.owner[c], pol_keep) == key;
+      const uint32_t hm = __ballot_sync(0xffffffffu, c >= 0);
+      const uint32_t om = __ballot_sync(0xffffffffu, own);
+      if (lane == wd) { my_has = hm; my_own = om; }
+    }
+    if (lane < W) {
+      B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + lane] = my_has;
+      B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + lane] = my_own;
+    }
+  }
+}
+
+// The walk of R6.3 on the two masks: from the outermost row inward with the running shared
+// budget; segments split at holes > max_gap_select; EMIT=false counts, EMIT=true writes the
+// track records and, per track, the masks of its accepted / shared rows (k_sel_ids turns
+// them into cluster lists).
 template <bool EMIT>
 __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, uint32_t& n_seg_out, uint32_t& n_id_out,
                                               uint32_t trk_ofs, uint32_t id_ofs) {
   const tpc_params& P = B.K->P;
-  const uint32_t stride = (uint32_t)B.K->n_rows;
-  const unsigned long long key = B.tl_key[sd];
-  const int r0 = B.tracklets[sd].row_first, r1 = B.tracklets[sd].row_last;
+  const tpc_tracklet& tl = B.tracklets[sd];
+  const int r0 = tl.row_first, r1 = tl.row_last;
   const int min_hits = P.min_hits_track, max_gap = P.max_gap_select;
-  const long long permille = P.shared_permille;
+  const int permille = P.shared_permille;
+  const int R = B.K->n_rows;
+  uint32_t has[TPC_MASK_WORDS], own[TPC_MASK_WORDS], acc[TPC_MASK_WORDS], shm[TPC_MASK_WORDS];
+#pragma unroll
+  for (int w = 0; w < TPC_MASK_WORDS; ++w) {
+    has[w] = 0u; own[w] = 0u; acc[w] = 0u; shm[w] = 0u;
+    if (w * 32 < R) {
+      has[w] = B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + w];
+      own[w] = B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + w];
+    }
+  }
   int n_acc = 0, n_sh = 0, gap = 0, seg_last = -1, seg_first = -1;
   uint32_t n_seg = 0, n_id = 0;
-  // decisions of the current segment, one bit per row (the ids are written in ascending row
-  // order only once the segment is known to survive)
-  uint32_t acc_bits[TPC_MAX_ROWS / 32], sh_bits[TPC_MAX_ROWS / 32];
-  if (EMIT) {
-#pragma unroll
-    for (int i = 0; i < TPC_MAX_ROWS / 32; ++i) { acc_bits[i] = 0u; sh_bits[i] = 0u; }
-  }
   auto close = [&]() {
     if (n_acc >= min_hits) {
       if (EMIT) {
-        uint32_t o = id_ofs + n_id;
-        for (int r = seg_first; r <= seg_last; ++r) {
-          if (!((acc_bits[r >> 5] >> (r & 31)) & 1u)) continue;
-          B.cluster_ids[o] = B.orig_id[B.row_hit[(size_t)sd * stride + r]];
-          B.cluster_shared[o] = (uint8_t)((sh_bits[r >> 5] >> (r & 31)) & 1u);
-          ++o;
+        const uint32_t ti = trk_ofs + n_seg;
+#pragma unroll
+        for (int w = 0; w < TPC_MASK_WORDS; ++w) {
+          if (w * 32 < R) {
+            B.trk_mask[(size_t)ti * (2 * TPC_MASK_WORDS) + w] = acc[w];
+            B.trk_mask[(size_t)ti * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + w] = shm[w];
+          }
         }
-        const tpc_tracklet& tl = B.tracklets[sd];
+        B.trk_sd[ti] = sd;
         tpc_track t;
         t.x = tl.x;
 #pragma unroll
@@ -1387,36 +1462,44 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
         t.n_hits_tracklet = (uint16_t)tl.n_hits;
         t.segment = (uint8_t)n_seg;
         t.pad_ = 0;
-        B.tracks[trk_ofs + n_seg] = t;
+        B.tracks[ti] = t;
       }
       ++n_seg;
       n_id += (uint32_t)n_acc;
     }
-    if (EMIT && n_acc > 0) {
-      for (int w = seg_first >> 5; w <= seg_last >> 5; ++w) { acc_bits[w] = 0u; sh_bits[w] = 0u; }
+    if (EMIT) {
+#pragma unroll
+      for (int w = 0; w < TPC_MASK_WORDS; ++w) { acc[w] = 0u; shm[w] = 0u; }
     }
     n_acc = 0; n_sh = 0; seg_last = -1; seg_first = -1;
   };
-  for (int r = r1; r >= r0; --r) {
-    int32_t c = B.row_hit[(size_t)sd * stride + r];
-    bool sh = false;
-    if (c >= 0 && B.owner[c] != key) {
-      if ((long long)(n_sh + 1) * 1000 <= permille * (long long)(n_acc + 1)) sh = true;
-      else c = -1;
-    }
-    if (c >= 0) {
-      if (n_acc == 0) seg_last = r;
-      seg_first = r;
-      if (EMIT) {
-        acc_bits[r >> 5] |= 1u << (r & 31);
-        if (sh) sh_bits[r >> 5] |= 1u << (r & 31);
+#pragma unroll
+  for (int w = TPC_MASK_WORDS - 1; w >= 0; --w) {
+    if (w * 32 > r1 || w * 32 + 31 < r0) continue;
+    const int b_hi = min(31, r1 - w * 32), b_lo = max(0, r0 - w * 32);
+    const uint32_t hw = has[w], ow = own[w];
+    for (int b = b_hi; b >= b_lo; --b) {
+      const int r = w * 32 + b;
+      bool c = (hw >> b) & 1u;
+      bool sh = false;
+      if (c && !((ow >> b) & 1u)) {
+        if ((n_sh + 1) * 1000 <= permille * (n_acc + 1)) sh = true;
+        else c = false;
       }
-      ++n_acc;
-      if (sh) ++n_sh;
-      gap = 0;
-    } else {
-      ++gap;
-      if (gap > max_gap && n_acc > 0) close();
+      if (c) {
+        if (n_acc == 0) seg_last = r;
+        seg_first = r;
+        if (EMIT) {
+          acc[w] |= 1u << b;
+          if (sh) shm[w] |= 1u << b;
+        }
+        ++n_acc;
+        if (sh) ++n_sh;
+        gap = 0;
+      } else {
+        ++gap;
+        if (gap > max_gap && n_acc > 0) close();
+      }
     }
   }
   close();
@@ -1424,7 +1507,7 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
   n_id_out = n_id;
 }
 
-// K5b: count tracks / cluster ids per tracklet + per-block partial sums (for the scans).
+// K5c: count tracks / cluster ids per tracklet + per-block partial sums (for the scans).
 __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
   __shared__ uint32_t sm[33];
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
@@ -1435,26 +1518,53 @@ __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
   for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
     const uint32_t sd = blk * blockDim.x + threadIdx.x;
     uint32_t ns = 0, ni = 0;
-    if (sd < n_seeds && B.tracklets[sd].n_hits > 0) walk_tracklet<false>(B, sd, ns, ni, 0, 0);
+    if (sd < n_seeds && B.tl_key[sd] != 0ull) walk_tracklet<false>(B, sd, ns, ni, 0, 0);
     uint32_t tot_s, tot_i;
     const uint32_t ps = block_excl_scan(ns, &tot_s, sm);
     const uint32_t pi = block_excl_scan(ni, &tot_i, sm);
-    if (sd < n_seeds) { B.seg_cnt[sd] = ps; B.id_cnt[sd] = pi; }  // block-local exclusive prefix
+    if (sd < n_seeds) { B.seg_cnt[sd] = ns ? ps : 0xFFFFFFFFu; B.id_cnt[sd] = pi; }  // block-local exclusive prefix
     if (threadIdx.x == 0) { part_seg[blk] = tot_s; part_id[blk] = tot_i; }
   }
 }
 
-// K5c: emit tracks + cluster lists at their scanned offsets (order = seed order).
+// K5d: emit the track records at their scanned offsets (order = seed order).
 __global__ void __launch_bounds__(256) k_sel_emit(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const uint32_t* part_seg = B.scan_partials;
   const uint32_t* part_id = B.scan_partials + (B.scan_blocks + 1) / 2;
   for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
-    if (B.tracklets[sd].n_hits <= 0) continue;
+    const uint32_t ps = B.seg_cnt[sd];
+    if (ps == 0xFFFFFFFFu) continue;   // no surviving segment
     const uint32_t blk = sd / blockDim.x;
     uint32_t ns, ni;
-    walk_tracklet<true>(B, sd, ns, ni, part_seg[blk] + B.seg_cnt[sd], part_id[blk] + B.id_cnt[sd]);
+    walk_tracklet<true>(B, sd, ns, ni, part_seg[blk] + ps, part_id[blk] + B.id_cnt[sd]);
+  }
+}
+
+// K5e: cluster lists (original ids ascending in row) and shared flags, one warp per track.
+__global__ void __launch_bounds__(256) k_sel_ids(TpcBuffers B) {
+  if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return;
+  const uint32_t n_tracks = B.cnt->n_tracks;
+  const uint32_t R = (uint32_t)B.K->n_rows;
+  const int lane = threadIdx.x & 31;
+  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t ti = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; ti < n_tracks; ti += n_warps) {
+    const tpc_track* __restrict__ t = B.tracks + ti;
+    const int r0 = t->row_first, r1 = t->row_last;
+    uint32_t o = t->cluster_ofs;
+    const uint32_t sd = B.trk_sd[ti];
+    const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
+    const uint32_t* __restrict__ mk = B.trk_mask + (size_t)ti * (2 * TPC_MASK_WORDS);
+    for (int wd = r0 >> 5; wd <= (r1 >> 5); ++wd) {
+      const uint32_t am = mk[wd], sm = mk[TPC_MASK_WORDS + wd];
+      if ((am >> lane) & 1u) {
+        const uint32_t pos = o + (uint32_t)__popc(am & ((1u << lane) - 1u));
+        B.cluster_ids[pos] = B.orig_id[hits[wd * 32 + lane]];
+        B.cluster_shared[pos] = (uint8_t)((sm >> lane) & 1u);
+      }
+      o += (uint32_t)__popc(am);
+    }
   }
 }
 
@@ -1549,8 +1659,10 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   // ---- K5 ambiguity solving
   k_zero_owner<<<grid_for(B.n / 2 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_owner");
-  k_sel_owner<<<grid_for(B.max_seeds, 128, n_sm, 8), 128, 0, st>>>(B);
+  k_sel_owner<<<grid_for((uint64_t)B.max_seeds * 32, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_owner");
+  k_sel_masks<<<grid_for((uint64_t)B.max_seeds * 32, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_sel_masks");
   k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_count");
   const uint32_t half = (B.scan_blocks + 1) / 2;
@@ -1562,6 +1674,8 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   TPC_LAUNCH_CHECK("k_scan_partials");
   k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_emit");
+  k_sel_ids<<<grid_for((uint64_t)B.max_tracks * 32, 256, n_sm, 8), 256, 0, st>>>(B);
+  TPC_LAUNCH_CHECK("k_sel_ids");
   if (timers) cudaEventRecord(E.ev[5], st);
   (void)flags;
   E.n_kernels = launches < TPC_MAX_KERNELS ? launches : TPC_MAX_KERNELS;
