@@ -81,6 +81,8 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   std::memset(&b, 0, sizeof(b));
   b.n = (uint32_t)n;
   b.n_sr = n_sr;
+  b.n_sectors = (uint32_t)c->geom.n_sectors;
+  b.n_rows = (uint32_t)c->geom.n_rows;
   b.max_bins = k.max_bins;
   b.max_seeds = k.max_seeds;
   b.max_tracks = k.max_tracks;
@@ -99,6 +101,8 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.link_dn2 = (int32_t*)take(4 * n);
   b.seed_len = (uint8_t*)take(n);
   b.scan_partials = (uint32_t*)take(4 * (size_t)(k.scan_blocks + 2));
+  b.item_cnt = (uint32_t*)take(4 * (size_t)n_sr * TPC_SEED_SLABS);
+  b.item_delta = (int32_t*)take(4 * (size_t)n_sr * TPC_SEED_SLABS);
   b.seeds = (uint32_t*)take(4 * (size_t)k.max_seeds);
   b.seed_sr = (uint16_t*)take(2 * (size_t)k.max_seeds);
   b.turn = (uint4*)take(32 * (size_t)k.max_seeds);

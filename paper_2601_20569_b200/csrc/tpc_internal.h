@@ -53,11 +53,17 @@ struct TpcRowStat {
 
 #define TPC_NF_TILE 256  // clusters per neighbour-finder tile (one CTA)
 
+// Seeds are handed to the follower / selector ordered by (sector, z-slab, row): tracklets that
+// run at the same time then touch the same z-range of every row, which keeps their random
+// accesses (grid, owner words) inside L2.  A slab is 1/TPC_SEED_SLABS of a row's z-bins.
+#define TPC_SEED_SLABS 64
+
 // All device buffers of one run (pointers into the caller's workspace, or ctx-owned).
 struct TpcBuffers {
   const tpc_cluster* clusters;
   uint32_t n;            // input clusters
   uint32_t n_sr;         // n_sectors*n_rows
+  uint32_t n_sectors, n_rows;
   uint64_t max_bins;
   uint32_t max_seeds, max_tracks, max_ids;
   uint32_t scan_blocks;  // capacity of scan_partials
@@ -77,7 +83,9 @@ struct TpcBuffers {
   int32_t* link_dn2;
   uint8_t* seed_len;      // [n] chain length if the cluster is a start hit of a seed, else 0
   uint32_t* scan_partials;// [scan_blocks+1]
-  uint32_t* seeds;        // [max_seeds] sorted index of start hits
+  uint32_t* item_cnt;     // [n_sr][TPC_SEED_SLABS] seeds per (sector,row,z-slab)
+  int32_t* item_delta;    // [n_sr][TPC_SEED_SLABS] list position in (sector,slab,row) order minus rank in sorted order
+  uint32_t* seeds;        // [max_seeds] sorted index of start hits, in (sector, z-slab, row, sorted index) order
   uint16_t* seed_sr;      // [max_seeds] sector*n_rows+row of each start hit
   uint4* turn;            // [max_seeds][2] state at the outermost hit (y,z,sin phi,tan lambda | q/pT,row,-,-)
   uint32_t* down_list;    // [max_seeds] seeds whose refit reached the start row (inward extrapolation pending)
