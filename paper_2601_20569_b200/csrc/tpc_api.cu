@@ -242,8 +242,8 @@ int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clu
   ctx->events.enabled = (flags & TPC_STAGE_TIMERS) != 0;
   (void)cudaGetLastError();
   const int launches = (flags & TPC_DETERMINISTIC)
-                           ? tpc_det::run_pipeline(B, ctx->stream, flags, ctx->events, ctx->n_sm)
-                           : tpc_fast::run_pipeline(B, ctx->stream, flags, ctx->events, ctx->n_sm);
+                           ? tpc_det::run_pipeline(B, &ctx->hconst, ctx->stream, flags, ctx->events, ctx->n_sm)
+                           : tpc_fast::run_pipeline(B, &ctx->hconst, ctx->stream, flags, ctx->events, ctx->n_sm);
   if (launches < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch");
   cudaError_t e = cudaMemcpyAsync(ctx->h_cnt, ctx->d_cnt, sizeof(TpcCounters), cudaMemcpyDeviceToHost, ctx->stream);
   if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(counters)");

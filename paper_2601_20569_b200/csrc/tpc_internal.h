@@ -113,10 +113,10 @@ struct TpcStageEvents {
 };
 
 namespace tpc_det {
-int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
+int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
-int run_pipeline(const TpcBuffers& B, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
+int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 
 #endif

@@ -626,8 +626,10 @@ __global__ void __launch_bounds__(1024) k_seed_flags(TpcBuffers B) {
     const uint32_t i = blk * blockDim.x + threadIdx.x;
     uint32_t len = 0;
     if (i < n && B.link_dn2[i] < 0 && B.link_up2[i] >= 0) {
+      // only "at least seed_min_len" is decided here; the full chain length is counted by the
+      // follower's chain fit, which walks the chain anyway (k_follow_up -> seed_len[])
       len = 1;
-      for (int32_t c = B.link_up2[i]; c >= 0; c = B.link_up2[c]) ++len;
+      for (int32_t c = B.link_up2[i]; c >= 0 && (int)len < min_len; c = B.link_up2[c]) ++len;
       if ((int)len < min_len) len = 0;
       if (len) atomicAdd(&B.item_cnt[seed_item(B, sr_of_position(B, i), i)], 1u);
     }
@@ -979,7 +981,9 @@ __device__ __forceinline__ bool queue_claim(uint32_t* counter, uint32_t n_items,
   return got;
 }
 
-__device__ __forceinline__ FollowConst follow_const(const TpcConst* __restrict__ K) {
+// Filled on the host and passed BY VALUE as a kernel parameter: the constants then sit in the
+// constant bank and cost no registers in the follower loops.
+static inline FollowConst follow_const(const TpcConst* K) {
   FollowConst F;
   F.dx = K->dx_row; F.cfield = K->cfield; F.max_sinphi = K->P.max_sinphi; F.max_qpt = K->P.max_qpt;
   F.vy = K->vy; F.vz = K->vz;
@@ -1045,13 +1049,12 @@ __device__ __forceinline__ void write_tracklet(const TpcBuffers& B, uint32_t sd,
 #endif
 
 // ---- R5.1-R5.3: init, chain fit, outward extrapolation
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_up(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_up(TpcBuffers B, const __grid_constant__ FollowConst F) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
   const TpcConst* __restrict__ K = B.K;
   for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_ylim[r] = K->ylim[r];
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
-  const FollowConst F = follow_const(K);
   const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const int32_t* __restrict__ up2 = B.link_up2;
@@ -1069,7 +1072,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
   kf_init_cov(k, F);
   uint32_t sd = 0, sr_base = 0;
   int32_t* __restrict__ hit_row = B.row_hit;  // this seed's row -> sorted index table
-  int r = 0, r_out = 0, gap = 0;
+  int r = 0, r_out = 0, gap = 0, chain_n = 0;
   float snap_s = 0.f, snap_t = 0.f, snap_q = 0.f, snap_y = 0.f, snap_z = 0.f;
   int32_t c_cur = -1, c_nxt = -1;   // chain hit of the coming row and the one after it
   float2 m_cur = make_float2(0.f, 0.f);
@@ -1103,6 +1106,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
         snap_s = k.s; snap_t = k.t; snap_q = k.q; snap_y = m0.x; snap_z = m0.y;
         gap = 0;
         c_cur = c1; m_cur = m1;
+        chain_n = 1;
         pb = TPC_NO_BIN;
         phase = PH_CHAIN;
       }
@@ -1162,8 +1166,15 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
             ++gap;
             if (gap > F.max_gap) fin = true;
           }
-          if (!extrap) { c_cur = c_nxt; m_cur = m_nxt; c_nxt = c_nxt2; }
+          if (!extrap) { c_cur = c_nxt; m_cur = m_nxt; c_nxt = c_nxt2; ++chain_n; }
         }
+      }
+      if (phase == PH_CHAIN && (fin || c_cur < 0)) {
+        // chain length of the seed (R4): hits fitted so far + links not reached when the leg
+        // ended inside the chain
+        int n_chain = chain_n;
+        for (int32_t c = c_cur; c >= 0; c = up2[c]) ++n_chain;
+        B.seed_len[B.seeds[sd]] = (uint8_t)n_chain;
       }
       if (fin) {
         // state for R5.4 (turn at the outermost accepted hit)
@@ -1180,14 +1191,13 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
 }
 
 // ---- R5.4-R5.5: turn at the outermost accepted hit, refit inward through the recorded hits
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) k_follow_refit(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) k_follow_refit(TpcBuffers B, const __grid_constant__ FollowConst F) {
   __shared__ float s_x[TPC_MAX_ROWS];
   __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];  // state at the innermost accepted hit (R5.7)
   const TpcConst* __restrict__ K = B.K;
   for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) s_x[r] = K->x[r];
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
-  const FollowConst F = follow_const(K);
   const uint32_t n_seeds = B.cnt->n_seeds;
   const float2* __restrict__ yz = B.yz;
   const int lane = threadIdx.x & 31;
@@ -1279,7 +1289,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) 
 }
 
 // ---- R5.6-R5.7: inward extrapolation below the start row, output
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_down(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_down(TpcBuffers B, const __grid_constant__ FollowConst F) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
   __shared__ float s_x[TPC_MAX_ROWS];
   __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];
@@ -1287,7 +1297,6 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
   for (int r = threadIdx.x; r < K->n_rows; r += blockDim.x) { s_ylim[r] = K->ylim[r]; s_x[r] = K->x[r]; }
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
-  const FollowConst F = follow_const(K);
   const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
   const uint32_t n_down = B.cnt->n_down;
   const float2* __restrict__ yz = B.yz;
@@ -1666,8 +1675,9 @@ static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.
-int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageEvents& E, int n_sm) {
+int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint32_t flags, TpcStageEvents& E, int n_sm) {
   int launches = 0;
+  const FollowConst F = follow_const(hK);
   const bool timers = E.enabled;
   if (timers) cudaEventRecord(E.kev[0], st);
   k_init<<<(B.n_sr + 255) / 256, 256, 0, st>>>(B);
@@ -1716,11 +1726,11 @@ int run_pipeline(const TpcBuffers& B, cudaStream_t st, uint32_t flags, TpcStageE
   TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
-  k_follow_up<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  k_follow_up<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_up");
-  k_follow_refit<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_REFIT_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  k_follow_refit<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_REFIT_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_refit");
-  k_follow_down<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B);
+  k_follow_down<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_down");
   if (timers) cudaEventRecord(E.ev[4], st);
   // ---- K5 ambiguity solving
