@@ -36,7 +36,8 @@ struct TpcConst {
 struct TpcCounters {
   uint32_t n_sorted, n_ignored, n_dropped, n_bad;
   uint32_t n_bins, n_tiles, n_seeds, n_tracklets;
-  uint32_t n_tracks, n_ids, error, pad_;
+  uint32_t n_tracks, n_ids, error;
+  uint32_t grid_rows;   // 1: every row's input records are contiguous and fit k_row_sort (the per-row grid build)
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
   unsigned long long follow_work[3][3];  // [kernel up/refit/down][steps, updates, candidates]
@@ -48,10 +49,21 @@ struct TpcCounters {
 // per (sector,row) statistics of pass 1
 struct TpcRowStat {
   uint32_t zmin_key, zmax_key;  // order-preserving uint image of the float
-  uint32_t count, pad_;
+  uint32_t count;               // clusters kept in the grid
+  uint32_t n_all;               // input records carrying this (sector,row), kept or not
+  uint32_t first, last;         // lowest / highest input index among them
+  uint32_t pad_[2];
 };
 
 #define TPC_NF_TILE 256  // clusters per neighbour-finder tile (one CTA)
+
+// Per-row grid build (k_row_sort): one CTA per (sector,row); the row's bin counters and its
+// permutation live in shared memory (16-bit entries).
+#define TPC_RS_THREADS 1024
+#define TPC_RS_SMEM_BYTES (224 * 1024)   // dynamic shared memory per CTA
+#ifndef TPC_RS_BATCH
+#define TPC_RS_BATCH 4                   // records requested together per thread
+#endif
 
 // Seeds are handed to the follower / selector ordered by (sector, z-slab, row): tracklets that
 // run at the same time then touch the same z-range of every row, which keeps their random

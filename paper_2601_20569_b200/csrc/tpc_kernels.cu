@@ -111,24 +111,38 @@ __global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
     n_drop += cls == 2;
     n_bad += cls == 3;
     const bool ok = cls == 0;
+    const bool in_row = cls <= 2;   // carries a valid (sector,row), kept in the grid or not
+    const unsigned rowmask = __ballot_sync(0xffffffffu, in_row);
+    if (rowmask == 0) continue;
     const unsigned okmask = __ballot_sync(0xffffffffu, ok);
-    if (okmask == 0) continue;
-    const int leader = __ffs(okmask) - 1;
+    const int leader = __ffs(rowmask) - 1;
     const int sr0 = __shfl_sync(0xffffffffu, sr, leader);
-    const bool uniform = __all_sync(0xffffffffu, !ok || sr == sr0);
+    const bool uniform = __all_sync(0xffffffffu, !in_row || sr == sr0);
     const uint32_t zk = f2key(z);
     if (uniform) {
       const uint32_t mn = __reduce_min_sync(0xffffffffu, ok ? zk : 0xFFFFFFFFu);
       const uint32_t mx = __reduce_max_sync(0xffffffffu, ok ? zk : 0u);
       if ((int)(threadIdx.x & 31) == leader) {
-        atomicMin(&B.row_stat[sr0].zmin_key, mn);
-        atomicMax(&B.row_stat[sr0].zmax_key, mx);
-        atomicAdd(&B.row_stat[sr0].count, (uint32_t)__popc(okmask));
+        TpcRowStat* rs = &B.row_stat[sr0];
+        if (okmask) {
+          atomicMin(&rs->zmin_key, mn);
+          atomicMax(&rs->zmax_key, mx);
+          atomicAdd(&rs->count, (uint32_t)__popc(okmask));
+        }
+        atomicAdd(&rs->n_all, (uint32_t)__popc(rowmask));
+        atomicMin(&rs->first, i);                                  // the leader is the lowest lane
+        atomicMax(&rs->last, (i - (uint32_t)leader) + (31u - (uint32_t)__clz(rowmask)));
       }
-    } else if (ok) {
-      atomicMin(&B.row_stat[sr].zmin_key, zk);
-      atomicMax(&B.row_stat[sr].zmax_key, zk);
-      atomicAdd(&B.row_stat[sr].count, 1u);
+    } else if (in_row) {
+      TpcRowStat* rs = &B.row_stat[sr];
+      if (ok) {
+        atomicMin(&rs->zmin_key, zk);
+        atomicMax(&rs->zmax_key, zk);
+        atomicAdd(&rs->count, 1u);
+      }
+      atomicAdd(&rs->n_all, 1u);
+      atomicMin(&rs->first, i);
+      atomicMax(&rs->last, i);
     }
   }
   n_ign = __reduce_add_sync(0xffffffffu, n_ign);
@@ -182,6 +196,7 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
   uint32_t base_bin = 0, base_clu = 0, base_tile = 0;
   unsigned long long bins64 = 0;
   bool overflow = false;
+  bool by_rows = true;   // every row qualifies for the per-row grid build (k_row_sort)
   for (uint32_t s0 = 0; s0 < B.n_sr; s0 += blockDim.x) {
     const uint32_t sr = s0 + threadIdx.x;
     uint32_t cnt = 0, nb = 0, nt = 0;
@@ -203,6 +218,11 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
         if (nb64 > B.max_bins) { overflow = true; nb = 0; nz = 0; }
         else nb = (uint32_t)nb64;
         nt = (cnt + TPC_NF_TILE - 1) / TPC_NF_TILE;
+        // k_row_sort needs the row's input records in one contiguous range, and its bin
+        // counters + permutation in the cluster's shared memory
+        const TpcRowStat rs = B.row_stat[sr];
+        const uint32_t bytes = 4u * ((nb + 1) / 2) + 2u * cnt;
+        if (rs.last - rs.first + 1u != rs.n_all || rs.n_all > 65535u || bytes > TPC_RS_SMEM_BYTES) by_rows = false;
       }
     }
     uint32_t tot_b, tot_c, tot_t;
@@ -223,7 +243,9 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
     base_bin += tot_b; base_clu += tot_c; base_tile += tot_t;
   }
   overflow = __syncthreads_or(overflow || bins64 > B.max_bins);
+  by_rows = __syncthreads_and(by_rows);
   if (threadIdx.x == 0) {
+    B.cnt->grid_rows = (by_rows && !overflow) ? 1u : 0u;
     B.tile_ofs[B.n_sr] = base_tile;
     B.cnt->n_sorted = base_clu;
     B.cnt->n_tiles = base_tile;
@@ -247,7 +269,7 @@ __global__ void __launch_bounds__(128) k_tile_rows(TpcBuffers B) {
 __global__ void __launch_bounds__(256) k_zero_bins(TpcBuffers B) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n_sr * TPC_SEED_SLABS; i += gridDim.x * blockDim.x)
     B.item_cnt[i] = 0u;
-  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
   const uint32_t n = B.cnt->n_bins + 1;
   uint4* p4 = reinterpret_cast<uint4*>(B.bin_start);
   const uint32_t n4 = n / 4;
@@ -266,7 +288,7 @@ __device__ __forceinline__ uint32_t bin_of(const tpc_row_desc& d, const TpcConst
 // so the scatter needs no second atomic.
 __global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
-  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
     const uint4 raw = ld_stream16(B.clusters + i);
     int sr, row;
@@ -285,7 +307,7 @@ __global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
 // (north star: "a per-row bin index built by a warp-level scan").
 __global__ void __launch_bounds__(512) k_bin_scan(TpcBuffers B) {
   __shared__ uint32_t sm[33];
-  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
   for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
     const tpc_row_desc d = B.row_desc[sr];
     const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
@@ -315,7 +337,7 @@ __global__ void __launch_bounds__(512) k_bin_scan(TpcBuffers B) {
 // K1e: scatter into bin order: sorted (y,z) pairs + original index.
 __global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
-  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
     const uint32_t s = B.slot[i];
     if (s == 0xFFFFFFFFu) continue;
@@ -339,7 +361,7 @@ __global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
 // K1f (deterministic mode only): order the clusters of every bin by ascending original index,
 // so that the sorted order is a function of the input alone (stable sort).
 __global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
-  if (B.cnt->error & TPC_DEVERR_BINS) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
   const uint32_t nb = B.cnt->n_bins;
   for (uint32_t b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
     const uint32_t lo = B.bin_start[b], hi = B.bin_start[b + 1];
@@ -358,6 +380,129 @@ __global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
   }
 }
 #endif
+
+// ------------------------------------------------------------------ K1 per-row build
+// The grid of one (sector,row) built by ONE CTA whose shared memory holds the row's bin
+// counters and its permutation (both 16-bit: a qualifying row has < 65536 records), so that
+// HBM sees only streaming traffic: the row's input records once (the later passes hit L2),
+// bin_start, yz and orig_id written once, coalesced.  Used when every row's input records are
+// contiguous (clusteriser order) and fit; otherwise the generic kernels above run (k_row_desc
+// decides).
+//   A  count: bin of every record -> shared-memory atomics (two 16-bit counters per word)
+//   S  scan : exclusive scan of the counters -> bin_start to HBM, counters become cursors
+//   B  place: cursor atomics hand out positions; inv[position] = record
+//   (deterministic build: records of a bin ordered by input index, rule R1.4)
+//   C  write: position-major, coalesced: record = inv[p] -> yz[p], orig_id[p]
+__global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
+  extern __shared__ uint32_t rs_mem[];   // [nbw] packed bin counters / cursors | inv (16-bit)
+  __shared__ uint32_t sm[33];
+  if ((B.cnt->error & TPC_DEVERR_BINS) || !B.cnt->grid_rows) return;
+  if (blockIdx.x == 0 && threadIdx.x == 0) B.bin_start[B.cnt->n_bins] = B.cnt->n_sorted;
+  const TpcConst* __restrict__ K = B.K;
+  const uint32_t tid = threadIdx.x;
+  const uint4 kSkip = make_uint4(0x7fc00000u, 0u, 0u, 0u);   // NaN y: classified "ignored"
+  for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
+    const tpc_row_desc d = B.row_desc[sr];
+    if (d.count == 0) continue;
+    const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
+    const uint32_t nbw = (nb + 1) / 2;                       // counter words
+    uint16_t* inv = reinterpret_cast<uint16_t*>(rs_mem + nbw);
+    const TpcRowStat rs = B.row_stat[sr];
+    const tpc_cluster* __restrict__ in = B.clusters + rs.first;
+    const uint32_t n_all = rs.n_all;
+    __syncthreads();                                         // the previous row is done with rs_mem
+    for (uint32_t w = tid; w < nbw; w += TPC_RS_THREADS) rs_mem[w] = 0u;
+    __syncthreads();
+    // ---- A: count.  TPC_RS_BATCH records per thread are requested together
+    for (uint32_t e0 = tid; e0 < n_all; e0 += TPC_RS_BATCH * TPC_RS_THREADS) {
+      uint4 raw[TPC_RS_BATCH];
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        const uint32_t e = e0 + u * TPC_RS_THREADS;
+        raw[u] = e < n_all ? ld_stream16(in + e) : kSkip;
+      }
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        int sr_e, row;
+        float y, z;
+        if (classify(raw[u], K, sr_e, y, z, row) != 0) continue;
+        const uint32_t bb = bin_of(d, K, y, z) - d.bin_ofs;
+        atomicAdd(&rs_mem[bb >> 1], 1u << ((bb & 1u) * 16u));
+      }
+    }
+    __syncthreads();
+    // ---- S: scan; runs of L consecutive counter words (2L bins) per thread
+    const uint32_t L = (nbw + TPC_RS_THREADS - 1) / TPC_RS_THREADS;
+    const uint32_t w0 = min(tid * L, nbw), w1 = min(w0 + L, nbw);
+    uint32_t run = 0;
+    for (uint32_t w = w0; w < w1; ++w) { const uint32_t c = rs_mem[w]; run += (c & 0xFFFFu) + (c >> 16); }
+    uint32_t tot;
+    uint32_t pre = block_excl_scan(run, &tot, sm);
+    for (uint32_t w = w0; w < w1; ++w) {
+      const uint32_t c = rs_mem[w];
+      const uint32_t p0 = pre, p1 = pre + (c & 0xFFFFu);
+      rs_mem[w] = p0 | (p1 << 16);                           // cursors, row-relative (< 65536)
+      B.bin_start[d.bin_ofs + 2 * w] = d.clu_ofs + p0;
+      if (2 * w + 1 < nb) B.bin_start[d.bin_ofs + 2 * w + 1] = d.clu_ofs + p1;
+      pre = p1 + (c >> 16);
+    }
+    __syncthreads();
+    // ---- B: place (the row's records now come from L2)
+    for (uint32_t e0 = tid; e0 < n_all; e0 += TPC_RS_BATCH * TPC_RS_THREADS) {
+      uint4 raw[TPC_RS_BATCH];
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        const uint32_t e = e0 + u * TPC_RS_THREADS;
+        raw[u] = e < n_all ? *reinterpret_cast<const uint4*>(in + e) : kSkip;
+      }
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        int sr_e, row;
+        float y, z;
+        if (classify(raw[u], K, sr_e, y, z, row) != 0) continue;
+        const uint32_t bb = bin_of(d, K, y, z) - d.bin_ofs;
+        const uint32_t sh = (bb & 1u) * 16u;
+        const uint32_t p = (atomicAdd(&rs_mem[bb >> 1], 1u << sh) >> sh) & 0xFFFFu;
+        inv[p] = (uint16_t)(e0 + u * TPC_RS_THREADS);
+      }
+    }
+    __syncthreads();
+#if TPC_DET
+    // ---- records of a bin in ascending input index (the cursors now point at the bin ends;
+    // a cursor that reached 65536 wrapped to 0 and its carry went into the upper half, which
+    // only happens for the last bin of a 65536-record row: excluded by k_row_desc)
+    for (uint32_t b = tid; b < nb; b += TPC_RS_THREADS) {
+      const uint32_t hi = (rs_mem[b >> 1] >> ((b & 1u) * 16u)) & 0xFFFFu;
+      const uint32_t lo = b ? ((rs_mem[(b - 1) >> 1] >> (((b - 1) & 1u) * 16u)) & 0xFFFFu) : 0u;
+      for (uint32_t i = lo + 1; i < hi; ++i) {   // insertion sort, bins hold a few clusters
+        const uint16_t v = inv[i];
+        uint32_t j = i;
+        while (j > lo && inv[j - 1] > v) { inv[j] = inv[j - 1]; --j; }
+        inv[j] = v;
+      }
+    }
+    __syncthreads();
+#endif
+    // ---- C: write the sorted arrays
+    for (uint32_t q0 = tid; q0 < d.count; q0 += TPC_RS_BATCH * TPC_RS_THREADS) {
+      uint32_t e[TPC_RS_BATCH];
+      uint2 v[TPC_RS_BATCH];
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        const uint32_t q = q0 + u * TPC_RS_THREADS;
+        e[u] = q < d.count ? (uint32_t)inv[q] : 0u;
+        v[u] = *reinterpret_cast<const uint2*>(in + e[u]);
+      }
+#pragma unroll
+      for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        const uint32_t q = q0 + u * TPC_RS_THREADS;
+        if (q >= d.count) continue;
+        B.yz[d.clu_ofs + q] = make_float2(__uint_as_float(v[u].x), __uint_as_float(v[u].y));
+        B.orig_id[d.clu_ofs + q] = rs.first + e[u];
+      }
+    }
+  }
+}
 
 // ================================================================== window queries
 // Visit the sorted clusters of one row whose bin intersects [ylo,yhi]x[zlo,zhi].  The margins
@@ -1641,14 +1786,16 @@ __global__ void k_init(TpcBuffers B) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < B.n_sr) {
     TpcRowStat s;
-    s.zmin_key = 0xFFFFFFFFu; s.zmax_key = 0u; s.count = 0u; s.pad_ = 0u;
+    s.zmin_key = 0xFFFFFFFFu; s.zmax_key = 0u; s.count = 0u; s.n_all = 0u;
+    s.first = 0xFFFFFFFFu; s.last = 0u; s.pad_[0] = s.pad_[1] = 0u;
     B.row_stat[i] = s;
   }
   if (i == 0) {
     TpcCounters c;
     c.n_sorted = c.n_ignored = c.n_dropped = c.n_bad = 0;
     c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
-    c.n_tracks = c.n_ids = c.error = c.pad_ = 0;
+    c.n_tracks = c.n_ids = c.error = 0;
+    c.grid_rows = 0;
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) c.follow_work[a][b] = 0ull;
     c.follow_next[0] = c.follow_next[1] = c.follow_next[2] = 0u; c.n_down = 0u;
@@ -1690,6 +1837,9 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   TPC_LAUNCH_CHECK("k_row_desc");
   k_tile_rows<<<grid_for((uint64_t)B.n_sr * 128, 128, n_sm, 8), 128, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_tile_rows");
+  cudaFuncSetAttribute(k_row_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, TPC_RS_SMEM_BYTES);
+  k_row_sort<<<min((uint32_t)n_sm, B.n_sr), TPC_RS_THREADS, TPC_RS_SMEM_BYTES, st>>>(B);
+  TPC_LAUNCH_CHECK("k_row_sort");
   k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_bins");
   k_bin_hist<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
