@@ -151,7 +151,7 @@ class ClockSampler:
 def make_frame(workload: str, rank: int, events: int | None, tracks: int | None):
     from paper_2601_20569_b200 import datagen as dg
     base = dg.preset(workload)
-    kw = dict(seed=base.seed + 1000 * rank)
+    kw = dict(seed=rank_seed(base.seed, rank))
     if events is not None:
         kw["n_events"] = events
         # a shorter frame at the SAME interaction rate (same cluster density per cm of drift)
@@ -221,6 +221,30 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------ N > 1: units and reductions
+def rank_seed(base_seed: int, rank: int) -> int:
+    """Every rank tracks its own independent time frame (no data-path collective)."""
+    return base_seed + 1000 * rank
+
+
+def reduce_over_ranks(x: float, op: str, world: int, device=None) -> float:
+    """Whole-job figures: op = "max" for the time of the slowest rank, "sum" for the units."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def whole_job_value(n_local: float, ms_local: float, steps: int, world: int, device=None):
+    """value = units all ranks processed / max-over-ranks time; returns (value, ms_total)."""
+    ms_total = reduce_over_ranks(ms_local, "max", world, device)
+    n_all = reduce_over_ranks(float(n_local), "sum", world, device)
+    return n_all * steps / (ms_total * 1e-3), ms_total
+
+
 # ------------------------------------------------------------------ the CUDA arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -242,18 +266,10 @@ def run_ours(args, rank, world, local_rank):
         torch.cuda.synchronize()
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_over_ranks(x, "max", world, dev)
 
     def sum_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return reduce_over_ranks(x, "sum", world, dev)
 
     cfg, clusters, labels, gen_s = make_frame(args.workload, rank, args.events, args.tracks)
     n = len(clusters)
