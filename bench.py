@@ -40,7 +40,7 @@ WORKLOAD_PARAMS = {
     "C1": dict(),
     "C2": dict(),
     "C3": dict(),
-    "C4": dict(grid_dy=4.0, grid_dz=4.0),
+    "C4": dict(grid_dy=3.0, grid_dz=3.0),
     "C5": dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6),
 }
 
@@ -57,6 +57,7 @@ def algorithmic_work(name: str, st: dict):
     W, NT, NI = (R + 31) // 32, st["n_tracks"], st["n_ids"]
     hbm = {
         "k_row_stats": 16 * N,
+        "k_row_sort": 16 * N + 12 * Ns + 4 * NB,         # records in (once; the re-reads are L2 by design), yz+id+bin_start out
         "k_zero_bins": 4 * NB,
         "k_bin_hist": 16 * N + 4 * N + 8 * Ns,          # cluster in, slot out, counter RMW
         "k_bin_scan": 8 * NB,
@@ -390,7 +391,7 @@ def run_ours(args, rank, world, local_rank):
             pass
     # north star: HBM fraction of the grid and neighbour stages
     stages = {}
-    grid_names = ("k_row_stats", "k_row_desc", "k_zero_bins", "k_bin_hist", "k_bin_scan", "k_scatter", "k_bin_sort")
+    grid_names = ("k_row_stats", "k_row_desc", "k_row_sort", "k_zero_bins", "k_bin_hist", "k_bin_scan", "k_scatter", "k_bin_sort")
     gb = sum(k["work_per_step"] for k in per_kernel if k["name"] in grid_names)
     gms = sum(k["ms_per_step"] for k in per_kernel if k["name"] in grid_names)
     nb = next((k for k in per_kernel if k["name"] == "k_neighbours"), None)

@@ -1567,7 +1567,7 @@ __global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
   const float w = B.K->P.sel_chi2_weight;
   const int lane = threadIdx.x & 31;
   const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
-  const uint64_t pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
+  const uint64_t pol_stream = l2_policy_evict_first();
   for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
     const tpc_tracklet* __restrict__ t = B.tracklets + sd;
     const int nh = t->n_hits;
@@ -1583,7 +1583,9 @@ __global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
         // read first: most hits lose against the current owner and then need no atomic; the
         // load also brings the sector into L2, where a red that misses would not stay
         // (C4 frame: 28.0 -> 16.3 ms)
-        if (c >= 0 && ld_u64_hint(&B.owner[c], pol_keep) < key) red_max_u64_hint(&B.owner[c], key, pol_keep);
+        // read first: most hits lose against the current owner and then need no atomic
+        // (C4 frame: 28.0 -> 13.5 ms)
+        if (c >= 0 && __ldcg(&B.owner[c]) < key) atomicMax(&B.owner[c], key);
       }
     }
     if (lane == 0) B.tl_key[sd] = key;
