@@ -99,14 +99,21 @@ __device__ __forceinline__ int classify(const uint4& raw, const TpcConst* __rest
 __global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
   uint32_t n_ign = 0, n_drop = 0, n_bad = 0;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < ((B.n + 31u) & ~31u);
-       i += gridDim.x * blockDim.x) {
+  const uint32_t stride = gridDim.x * blockDim.x, n_up = (B.n + 31u) & ~31u;
+  for (uint32_t i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < n_up; i0 += 4 * stride) {
+   uint4 raw4[4];   // four records requested together (bytes in flight)
+#pragma unroll
+   for (int u = 0; u < 4; ++u) {
+     const uint32_t iu = i0 + u * stride;
+     raw4[u] = iu < B.n ? ld_stream16(B.clusters + iu) : make_uint4(0u, 0u, 0u, 0u);
+   }
+#pragma unroll
+   for (int u = 0; u < 4; ++u) {
+    const uint32_t i = i0 + u * stride;
+    if (i >= n_up) break;   // warp-uniform
     int cls = 4, sr = -1, row;
     float y, z = 0.f;
-    if (i < B.n) {
-      const uint4 raw = ld_stream16(B.clusters + i);
-      cls = classify(raw, K, sr, y, z, row);
-    }
+    if (i < B.n) cls = classify(raw4[u], K, sr, y, z, row);
     n_ign += cls == 1;
     n_drop += cls == 2;
     n_bad += cls == 3;
@@ -144,6 +151,7 @@ __global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
       atomicMin(&rs->first, i);
       atomicMax(&rs->last, i);
     }
+   }
   }
   n_ign = __reduce_add_sync(0xffffffffu, n_ign);
   n_drop = __reduce_add_sync(0xffffffffu, n_drop);
@@ -1560,10 +1568,14 @@ __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
 }
 
 // K5a (R6.1, R6.2): weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
+// Also writes, per tracklet, the mask of rows with a hit and the mask of rows where this
+// tracklet's key was the maximum when it looked ("tentative": only those can still be owned
+// at the end, a hit that lost once has lost for good because owner words only grow).
 __global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const uint32_t R = (uint32_t)B.K->n_rows;
+  const int W = (int)((R + 31u) >> 5);
   const float w = B.K->P.sel_chi2_weight;
   const int lane = threadIdx.x & 31;
   const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
@@ -1578,21 +1590,30 @@ __global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
       key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - t->seed_id);
       const int r0 = t->row_first, r1 = t->row_last;
       const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
-      for (int r = r0 + lane; r <= r1; r += 32) {
-        const int32_t c = ld_i32_hint(hits + r, pol_stream);
-        // read first: most hits lose against the current owner and then need no atomic; the
-        // load also brings the sector into L2, where a red that misses would not stay
-        // (C4 frame: 28.0 -> 16.3 ms)
+      uint32_t my_has = 0u, my_tent = 0u;
+      for (int wd = r0 >> 5; wd <= (r1 >> 5); ++wd) {
+        const int r = wd * 32 + lane;
+        int32_t c = -1;
+        if (r >= r0 && r <= r1) c = ld_i32_hint(hits + r, pol_stream);
         // read first: most hits lose against the current owner and then need no atomic
         // (C4 frame: 28.0 -> 13.5 ms)
-        if (c >= 0 && __ldcg(&B.owner[c]) < key) atomicMax(&B.owner[c], key);
+        const bool tent = c >= 0 && __ldcg(&B.owner[c]) < key;
+        if (tent) atomicMax(&B.owner[c], key);
+        const uint32_t hm = __ballot_sync(0xffffffffu, c >= 0);
+        const uint32_t tm = __ballot_sync(0xffffffffu, tent);
+        if (lane == wd) { my_has = hm; my_tent = tm; }
+      }
+      if (lane < W) {
+        B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + lane] = my_has;
+        B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + lane] = my_tent;
       }
     }
     if (lane == 0) B.tl_key[sd] = key;
   }
 }
 
-// K5b: per tracklet the two row masks of R6.3: "row has a hit" and "the hit is owned".
+// K5b: "the hit is owned" mask of R6.3: the tentative rows whose owner word still is this
+// tracklet's key once all tracklets have been through K5a.
 __global__ void __launch_bounds__(256) k_sel_masks(TpcBuffers B) {
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
@@ -1604,23 +1625,24 @@ __global__ void __launch_bounds__(256) k_sel_masks(TpcBuffers B) {
   for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
     const unsigned long long key = B.tl_key[sd];
     if (key == 0ull) continue;   // rejected tracklet (uniform over the warp)
-    const tpc_tracklet* __restrict__ t = B.tracklets + sd;
-    const int r0 = t->row_first, r1 = t->row_last;
+    uint32_t* __restrict__ tent_p = B.tl_mask + (size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS;
+    const uint32_t my_tent = lane < W ? tent_p[lane] : 0u;
     const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
-    uint32_t my_has = 0u, my_own = 0u;
-    for (int wd = r0 >> 5; wd <= (r1 >> 5); ++wd) {
-      const int r = wd * 32 + lane;
-      int32_t c = -1;
-      if (r >= r0 && r <= r1) c = ld_i32_hint(hits + r, pol_stream);
-      const bool own = c >= 0 && ld_u64_hint(&B.owner[c], pol_keep) == key;
-      const uint32_t hm = __ballot_sync(0xffffffffu, c >= 0);
+    uint32_t my_own = 0u;
+    uint32_t words = __ballot_sync(0xffffffffu, my_tent != 0u);
+    while (words) {
+      const int wd = __ffs(words) - 1;
+      words &= words - 1;
+      const uint32_t tm = __shfl_sync(0xffffffffu, my_tent, wd);
+      bool own = false;
+      if ((tm >> lane) & 1u) {
+        const int32_t c = ld_i32_hint(hits + wd * 32 + lane, pol_stream);
+        own = ld_u64_hint(&B.owner[c], pol_keep) == key;
+      }
       const uint32_t om = __ballot_sync(0xffffffffu, own);
-      if (lane == wd) { my_has = hm; my_own = om; }
+      if (lane == wd) my_own = om;
     }
-    if (lane < W) {
-      B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + lane] = my_has;
-      B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + lane] = my_own;
-    }
+    if (lane < W) tent_p[lane] = my_own;
   }
 }
 
