@@ -392,10 +392,16 @@ def run_ours(args, rank, world, local_rank):
     # north star: HBM fraction of the grid and neighbour stages
     stages = {}
     grid_names = ("k_row_stats", "k_row_desc", "k_row_sort", "k_zero_bins", "k_bin_hist", "k_bin_scan", "k_scatter", "k_bin_sort")
-    gb = sum(k["work_per_step"] for k in per_kernel if k["name"] in grid_names)
+    # both grid paths are enqueued, the one k_row_desc did not choose returns at once: count only
+    # the path that ran (the other's launches cost a few microseconds and move no data)
+    kms = {k["name"]: k["ms_per_step"] for k in per_kernel}
+    by_rows = kms.get("k_row_sort", 0.0) > kms.get("k_scatter", 0.0)
+    idle = ("k_zero_bins", "k_bin_hist", "k_bin_scan", "k_scatter", "k_bin_sort") if by_rows else ("k_row_sort",)
+    gb = sum(k["work_per_step"] for k in per_kernel if k["name"] in grid_names and k["name"] not in idle)
     gms = sum(k["ms_per_step"] for k in per_kernel if k["name"] in grid_names)
     nb = next((k for k in per_kernel if k["name"] == "k_neighbours"), None)
     if gms:
+        stages["grid_path"] = "per-row build (k_row_sort)" if by_rows else "generic (histogram, scan, scatter)"
         stages["grid"] = {"ms": gms, "GB/s": gb / gms / 1e6, "frac_hbm": gb / gms / 1e6 / hbm_peak}
     if nb and nb["ms_per_step"]:
         stages["neighbours"] = {"ms": nb["ms_per_step"], "GB/s": nb["work_per_step"] / nb["ms_per_step"] / 1e6,
@@ -421,7 +427,7 @@ def run_ours(args, rank, world, local_rank):
                    "l2": "inputs larger than L2 (frame %.2f GB + workspace %.1f GB)" % (n * 16 / 1e9, ws_bytes / 1e9),
                    "n_seeds": int(v.n_seeds), "n_tracklets": int(v.n_tracklets), "n_tracks": int(v.n_tracks),
                    "n_bins": int(v.n_bins), "follow_steps": st["follow_steps"],
-                   "follow_updates": st["follow_updates"], "follow_cands": st["follow_cands"],
+                   "follow_updates": st["follow_updates"], "follow_cands": st["follow_cands"], "follow_work": st["follow_work"],
                    "generator_s": gen_s},
         "time_frames_per_s": world * args.steps / (ms_total * 1e-3),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,

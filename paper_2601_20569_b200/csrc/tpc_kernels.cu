@@ -1269,7 +1269,6 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
       const bool extrap = phase == PH_UP;
       const int rn = r + 1;
       bool fin = false;
-      if (extrap && pb != TPC_NO_BIN) prefetch_l1(yz + pb);
       if (rn >= F.R) {
         fin = true;  // ran off the pad plane
       } else {
@@ -1283,12 +1282,15 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
           int32_t c_nxt2 = -1;
           float2 m_nxt = make_float2(0.f, 0.f);
           if (extrap) {
+            // two rows ahead: the bin index entry of row r+2 is requested now, the clusters of
+            // row r+1 (entry requested one step ago) are pulled into L1 now
+            if (pb != TPC_NO_BIN) prefetch_l1(yz + pb);
             pb = TPC_NO_BIN;
-            if (r + 1 < F.R) {
-              const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)(r + 1));
+            if (r + 2 < F.R) {
+              const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)(r + 2));
               if (dn.count) {  // linear continuation of this step
-                const int by = bin_coord(k.y + (k.y - y_prev), dn.y0, inv_dy, dn.ny);
-                const int bz = bin_coord(k.z + (k.z - z_prev), dn.z0, inv_dz, dn.nz);
+                const int by = bin_coord(k.y + 2.f * (k.y - y_prev), dn.y0, inv_dy, dn.ny);
+                const int bz = bin_coord(k.z + 2.f * (k.z - z_prev), dn.z0, inv_dz, dn.nz);
                 pb = bin_start[dn.bin_ofs + (uint32_t)bz * (uint32_t)dn.ny + (uint32_t)by];
               }
             }
@@ -1504,7 +1506,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
           fin = true;
         } else {
           r = rn;
-          pb = TPC_NO_BIN;
+          pb = TPC_NO_BIN;   // (inward legs are short: one row ahead measured better than two)
           if (r - 1 >= 0) {
             const tpc_row_desc dn = ld_row_desc(B.row_desc + sr_base + (uint32_t)(r - 1));
             if (dn.count) {
