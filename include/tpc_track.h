@@ -141,6 +141,9 @@ typedef struct tpc_track_view {
   uint64_t n_follow_candidates;     /* ... and chi2 evaluations of road candidates       */
   uint64_t follow_work[3][3];       /* the same three counters per follower kernel:
                                        [outward | refit | inward][steps, updates, candidates] */
+  uint64_t grid_by_rows;            /* 1: the grid was built row by row in shared memory (every
+                                       row's records contiguous in the input and small enough),
+                                       0: by the generic histogram / scan / scatter kernels  */
 } tpc_track_view;
 
 /* One row of the search grid. */

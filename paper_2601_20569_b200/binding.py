@@ -67,7 +67,8 @@ class TrackView(C.Structure):
                 ("n_ignored", C.c_uint64), ("n_dropped", C.c_uint64), ("n_seeds", C.c_uint64),
                 ("n_tracklets", C.c_uint64), ("n_bins", C.c_uint64),
                 ("n_follow_steps", C.c_uint64), ("n_follow_updates", C.c_uint64),
-                ("n_follow_candidates", C.c_uint64), ("follow_work", (C.c_uint64 * 3) * 3)]
+                ("n_follow_candidates", C.c_uint64), ("follow_work", (C.c_uint64 * 3) * 3),
+                ("grid_by_rows", C.c_uint64)]
 
 
 class DebugView(C.Structure):

@@ -294,6 +294,7 @@ int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out) {
     out->n_follow_candidates += c.follow_work[a][2];
     for (int b = 0; b < 3; ++b) out->follow_work[a][b] = c.follow_work[a][b];
   }
+  out->grid_by_rows = c.grid_rows;
   return rc;
 }
 

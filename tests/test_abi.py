@@ -25,7 +25,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.GeomDesc) == 40
     assert ctypes.sizeof(B.Params) == 120
     assert B.Params.max_bins.offset == 96 and B.Params.max_seeds.offset == 104
-    assert ctypes.sizeof(B.TrackView) == 176 and ctypes.sizeof(B.DebugView) == 136
+    assert ctypes.sizeof(B.TrackView) == 184 and ctypes.sizeof(B.DebugView) == 136
 
 
 def test_host_only_calls_without_gpu():

@@ -41,7 +41,7 @@ def run_gpu(B, clusters, gparams=None, flags=DET, geom=None):
         trk.close()
 
 
-def assert_det_parity(B, clusters, **pkw):
+def assert_det_parity(B, clusters, grid_by_rows=None, **pkw):
     gp, op = params_pair(B, **pkw)
     tracks, ids, shared, view, gi = run_gpu(B, clusters, gp, DET)
     o = oracle.run(clusters, params=op, n_threads=8)
@@ -54,24 +54,26 @@ def assert_det_parity(B, clusters, **pkw):
     assert view.n_seeds == o.n_seeds and view.n_tracklets == o.n_tracklets
     assert view.n_tracks == o.n_tracks and view.n_cluster_ids == o.n_cluster_ids
     assert view.n_ignored == o.n_ignored and view.n_dropped == o.n_dropped
+    if grid_by_rows is not None:   # which of the two grid builds ran (both are checked against the oracle)
+        assert view.grid_by_rows == grid_by_rows
     return o, tracks
 
 
 def test_det_parity_c1(B):
     cl, _, _ = dg.generate(dg.preset("C1"))
-    o, _ = assert_det_parity(B, cl)
+    o, _ = assert_det_parity(B, cl, grid_by_rows=1)
     assert o.n_tracks > 50
 
 
 def test_det_parity_c2_reduced_all_sectors(B):
     cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=1500))
-    o, _ = assert_det_parity(B, cl)
+    o, _ = assert_det_parity(B, cl, grid_by_rows=1)
     assert o.n_tracks > 1500 and len(np.unique(o.tracks["sector"])) == 36
 
 
 def test_det_parity_c3_reduced_overlapping_events(B):
     cl, _, _ = dg.generate(dg.preset("C3", tracks_per_event=500))
-    o, _ = assert_det_parity(B, cl)
+    o, _ = assert_det_parity(B, cl, grid_by_rows=1)
     assert o.n_tracks > 1500
 
 
@@ -94,7 +96,7 @@ def test_det_parity_shuffled_input_and_ragged_sizes(B):
     cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=700, seed=31))
     rng = np.random.default_rng(0)
     cl = cl[rng.permutation(len(cl))][: len(cl) - 37]
-    assert_det_parity(B, cl)
+    assert_det_parity(B, cl, grid_by_rows=0)      # generic histogram / scan / scatter path
 
 
 def test_det_parity_other_bin_sizes(B):
@@ -207,16 +209,19 @@ def test_det_parity_full_c2_bench_configuration(B):
 
 
 def test_det_parity_full_c4_sampled_sectors(B):
-    """BASELINE.json configs[3], the headline workload, at a size the oracle can still check:
-    the whole 2.8 ms frame shape (140 events) at 1/4 of the track multiplicity is tracked in
-    the launch configuration bench.py times; two sampled sectors are compared bit by bit with
-    the oracle (sectors are independent, tests/test_oracle_path.py::test_sectors_are_independent)."""
-    cl, lab, _ = dg.generate(dg.preset("C4", tracks_per_event=3000))
-    gp = B.tpc_default_params(grid_dy=4.0, grid_dz=4.0)
+    """BASELINE.json configs[3], the headline workload, at FULL size (140 events x 12000 tracks,
+    ~2.4e8 clusters) with the tracker parameters and launch configuration bench.py times; two
+    sampled sectors are compared bit by bit with the oracle (sectors are independent,
+    tests/test_oracle_path.py::test_sectors_are_independent; one sector takes the oracle ~12 s)."""
+    import bench
+    pkw = bench.WORKLOAD_PARAMS["C4"]
+    cl, lab, _ = dg.generate(dg.preset("C4"))
+    assert len(cl) > 2.0e8
+    gp = B.tpc_default_params(**pkw)
     tracks, ids, shared, view, _ = run_gpu(B, cl, gp, 1)
+    assert view.grid_by_rows == 1                  # the per-row grid build, as in the bench
     for s in (5, 23):
-        o = oracle.run(cl, params=oracle.default_params(grid_dy=4.0, grid_dz=4.0), sector_lo=s, sector_hi=s + 1,
-                       want=("tracks",))
+        o = oracle.run(cl, params=oracle.default_params(**pkw), sector_lo=s, sector_hi=s + 1, want=("tracks",))
         bad = parity.compare_tracks(tracks, ids, shared, o, sector=s)
         assert parity.all_zero(bad), (s, bad)
-        assert o.n_tracks > 1000
+        assert o.n_tracks > 10000
