@@ -1569,82 +1569,159 @@ __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
     p4[i] = make_uint4(0, 0, 0, 0);
 }
 
+// K5a / K5b work on TILES of 32 consecutive tracklets of the seed list (one CTA per tile at a
+// time, lane = tracklet, the 8 warps share the rows in groups of four: one 16-byte load per
+// lane, the other half of each sector is read by the next warp).  The tracklets of a tile (and
+// of the tiles that run at the same time) come from the same z-slab of one sector and are
+// processed row by row, so their owner words sit in a few KB per row and stay in L2.  The per-row ballots are transposed through shared
+// memory into per-tracklet row masks, stored [word][tracklet].
+#define TPC_SEL_BLOCK 256
+#define TPC_SEL_UNROLL 4   // rows per load: row_hit rows are 16-byte aligned when n_rows % 4 == 0
+
+// hits of rows rb..rb+3 of one tracklet (p = its row_hit row), -1 where `want` is false
+__device__ __forceinline__ void load_hits4(const int32_t* __restrict__ p, int rb, int R, bool vec, const bool (&want)[4],
+                                           int32_t (&c)[4]) {
+  c[0] = c[1] = c[2] = c[3] = -1;
+  if (!(want[0] || want[1] || want[2] || want[3])) return;
+  if (vec) {
+    const int4 v = __ldcs(reinterpret_cast<const int4*>(p + rb));
+    if (want[0]) c[0] = v.x;
+    if (want[1]) c[1] = v.y;
+    if (want[2]) c[2] = v.z;
+    if (want[3]) c[3] = v.w;
+  } else {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) if (want[u] && rb + u < R) c[u] = __ldcs(p + rb + u);
+  }
+}
+
+__device__ __forceinline__ unsigned long long tracklet_key(const tpc_tracklet* __restrict__ t, float w) {
+  const int nh = t->n_hits;
+  if (nh <= 0) return 0ull;
+  const int ndf = 2 * nh - 5;
+  const float Q = (float)nh - w * (t->chi2 / (float)ndf);
+  return ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - t->seed_id);
+}
+
+// bits[r] holds, for row r, one bit per tracklet of the tile -> word w of tracklet `lane`
+__device__ __forceinline__ uint32_t transpose_rows(const uint32_t* __restrict__ bits, int w, int lane, int R) {
+  uint32_t m = 0u;
+#pragma unroll 8
+  for (int b = 0; b < 32; ++b) {
+    const int r = w * 32 + b;
+    if (r < R) m |= ((bits[r] >> lane) & 1u) << b;
+  }
+  return m;
+}
+
 // K5a (R6.1, R6.2): weight -> 64-bit key; per-cluster owner = max key (64-bit atomicMax).
 // Also writes, per tracklet, the mask of rows with a hit and the mask of rows where this
 // tracklet's key was the maximum when it looked ("tentative": only those can still be owned
 // at the end, a hit that lost once has lost for good because owner words only grow).
-__global__ void __launch_bounds__(256) k_sel_owner(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_SEL_BLOCK) k_sel_owner(TpcBuffers B) {
+  __shared__ unsigned long long s_key[32];
+  __shared__ int s_r0[32], s_r1[32];
+  __shared__ uint32_t s_has[TPC_MAX_ROWS], s_tent[TPC_MAX_ROWS];
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
-  const uint32_t R = (uint32_t)B.K->n_rows;
-  const int W = (int)((R + 31u) >> 5);
+  const int R = B.K->n_rows;
+  const int W = (R + 31) >> 5;
   const float w = B.K->P.sel_chi2_weight;
-  const int lane = threadIdx.x & 31;
-  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
-  const uint64_t pol_stream = l2_policy_evict_first();
-  for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
-    const tpc_tracklet* __restrict__ t = B.tracklets + sd;
-    const int nh = t->n_hits;
-    unsigned long long key = 0ull;
-    if (nh > 0) {
-      const int ndf = 2 * nh - 5;
-      const float Q = (float)nh - w * (t->chi2 / (float)ndf);
-      key = ((unsigned long long)f2key(Q) << 32) | (unsigned long long)(0xFFFFFFFFu - t->seed_id);
-      const int r0 = t->row_first, r1 = t->row_last;
-      const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
-      uint32_t my_has = 0u, my_tent = 0u;
-      for (int wd = r0 >> 5; wd <= (r1 >> 5); ++wd) {
-        const int r = wd * 32 + lane;
-        int32_t c = -1;
-        if (r >= r0 && r <= r1) c = ld_i32_hint(hits + r, pol_stream);
-        // read first: most hits lose against the current owner and then need no atomic
-        // (C4 frame: 28.0 -> 13.5 ms)
-        const bool tent = c >= 0 && __ldcg(&B.owner[c]) < key;
-        if (tent) atomicMax(&B.owner[c], key);
-        const uint32_t hm = __ballot_sync(0xffffffffu, c >= 0);
-        const uint32_t tm = __ballot_sync(0xffffffffu, tent);
-        if (lane == wd) { my_has = hm; my_tent = tm; }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t hstride = B.max_seeds;
+  const uint32_t n_tiles = (n_seeds + 31u) >> 5;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const uint32_t sd = tile * 32u + (uint32_t)lane;
+    __syncthreads();   // the previous tile is done with the shared arrays
+    if (warp == 0) {
+      unsigned long long key = 0ull;
+      int r0 = 0x7fffffff, r1 = -1;
+      if (sd < n_seeds) {
+        const tpc_tracklet* __restrict__ t = B.tracklets + sd;
+        key = tracklet_key(t, w);
+        if (key) { r0 = t->row_first; r1 = t->row_last; }
+        B.tl_key[sd] = key;
       }
-      if (lane < W) {
-        B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + lane] = my_has;
-        B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + lane] = my_tent;
+      s_key[lane] = key; s_r0[lane] = r0; s_r1[lane] = r1;
+    }
+    for (int r = threadIdx.x; r < R; r += TPC_SEL_BLOCK) { s_has[r] = 0u; s_tent[r] = 0u; }
+    __syncthreads();
+    const unsigned long long key = s_key[lane];
+    const int r0 = s_r0[lane], r1 = s_r1[lane];
+    const int t0 = __reduce_min_sync(0xffffffffu, r0), t1 = __reduce_max_sync(0xffffffffu, r1);
+    const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * (size_t)R;
+    const bool vec = (R & 3) == 0;
+    for (int rb = (t0 & ~3) + warp * TPC_SEL_UNROLL; rb <= t1; rb += (TPC_SEL_BLOCK / 32) * TPC_SEL_UNROLL) {
+      int32_t c[TPC_SEL_UNROLL];
+      unsigned long long o[TPC_SEL_UNROLL];
+      bool want[TPC_SEL_UNROLL];
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) want[u] = rb + u >= r0 && rb + u <= r1;
+      load_hits4(hits, rb, R, vec, want, c);
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) o[u] = c[u] >= 0 ? __ldcg(&B.owner[c[u]]) : ~0ull;
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) {
+        // read first: most hits lose against the current owner and then need no atomic
+        const bool tent = o[u] < key;
+        if (tent) atomicMax(&B.owner[c[u]], key);
+        const uint32_t hm = __ballot_sync(0xffffffffu, c[u] >= 0);
+        const uint32_t tm = __ballot_sync(0xffffffffu, tent);
+        if (lane == 0 && rb + u < R) { s_has[rb + u] = hm; s_tent[rb + u] = tm; }
       }
     }
-    if (lane == 0) B.tl_key[sd] = key;
+    __syncthreads();
+    if (warp < W && sd < n_seeds && key) {
+      B.tl_mask[(size_t)warp * hstride + sd] = transpose_rows(s_has, warp, lane, R);
+      B.tl_mask[(size_t)(TPC_MASK_WORDS + warp) * hstride + sd] = transpose_rows(s_tent, warp, lane, R);
+    }
   }
 }
 
 // K5b: "the hit is owned" mask of R6.3: the tentative rows whose owner word still is this
 // tracklet's key once all tracklets have been through K5a.
-__global__ void __launch_bounds__(256) k_sel_masks(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_SEL_BLOCK) k_sel_masks(TpcBuffers B) {
+  __shared__ uint32_t s_tw[TPC_MASK_WORDS][32];   // tentative words of the tile's tracklets
+  __shared__ uint32_t s_own[TPC_MAX_ROWS];
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
-  const uint32_t R = (uint32_t)B.K->n_rows;
-  const int W = (int)((R + 31u) >> 5);
-  const int lane = threadIdx.x & 31;
-  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
-  const uint64_t pol_stream = l2_policy_evict_first(), pol_keep = l2_policy_evict_last();
-  for (uint32_t sd = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; sd < n_seeds; sd += n_warps) {
-    const unsigned long long key = B.tl_key[sd];
-    if (key == 0ull) continue;   // rejected tracklet (uniform over the warp)
-    uint32_t* __restrict__ tent_p = B.tl_mask + (size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS;
-    const uint32_t my_tent = lane < W ? tent_p[lane] : 0u;
-    const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * R;
-    uint32_t my_own = 0u;
-    uint32_t words = __ballot_sync(0xffffffffu, my_tent != 0u);
-    while (words) {
-      const int wd = __ffs(words) - 1;
-      words &= words - 1;
-      const uint32_t tm = __shfl_sync(0xffffffffu, my_tent, wd);
-      bool own = false;
-      if ((tm >> lane) & 1u) {
-        const int32_t c = ld_i32_hint(hits + wd * 32 + lane, pol_stream);
-        own = ld_u64_hint(&B.owner[c], pol_keep) == key;
+  const int R = B.K->n_rows;
+  const int W = (R + 31) >> 5;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t hstride = B.max_seeds;
+  const uint32_t n_tiles = (n_seeds + 31u) >> 5;
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const uint32_t sd = tile * 32u + (uint32_t)lane;
+    const unsigned long long key = sd < n_seeds ? B.tl_key[sd] : 0ull;
+    __syncthreads();
+    if (warp < W) s_tw[warp][lane] = key ? B.tl_mask[(size_t)(TPC_MASK_WORDS + warp) * hstride + sd] : 0u;
+    for (int r = threadIdx.x; r < R; r += TPC_SEL_BLOCK) s_own[r] = 0u;
+    __syncthreads();
+    const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * (size_t)R;
+    const bool vec = (R & 3) == 0;
+    for (int rb = warp * TPC_SEL_UNROLL; rb < R; rb += (TPC_SEL_BLOCK / 32) * TPC_SEL_UNROLL) {
+      int32_t c[TPC_SEL_UNROLL];
+      bool own[TPC_SEL_UNROLL];
+      bool want[TPC_SEL_UNROLL];
+      bool any = false;
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) {
+        const int r = rb + u;
+        want[u] = r < R && ((s_tw[r >> 5][lane] >> (r & 31)) & 1u);
+        any |= want[u];
       }
-      const uint32_t om = __ballot_sync(0xffffffffu, own);
-      if (lane == wd) my_own = om;
+      if (!__any_sync(0xffffffffu, any)) continue;
+      load_hits4(hits, rb, R, vec, want, c);
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) own[u] = c[u] >= 0 && __ldcg(&B.owner[c[u]]) == key;
+#pragma unroll
+      for (int u = 0; u < TPC_SEL_UNROLL; ++u) {
+        const uint32_t om = __ballot_sync(0xffffffffu, own[u]);
+        if (lane == 0 && rb + u < R) s_own[rb + u] = om;
+      }
     }
-    if (lane < W) tent_p[lane] = my_own;
+    __syncthreads();
+    if (warp < W && key) B.tl_mask[(size_t)(TPC_MASK_WORDS + warp) * hstride + sd] = transpose_rows(s_own, warp, lane, R);
   }
 }
 
@@ -1666,8 +1743,8 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
   for (int w = 0; w < TPC_MASK_WORDS; ++w) {
     has[w] = 0u; own[w] = 0u; acc[w] = 0u; shm[w] = 0u;
     if (w * 32 < R) {
-      has[w] = B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + w];
-      own[w] = B.tl_mask[(size_t)sd * (2 * TPC_MASK_WORDS) + TPC_MASK_WORDS + w];
+      has[w] = B.tl_mask[(size_t)w * B.max_seeds + sd];                      // [word][tracklet]
+      own[w] = B.tl_mask[(size_t)(TPC_MASK_WORDS + w) * B.max_seeds + sd];
     }
   }
   int n_acc = 0, n_sh = 0, gap = 0, seg_last = -1, seg_first = -1;
@@ -1912,9 +1989,9 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   // ---- K5 ambiguity solving
   k_zero_owner<<<grid_for(B.n / 2 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_owner");
-  k_sel_owner<<<grid_for((uint64_t)B.max_seeds * 32, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_sel_owner<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, 8), TPC_SEL_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_owner");
-  k_sel_masks<<<grid_for((uint64_t)B.max_seeds * 32, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_sel_masks<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, 8), TPC_SEL_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_masks");
   k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_count");
