@@ -769,26 +769,65 @@ __device__ __forceinline__ uint32_t seed_item(const TpcBuffers& B, uint32_t sr, 
 }
 
 // R4 pass A: start hits (no down link, an up link, chain >= seed_min_len); per-block counts.
-__global__ void __launch_bounds__(1024) k_seed_flags(TpcBuffers B) {
+// A block covers TPC_SEED_SPAN consecutive sorted positions, four per thread (16-byte loads of
+// the links, one packed store of the four flags).
+#define TPC_SEED_BLOCK 256
+#define TPC_SEED_SPAN (4 * TPC_SEED_BLOCK)
+
+// (sector,row) of position i, searched upward from the row of the block's first position
+// (rows are long against a block's span, so this is zero or one step)
+__device__ __forceinline__ uint32_t sr_from(const TpcBuffers& B, uint32_t sr, uint32_t i) {
+  while (sr + 1 < B.n_sr && B.row_desc[sr + 1].clu_ofs <= i) ++sr;
+  return sr;
+}
+
+__global__ void __launch_bounds__(TPC_SEED_BLOCK) k_seed_flags(TpcBuffers B) {
   __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_sr;
   if (B.cnt->error & TPC_DEVERR_BINS) return;
   const uint32_t n = B.cnt->n_sorted;
   const int min_len = B.K->P.seed_min_len;
-  const uint32_t n_blocks = (n + blockDim.x - 1) / blockDim.x;
+  const uint32_t n_blocks = (n + TPC_SEED_SPAN - 1) / TPC_SEED_SPAN;
+  const int32_t* __restrict__ up2 = B.link_up2;
   for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
-    const uint32_t i = blk * blockDim.x + threadIdx.x;
-    uint32_t len = 0;
-    if (i < n && B.link_dn2[i] < 0 && B.link_up2[i] >= 0) {
-      // only "at least seed_min_len" is decided here; the full chain length is counted by the
-      // follower's chain fit, which walks the chain anyway (k_follow_up -> seed_len[])
-      len = 1;
-      for (int32_t c = B.link_up2[i]; c >= 0 && (int)len < min_len; c = B.link_up2[c]) ++len;
-      if ((int)len < min_len) len = 0;
-      if (len) atomicAdd(&B.item_cnt[seed_item(B, sr_of_position(B, i), i)], 1u);
+    const uint32_t i0 = blk * TPC_SEED_SPAN + threadIdx.x * 4;
+    __syncthreads();
+    if (threadIdx.x == 0) s_sr = sr_of_position(B, blk * TPC_SEED_SPAN);
+    int32_t dn[4] = {0, 0, 0, 0}, up[4] = {-1, -1, -1, -1};
+    if (i0 + 3 < n) {   // link arrays are 256-byte aligned, i0 is a multiple of 4
+      const int4 d4 = *reinterpret_cast<const int4*>(B.link_dn2 + i0);
+      const int4 u4 = *reinterpret_cast<const int4*>(up2 + i0);
+      dn[0] = d4.x; dn[1] = d4.y; dn[2] = d4.z; dn[3] = d4.w;
+      up[0] = u4.x; up[1] = u4.y; up[2] = u4.z; up[3] = u4.w;
+    } else {
+      for (int u = 0; u < 4; ++u) if (i0 + u < n) { dn[u] = B.link_dn2[i0 + u]; up[u] = up2[i0 + u]; }
     }
-    if (i < n) B.seed_len[i] = (uint8_t)len;
+    uint32_t flags = 0, cnt = 0;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (dn[u] < 0 && up[u] >= 0) {
+        // only "at least seed_min_len" is decided here; the full chain length is counted by the
+        // follower's chain fit, which walks the chain anyway (k_follow_up -> seed_len[])
+        int len = 1;
+        for (int32_t c = up[u]; c >= 0 && len < min_len; c = up2[c]) ++len;
+        if (len >= min_len) { flags |= 1u << (8 * u); ++cnt; }
+      }
+    }
+    __syncthreads();   // s_sr
+    if (flags) {
+      uint32_t sr = s_sr;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if ((flags >> (8 * u)) & 1u) {
+          sr = sr_from(B, sr, i0 + u);
+          atomicAdd(&B.item_cnt[seed_item(B, sr, i0 + u)], 1u);
+        }
+      }
+    }
+    if (i0 + 3 < n) *reinterpret_cast<uint32_t*>(B.seed_len + i0) = flags;
+    else for (int u = 0; u < 4; ++u) if (i0 + u < n) B.seed_len[i0 + u] = (uint8_t)((flags >> (8 * u)) & 1u);
     uint32_t tot;
-    block_excl_scan(len ? 1u : 0u, &tot, sm);
+    block_excl_scan(cnt, &tot, sm);
     if (threadIdx.x == 0) B.scan_partials[blk] = tot;
   }
 }
@@ -853,21 +892,34 @@ __global__ void __launch_bounds__(1024) k_seed_items(TpcBuffers B) {
 
 // R4 pass B: write the seed list, ordered by (sector, z-slab, row, sorted index) — a pure
 // function of the input in deterministic mode.
-__global__ void __launch_bounds__(1024) k_seed_write(TpcBuffers B) {
+__global__ void __launch_bounds__(TPC_SEED_BLOCK) k_seed_write(TpcBuffers B) {
   __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_sr;
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n = B.cnt->n_sorted;
-  const uint32_t n_blocks = (n + blockDim.x - 1) / blockDim.x;
+  const uint32_t n_blocks = (n + TPC_SEED_SPAN - 1) / TPC_SEED_SPAN;
   for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
-    const uint32_t i = blk * blockDim.x + threadIdx.x;
-    const uint32_t f = (i < n && B.seed_len[i]) ? 1u : 0u;
+    const uint32_t i0 = blk * TPC_SEED_SPAN + threadIdx.x * 4;
+    __syncthreads();
+    if (threadIdx.x == 0) s_sr = sr_of_position(B, blk * TPC_SEED_SPAN);
+    uint32_t flags = 0;
+    if (i0 + 3 < n) flags = *reinterpret_cast<const uint32_t*>(B.seed_len + i0);
+    else for (int u = 0; u < 4; ++u) if (i0 + u < n && B.seed_len[i0 + u]) flags |= 1u << (8 * u);
+    flags &= 0x01010101u;
     uint32_t tot;
-    const uint32_t pre = block_excl_scan(f, &tot, sm);
-    if (f) {
-      const uint32_t sr = sr_of_position(B, i);
-      const uint32_t pos = (uint32_t)((int32_t)(B.scan_partials[blk] + pre) + B.item_delta[seed_item(B, sr, i)]);
-      B.seeds[pos] = i;
-      B.seed_sr[pos] = (uint16_t)sr;
+    uint32_t pre = block_excl_scan((uint32_t)__popc(flags), &tot, sm) + B.scan_partials[blk];   // syncs: s_sr is visible
+    if (flags) {
+      uint32_t sr = s_sr;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if ((flags >> (8 * u)) & 1u) {
+          sr = sr_from(B, sr, i0 + u);
+          const uint32_t pos = (uint32_t)((int32_t)pre + B.item_delta[seed_item(B, sr, i0 + u)]);
+          B.seeds[pos] = i0 + u;
+          B.seed_sr[pos] = (uint16_t)sr;
+          ++pre;
+        }
+      }
     }
   }
 }
@@ -1963,7 +2015,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   // ---- K3 cleanup + seeds
   k_link_cleanup<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_link_cleanup");
-  k_seed_flags<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
+  k_seed_flags<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, 8), TPC_SEED_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_seed_flags");
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_sorted, 1024u, &B.cnt->n_seeds, B.max_seeds,
                                       &B.cnt->error, TPC_DEVERR_SEEDS);
@@ -1975,7 +2027,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
     k_seed_items<<<B.n_sectors, 1024, smem, st>>>(B);
   }
   TPC_LAUNCH_CHECK("k_seed_items");
-  k_seed_write<<<grid_for(B.n, 1024, n_sm, 2), 1024, 0, st>>>(B);
+  k_seed_write<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, 8), TPC_SEED_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
