@@ -261,6 +261,24 @@ int tpc_sector_track_host(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t 
                           uint64_t cap_tracks, uint32_t* h_cluster_ids, uint8_t* h_cluster_shared,
                           uint64_t cap_ids, tpc_track_view* out);
 
+/* The same end-to-end call for a frame handed over as n_chunks consecutive parts of
+ * h_clusters: chunk c = records [chunk_ofs[c], chunk_ofs[c+1]) (chunk_ofs: HOST, n_chunks+1
+ * entries, chunk_ofs[0] = 0, chunk_ofs[n_chunks] = n_clusters).  No sector may have records in
+ * two chunks: sectors are the independent units of the sector tracking, so
+ * the chunks are tracked one after the other while the next one is copied in and the previous
+ * one's tracks are copied out (two library-owned copy streams; the kernels run on cuda_stream).
+ * Results: those of one call on the whole frame (cluster ids are indices into h_clusters),
+ * tracks concatenated in chunk order; *out holds the summed counts, its d_* pointers are NULL.
+ * d_staging (DEVICE) holds the whole frame; the workspace must be at least twice
+ * tpc_workspace_bytes(ctx, largest chunk) (else TPC_E_WORKSPACE).  A sector found in two
+ * chunks gives TPC_E_ARG. */
+int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t n_clusters,
+                                 const uint64_t* chunk_ofs, int n_chunks, void* d_staging,
+                                 void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                                 uint32_t flags, tpc_track* h_tracks, uint64_t cap_tracks,
+                                 uint32_t* h_cluster_ids, uint8_t* h_cluster_shared, uint64_t cap_ids,
+                                 tpc_track_view* out);
+
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);
 

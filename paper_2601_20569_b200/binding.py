@@ -82,7 +82,7 @@ class DebugView(C.Structure):
 
 EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
            "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
-           "tpc_sector_track_host", "tpc_last_launch_count",
+           "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -115,6 +115,9 @@ def load_library():
     L.tpc_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.tpc_get_kernel_ms.restype = C.c_int
     L.tpc_get_kernel_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    L.tpc_sector_track_host_chunks.restype = C.c_int
+    L.tpc_sector_track_host_chunks.argtypes = [vp, vp, C.c_uint64, C.POINTER(C.c_uint64), C.c_int, vp, vp, C.c_size_t, vp,
+                                               C.c_uint32, vp, C.c_uint64, vp, vp, C.c_uint64, vp]
     L.tpc_sector_track_host.restype = C.c_int
     L.tpc_sector_track_host.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_size_t, vp, C.c_uint32, vp, C.c_uint64,
                                         vp, vp, C.c_uint64, C.POINTER(TrackView)]
@@ -206,6 +209,18 @@ def tpc_sector_track_host(ctx: int, h_clusters: int, n_clusters: int, d_staging:
     rc = load_library().tpc_sector_track_host(ctx, h_clusters, n_clusters, d_staging, d_workspace, workspace_bytes,
                                               cuda_stream, flags, h_tracks, cap_tracks, h_cluster_ids,
                                               h_cluster_shared, cap_ids, C.byref(v))
+    return rc, v
+
+
+def tpc_sector_track_host_chunks(ctx: int, h_clusters: int, n_clusters: int, chunk_ofs, d_staging: int,
+                                 d_workspace: int, workspace_bytes: int, cuda_stream: int, flags: int,
+                                 h_tracks: int, cap_tracks: int, h_cluster_ids: int, h_cluster_shared: int,
+                                 cap_ids: int):
+    v = TrackView()
+    ofs = (C.c_uint64 * len(chunk_ofs))(*[int(x) for x in chunk_ofs])
+    rc = load_library().tpc_sector_track_host_chunks(ctx, h_clusters, n_clusters, ofs, len(chunk_ofs) - 1, d_staging,
+                                                     d_workspace, workspace_bytes, cuda_stream, flags, h_tracks,
+                                                     cap_tracks, h_cluster_ids, h_cluster_shared, cap_ids, C.byref(v))
     return rc, v
 
 
@@ -328,6 +343,28 @@ class SectorTracker:
                                       h_shared.data_ptr(), min(h_ids.numel() // 4, h_shared.numel()))
         if rc != TPC_OK:
             raise TpcError(rc, "tpc_sector_track_host", tpc_last_cuda_error(self.ctx))
+        self.n = n
+        return v
+
+    def track_host_chunks(self, h_clusters, chunk_ofs, d_staging, h_tracks, h_ids, h_shared, flags: int = 0,
+                          stream=None):
+        """track_host for a frame given as consecutive chunks of whole sectors (chunk_ofs: record
+        offsets, first 0, last n): copy-in, tracking and copy-out of successive chunks overlap."""
+        n = h_clusters.numel() // 16
+        n_max = max(int(chunk_ofs[i + 1]) - int(chunk_ofs[i]) for i in range(len(chunk_ofs) - 1))
+        one = (tpc_workspace_bytes(self.ctx, n_max) + 255) // 256 * 256
+        need = 2 * one
+        if self.workspace is None or self.workspace.numel() < need + 256:
+            self.workspace = None
+            self.workspace = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc, v = tpc_sector_track_host_chunks(self.ctx, h_clusters.data_ptr(), n, chunk_ofs, d_staging.data_ptr(), ws_ptr,
+                                             need, st.cuda_stream, flags, h_tracks.data_ptr(),
+                                             h_tracks.numel() // TRACK_DTYPE.itemsize, h_ids.data_ptr(),
+                                             h_shared.data_ptr(), min(h_ids.numel() // 4, h_shared.numel()))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_sector_track_host_chunks", tpc_last_cuda_error(self.ctx))
         self.n = n
         return v
 

@@ -17,6 +17,10 @@ struct tpc_ctx {
   TpcCounters* d_cnt = nullptr;
   TpcRowStat* d_row_stat = nullptr;
   TpcCounters* h_cnt = nullptr;  // pinned
+  uint32_t* d_sector_seen = nullptr;
+  // chunked host call: copy-in / copy-out streams and their events (ping-pong)
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  cudaEvent_t ev_in[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr}, ev_out[2] = {nullptr, nullptr};
   TpcStageEvents events;
   int n_sm = 148;
   int device = 0;
@@ -193,6 +197,9 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
       (e = cudaMalloc(&c->d_cnt, sizeof(TpcCounters))) != cudaSuccess ||
       (e = cudaMalloc(&c->d_row_stat, sizeof(TpcRowStat) * n_sr)) != cudaSuccess ||
       (e = cudaMallocHost(&c->h_cnt, sizeof(TpcCounters))) != cudaSuccess ||
+      (e = cudaMalloc(&c->d_sector_seen, sizeof(uint32_t) * (size_t)geom->n_sectors)) != cudaSuccess ||
+      (e = cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking)) != cudaSuccess ||
+      (e = cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking)) != cudaSuccess ||
       (e = cudaMemcpy(c->d_const, &K, sizeof(TpcConst), cudaMemcpyHostToDevice)) != cudaSuccess) {
     std::fprintf(stderr, "tpc_geom_init: %s\n", cudaGetErrorString(e));
     tpc_destroy(c);
@@ -214,6 +221,14 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
       return TPC_E_CUDA;
     }
   }
+  for (int i = 0; i < 2; ++i) {
+    if ((e = cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev_out[i], cudaEventDisableTiming)) != cudaSuccess) {
+      tpc_destroy(c);
+      return TPC_E_CUDA;
+    }
+  }
   *out = c;
   return TPC_OK;
 }
@@ -223,8 +238,8 @@ size_t tpc_workspace_bytes(const tpc_ctx* ctx, uint64_t n_clusters) {
   return carve(ctx, n_clusters, nullptr, nullptr);
 }
 
-int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters, void* d_workspace,
-                     size_t workspace_bytes, void* cuda_stream, uint32_t flags) {
+static int enqueue_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters, void* d_workspace,
+                         size_t workspace_bytes, void* cuda_stream, uint32_t flags, uint32_t id_base, uint32_t chunk_tag) {
   if (!ctx || !d_workspace || (!d_clusters && n_clusters) || n_clusters >= (1ull << 30)) return TPC_E_ARG;
   if (((uintptr_t)d_clusters & 15u) || ((uintptr_t)d_workspace & 255u)) return TPC_E_ARG;
   TpcBuffers B;
@@ -234,6 +249,9 @@ int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clu
   B.K = ctx->d_const;
   B.cnt = ctx->d_cnt;
   B.row_stat = ctx->d_row_stat;
+  B.id_base = id_base;
+  B.chunk_tag = chunk_tag;
+  B.sector_seen = ctx->d_sector_seen;
   ctx->buf = B;
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->flags = flags;
@@ -252,6 +270,11 @@ int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clu
   return TPC_OK;
 }
 
+int tpc_sector_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters, void* d_workspace,
+                     size_t workspace_bytes, void* cuda_stream, uint32_t flags) {
+  return enqueue_track(ctx, d_clusters, n_clusters, d_workspace, workspace_bytes, cuda_stream, flags, 0u, 0u);
+}
+
 static int sync_run(tpc_ctx* ctx) {
   if (!ctx) return TPC_E_ARG;
   if (!ctx->ran) return TPC_E_STATE;
@@ -266,7 +289,7 @@ static int sync_run(tpc_ctx* ctx) {
 static int device_status(const tpc_ctx* ctx) {
   const uint32_t err = ctx->h_cnt->error;
   if (err & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return TPC_E_OVERFLOW;
-  if (err & TPC_DEVERR_BAD_CLUSTER) return TPC_E_ARG;
+  if (err & (TPC_DEVERR_BAD_CLUSTER | TPC_DEVERR_CHUNKS)) return TPC_E_ARG;
   return TPC_OK;
 }
 
@@ -388,6 +411,94 @@ int tpc_sector_track_host(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t 
   return TPC_OK;
 }
 
+// cluster_ofs of a chunk's tracks refers to the chunk's own id list: shift it to the frame's
+__global__ void k_shift_tracks(tpc_track* tracks, uint32_t n, uint32_t ids_base) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) tracks[i].cluster_ofs += ids_base;
+}
+
+int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t n_clusters,
+                                 const uint64_t* chunk_ofs, int n_chunks, void* d_staging, void* d_workspace,
+                                 size_t workspace_bytes, void* cuda_stream, uint32_t flags, tpc_track* h_tracks,
+                                 uint64_t cap_tracks, uint32_t* h_cluster_ids, uint8_t* h_cluster_shared,
+                                 uint64_t cap_ids, tpc_track_view* out) {
+  if (!ctx || !out || !chunk_ofs || n_chunks < 1 || (!h_clusters && n_clusters) || (!d_staging && n_clusters) ||
+      !d_workspace || n_clusters >= (1ull << 30))
+    return TPC_E_ARG;
+  if (chunk_ofs[0] != 0 || chunk_ofs[n_chunks] != n_clusters) return TPC_E_ARG;
+  uint64_t n_max = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    if (chunk_ofs[c + 1] < chunk_ofs[c]) return TPC_E_ARG;
+    const uint64_t nc = chunk_ofs[c + 1] - chunk_ofs[c];
+    n_max = nc > n_max ? nc : n_max;
+  }
+  // two workspaces, used alternately: the results of chunk c are read back while chunk c+1 runs
+  const size_t ws_one = align_up(carve(ctx, n_max, nullptr, nullptr), 256);
+  if (((uintptr_t)d_workspace & 255u) || workspace_bytes < 2 * ws_one) return TPC_E_WORKSPACE;
+  char* ws[2] = {(char*)d_workspace, (char*)d_workspace + ws_one};
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t e;
+  std::memset(out, 0, sizeof(*out));
+  if ((e = cudaMemsetAsync(ctx->d_sector_seen, 0, sizeof(uint32_t) * (size_t)ctx->geom.n_sectors, st)) != cudaSuccess)
+    return set_cuda_err(ctx, e, "cudaMemsetAsync(sector_seen)");
+  // the copy streams start after whatever the caller has enqueued on `st`
+  if ((e = cudaEventRecord(ctx->ev_done[0], st)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaEventRecord");
+  cudaStreamWaitEvent(ctx->s_in, ctx->ev_done[0], 0);
+  cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[0], 0);
+  auto copy_in = [&](int c) -> cudaError_t {
+    const uint64_t o = chunk_ofs[c], nc = chunk_ofs[c + 1] - o;
+    if (nc) {
+      cudaError_t ee = cudaMemcpyAsync((tpc_cluster*)d_staging + o, h_clusters + o, nc * sizeof(tpc_cluster),
+                                       cudaMemcpyHostToDevice, ctx->s_in);
+      if (ee != cudaSuccess) return ee;
+    }
+    return cudaEventRecord(ctx->ev_in[c & 1], ctx->s_in);
+  };
+  if ((e = copy_in(0)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(clusters)");
+  uint64_t n_tracks = 0, n_ids = 0;
+  int rc_all = TPC_OK, launches = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const uint64_t o = chunk_ofs[c], nc = chunk_ofs[c + 1] - o;
+    cudaStreamWaitEvent(st, ctx->ev_in[c & 1], 0);                    // chunk c is on the device
+    if (c >= 2) cudaStreamWaitEvent(st, ctx->ev_out[c & 1], 0);       // workspace c&1 has been read back
+    int rc = enqueue_track(ctx, (const tpc_cluster*)d_staging + o, nc, ws[c & 1], ws_one, cuda_stream, flags,
+                           (uint32_t)o, (uint32_t)c + 1u);
+    if (rc != TPC_OK) { cudaDeviceSynchronize(); return rc; }
+    launches += ctx->launches;
+    if (c + 1 < n_chunks) {   // next chunk's copy-in runs behind this chunk's kernels
+      if ((e = copy_in(c + 1)) != cudaSuccess) { cudaDeviceSynchronize(); return set_cuda_err(ctx, e, "cudaMemcpyAsync(clusters)"); }
+    }
+    tpc_track_view v;
+    rc = tpc_get_tracks(ctx, &v);                                     // syncs `st`: counts of chunk c
+    if (rc != TPC_OK) { cudaDeviceSynchronize(); return rc; }
+    if (n_tracks + v.n_tracks > cap_tracks || n_ids + v.n_cluster_ids > cap_ids) { cudaDeviceSynchronize(); return TPC_E_OVERFLOW; }
+    if (v.n_tracks) k_shift_tracks<<<(unsigned)((v.n_tracks + 255) / 256), 256, 0, st>>>((tpc_track*)v.d_tracks, (uint32_t)v.n_tracks, (uint32_t)n_ids);
+    cudaEventRecord(ctx->ev_done[c & 1], st);
+    cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c & 1], 0);
+    if (h_tracks && v.n_tracks)
+      cudaMemcpyAsync(h_tracks + n_tracks, v.d_tracks, v.n_tracks * sizeof(tpc_track), cudaMemcpyDeviceToHost, ctx->s_out);
+    if (h_cluster_ids && v.n_cluster_ids)
+      cudaMemcpyAsync(h_cluster_ids + n_ids, v.d_cluster_ids, v.n_cluster_ids * 4, cudaMemcpyDeviceToHost, ctx->s_out);
+    if (h_cluster_shared && v.n_cluster_ids)
+      cudaMemcpyAsync(h_cluster_shared + n_ids, v.d_cluster_shared, v.n_cluster_ids, cudaMemcpyDeviceToHost, ctx->s_out);
+    cudaEventRecord(ctx->ev_out[c & 1], ctx->s_out);
+    n_tracks += v.n_tracks; n_ids += v.n_cluster_ids;
+    out->n_ignored += v.n_ignored; out->n_dropped += v.n_dropped; out->n_seeds += v.n_seeds;
+    out->n_tracklets += v.n_tracklets; out->n_bins += v.n_bins;
+    out->n_follow_steps += v.n_follow_steps; out->n_follow_updates += v.n_follow_updates;
+    out->n_follow_candidates += v.n_follow_candidates;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) out->follow_work[a][b] += v.follow_work[a][b];
+    out->grid_by_rows = (c == 0) ? v.grid_by_rows : (out->grid_by_rows & v.grid_by_rows);
+  }
+  if ((e = cudaStreamSynchronize(ctx->s_out)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize(copy-out)");
+  if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize");
+  out->n_tracks = n_tracks;
+  out->n_cluster_ids = n_ids;
+  ctx->launches = launches;
+  return rc_all;
+}
+
 int tpc_last_launch_count(const tpc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 void tpc_destroy(tpc_ctx* c) {
@@ -400,6 +511,14 @@ void tpc_destroy(tpc_ctx* c) {
   if (c->d_cnt) cudaFree(c->d_cnt);
   if (c->d_row_stat) cudaFree(c->d_row_stat);
   if (c->h_cnt) cudaFreeHost(c->h_cnt);
+  if (c->d_sector_seen) cudaFree(c->d_sector_seen);
+  if (c->s_in) cudaStreamDestroy(c->s_in);
+  if (c->s_out) cudaStreamDestroy(c->s_out);
+  for (int i = 0; i < 2; ++i) {
+    if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
+    if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+    if (c->ev_out[i]) cudaEventDestroy(c->ev_out[i]);
+  }
   delete c;
 }
 

@@ -32,6 +32,7 @@ struct TpcConst {
 #define TPC_DEVERR_BINS 2u          // bin index capacity            -> TPC_E_OVERFLOW
 #define TPC_DEVERR_SEEDS 4u         // seed capacity                 -> TPC_E_OVERFLOW
 #define TPC_DEVERR_TRACKS 8u        // track / cluster-id capacity   -> TPC_E_OVERFLOW
+#define TPC_DEVERR_CHUNKS 16u       // a sector has records in two chunks of a chunked frame -> TPC_E_ARG
 
 struct TpcCounters {
   uint32_t n_sorted, n_ignored, n_dropped, n_bad;
@@ -76,6 +77,9 @@ struct TpcBuffers {
   uint32_t n;            // input clusters
   uint32_t n_sr;         // n_sectors*n_rows
   uint32_t n_sectors, n_rows;
+  uint32_t id_base;      // added to every original index (chunked frames: position of the chunk in the frame)
+  uint32_t chunk_tag;    // 0: whole frame; else 1 + chunk number (sector_seen check)
+  uint32_t* sector_seen; // [n_sectors] tag of the chunk that brought records of the sector (ctx-owned)
   uint64_t max_bins;
   uint32_t max_seeds, max_tracks, max_ids;
   uint32_t scan_blocks;  // capacity of scan_partials

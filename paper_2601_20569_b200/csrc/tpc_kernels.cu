@@ -233,6 +233,10 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
         if (rs.last - rs.first + 1u != rs.n_all || rs.n_all > 65535u || bytes > TPC_RS_SMEM_BYTES) by_rows = false;
       }
     }
+    if (B.chunk_tag && sr < B.n_sr && B.row_stat[sr].n_all) {   // chunked frame: sectors must not straddle chunks
+      const uint32_t seen = atomicCAS(&B.sector_seen[sr / (uint32_t)K->n_rows], 0u, B.chunk_tag);
+      if (seen != 0u && seen != B.chunk_tag) atomicOr(&B.cnt->error, TPC_DEVERR_CHUNKS);
+    }
     uint32_t tot_b, tot_c, tot_t;
     const uint32_t pb = block_excl_scan(nb, &tot_b, sm);
     const uint32_t pc = block_excl_scan(cnt, &tot_c, sm);
@@ -361,7 +365,7 @@ __global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(B.yz + pos));
     asm volatile("prefetch.global.L2 [%0];" ::"l"(B.orig_id + pos));
     B.yz[pos] = make_float2(y, z);
-    B.orig_id[pos] = i;
+    B.orig_id[pos] = B.id_base + i;
   }
 }
 
@@ -506,7 +510,7 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
         const uint32_t q = q0 + u * TPC_RS_THREADS;
         if (q >= d.count) continue;
         B.yz[d.clu_ofs + q] = make_float2(__uint_as_float(v[u].x), __uint_as_float(v[u].y));
-        B.orig_id[d.clu_ofs + q] = rs.first + e[u];
+        B.orig_id[d.clu_ofs + q] = B.id_base + rs.first + e[u];
       }
     }
   }

@@ -225,3 +225,50 @@ def test_det_parity_full_c4_sampled_sectors(B):
         bad = parity.compare_tracks(tracks, ids, shared, o, sector=s)
         assert parity.all_zero(bad), (s, bad)
         assert o.n_tracks > 10000
+
+
+def _host_run(B, cl, chunk_ofs=None, flags=DET & 1):
+    import torch
+    n = len(cl)
+    h = torch.from_numpy(cl.view(np.uint8).reshape(-1).copy()).pin_memory()
+    d = torch.empty(n * 16, dtype=torch.uint8, device="cuda")
+    h_tracks = torch.empty(200000 * B.TRACK_DTYPE.itemsize, dtype=torch.uint8).pin_memory()
+    h_ids = torch.empty(4 * 4_000_000, dtype=torch.uint8).pin_memory()
+    h_sh = torch.empty(4_000_000, dtype=torch.uint8).pin_memory()
+    trk = B.SectorTracker()
+    try:
+        if chunk_ofs is None:
+            v = trk.track_host(h, d, h_tracks, h_ids, h_sh, flags=flags)
+        else:
+            v = trk.track_host_chunks(h, chunk_ofs, d, h_tracks, h_ids, h_sh, flags=flags)
+        nt, ni = int(v.n_tracks), int(v.n_cluster_ids)
+        tracks = h_tracks.numpy()[: nt * B.TRACK_DTYPE.itemsize].view(B.TRACK_DTYPE).copy()
+        ids = h_ids.numpy()[: 4 * ni].view(np.uint32).copy()
+        sh = h_sh.numpy()[:ni].copy()
+        return tracks, ids, sh, v
+    finally:
+        trk.close()
+
+
+def test_chunked_host_call_equals_whole_frame_and_oracle(B):
+    """tpc_sector_track_host_chunks: chunks of whole sectors, pipelined copy-in / tracking /
+    copy-out; the result is that of the whole frame (bit-exact vs the oracle, deterministic mode)."""
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=1500, seed=41))
+    bounds = np.searchsorted(cl["sector"], [0, 7, 8, 20, 36])          # ragged chunks: 7, 1, 12, 16 sectors
+    tracks, ids, sh, v = _host_run(B, cl, [int(x) for x in bounds], flags=1)
+    o = oracle.run(cl, n_threads=8, want=("tracks",))
+    assert parity.all_zero(parity.compare_tracks(tracks, ids, sh, o))
+    assert v.n_tracks == o.n_tracks and v.n_seeds == o.n_seeds and v.grid_by_rows == 1
+    t1, i1, s1, v1 = _host_run(B, cl, None, flags=1)
+    assert parity.all_zero(parity.compare_tracks(t1, i1, s1, o)) and v1.n_tracks == v.n_tracks
+    # an empty chunk and a single chunk are fine
+    tracks, ids, sh, v = _host_run(B, cl, [0, 0, len(cl)], flags=1)
+    assert parity.all_zero(parity.compare_tracks(tracks, ids, sh, o))
+
+
+def test_chunked_host_call_rejects_a_sector_in_two_chunks(B):
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=300, seed=42))
+    mid = int(np.searchsorted(cl["sector"], 10)) + 5                    # cuts sector 10 in two
+    with pytest.raises(B.TpcError) as e:
+        _host_run(B, cl, [0, mid, len(cl)], flags=1)
+    assert e.value.code == B.TPC_E_ARG
