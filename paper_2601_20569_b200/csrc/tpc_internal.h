@@ -56,7 +56,9 @@ struct TpcRowStat {
   uint32_t pad_[2];
 };
 
+#ifndef TPC_NF_TILE
 #define TPC_NF_TILE 256  // clusters per neighbour-finder tile (one CTA)
+#endif
 
 // Per-row grid build (k_row_sort): one CTA per (sector,row); the row's bin counters and its
 // permutation live in shared memory (16-bit entries).

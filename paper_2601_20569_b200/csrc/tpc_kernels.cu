@@ -552,8 +552,13 @@ __device__ __forceinline__ BinWindow make_window(const tpc_row_desc& d, const Tp
 // minimum of (d2, original id of up, original id of down) (rule D2), which makes the result
 // independent of the visiting order.  Tiles whose slab does not fit (very sparse or very
 // dense rows) take the same search on global memory (nf_generic).
+#ifndef TPC_NF_SLAB
 #define TPC_NF_SLAB 1024   // clusters staged per neighbour row
-#define TPC_NF_BINS 1023   // bins staged per neighbour row (+1 end marker)
+#endif
+#define TPC_NF_BINS (TPC_NF_SLAB - 1)   // bins staged per neighbour row (+1 end marker)
+#ifndef TPC_NF_MINBLOCKS
+#define TPC_NF_MINBLOCKS 6
+#endif
 #define TPC_NF_LIST 12     // window members kept per thread and side
 
 // The search of one cluster directly on global memory.
@@ -626,10 +631,67 @@ __device__ __forceinline__ int nf_collect(const BinWindow& w, int bz_lo, uint32_
   return n;
 }
 
-__global__ void __launch_bounds__(TPC_NF_TILE, 6) k_neighbours(TpcBuffers B) {
+// The down side of the search: every member of the down window is paired at once with the
+// (few) members of the up window collected before, so that no second list and no separate
+// pair loop are needed.  The first two up members sit in registers.  Best pair = minimum of
+// (d2, original id of up, original id of down): independent of the visiting order (rule D2).
+__device__ __forceinline__ void nf_down_pairs(const BinWindow& w, int bz_lo, uint32_t bin_ofs, uint32_t c0,
+                                              const uint32_t* __restrict__ s_bin, const float2* __restrict__ s_yz_d,
+                                              const float2* __restrict__ s_yz_u, const uint16_t* __restrict__ s_list_u,
+                                              int nU, float yi, float zi, float ty, float wy, float wz, float max_d2,
+                                              const uint32_t* __restrict__ orig, uint32_t cu0, uint32_t cd0,
+                                              int32_t& bj, int32_t& bk) {
+  const int nzr = w.bz1 - w.bz0;  // 0..2 extra z-rows
+  const uint32_t b = (w.base - bin_ofs) + (uint32_t)(w.bz0 - bz_lo) * (uint32_t)w.ny;
+  const uint32_t a0 = s_bin[b] - c0, l0 = (s_bin[b + w.by_span] - c0) - a0;
+  uint32_t a1 = 0, l1 = 0, a2 = 0, l2 = 0;
+  if (nzr >= 1) { a1 = s_bin[b + w.ny] - c0; l1 = (s_bin[b + w.ny + w.by_span] - c0) - a1; }
+  if (nzr >= 2) { a2 = s_bin[b + 2 * w.ny] - c0; l2 = (s_bin[b + 2 * w.ny + w.by_span] - c0) - a2; }
+  const uint32_t l01 = l0 + l1, total = l01 + l2;
+  const uint32_t o1 = a1 - l0, o2 = a2 - l01;
+  const uint32_t ju0 = s_list_u[0];
+  const float2 cj0 = s_yz_u[ju0];
+  const float ux0 = cj0.x - yi, uz0 = cj0.y - zi;
+  uint32_t ju1 = 0;
+  float ux1 = 0.f, uz1 = 0.f;
+  if (nU > 1) {
+    ju1 = s_list_u[TPC_NF_TILE];
+    const float2 cj1 = s_yz_u[ju1];
+    ux1 = cj1.x - yi; uz1 = cj1.y - zi;
+  }
+  float best = 0.f;
+  for (uint32_t t = 0; t < total; ++t) {
+    const uint32_t kd = t + (t < l0 ? a0 : (t < l01 ? o1 : o2));
+    const float2 ck = s_yz_d[kd];
+    if (!(fabsf((yi - ck.x) - ty) <= wy && fabsf(zi - ck.y) <= wz)) continue;
+    const float vx = ck.x - yi, vz = ck.y - zi;
+    auto pair = [&](uint32_t ju, float ux, float uz) {
+      const float dy = ux + vx;
+      const float dz = uz + vz;
+      const float d2 = dy * dy + dz * dz;
+      if (d2 <= max_d2) {
+        bool better = bj < 0 || d2 < best;
+        if (!better && d2 == best) {  // exact tie: rule D2 (rare, ids fetched only here)
+          const uint32_t jid = orig[cu0 + ju], bjid = orig[cu0 + (uint32_t)bj];
+          better = jid < bjid || (jid == bjid && orig[cd0 + kd] < orig[cd0 + (uint32_t)bk]);
+        }
+        if (better) { best = d2; bj = (int32_t)ju; bk = (int32_t)kd; }
+      }
+    };
+    pair(ju0, ux0, uz0);
+    if (nU > 1) pair(ju1, ux1, uz1);
+    for (int a = 2; a < nU; ++a) {
+      const uint32_t ju = s_list_u[a * TPC_NF_TILE];
+      const float2 cj = s_yz_u[ju];
+      pair(ju, cj.x - yi, cj.y - zi);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(TPC_NF_TILE, TPC_NF_MINBLOCKS) k_neighbours(TpcBuffers B) {
   __shared__ float2 s_yz[2][TPC_NF_SLAB];
   __shared__ uint32_t s_bin[2][TPC_NF_BINS + 1];
-  __shared__ uint16_t s_list[2][TPC_NF_LIST * TPC_NF_TILE];
+  __shared__ uint16_t s_list[1][TPC_NF_LIST * TPC_NF_TILE];   // up-window members per thread
   __shared__ int s_red[4];
   const TpcConst* __restrict__ K = B.K;
   if (B.cnt->error & TPC_DEVERR_BINS) return;
@@ -701,37 +763,11 @@ __global__ void __launch_bounds__(TPC_NF_TILE, 6) k_neighbours(TpcBuffers B) {
         nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);     // bins much smaller than the window
       } else if (have) {
         const int nU = nf_collect<true>(wu, ulo, du.bin_ofs, cu0, s_bin[0], s_yz[0], &s_list[0][tx], yi, zi, ty, wy, wz);
-        const int nD = nU ? nf_collect<false>(wd, dlo, dd.bin_ofs, cd0, s_bin[1], s_yz[1], &s_list[1][tx], yi, zi, ty,
-                                              wy, wz)
-                          : 0;
-        if (nU > TPC_NF_LIST || nD > TPC_NF_LIST) {
-          nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);   // rare: crowded windows
-        } else if (nU && nD) {
-          // flat pair loop over the two lists
-          float best = 0.f;
-          int a = 0, b = 0;
-          uint32_t ju = s_list[0][tx];
-          float2 cj = s_yz[0][ju];
-          const int total = nU * nD;
-          for (int t = 0; t < total; ++t) {
-            const uint32_t kd = s_list[1][b * TPC_NF_TILE + tx];
-            const float2 ck = s_yz[1][kd];
-            const float dy = (cj.x - yi) + (ck.x - yi);
-            const float dz = (cj.y - zi) + (ck.y - zi);
-            const float d2 = dy * dy + dz * dz;
-            if (d2 <= max_d2) {
-              bool better = bj < 0 || d2 < best;
-              if (!better && d2 == best) {  // exact tie: rule D2 (rare, ids fetched only here)
-                const uint32_t jid = orig[cu0 + ju], bjid = orig[cu0 + (uint32_t)bj];
-                better = jid < bjid || (jid == bjid && orig[cd0 + kd] < orig[cd0 + (uint32_t)bk]);
-              }
-              if (better) { best = d2; bj = (int32_t)ju; bk = (int32_t)kd; }
-            }
-            if (++b == nD) {
-              b = 0;
-              if (++a < nU) { ju = s_list[0][a * TPC_NF_TILE + tx]; cj = s_yz[0][ju]; }
-            }
-          }
+        if (nU > TPC_NF_LIST) {
+          nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);   // rare: crowded window
+        } else if (nU) {
+          nf_down_pairs(wd, dlo, dd.bin_ofs, cd0, s_bin[1], s_yz[1], s_yz[0], &s_list[0][tx], nU, yi, zi, ty, wy, wz,
+                        max_d2, orig, cu0, cd0, bj, bk);
           if (bj >= 0) { bj += (int32_t)cu0; bk += (int32_t)cd0; }
         }
       }
@@ -1973,6 +2009,16 @@ __global__ void k_init(TpcBuffers B) {
     ++launches;                                                     \
   } while (0)
 
+// CTAs of `kernel` that are resident on one SM at this block size / dynamic shared memory.
+// Every kernel here is a grid-stride (persistent) loop: a grid larger than what is resident
+// runs in waves and leaves a tail, a smaller one leaves SMs short of warps.
+template <class K>
+static inline int resident_ctas(K kernel, int block, size_t smem = 0) {
+  int n = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kernel, block, smem) != cudaSuccess || n < 1) n = 1;
+  return n;
+}
+
 static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
   uint64_t g = (n + block - 1) / block;
   const uint64_t cap = (uint64_t)n_sm * ctas_per_sm;
@@ -1990,7 +2036,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   TPC_LAUNCH_CHECK("k_init");
   if (timers) cudaEventRecord(E.ev[0], st);
   // ---- K1 grid
-  k_row_stats<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_row_stats<<<grid_for(B.n, 256, n_sm, resident_ctas(k_row_stats, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_row_stats");
   k_row_desc<<<1, 1024, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_row_desc");
@@ -2001,25 +2047,25 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   TPC_LAUNCH_CHECK("k_row_sort");
   k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_bins");
-  k_bin_hist<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_bin_hist<<<grid_for(B.n, 256, n_sm, resident_ctas(k_bin_hist, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_bin_hist");
-  k_bin_scan<<<grid_for((uint64_t)B.n_sr * 512, 512, n_sm, 4), 512, 0, st>>>(B);
+  k_bin_scan<<<grid_for((uint64_t)B.n_sr * 512, 512, n_sm, resident_ctas(k_bin_scan, 512)), 512, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_bin_scan");
-  k_scatter<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_scatter<<<grid_for(B.n, 256, n_sm, resident_ctas(k_scatter, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_scatter");
 #if TPC_DET
-  k_bin_sort<<<grid_for(B.max_bins, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_bin_sort<<<grid_for(B.max_bins, 256, n_sm, resident_ctas(k_bin_sort, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_bin_sort");
 #endif
   if (timers) cudaEventRecord(E.ev[1], st);
   // ---- K2 neighbour finder
-  k_neighbours<<<grid_for((uint64_t)(B.n / TPC_NF_TILE + B.n_sr) * TPC_NF_TILE, TPC_NF_TILE, n_sm, 8), TPC_NF_TILE, 0, st>>>(B);
+  k_neighbours<<<grid_for((uint64_t)(B.n / TPC_NF_TILE + B.n_sr) * TPC_NF_TILE, TPC_NF_TILE, n_sm, resident_ctas(k_neighbours, TPC_NF_TILE)), TPC_NF_TILE, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_neighbours");
   if (timers) cudaEventRecord(E.ev[2], st);
   // ---- K3 cleanup + seeds
-  k_link_cleanup<<<grid_for(B.n, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_link_cleanup<<<grid_for(B.n, 256, n_sm, resident_ctas(k_link_cleanup, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_link_cleanup");
-  k_seed_flags<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, 8), TPC_SEED_BLOCK, 0, st>>>(B);
+  k_seed_flags<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, resident_ctas(k_seed_flags, TPC_SEED_BLOCK)), TPC_SEED_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_seed_flags");
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_sorted, 1024u, &B.cnt->n_seeds, B.max_seeds,
                                       &B.cnt->error, TPC_DEVERR_SEEDS);
@@ -2031,25 +2077,25 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
     k_seed_items<<<B.n_sectors, 1024, smem, st>>>(B);
   }
   TPC_LAUNCH_CHECK("k_seed_items");
-  k_seed_write<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, 8), TPC_SEED_BLOCK, 0, st>>>(B);
+  k_seed_write<<<grid_for((B.n + 3) / 4, TPC_SEED_BLOCK, n_sm, resident_ctas(k_seed_write, TPC_SEED_BLOCK)), TPC_SEED_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_seed_write");
   if (timers) cudaEventRecord(E.ev[3], st);
   // ---- K4 follower
-  k_follow_up<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
+  k_follow_up<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, resident_ctas(k_follow_up, TPC_FOLLOW_BLOCK)), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_up");
-  k_follow_refit<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_REFIT_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
+  k_follow_refit<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, resident_ctas(k_follow_refit, TPC_FOLLOW_BLOCK)), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_refit");
-  k_follow_down<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, TPC_FOLLOW_UP_MINBLOCKS), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
+  k_follow_down<<<grid_for(B.max_seeds, TPC_FOLLOW_BLOCK, n_sm, resident_ctas(k_follow_down, TPC_FOLLOW_BLOCK)), TPC_FOLLOW_BLOCK, 0, st>>>(B, F);
   TPC_LAUNCH_CHECK("k_follow_down");
   if (timers) cudaEventRecord(E.ev[4], st);
   // ---- K5 ambiguity solving
   k_zero_owner<<<grid_for(B.n / 2 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_owner");
-  k_sel_owner<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, 8), TPC_SEL_BLOCK, 0, st>>>(B);
+  k_sel_owner<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, resident_ctas(k_sel_owner, TPC_SEL_BLOCK)), TPC_SEL_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_owner");
-  k_sel_masks<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, 8), TPC_SEL_BLOCK, 0, st>>>(B);
+  k_sel_masks<<<grid_for((uint64_t)(B.max_seeds / 32 + 1) * TPC_SEL_BLOCK, TPC_SEL_BLOCK, n_sm, resident_ctas(k_sel_masks, TPC_SEL_BLOCK)), TPC_SEL_BLOCK, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_masks");
-  k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_sel_count<<<grid_for(B.max_seeds, 256, n_sm, resident_ctas(k_sel_count, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_count");
   const uint32_t half = (B.scan_blocks + 1) / 2;
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials, &B.cnt->n_seeds, 256u, &B.cnt->n_tracks, B.max_tracks,
@@ -2058,9 +2104,9 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials + half, &B.cnt->n_seeds, 256u, &B.cnt->n_ids, B.max_ids,
                                       &B.cnt->error, TPC_DEVERR_TRACKS);
   TPC_LAUNCH_CHECK("k_scan_partials");
-  k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, resident_ctas(k_sel_emit, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_emit");
-  k_sel_ids<<<grid_for((uint64_t)B.max_tracks * 32, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_sel_ids<<<grid_for((uint64_t)B.max_tracks * 32, 256, n_sm, resident_ctas(k_sel_ids, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_ids");
   if (timers) cudaEventRecord(E.ev[5], st);
   (void)flags;
