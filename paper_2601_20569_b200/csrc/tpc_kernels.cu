@@ -1841,6 +1841,15 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
   }
   int n_acc = 0, n_sh = 0, gap = 0, seg_last = -1, seg_first = -1;
   uint32_t n_seg = 0, n_id = 0;
+  if (!EMIT) {
+    // A segment holds at least (1 - shared fraction) owned hits at every moment of the walk
+    // (running rule of R6.3), so a tracklet that owns too few hits cannot reach min_hits_track
+    // in any segment: most clone instances leave here.
+    int n_own = 0;
+#pragma unroll
+    for (int w = 0; w < TPC_MASK_WORDS; ++w) n_own += __popc(own[w]);
+    if (n_own * 1000 < min_hits * (1000 - permille)) { n_seg_out = 0; n_id_out = 0; return; }
+  }
   auto close = [&]() {
     if (n_acc >= min_hits) {
       if (EMIT) {
