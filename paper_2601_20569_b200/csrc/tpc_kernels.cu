@@ -1527,7 +1527,6 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) 
         // the start row is reached (its hit is always present, so the saved state is the live one)
         const bool pending = r0 > 0;   // rows below to extrapolate into
         write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, pending);
-        if (pending) B.down_list[atomicAdd(&B.cnt->n_down, 1u)] = sd;
         active = false;
       }
     }
@@ -1545,7 +1544,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
   __syncthreads();
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const float inv_dy = K->inv_dy, inv_dz = K->inv_dz;
-  const uint32_t n_down = B.cnt->n_down;
+  const uint32_t n_seeds = B.cnt->n_seeds;
   const float2* __restrict__ yz = B.yz;
   const uint32_t* __restrict__ bin_start = B.bin_start;
   const int lane = threadIdx.x & 31;
@@ -1567,8 +1566,12 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_f
   for (;;) {
     if (__ballot_sync(0xffffffffu, !active)) {
       uint32_t item = 0;
-      if (queue_claim(&B.cnt->follow_next[2], n_down, lane, !active, chunk_next, chunk_end, exhausted, item)) {
-        sd = B.down_list[item];
+      // seeds are taken in LIST order (not in the order the refit finished them): the lanes of a
+      // warp then hold seeds of the same (sector, z-slab, row), walk the same rows and read
+      // neighbouring bins
+      if (queue_claim(&B.cnt->follow_next[2], n_seeds, lane, !active, chunk_next, chunk_end, exhausted, item) &&
+          B.tracklets[item].pad_ == (uint16_t)TPC_TL_PENDING) {
+        sd = item;
         const tpc_tracklet* __restrict__ t = B.tracklets + sd;
         k.y = t->p[0]; k.z = t->p[1]; k.s = t->p[2]; k.t = t->p[3]; k.q = t->p[4];
         k.c00 = t->c[0]; k.c10 = t->c[1]; k.c11 = t->c[2]; k.c20 = t->c[3]; k.c21 = t->c[4]; k.c22 = t->c[5];
