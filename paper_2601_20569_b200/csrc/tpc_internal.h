@@ -71,7 +71,12 @@ struct TpcRowStat {
 // Seeds are handed to the follower / selector ordered by (sector, z-slab, row): tracklets that
 // run at the same time then touch the same z-range of every row, which keeps their random
 // accesses (grid, owner words) inside L2.  A slab is 1/TPC_SEED_SLABS of a row's z-bins.
+#ifndef TPC_SEED_GROUP
+#define TPC_SEED_GROUP 1    // z-slabs interleaved row by row in the seed list (must divide TPC_SEED_SLABS)
+#endif
+#ifndef TPC_SEED_SLABS
 #define TPC_SEED_SLABS 64
+#endif
 
 // All device buffers of one run (pointers into the caller's workspace, or ctx-owned).
 struct TpcBuffers {

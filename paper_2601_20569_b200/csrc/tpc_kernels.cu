@@ -918,12 +918,17 @@ __global__ void __launch_bounds__(1024) k_seed_items(TpcBuffers B) {
     for (uint32_t e = e0; e < e1; ++e) { B.item_delta[base + e] = -(int32_t)pre; pre += s_cnt[e]; }
   }
   __syncthreads();
-  {  // list order: element e = slab*R + row
+  // list order: groups of TPC_SEED_GROUP z-slabs, row-major inside a group (group 1: slab-major)
+  auto list_to_item = [&](uint32_t e) -> uint32_t {
+    const uint32_t g = e / (R * TPC_SEED_GROUP), rem = e % (R * TPC_SEED_GROUP);
+    return (rem / TPC_SEED_GROUP) * S + g * TPC_SEED_GROUP + rem % TPC_SEED_GROUP;
+  };
+  {
     uint32_t sum = 0;
-    for (uint32_t e = e0; e < e1; ++e) sum += s_cnt[(e % R) * S + e / R];
+    for (uint32_t e = e0; e < e1; ++e) sum += s_cnt[list_to_item(e)];
     uint32_t pre = block_excl_scan(sum, &tot, sm);
     for (uint32_t e = e0; e < e1; ++e) {
-      const uint32_t k = (e % R) * S + e / R;
+      const uint32_t k = list_to_item(e);
       B.item_delta[base + k] += (int32_t)pre;
       pre += s_cnt[k];
     }
@@ -1207,7 +1212,9 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
 #ifndef TPC_REFILL_DOWN
 #define TPC_REFILL_DOWN 4
 #endif
-#define TPC_FOLLOW_CHUNK 64
+#ifndef TPC_FOLLOW_CHUNK
+#define TPC_FOLLOW_CHUNK 8    // seeds a warp claims at a time: small keeps the seeds in flight close in the list (64 -> 8: -5 ms)
+#endif
 #define TPC_NO_BIN 0xFFFFFFFFu
 #define TPC_TL_PENDING 1u   // tracklet.pad_: handed from the refit to the inward extrapolation
 
@@ -1681,7 +1688,9 @@ __global__ void __launch_bounds__(256) k_zero_owner(TpcBuffers B) {
 // of the tiles that run at the same time) come from the same z-slab of one sector and are
 // processed row by row, so their owner words sit in a few KB per row and stay in L2.  The per-row ballots are transposed through shared
 // memory into per-tracklet row masks, stored [word][tracklet].
+#ifndef TPC_SEL_BLOCK
 #define TPC_SEL_BLOCK 256
+#endif
 #define TPC_SEL_UNROLL 4   // rows per load: row_hit rows are 16-byte aligned when n_rows % 4 == 0
 
 // hits of rows rb..rb+3 of one tracklet (p = its row_hit row), -1 where `want` is false
