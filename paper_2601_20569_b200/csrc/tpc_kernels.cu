@@ -1304,11 +1304,16 @@ __device__ __forceinline__ void write_tracklet(const TpcBuffers& B, uint32_t sd,
   if (!pending && keep) atomicAdd(&B.cnt->n_tracklets, 1u);
 }
 
+// resident CTAs per SM the register budgets are sized for (measured on the C4 frame: fewer,
+// fatter CTAs are better for the outward pass, the other two take 6)
 #ifndef TPC_FOLLOW_UP_MINBLOCKS
-#define TPC_FOLLOW_UP_MINBLOCKS 6   // resident CTAs per SM the register budget is sized for
+#define TPC_FOLLOW_UP_MINBLOCKS 5
+#endif
+#ifndef TPC_FOLLOW_DOWN_MINBLOCKS
+#define TPC_FOLLOW_DOWN_MINBLOCKS 6
 #endif
 #ifndef TPC_FOLLOW_REFIT_MINBLOCKS
-#define TPC_FOLLOW_REFIT_MINBLOCKS 8
+#define TPC_FOLLOW_REFIT_MINBLOCKS 6
 #endif
 
 // ---- R5.1-R5.3: init, chain fit, outward extrapolation
@@ -1553,7 +1558,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) 
 }
 
 // ---- R5.6-R5.7: inward extrapolation below the start row, output
-__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_UP_MINBLOCKS) k_follow_down(TpcBuffers B, const __grid_constant__ FollowConst F) {
+__global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_DOWN_MINBLOCKS) k_follow_down(TpcBuffers B, const __grid_constant__ FollowConst F) {
   __shared__ float s_ylim[TPC_MAX_ROWS];
   __shared__ float s_x[TPC_MAX_ROWS];
   __shared__ float s_kin[20][TPC_FOLLOW_BLOCK];
