@@ -33,7 +33,10 @@ def build_tpctrack(force: bool = False, verbose: bool = False) -> str:
     det_o, fast_o, api_o = (os.path.join(CSRC, f"tpc_{n}{tag}.o") for n in ("kernels_det", "kernels_fast", "api"))
     cmds = [
         _NVCC_BASE + extra + ["-DTPC_DET=1", "--fmad=false", "-c", srcs[0], "-o", det_o],
-        _NVCC_BASE + extra + ["-DTPC_DET=0", "--fmad=true"] + os.environ.get("TPCTRACK_FAST_FLAGS", "").split()
+        # fast build: FMA contraction, approximate division / square root (MUFU based), denormals
+        # flushed: rounding-level differences only, which is all fast mode may differ by
+        _NVCC_BASE + extra + ["-DTPC_DET=0", "--fmad=true"]
+        + os.environ.get("TPCTRACK_FAST_FLAGS", "--use_fast_math").split()
         + ["-c", srcs[0], "-o", fast_o],
         _NVCC_BASE + ["-c", srcs[1], "-o", api_o],
         ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB_PATH, det_o, fast_o, api_o],

@@ -4,7 +4,8 @@
 // This translation unit is compiled TWICE:
 //   -DTPC_DET=1 --fmad=false  -> namespace tpc_det  : deterministic mode: no FMA
 //                                contraction, stable grid order; bit-comparable to the CPU oracle
-//   -DTPC_DET=0 --fmad=true   -> namespace tpc_fast : FMA contraction allowed, no in-bin sort
+//   -DTPC_DET=0 --fmad=true --use_fast_math -> namespace tpc_fast : FMA contraction, approximate
+//                                division / sqrt, no in-bin sort
 // Both use only + - * / sqrt on the decision path; every argmin carries an integer tie-break on
 // the ORIGINAL cluster index (rule D2), so atomics / thread order never change a result.
 //
