@@ -1974,18 +1974,39 @@ __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
   }
 }
 
-// K5d: emit the track records at their scanned offsets (order = seed order).
+// K5d: emit the track records at their scanned offsets (order = seed order).  Only about one
+// tracklet in five emits anything, so a CTA first compacts the emitting tracklets of a span of
+// TPC_EMIT_SPAN seeds into shared memory and then walks them with full warps.
+#define TPC_EMIT_SPAN 1024
 __global__ void __launch_bounds__(256) k_sel_emit(TpcBuffers B) {
+  __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_list[TPC_EMIT_SPAN];
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS | TPC_DEVERR_TRACKS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const uint32_t* part_seg = B.scan_partials;
   const uint32_t* part_id = B.scan_partials + (B.scan_blocks + 1) / 2;
-  for (uint32_t sd = blockIdx.x * blockDim.x + threadIdx.x; sd < n_seeds; sd += gridDim.x * blockDim.x) {
-    const uint32_t ps = B.seg_cnt[sd];
-    if (ps == 0xFFFFFFFFu) continue;   // no surviving segment
-    const uint32_t blk = sd / blockDim.x;
-    uint32_t ns, ni;
-    walk_tracklet<true>(B, sd, ns, ni, part_seg[blk] + ps, part_id[blk] + B.id_cnt[sd]);
+  const uint32_t n_spans = (n_seeds + TPC_EMIT_SPAN - 1) / TPC_EMIT_SPAN;
+  for (uint32_t span = blockIdx.x; span < n_spans; span += gridDim.x) {
+    const uint32_t sd0 = span * TPC_EMIT_SPAN + threadIdx.x * 4;
+    uint32_t ps[4];
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      ps[u] = sd0 + u < n_seeds ? B.seg_cnt[sd0 + u] : 0xFFFFFFFFu;
+      cnt += ps[u] != 0xFFFFFFFFu;   // has a surviving segment
+    }
+    uint32_t tot;
+    uint32_t pre = block_excl_scan(cnt, &tot, sm);   // (its first barrier also frees s_list of the previous span)
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (ps[u] != 0xFFFFFFFFu) s_list[pre++] = sd0 + u;
+    __syncthreads();
+    for (uint32_t e = threadIdx.x; e < tot; e += blockDim.x) {
+      const uint32_t sd = s_list[e];
+      const uint32_t blk = sd / 256u;   // block of k_sel_count that scanned this tracklet
+      uint32_t ns, ni;
+      walk_tracklet<true>(B, sd, ns, ni, part_seg[blk] + B.seg_cnt[sd], part_id[blk] + B.id_cnt[sd]);
+    }
   }
 }
 
@@ -2142,7 +2163,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   k_scan_partials<<<1, 1024, 0, st>>>(B.scan_partials + half, &B.cnt->n_seeds, 256u, &B.cnt->n_ids, B.max_ids,
                                       &B.cnt->error, TPC_DEVERR_TRACKS);
   TPC_LAUNCH_CHECK("k_scan_partials");
-  k_sel_emit<<<grid_for(B.max_seeds, 256, n_sm, resident_ctas(k_sel_emit, 256)), 256, 0, st>>>(B);
+  k_sel_emit<<<grid_for((uint64_t)(B.max_seeds / TPC_EMIT_SPAN + 1) * 256, 256, n_sm, resident_ctas(k_sel_emit, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_emit");
   k_sel_ids<<<grid_for((uint64_t)B.max_tracks * 32, 256, n_sm, resident_ctas(k_sel_ids, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_sel_ids");
