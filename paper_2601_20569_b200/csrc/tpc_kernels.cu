@@ -1957,6 +1957,8 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
 // K5c: count tracks / cluster ids per tracklet + per-block partial sums (for the scans).
 __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
   __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_ns[256], s_ni[256];
+  __shared__ uint16_t s_list[256];
   if (B.cnt->error & (TPC_DEVERR_BINS | TPC_DEVERR_SEEDS)) return;
   const uint32_t n_seeds = B.cnt->n_seeds;
   const uint32_t n_blocks = (n_seeds + blockDim.x - 1) / blockDim.x;
@@ -1964,8 +1966,29 @@ __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
   uint32_t* part_id = B.scan_partials + (B.scan_blocks + 1) / 2;
   for (uint32_t blk = blockIdx.x; blk < n_blocks; blk += gridDim.x) {
     const uint32_t sd = blk * blockDim.x + threadIdx.x;
-    uint32_t ns = 0, ni = 0;
-    if (sd < n_seeds && B.tl_key[sd] != 0ull) walk_tracklet<false>(B, sd, ns, ni, 0, 0);
+    // tracklets that can hold a segment at all (the bound of walk_tracklet) are compacted and
+    // walked with full warps; the others count zero
+    bool cand = false;
+    if (sd < n_seeds && B.tl_key[sd] != 0ull) {
+      int n_own = 0;
+#pragma unroll
+      for (int w = 0; w < TPC_MASK_WORDS; ++w)
+        if (w * 32 < B.K->n_rows) n_own += __popc(B.tl_mask[(size_t)(TPC_MASK_WORDS + w) * B.max_seeds + sd]);
+      cand = n_own * 1000 >= B.K->P.min_hits_track * (1000 - B.K->P.shared_permille);
+    }
+    s_ns[threadIdx.x] = 0u; s_ni[threadIdx.x] = 0u;
+    uint32_t n_cand;
+    const uint32_t slot = block_excl_scan(cand ? 1u : 0u, &n_cand, sm);
+    if (cand) s_list[slot] = (uint16_t)threadIdx.x;
+    __syncthreads();
+    if (threadIdx.x < n_cand) {
+      const uint32_t t = s_list[threadIdx.x];
+      uint32_t a = 0, b = 0;
+      walk_tracklet<false>(B, blk * blockDim.x + t, a, b, 0, 0);
+      s_ns[t] = a; s_ni[t] = b;
+    }
+    __syncthreads();
+    const uint32_t ns = s_ns[threadIdx.x], ni = s_ni[threadIdx.x];
     uint32_t tot_s, tot_i;
     const uint32_t ps = block_excl_scan(ns, &tot_s, sm);
     const uint32_t pi = block_excl_scan(ni, &tot_i, sm);
