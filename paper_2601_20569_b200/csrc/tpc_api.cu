@@ -110,7 +110,6 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.seeds = (uint32_t*)take(4 * (size_t)k.max_seeds);
   b.seed_sr = (uint16_t*)take(2 * (size_t)k.max_seeds);
   b.turn = (uint4*)take(32 * (size_t)k.max_seeds);
-  b.down_list = (uint32_t*)take(4 * (size_t)k.max_seeds);
   b.tracklets = (tpc_tracklet*)take(sizeof(tpc_tracklet) * (size_t)k.max_seeds);
   b.row_hit = (int32_t*)take(4 * (size_t)c->geom.n_rows * k.max_seeds);
   b.owner = (unsigned long long*)take(8 * n);

@@ -42,9 +42,8 @@ struct TpcCounters {
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
   unsigned long long follow_work[3][3];  // [kernel up/refit/down][steps, updates, candidates]
-  // work queues of the three follower kernels (next unclaimed item) and the number of seeds
-  // handed from the refit to the inward extrapolation
-  uint32_t follow_next[3], n_down;
+  // work queues of the three follower kernels (next unclaimed seed)
+  uint32_t follow_next[3], pad_;
 };
 
 // per (sector,row) statistics of pass 1
@@ -111,7 +110,6 @@ struct TpcBuffers {
   uint32_t* seeds;        // [max_seeds] sorted index of start hits, in (sector, z-slab, row, sorted index) order
   uint16_t* seed_sr;      // [max_seeds] sector*n_rows+row of each start hit
   uint4* turn;            // [max_seeds][2] state at the outermost hit (y,z,sin phi,tan lambda | q/pT,row,-,-)
-  uint32_t* down_list;    // [max_seeds] seeds whose refit reached the start row (inward extrapolation pending)
   tpc_tracklet* tracklets;// [max_seeds]
   int32_t* row_hit;       // [max_seeds][n_rows]
   unsigned long long* owner;     // [n]

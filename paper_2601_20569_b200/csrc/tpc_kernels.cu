@@ -2075,7 +2075,7 @@ __global__ void k_init(TpcBuffers B) {
     c.grid_rows = 0;
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) c.follow_work[a][b] = 0ull;
-    c.follow_next[0] = c.follow_next[1] = c.follow_next[2] = 0u; c.n_down = 0u;
+    c.follow_next[0] = c.follow_next[1] = c.follow_next[2] = 0u; c.pad_ = 0u;
     *B.cnt = c;
   }
 }
