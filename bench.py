@@ -339,8 +339,17 @@ def run_ours(args, rank, world, local_rank):
     # tracking and copy-out of successive chunks overlap inside tpc_sector_track_host_chunks.  The
     # chunk offsets are part of the input's description (the generator emits sectors in order).
     sec = clusters["sector"]
-    n_chunks = max(1, min(args.e2e_chunks, int(sec.max()) + 1 if n else 1))
+    n_chunks = max(1, min(args.e2e_chunks or 1, int(sec.max()) + 1 if n else 1))
     cuts = [int(round((int(sec.max()) + 1) * c / n_chunks)) for c in range(n_chunks + 1)] if n else [0, 0]
+    if args.e2e_cuts and n:       # explicit sector boundaries, e.g. "0,2,6,12,20,28,34,36"
+        cuts = [int(x) for x in args.e2e_cuts.split(",")]
+        n_chunks = len(cuts) - 1
+    elif args.e2e_chunks == 0 and n:
+        # default: small chunks first and last (short pipeline fill and drain), large ones between
+        # (measured on the C4 frame: 112.0 ms against 119.7 ms for six equal chunks)
+        ns = int(sec.max()) + 1
+        cuts = sorted({int(round(ns * f)) for f in (0, 1 / 18, 1 / 6, 1 / 3, 5 / 9, 7 / 9, 17 / 18, 1)})
+        n_chunks = len(cuts) - 1
     chunk_ofs = [int(x) for x in np.searchsorted(sec, cuts[:-1])] + [n]
 
     def e2e_step():
@@ -473,7 +482,8 @@ def main():
     ap.add_argument("--max-bins", type=int, default=0, help="bin-index capacity (0 = library default)")
     ap.add_argument("--oracle-budget", type=int, default=7_000_000,
                     help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
-    ap.add_argument("--e2e-chunks", type=int, default=6, help="chunks of whole sectors in the end-to-end leg (1 = one shot)")
+    ap.add_argument("--e2e-chunks", type=int, default=0, help="equal chunks of whole sectors in the end-to-end leg (1 = one shot, 0 = ramped schedule)")
+    ap.add_argument("--e2e-cuts", default="", help="sector boundaries of the chunks of the end-to-end leg (overrides --e2e-chunks)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
