@@ -1772,23 +1772,35 @@ __global__ void __launch_bounds__(TPC_SEL_BLOCK) k_sel_owner(TpcBuffers B) {
     const int t0 = __reduce_min_sync(0xffffffffu, r0), t1 = __reduce_max_sync(0xffffffffu, r1);
     const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * (size_t)R;
     const bool vec = (R & 3) == 0;
-    for (int rb = (t0 & ~3) + warp * TPC_SEL_UNROLL; rb <= t1; rb += (TPC_SEL_BLOCK / 32) * TPC_SEL_UNROLL) {
-      int32_t c[TPC_SEL_UNROLL];
-      unsigned long long o[TPC_SEL_UNROLL];
-      bool want[TPC_SEL_UNROLL];
+    // two row groups per iteration: eight independent hit -> owner chains in flight per lane
+    constexpr int kStride = (TPC_SEL_BLOCK / 32) * TPC_SEL_UNROLL;
+    for (int rb0 = (t0 & ~3) + warp * TPC_SEL_UNROLL; rb0 <= t1; rb0 += 2 * kStride) {
+      int32_t c[2][TPC_SEL_UNROLL];
+      unsigned long long o[2][TPC_SEL_UNROLL];
 #pragma unroll
-      for (int u = 0; u < TPC_SEL_UNROLL; ++u) want[u] = rb + u >= r0 && rb + u <= r1;
-      load_hits4(hits, rb, R, vec, want, c);
+      for (int g = 0; g < 2; ++g) {
+        const int rb = rb0 + g * kStride;
+        bool want[TPC_SEL_UNROLL];
 #pragma unroll
-      for (int u = 0; u < TPC_SEL_UNROLL; ++u) o[u] = c[u] >= 0 ? __ldcg(&B.owner[c[u]]) : ~0ull;
+        for (int u = 0; u < TPC_SEL_UNROLL; ++u) want[u] = rb + u >= r0 && rb + u <= r1;
+        load_hits4(hits, rb, R, vec && rb + 3 < R, want, c[g]);
+      }
 #pragma unroll
-      for (int u = 0; u < TPC_SEL_UNROLL; ++u) {
-        // read first: most hits lose against the current owner and then need no atomic
-        const bool tent = o[u] < key;
-        if (tent) atomicMax(&B.owner[c[u]], key);
-        const uint32_t hm = __ballot_sync(0xffffffffu, c[u] >= 0);
-        const uint32_t tm = __ballot_sync(0xffffffffu, tent);
-        if (lane == 0 && rb + u < R) { s_has[rb + u] = hm; s_tent[rb + u] = tm; }
+      for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int u = 0; u < TPC_SEL_UNROLL; ++u) o[g][u] = c[g][u] >= 0 ? __ldcg(&B.owner[c[g][u]]) : ~0ull;
+#pragma unroll
+      for (int g = 0; g < 2; ++g) {
+        const int rb = rb0 + g * kStride;
+#pragma unroll
+        for (int u = 0; u < TPC_SEL_UNROLL; ++u) {
+          // read first: most hits lose against the current owner and then need no atomic
+          const bool tent = o[g][u] < key;
+          if (tent) atomicMax(&B.owner[c[g][u]], key);
+          const uint32_t hm = __ballot_sync(0xffffffffu, c[g][u] >= 0);
+          const uint32_t tm = __ballot_sync(0xffffffffu, tent);
+          if (lane == 0 && rb + u < R) { s_has[rb + u] = hm; s_tent[rb + u] = tm; }
+        }
       }
     }
     __syncthreads();
