@@ -197,6 +197,36 @@ def test_fast_mode_tolerances(B):
     assert qo["efficiency"] > 0.95
 
 
+@pytest.mark.parametrize("name", ["C2_full", "C4_20_events", "C5_reduced"])
+def test_fast_mode_tolerances_other_configs(B, name):
+    """The fast build (FMA, approximate division / sqrt) against the oracle on the other workload
+    shapes: same bars as above (parameters 1e-3 relative on key-paired tracks, efficiency and
+    clone rate within 0.2 % absolute)."""
+    import bench
+    if name == "C2_full":
+        cl, lab, _ = dg.generate(dg.preset("C2"))
+        pkw = {}
+    elif name == "C4_20_events":
+        base = dg.preset("C4")
+        cl, lab, _ = dg.generate(dg.preset("C4", n_events=20, t_window_us=base.t_window_us * 20 / base.n_events))
+        pkw = dict(bench.WORKLOAD_PARAMS["C4"])
+        sel = cl["sector"] < 4                      # four sectors keep the oracle's share short
+        cl, lab = cl[sel], lab[sel]
+    else:
+        cl, lab, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(bench.WORKLOAD_PARAMS["C5"])
+    gp, op = params_pair(B, **pkw)
+    tracks, ids, shared, view, _ = run_gpu(B, cl, gp, 0)
+    o = oracle.run(cl, params=op, n_threads=8, want=("tracks",))
+    st = parity.compare_tracks_fast(tracks, ids, shared, o)
+    assert st["n_paired"] >= 0.995 * st["n_oracle"], st
+    assert st["n_param_bad"] <= 0.002 * st["n_paired"], st
+    assert st["n_list_diff"] <= 0.01 * st["n_paired"], st
+    qg, qo = quality(tracks, ids, lab), quality(o.tracks, o.cluster_ids, lab)
+    assert abs(qg["efficiency"] - qo["efficiency"]) <= 0.002, (qg, qo)
+    assert abs(qg["clone_rate"] - qo["clone_rate"]) <= 0.002, (qg, qo)
+
+
 def test_det_parity_full_c2_bench_configuration(B):
     """BASELINE.json configs[1] at full size (~1.8 M clusters, 36 sectors)."""
     cl, lab, _ = dg.generate(dg.preset("C2"))
