@@ -13,8 +13,11 @@ from __future__ import annotations
 import numpy as np
 
 
+FINDABLE_MIN_HITS = 70   # findable = at least 70 hits in the TPC
+
+
 def track_quality(n_clusters_per_track, cluster_ofs, cluster_ids, track_sector, labels,
-                  min_findable: int = 70, purity: float = 0.9) -> dict:
+                  min_findable: int = FINDABLE_MIN_HITS, purity: float = 0.9) -> dict:
     """Efficiency / clone rate / fake rate.
 
     n_clusters_per_track, cluster_ofs, track_sector: per-track arrays; cluster_ids: the
