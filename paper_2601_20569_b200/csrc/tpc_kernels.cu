@@ -444,20 +444,37 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
       }
     }
     __syncthreads();
-    // ---- S: scan; runs of L consecutive counter words (2L bins) per thread
-    const uint32_t L = (nbw + TPC_RS_THREADS - 1) / TPC_RS_THREADS;
-    const uint32_t w0 = min(tid * L, nbw), w1 = min(w0 + L, nbw);
-    uint32_t run = 0;
-    for (uint32_t w = w0; w < w1; ++w) { const uint32_t c = rs_mem[w]; run += (c & 0xFFFFu) + (c >> 16); }
-    uint32_t tot;
-    uint32_t pre = block_excl_scan(run, &tot, sm);
-    for (uint32_t w = w0; w < w1; ++w) {
-      const uint32_t c = rs_mem[w];
-      const uint32_t p0 = pre, p1 = pre + (c & 0xFFFFu);
-      rs_mem[w] = p0 | (p1 << 16);                           // cursors, row-relative (< 65536)
-      B.bin_start[d.bin_ofs + 2 * w] = d.clu_ofs + p0;
-      if (2 * w + 1 < nb) B.bin_start[d.bin_ofs + 2 * w + 1] = d.clu_ofs + p1;
-      pre = p1 + (c >> 16);
+    // ---- S: scan.  Each warp owns a contiguous chunk of the counter words and walks it 32 words
+    // at a time (lane = word: conflict-free shared-memory access, warp scan by shuffles, coalesced
+    // bin_start stores); the chunk totals are scanned by the block in between.
+    {
+      const uint32_t lane = tid & 31u, wid = tid >> 5;
+      const uint32_t chunk = ((nbw + 1023u) / 1024u) * 32u;            // words per warp, a multiple of 32
+      const uint32_t c_lo = min(wid * chunk, nbw), c_hi = min(c_lo + chunk, nbw);
+      uint32_t part = 0;
+      for (uint32_t w = c_lo + lane; w < c_hi; w += 32) { const uint32_t c = rs_mem[w]; part += (c & 0xFFFFu) + (c >> 16); }
+      part = __reduce_add_sync(0xffffffffu, part);
+      uint32_t tot;
+      const uint32_t warp_pre = block_excl_scan(lane == 0 ? part : 0u, &tot, sm);   // exclusive prefix lands on lane 0
+      uint32_t carry = __shfl_sync(0xffffffffu, warp_pre, 0);
+      for (uint32_t w0 = c_lo; w0 < c_hi; w0 += 32) {
+        const uint32_t w = w0 + lane;
+        const uint32_t c = w < c_hi ? rs_mem[w] : 0u;
+        const uint32_t lo = c & 0xFFFFu, both = lo + (c >> 16);
+        uint32_t inc = both;
+#pragma unroll
+        for (int dlt = 1; dlt < 32; dlt <<= 1) {
+          const uint32_t t = __shfl_up_sync(0xffffffffu, inc, dlt);
+          if ((int)lane >= dlt) inc += t;
+        }
+        const uint32_t p0 = carry + inc - both, p1 = p0 + lo;
+        if (w < c_hi) {
+          rs_mem[w] = p0 | (p1 << 16);                       // cursors, row-relative (< 65536)
+          B.bin_start[d.bin_ofs + 2 * w] = d.clu_ofs + p0;
+          if (2 * w + 1 < nb) B.bin_start[d.bin_ofs + 2 * w + 1] = d.clu_ofs + p1;
+        }
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+      }
     }
     __syncthreads();
     // ---- B: place (the row's records now come from L2)
