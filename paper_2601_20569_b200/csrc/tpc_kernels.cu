@@ -423,6 +423,7 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
     const TpcRowStat rs = B.row_stat[sr];
     const tpc_cluster* __restrict__ in = B.clusters + rs.first;
     const uint32_t n_all = rs.n_all;
+    float2* __restrict__ yz_in = reinterpret_cast<float2*>(B.owner) + rs.first;   // (the owner words are not in use yet)
     __syncthreads();                                         // the previous row is done with rs_mem
     for (uint32_t w = tid; w < nbw; w += TPC_RS_THREADS) rs_mem[w] = 0u;
     __syncthreads();
@@ -436,9 +437,15 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
       }
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
+        const uint32_t e = e0 + u * TPC_RS_THREADS;
+        if (e >= n_all) continue;
         int sr_e, row;
         float y, z;
-        if (classify(raw[u], K, sr_e, y, z, row) != 0) continue;
+        const bool kept = classify(raw[u], K, sr_e, y, z, row) == 0;
+        // compact copy of the row for the later passes: 8 bytes per record instead of 16, so that
+        // the rows in flight (148 x ~350 KB) stay in L2; NaN marks a record that is not in the grid
+        yz_in[e] = kept ? make_float2(y, z) : make_float2(__uint_as_float(0x7fc00000u), 0.f);
+        if (!kept) continue;
         const uint32_t bb = bin_of(d, K, y, z) - d.bin_ofs;
         atomicAdd(&rs_mem[bb >> 1], 1u << ((bb & 1u) * 16u));
       }
@@ -479,18 +486,16 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
     __syncthreads();
     // ---- B: place (the row's records now come from L2)
     for (uint32_t e0 = tid; e0 < n_all; e0 += TPC_RS_BATCH * TPC_RS_THREADS) {
-      uint4 raw[TPC_RS_BATCH];
+      float2 v[TPC_RS_BATCH];
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
         const uint32_t e = e0 + u * TPC_RS_THREADS;
-        raw[u] = e < n_all ? *reinterpret_cast<const uint4*>(in + e) : kSkip;
+        v[u] = e < n_all ? yz_in[e] : make_float2(__uint_as_float(0x7fc00000u), 0.f);
       }
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
-        int sr_e, row;
-        float y, z;
-        if (classify(raw[u], K, sr_e, y, z, row) != 0) continue;
-        const uint32_t bb = bin_of(d, K, y, z) - d.bin_ofs;
+        if (!(v[u].x == v[u].x)) continue;   // not in the grid
+        const uint32_t bb = bin_of(d, K, v[u].x, v[u].y) - d.bin_ofs;
         const uint32_t sh = (bb & 1u) * 16u;
         const uint32_t p = (atomicAdd(&rs_mem[bb >> 1], 1u << sh) >> sh) & 0xFFFFu;
         inv[p] = (uint16_t)(e0 + u * TPC_RS_THREADS);
@@ -521,7 +526,7 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
         const uint32_t q = q0 + u * TPC_RS_THREADS;
         e[u] = q < d.count ? (uint32_t)inv[q] : 0u;
-        v[u] = *reinterpret_cast<const uint2*>(in + e[u]);
+        v[u] = *reinterpret_cast<const uint2*>(yz_in + e[u]);
       }
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
