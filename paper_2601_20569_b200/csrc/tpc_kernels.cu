@@ -101,6 +101,7 @@ __global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
   uint32_t n_ign = 0, n_drop = 0, n_bad = 0;
   const uint32_t stride = gridDim.x * blockDim.x, n_up = (B.n + 31u) & ~31u;
+  float2* __restrict__ yz_all = reinterpret_cast<float2*>(B.owner);   // (the owner words are not in use yet)
   for (uint32_t i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < n_up; i0 += 4 * stride) {
    uint4 raw4[4];   // four records requested together (bytes in flight)
 #pragma unroll
@@ -114,7 +115,11 @@ __global__ void __launch_bounds__(256) k_row_stats(TpcBuffers B) {
     if (i >= n_up) break;   // warp-uniform
     int cls = 4, sr = -1, row;
     float y, z = 0.f;
-    if (i < B.n) cls = classify(raw4[u], K, sr, y, z, row);
+    if (i < B.n) {
+      cls = classify(raw4[u], K, sr, y, z, row);
+      // compact copy of the frame for the per-row grid build: 8 bytes per record, NaN = not in the grid
+      yz_all[i] = cls == 0 ? make_float2(y, z) : make_float2(__uint_as_float(0x7fc00000u), 0.f);
+    }
     n_ign += cls == 1;
     n_drop += cls == 2;
     n_bad += cls == 3;
@@ -396,11 +401,12 @@ __global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
 
 // ------------------------------------------------------------------ K1 per-row build
 // The grid of one (sector,row) built by ONE CTA whose shared memory holds the row's bin
-// counters and its permutation (both 16-bit: a qualifying row has < 65536 records), so that
-// HBM sees only streaming traffic: the row's input records once (the later passes hit L2),
-// bin_start, yz and orig_id written once, coalesced.  Used when every row's input records are
-// contiguous (clusteriser order) and fit; otherwise the generic kernels above run (k_row_desc
-// decides).
+// counters and its permutation (both 16-bit: a qualifying row has < 65536 records).  It works
+// on the compact 8-byte (y,z) copy of the frame that k_row_stats leaves in the (not yet used)
+// owner words: the copies of the ~148 rows in flight fit in L2, so HBM sees the records twice
+// in all (k_row_stats, pass A) and bin_start, yz, orig_id once, coalesced.  Used when every
+// row's input records are contiguous (clusteriser order) and fit; otherwise the generic kernels
+// above run (k_row_desc decides).
 //   A  count: bin of every record -> shared-memory atomics (two 16-bit counters per word)
 //   S  scan : exclusive scan of the counters -> bin_start to HBM, counters become cursors
 //   B  place: cursor atomics hand out positions; inv[position] = record
@@ -413,7 +419,6 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
   if (blockIdx.x == 0 && threadIdx.x == 0) B.bin_start[B.cnt->n_bins] = B.cnt->n_sorted;
   const TpcConst* __restrict__ K = B.K;
   const uint32_t tid = threadIdx.x;
-  const uint4 kSkip = make_uint4(0x7fc00000u, 0u, 0u, 0u);   // NaN y: classified "ignored"
   for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
     const tpc_row_desc d = B.row_desc[sr];
     if (d.count == 0) continue;
@@ -421,32 +426,25 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
     const uint32_t nbw = (nb + 1) / 2;                       // counter words
     uint16_t* inv = reinterpret_cast<uint16_t*>(rs_mem + nbw);
     const TpcRowStat rs = B.row_stat[sr];
-    const tpc_cluster* __restrict__ in = B.clusters + rs.first;
     const uint32_t n_all = rs.n_all;
-    float2* __restrict__ yz_in = reinterpret_cast<float2*>(B.owner) + rs.first;   // (the owner words are not in use yet)
+    const float2* __restrict__ yz_in = reinterpret_cast<const float2*>(B.owner) + rs.first;   // written by k_row_stats
     __syncthreads();                                         // the previous row is done with rs_mem
     for (uint32_t w = tid; w < nbw; w += TPC_RS_THREADS) rs_mem[w] = 0u;
     __syncthreads();
-    // ---- A: count.  TPC_RS_BATCH records per thread are requested together
+    // ---- A: count, from the compact (y,z) copy k_row_stats left (NaN = record not in the grid).
+    // TPC_RS_BATCH records per thread are requested together
+    const float2 kNone = make_float2(__uint_as_float(0x7fc00000u), 0.f);
     for (uint32_t e0 = tid; e0 < n_all; e0 += TPC_RS_BATCH * TPC_RS_THREADS) {
-      uint4 raw[TPC_RS_BATCH];
+      float2 v[TPC_RS_BATCH];
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
         const uint32_t e = e0 + u * TPC_RS_THREADS;
-        raw[u] = e < n_all ? ld_stream16(in + e) : kSkip;
+        v[u] = e < n_all ? yz_in[e] : kNone;
       }
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
-        const uint32_t e = e0 + u * TPC_RS_THREADS;
-        if (e >= n_all) continue;
-        int sr_e, row;
-        float y, z;
-        const bool kept = classify(raw[u], K, sr_e, y, z, row) == 0;
-        // compact copy of the row for the later passes: 8 bytes per record instead of 16, so that
-        // the rows in flight (148 x ~350 KB) stay in L2; NaN marks a record that is not in the grid
-        yz_in[e] = kept ? make_float2(y, z) : make_float2(__uint_as_float(0x7fc00000u), 0.f);
-        if (!kept) continue;
-        const uint32_t bb = bin_of(d, K, y, z) - d.bin_ofs;
+        if (!(v[u].x == v[u].x)) continue;
+        const uint32_t bb = bin_of(d, K, v[u].x, v[u].y) - d.bin_ofs;
         atomicAdd(&rs_mem[bb >> 1], 1u << ((bb & 1u) * 16u));
       }
     }
@@ -490,7 +488,7 @@ __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
         const uint32_t e = e0 + u * TPC_RS_THREADS;
-        v[u] = e < n_all ? yz_in[e] : make_float2(__uint_as_float(0x7fc00000u), 0.f);
+        v[u] = e < n_all ? yz_in[e] : kNone;
       }
 #pragma unroll
       for (int u = 0; u < TPC_RS_BATCH; ++u) {
