@@ -378,6 +378,9 @@ def run_ours(args, rank, world, local_rank):
 
     if rank != 0:
         trk.close()
+        if world > 1:
+            dist.barrier()            # rank 0 prints after its CPU-side bookkeeping; leave together
+            dist.destroy_process_group()
         return
 
     # ---- roofline of the dominant kernel (live CUDA-event times over the timed region)
@@ -464,6 +467,7 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
     trk.close()
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
 
 
