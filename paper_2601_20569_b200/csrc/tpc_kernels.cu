@@ -9,9 +9,10 @@
 // Both use only + - * / sqrt on the decision path; every argmin carries an integer tie-break on
 // the ORIGINAL cluster index (rule D2), so atomics / thread order never change a result.
 //
-// Kernel groups:  K1 grid (row stats -> row descriptors -> histogram -> per-row scan -> scatter
-//                 [-> in-bin sort]),  K2 neighbour finder,  K3 link cleanup + seeds,
-//                 K4 Kalman track follower,  K5 ambiguity solving.
+// Kernel groups:  K1 grid (row stats -> row descriptors -> per-row build in shared memory, or,
+//                 for unordered input, histogram -> per-row scan -> scatter [-> in-bin sort]),
+//                 K2 neighbour finder,  K3 link cleanup + seeds,  K4 Kalman track follower
+//                 (outward / refit / inward kernels),  K5 ambiguity solving.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
