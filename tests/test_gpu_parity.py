@@ -238,6 +238,21 @@ def test_det_parity_full_c2_bench_configuration(B):
     assert q["efficiency"] >= 0.95 and q["clone_rate"] <= 0.10 and q["fake_rate"] <= 0.02
 
 
+def test_det_parity_full_c3_and_c5(B):
+    """BASELINE.json configs[2] and configs[4] at FULL size (C3: 5 overlapping events, ~8.5e6
+    clusters; C5: 50000 low-pT tracks in the 63 inner rows of one sector), final tracks bit-exact."""
+    import bench
+    for name in ("C3", "C5"):
+        pkw = dict(bench.WORKLOAD_PARAMS[name])
+        cl, lab, _ = dg.generate(dg.preset(name))
+        gp, op = params_pair(B, **pkw)
+        tracks, ids, shared, view, _ = run_gpu(B, cl, gp, 1)
+        o = oracle.run(cl, params=op, n_threads=8, want=("tracks",))
+        bad = parity.compare_tracks(tracks, ids, shared, o)
+        assert parity.all_zero(bad), (name, bad)
+        assert view.n_tracks == o.n_tracks and o.n_tracks > 1000, (name, o.n_tracks)
+
+
 def test_det_parity_full_c4_sampled_sectors(B):
     """BASELINE.json configs[3], the headline workload, at FULL size (140 events x 12000 tracks,
     ~2.4e8 clusters) with the tracker parameters and launch configuration bench.py times; two
