@@ -105,6 +105,7 @@ typedef struct tpc_params {
 
 /* ------------------------------------------------------------------ output */
 #define TPC_TRACK_PARAMS_STALE 1u /* segment does not contain the row the parameters refer to */
+#define TPC_TRACK_ITER2 2u        /* found by the second seeding iteration (tpc_sector_track_two_iterations) */
 
 /* One sector track (108 bytes).  Parameters are (y, z, sin(phi), tan(lambda), q/pT) at
  * local x of the tracklet's innermost row, c[] the lower-triangular covariance
@@ -278,6 +279,20 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
                                  uint32_t flags, tpc_track* h_tracks, uint64_t cap_tracks,
                                  uint32_t* h_cluster_ids, uint8_t* h_cluster_shared, uint64_t cap_ids,
                                  tpc_track_view* out);
+
+/* Sector tracking with a SECOND SEEDING ITERATION on the leftover clusters (section 3:
+ * "seeding ... in multiple iterations on the leftover clusters after ambiguity solving"; DESIGN.md
+ * reading R7): the path runs on the frame, every cluster attached to a track (owned or shared) is
+ * removed, and the path runs again on the remaining records.  Results: iteration-1 tracks followed
+ * by iteration-2 tracks (flag TPC_TRACK_ITER2), cluster ids in original input indices; read them
+ * with tpc_get_tracks (counts are the sums of both iterations; tpc_get_intermediates is not
+ * available).  d_clusters: DEVICE, as for tpc_sector_track.  The workspace must hold
+ * tpc_workspace_bytes_two_iterations(ctx, n_clusters) bytes.  Unlike tpc_sector_track this call
+ * synchronises cuda_stream (the size of the leftover frame has to reach the host). */
+size_t tpc_workspace_bytes_two_iterations(const tpc_ctx* ctx, uint64_t n_clusters);
+int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters,
+                                    void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+                                    uint32_t flags);
 
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);

@@ -82,7 +82,8 @@ class DebugView(C.Structure):
 
 EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
            "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
-           "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_last_launch_count",
+           "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
+           "tpc_sector_track_two_iterations", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -115,6 +116,10 @@ def load_library():
     L.tpc_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.tpc_get_kernel_ms.restype = C.c_int
     L.tpc_get_kernel_ms.argtypes = [vp, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_float)]
+    L.tpc_workspace_bytes_two_iterations.restype = C.c_size_t
+    L.tpc_workspace_bytes_two_iterations.argtypes = [vp, C.c_uint64]
+    L.tpc_sector_track_two_iterations.restype = C.c_int
+    L.tpc_sector_track_two_iterations.argtypes = [vp, vp, C.c_uint64, vp, C.c_size_t, vp, C.c_uint32]
     L.tpc_sector_track_host_chunks.restype = C.c_int
     L.tpc_sector_track_host_chunks.argtypes = [vp, vp, C.c_uint64, C.POINTER(C.c_uint64), C.c_int, vp, vp, C.c_size_t, vp,
                                                C.c_uint32, vp, C.c_uint64, vp, vp, C.c_uint64, vp]
@@ -224,6 +229,16 @@ def tpc_sector_track_host_chunks(ctx: int, h_clusters: int, n_clusters: int, chu
     return rc, v
 
 
+def tpc_workspace_bytes_two_iterations(ctx: int, n_clusters: int) -> int:
+    return load_library().tpc_workspace_bytes_two_iterations(ctx, n_clusters)
+
+
+def tpc_sector_track_two_iterations(ctx: int, d_clusters: int, n_clusters: int, d_workspace: int, workspace_bytes: int,
+                                    cuda_stream: int, flags: int) -> int:
+    return load_library().tpc_sector_track_two_iterations(ctx, d_clusters, n_clusters, d_workspace, workspace_bytes,
+                                                          cuda_stream, flags)
+
+
 def tpc_last_launch_count(ctx: int) -> int:
     return load_library().tpc_last_launch_count(ctx)
 
@@ -329,6 +344,22 @@ class SectorTracker:
         if rc < 0:
             raise TpcError(rc, "tpc_get_kernel_ms")
         return out
+
+    def track_two_iterations(self, d_clusters, flags: int = 0, stream=None) -> None:
+        """The path plus a second seeding iteration on the leftover clusters; read the
+        combined result with tracks()."""
+        n = d_clusters.numel() // 16
+        need = tpc_workspace_bytes_two_iterations(self.ctx, n)
+        if self.workspace is None or self.workspace.numel() < need + 256:
+            self.workspace = None
+            self.workspace = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        ws_ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc = tpc_sector_track_two_iterations(self.ctx, d_clusters.data_ptr(), n, ws_ptr, need, st.cuda_stream, flags)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_sector_track_two_iterations", tpc_last_cuda_error(self.ctx))
+        self.n = n
+        self._clusters = d_clusters
 
     def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
         """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the

@@ -498,6 +498,173 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
   return rc_all;
 }
 
+// ---------------------------------------------------------------- second seeding iteration (R7)
+// used[i] = 1 for every cluster attached to an iteration-1 track
+__global__ void k_mark_used(const uint32_t* __restrict__ ids, uint32_t n_ids, uint8_t* __restrict__ used) {
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n_ids; j += gridDim.x * blockDim.x) used[ids[j]] = 1;
+}
+// stable compaction of the unused records: per-block counts, one-CTA scan, write
+__global__ void __launch_bounds__(1024) k_left_count(const uint8_t* __restrict__ used, uint32_t n, uint32_t* partials) {
+  const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
+  const int c = __syncthreads_count(i < n && !used[i]);
+  if (threadIdx.x == 0) partials[blockIdx.x] = (uint32_t)c;
+}
+__global__ void __launch_bounds__(1024) k_left_scan(uint32_t* partials, uint32_t n_blocks, uint32_t* total) {
+  __shared__ uint32_t wsum[32];
+  __shared__ uint32_t s_chunk;
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  uint32_t carry = 0;
+  for (uint32_t b0 = 0; b0 < n_blocks; b0 += 1024) {
+    const uint32_t b = b0 + threadIdx.x;
+    const uint32_t v = b < n_blocks ? partials[b] : 0u;
+    uint32_t inc = v;
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if ((int)lane >= d) inc += t; }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+      const uint32_t x = wsum[lane];
+      uint32_t xi = x;
+      for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, xi, d); if ((int)lane >= d) xi += t; }
+      wsum[lane] = xi - x;
+      if (lane == 31) s_chunk = xi;
+    }
+    __syncthreads();
+    if (b < n_blocks) partials[b] = carry + wsum[w] + inc - v;
+    carry += s_chunk;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *total = carry;
+}
+__global__ void __launch_bounds__(1024) k_left_write(const uint8_t* __restrict__ used, const tpc_cluster* __restrict__ in,
+                                                     uint32_t n, const uint32_t* __restrict__ partials,
+                                                     uint32_t* __restrict__ map, tpc_cluster* __restrict__ left) {
+  __shared__ uint32_t wsum[32];
+  const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
+  const bool keep = i < n && !used[i];
+  const uint32_t m = __ballot_sync(0xffffffffu, keep);
+  const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0) wsum[w] = (uint32_t)__popc(m);
+  __syncthreads();
+  if (w == 0) {
+    const uint32_t v = wsum[lane];
+    uint32_t inc = v;
+    for (int d = 1; d < 32; d <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d); if ((int)lane >= d) inc += t; }
+    wsum[lane] = inc - v;
+  }
+  __syncthreads();
+  if (keep) {
+    const uint32_t pos = partials[blockIdx.x] + wsum[w] + (uint32_t)__popc(m & ((1u << lane) - 1u));
+    map[pos] = i;
+    left[pos] = in[i];
+  }
+}
+// iteration-2 results behind the iteration-1 results, in original cluster indices
+__global__ void k_append_iter2(tpc_track* __restrict__ t1, uint32_t n_t1, const tpc_track* __restrict__ t2, uint32_t n_t2,
+                               uint32_t* __restrict__ ids1, uint8_t* __restrict__ sh1, uint32_t n_i1,
+                               const uint32_t* __restrict__ ids2, const uint8_t* __restrict__ sh2, uint32_t n_i2,
+                               const uint32_t* __restrict__ map) {
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n_t2; j += stride) {
+    tpc_track t = t2[j];
+    t.seed_id = map[t.seed_id];
+    t.cluster_ofs += n_i1;
+    t.flags |= TPC_TRACK_ITER2;
+    t1[n_t1 + j] = t;
+  }
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n_i2; j += stride) {
+    ids1[n_i1 + j] = map[ids2[j]];
+    sh1[n_i1 + j] = sh2[j];
+  }
+}
+
+namespace {
+struct Iter2Layout { size_t ws_one, used, map, left, partials, total; uint32_t n_blocks; };
+Iter2Layout iter2_layout(const tpc_ctx* c, uint64_t n) {
+  Iter2Layout L;
+  L.ws_one = align_up(carve(c, n, nullptr, nullptr), 256);
+  L.n_blocks = (uint32_t)((n + 1023) / 1024);
+  size_t off = 2 * L.ws_one;
+  L.used = off; off = align_up(off + n, 256);
+  L.map = off; off = align_up(off + 4 * n, 256);
+  L.left = off; off = align_up(off + 16 * n, 256);
+  L.partials = off; off = align_up(off + 4 * ((size_t)L.n_blocks + 2), 256);
+  L.total = off;
+  return L;
+}
+}  // namespace
+
+size_t tpc_workspace_bytes_two_iterations(const tpc_ctx* ctx, uint64_t n_clusters) {
+  if (!ctx || n_clusters >= (1ull << 30)) return 0;
+  return iter2_layout(ctx, n_clusters).total;
+}
+
+int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters, void* d_workspace,
+                                    size_t workspace_bytes, void* cuda_stream, uint32_t flags) {
+  if (!ctx || !d_workspace || (!d_clusters && n_clusters) || n_clusters >= (1ull << 30)) return TPC_E_ARG;
+  if (((uintptr_t)d_workspace & 255u)) return TPC_E_ARG;
+  const Iter2Layout L = iter2_layout(ctx, n_clusters);
+  if (workspace_bytes < L.total) return TPC_E_WORKSPACE;
+  char* base = (char*)d_workspace;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const uint32_t n = (uint32_t)n_clusters;
+  flags &= ~(uint32_t)TPC_KEEP_INTERMEDIATES;
+  // ---- iteration 1 (R1..R6)
+  int rc = enqueue_track(ctx, d_clusters, n_clusters, base, L.ws_one, cuda_stream, flags, 0u, 0u);
+  if (rc != TPC_OK) return rc;
+  tpc_track_view v1;
+  rc = tpc_get_tracks(ctx, &v1);
+  if (rc != TPC_OK) return rc;
+  const TpcBuffers B1 = ctx->buf;
+  const TpcCounters c1 = *ctx->h_cnt;
+  const int launches1 = ctx->launches;
+  // ---- R7.1 / R7.2: leftover frame
+  uint8_t* used = (uint8_t*)(base + L.used);
+  uint32_t* map = (uint32_t*)(base + L.map);
+  tpc_cluster* left = (tpc_cluster*)(base + L.left);
+  uint32_t* partials = (uint32_t*)(base + L.partials);
+  uint32_t* d_total = partials + L.n_blocks;
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(used, 0, n_clusters, st)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemsetAsync(used)");
+  uint32_t n_left = 0;
+  if (n) {
+    if (c1.n_ids) k_mark_used<<<ctx->n_sm * 8, 256, 0, st>>>(B1.cluster_ids, c1.n_ids, used);
+    k_left_count<<<L.n_blocks, 1024, 0, st>>>(used, n, partials);
+    k_left_scan<<<1, 1024, 0, st>>>(partials, L.n_blocks, d_total);
+    k_left_write<<<L.n_blocks, 1024, 0, st>>>(used, d_clusters, n, partials, map, left);
+    if ((e = cudaMemcpyAsync(&n_left, d_total, 4, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(st)) != cudaSuccess)
+      return set_cuda_err(ctx, e, "leftover frame");
+  }
+  // ---- R7.3: the path on the leftover frame
+  rc = enqueue_track(ctx, left, n_left, base + L.ws_one, L.ws_one, cuda_stream, flags, 0u, 0u);
+  if (rc != TPC_OK) return rc;
+  tpc_track_view v2;
+  rc = tpc_get_tracks(ctx, &v2);
+  if (rc != TPC_OK) return rc;
+  const TpcCounters c2 = *ctx->h_cnt;
+  // ---- R7.4: append in original indices
+  if ((uint64_t)c1.n_tracks + c2.n_tracks > B1.max_tracks || (uint64_t)c1.n_ids + c2.n_ids > B1.max_ids) return TPC_E_OVERFLOW;
+  if (c2.n_tracks || c2.n_ids) {
+    k_append_iter2<<<ctx->n_sm * 8, 256, 0, st>>>(B1.tracks, c1.n_tracks, ctx->buf.tracks, c2.n_tracks, B1.cluster_ids,
+                                                  B1.cluster_shared, c1.n_ids, ctx->buf.cluster_ids,
+                                                  ctx->buf.cluster_shared, c2.n_ids, map);
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return set_cuda_err(ctx, e, "append");
+  }
+  // the context now describes the combined result (tpc_get_tracks reads it)
+  TpcCounters c = c1;
+  c.n_tracks += c2.n_tracks; c.n_ids += c2.n_ids; c.n_seeds += c2.n_seeds; c.n_tracklets += c2.n_tracklets;
+  c.n_bins += c2.n_bins; c.error |= c2.error;
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) c.follow_work[a][b] += c2.follow_work[a][b];
+  *ctx->h_cnt = c;
+  ctx->buf = B1;
+  ctx->flags = flags;
+  ctx->launches = launches1 + ctx->launches + 5;
+  ctx->ran = true;
+  ctx->synced = true;
+  return TPC_OK;
+}
+
 int tpc_last_launch_count(const tpc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 void tpc_destroy(tpc_ctx* c) {

@@ -317,3 +317,48 @@ def test_chunked_host_call_rejects_a_sector_in_two_chunks(B):
     with pytest.raises(B.TpcError) as e:
         _host_run(B, cl, [0, mid, len(cl)], flags=1)
     assert e.value.code == B.TPC_E_ARG
+
+
+def _canonical_two(tracks, ids, shared):
+    """Canonical order for a two-iteration result: (iteration, sector, seed id, segment)."""
+    it = (tracks["flags"].astype(np.int64) >> 1) & 1
+    order = np.lexsort((tracks["segment"], tracks["seed_id"], tracks["sector"], it))
+    tr = tracks[order]
+    n_per = tr["n_clusters"].astype(np.int64)
+    ofs = tr["cluster_ofs"].astype(np.int64)
+    within = np.arange(int(n_per.sum()), dtype=np.int64) - np.repeat(np.cumsum(n_per) - n_per, n_per)
+    g = np.repeat(ofs, n_per) + within
+    return tr, np.asarray(ids)[g], np.asarray(shared)[g]
+
+
+@pytest.mark.parametrize("name", ["C5_reduced", "C2_reduced"])
+def test_det_parity_second_seeding_iteration(B, name):
+    """the path, then the path again on the leftover
+    clusters; deterministic mode, bit-exact against oracle/second_iteration.py."""
+    from oracle import second_iteration as si
+    if name == "C5_reduced":
+        cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+    else:
+        cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=3000, seed=17))
+        pkw = {}
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        trk.track_two_iterations(trk.upload(cl), flags=1)
+        tracks, ids, shared, view = trk.tracks()
+    finally:
+        trk.close()
+    o = si.run_two_iterations(cl, params=op, n_threads=8)
+    assert view.n_tracks == o.n_tracks and view.n_cluster_ids == o.n_cluster_ids
+    tr, ci, sh = _canonical_two(tracks, ids, shared)
+    otr, oci, osh = _canonical_two(o.tracks, o.cluster_ids, o.cluster_shared)
+    for f in ("seed_id", "n_clusters", "n_shared", "sector", "row_first", "row_last", "flags", "n_hits_tracklet", "segment"):
+        assert (tr[f].astype(np.int64) == otr[f].astype(np.int64)).all(), f
+    for f in ("x", "p", "c", "chi2"):
+        assert (np.ascontiguousarray(tr[f]).view(np.uint32) == np.ascontiguousarray(otr[f]).view(np.uint32)).all(), f
+    assert (ci == oci).all() and (sh == osh).all()
+    n2 = int(((tracks["flags"] >> 1) & 1).sum())
+    assert n2 == o.second.n_tracks
+    if name == "C5_reduced":
+        assert n2 > 0
