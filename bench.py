@@ -290,11 +290,15 @@ def run_ours(args, rank, world, local_rank):
     h_clusters.numpy()[:] = clusters.view(np.uint8).reshape(-1)
     d_clusters = torch.empty(n * 16, dtype=torch.uint8, device=dev)
     d_clusters.copy_(h_clusters)
-    ws_bytes = trk.ensure_workspace(n)
+    ws_bytes = (B.tpc_workspace_bytes_two_iterations(trk.ctx, n) if args.second_iteration
+                else trk.ensure_workspace(n))
     torch.cuda.synchronize()
 
     def step():
-        trk.track(d_clusters, flags=flags, stream=stream)
+        if args.second_iteration:     # the path, then the path on the leftover clusters
+            trk.track_two_iterations(d_clusters, flags=flags, stream=stream)
+        else:
+            trk.track(d_clusters, flags=flags, stream=stream)
         rc, v = trk.counts()          # tpc_get_tracks: syncs the stream, reads the counters
         return v
 
@@ -327,6 +331,24 @@ def run_ours(args, rank, world, local_rank):
     launches = trk.launch_count() * args.steps
     stage_ms = trk.stage_ms()
     value = n_all * args.steps / (ms_total * 1e-3)
+
+    if args.second_iteration:
+        # reduced line: kernel times / roofline would describe the second pass only
+        if rank == 0:
+            print(json.dumps({
+                "metric": METRIC + ", with a second seeding iteration on the leftover clusters", "value": value,
+                "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"{args.workload} + second iteration (SURVEY.md 8(f) row 1)", "n_clusters_per_gpu": n,
+                           "mode": args.mode, "tracker_params": pkw, "n_tracks": int(v.n_tracks),
+                           "n_seeds_both_iterations": int(v.n_seeds), "workspace_gb": ws_bytes / 1e9},
+                "gpu_launches": launches}), flush=True)
+        trk.close()
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
 
     # ---- end-to-end: HOST buffers through the C ABI, copies inside the timed region
     cap_tracks = int(v.n_tracks * 1.05) + 1024
@@ -488,6 +510,8 @@ def main():
                     help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="equal chunks of whole sectors in the end-to-end leg (1 = one shot, 0 = ramped schedule)")
     ap.add_argument("--e2e-cuts", default="", help="sector boundaries of the chunks of the end-to-end leg (overrides --e2e-chunks)")
+    ap.add_argument("--second-iteration", action="store_true",
+                    help="time tpc_sector_track_two_iterations (the path + a second seeding iteration) instead")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
