@@ -331,16 +331,16 @@ def _canonical_two(tracks, ids, shared):
     return tr, np.asarray(ids)[g], np.asarray(shared)[g]
 
 
-@pytest.mark.parametrize("name", ["C5_reduced", "C2_reduced"])
+@pytest.mark.parametrize("name", ["C5_reduced", "C2_reduced", "C2_full", "C5_full"])
 def test_det_parity_second_seeding_iteration(B, name):
     """the path, then the path again on the leftover
     clusters; deterministic mode, bit-exact against oracle/second_iteration.py."""
     from oracle import second_iteration as si
-    if name == "C5_reduced":
-        cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+    if name.startswith("C5"):
+        cl, _, _ = dg.generate(dg.preset("C5", **({} if name == "C5_full" else dict(tracks_per_event=8000))))
         pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
     else:
-        cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=3000, seed=17))
+        cl, _, _ = dg.generate(dg.preset("C2", **({} if name == "C2_full" else dict(tracks_per_event=3000, seed=17))))
         pkw = {}
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
@@ -360,5 +360,5 @@ def test_det_parity_second_seeding_iteration(B, name):
     assert (ci == oci).all() and (sh == osh).all()
     n2 = int(((tracks["flags"] >> 1) & 1).sum())
     assert n2 == o.second.n_tracks
-    if name == "C5_reduced":
+    if name.startswith("C5"):
         assert n2 > 0
