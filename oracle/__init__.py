@@ -50,7 +50,7 @@ class Params(C.Structure):
                 ("max_gap_follow", C.c_int32), ("min_hits_tracklet", C.c_int32),
                 ("sel_chi2_weight", C.c_float),
                 ("shared_permille", C.c_int32), ("max_gap_select", C.c_int32), ("min_hits_track", C.c_int32),
-                ("grid_dy", C.c_float), ("grid_dz", C.c_float)]
+                ("grid_dy", C.c_float), ("grid_dz", C.c_float), ("shared_fixed_cap", C.c_int32)]
 
 
 def default_geom(**kw) -> Geom:

@@ -517,7 +517,11 @@ void select_tracks(int R, const orc_params& P, size_t n_idx, size_t n_t, const o
       int32_t c = row_hit[k * (size_t)R + r];
       bool sh = false;
       if (c >= 0 && owner[c] != key[k]) {
-        if ((int64_t)(n_sh + 1) * 1000 <= (int64_t)P.shared_permille * (n_acc + 1)) sh = true;
+        // R6.3: Phase-I running fraction counted from the outermost row, or, as the
+        // variant of SURVEY.md 8(f), the fixed cap of the rule before Phase I (shared_fixed_cap)
+        const int64_t budget = P.shared_fixed_cap ? (int64_t)P.shared_permille * tl[k].n_hits
+                                                  : (int64_t)P.shared_permille * (n_acc + 1);
+        if ((int64_t)(n_sh + 1) * 1000 <= budget) sh = true;
         else c = -1;
       }
       if (c >= 0) {
@@ -582,6 +586,7 @@ void orc_default_params(orc_params* p) {
   p->max_gap_follow = 4; p->min_hits_tracklet = 10;
   p->sel_chi2_weight = 2.0f;
   p->shared_permille = 100; p->max_gap_select = 4; p->min_hits_track = 20;
+  p->shared_fixed_cap = 0;
   p->grid_dy = 2.0f; p->grid_dz = 2.0f;
 }
 

@@ -55,6 +55,8 @@ typedef struct orc_params { /* DESIGN.md "Parameters" */
   float sel_chi2_weight;
   int32_t shared_permille, max_gap_select, min_hits_track;
   float grid_dy, grid_dz;
+  int32_t shared_fixed_cap; /* 0: running fraction from the outermost row (Phase I); 1: fixed cap
+                               floor(shared_permille * nHits / 1000) per segment (the rule before Phase I) */
 } orc_params;
 
 typedef struct orc_row_desc {

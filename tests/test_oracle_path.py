@@ -424,3 +424,25 @@ def test_sectors_are_independent():
     single = oracle.run(cl, n_threads=1)
     assert single.tracks.tobytes() == full.tracks.tobytes()
     assert np.array_equal(single.cluster_ids, full.cluster_ids)
+
+
+def test_selector_fixed_cap_variant_spends_the_budget_on_the_outer_rows():
+    """SURVEY.md 8(f) variant (the rule before Phase I): with a fixed cap floor(f*nHits) the shared
+    budget is spent where the walk starts, on the OUTER rows, and nothing is left for the inner
+    ones; the Phase-I running fraction does the opposite.  Hand-computed expectation:
+    tracklet A (rows 0..99) loses rows 90..99 and 0..9 to a better, short tracklet B."""
+    rows = np.arange(0, 100)
+    a = straight_tracklet(rows, 0)
+    b = np.full(152, -1, dtype=np.int32)
+    b[0:10] = a[0:10]
+    b[90:100] = a[90:100]
+    args = (np.stack([a, b]), [100, 20], [45.0 * 195, 0.0], [1, 2])      # Q_A = 100 - 2*45 = 10 < Q_B = 20
+    running = oracle.select_only(*args, n_clusters=3000)
+    t = running.tracks[running.tracks["seed_id"] == 1][0]
+    # outer foreign rows refused (no budget yet); own rows 10..89; inner: (k)*1000 <= 100*(80+k) -> k <= 8
+    assert (t["n_clusters"], t["n_shared"], t["row_first"], t["row_last"]) == (88, 8, 2, 89)
+    fixed = oracle.select_only(*args, n_clusters=3000, params=oracle.default_params(shared_fixed_cap=1))
+    t = fixed.tracks[fixed.tracks["seed_id"] == 1][0]
+    # cap = floor(0.1*100) = 10, spent on rows 99..90; rows 9..0 refused
+    assert (t["n_clusters"], t["n_shared"], t["row_first"], t["row_last"]) == (90, 10, 10, 99)
+    assert running.n_tracks == fixed.n_tracks == 1                        # B: two 10-hit segments, below min_hits_track
