@@ -100,7 +100,10 @@ typedef struct tpc_params {
   uint64_t max_bins;             /* bin-index capacity; 0 = default
                                     4*n_clusters + n_sectors*n_rows*ny_max*(z_max/grid_dz+2)   */
   uint32_t max_seeds;            /* seed/tracklet capacity; 0 = default n_clusters/8 + 4096     */
-  uint32_t reserved[3];
+  uint32_t shared_fixed_cap;     /* 0: shared clusters by the running fraction counted from the outermost
+                                    row (Phase I); 1: fixed cap shared_permille*nHits/1000
+                                    per segment (the rule before Phase I; A/B variant)             */
+  uint32_t reserved[2];
 } tpc_params;
 
 /* ------------------------------------------------------------------ output */

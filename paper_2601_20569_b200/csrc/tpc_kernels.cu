@@ -1891,6 +1891,7 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
   const int r0 = tl.row_first, r1 = tl.row_last;
   const int min_hits = P.min_hits_track, max_gap = P.max_gap_select;
   const int permille = P.shared_permille;
+  const bool fixed_cap = P.shared_fixed_cap != 0;   // variant: the rule before Phase I
   const int R = B.K->n_rows;
   uint32_t has[TPC_MASK_WORDS], own[TPC_MASK_WORDS], acc[TPC_MASK_WORDS], shm[TPC_MASK_WORDS];
 #pragma unroll
@@ -1910,7 +1911,8 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
     int n_own = 0;
 #pragma unroll
     for (int w = 0; w < TPC_MASK_WORDS; ++w) n_own += __popc(own[w]);
-    if (n_own * 1000 < min_hits * (1000 - permille)) { n_seg_out = 0; n_id_out = 0; return; }
+    if (fixed_cap ? n_own * 1000 + permille * (int)tl.n_hits < min_hits * 1000
+                  : n_own * 1000 < min_hits * (1000 - permille)) { n_seg_out = 0; n_id_out = 0; return; }
   }
   auto close = [&]() {
     if (n_acc >= min_hits) {
@@ -1963,7 +1965,7 @@ __device__ __forceinline__ void walk_tracklet(const TpcBuffers& B, uint32_t sd, 
       bool c = (hw >> b) & 1u;
       bool sh = false;
       if (c && !((ow >> b) & 1u)) {
-        if ((n_sh + 1) * 1000 <= permille * (n_acc + 1)) sh = true;
+        if ((n_sh + 1) * 1000 <= (fixed_cap ? permille * (int)tl.n_hits : permille * (n_acc + 1))) sh = true;
         else c = false;
       }
       if (c) {
@@ -2007,7 +2009,9 @@ __global__ void __launch_bounds__(256) k_sel_count(TpcBuffers B) {
 #pragma unroll
       for (int w = 0; w < TPC_MASK_WORDS; ++w)
         if (w * 32 < B.K->n_rows) n_own += __popc(B.tl_mask[(size_t)(TPC_MASK_WORDS + w) * B.max_seeds + sd]);
-      cand = n_own * 1000 >= B.K->P.min_hits_track * (1000 - B.K->P.shared_permille);
+      const tpc_params& P = B.K->P;
+      cand = P.shared_fixed_cap ? n_own * 1000 + P.shared_permille * (int)B.tracklets[sd].n_hits >= P.min_hits_track * 1000
+                                : n_own * 1000 >= P.min_hits_track * (1000 - P.shared_permille);
     }
     s_ns[threadIdx.x] = 0u; s_ni[threadIdx.x] = 0u;
     uint32_t n_cand;

@@ -91,6 +91,19 @@ def test_det_parity_c5_reduced_dense_shared(B):
     assert o.cluster_shared.sum() > 0
 
 
+def test_det_parity_selector_variants(B):
+    """SURVEY.md 8(f) variant switch: the selector before Phase I (length-dominated weight, fixed
+    shared cap) and the loose 20 % setting, deterministic, bit-exact."""
+    cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+    base = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+    n = []
+    for kw in (dict(shared_fixed_cap=1), dict(shared_fixed_cap=1, sel_chi2_weight=0.0),
+               dict(shared_fixed_cap=1, shared_permille=200), dict(sel_chi2_weight=0.0)):
+        o, tracks = assert_det_parity(B, cl, **base, **kw)
+        n.append(o.n_tracks)
+    assert len(set(n)) > 1          # the variants do change the result
+
+
 def test_det_parity_shuffled_input_and_ragged_sizes(B):
     """Input in any order (not grouped by row), sizes that are not multiples of any tile."""
     cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=700, seed=31))
