@@ -102,6 +102,8 @@ def lib():
         L.orc_update_d.argtypes = [vp] + [C.c_double] * 6 + [vp]
         L.orc_fit_hits.restype = C.c_float
         L.orc_fit_hits.argtypes = [C.POINTER(Geom), C.POINTER(Params), vp, vp, vp, C.c_int, vp]
+        L.orc_refit_hits.restype = C.c_float
+        L.orc_refit_hits.argtypes = [C.POINTER(Geom), C.POINTER(Params), vp, vp, vp, C.c_int, vp]
         L.orc_select_only.restype = vp
         L.orc_select_only.argtypes = [C.POINTER(Geom), C.POINTER(Params), C.c_uint64, C.c_int, vp, vp, vp, vp]
         _lib = L
@@ -246,3 +248,34 @@ def fit_hits(rows, y, z, geom: Geom | None = None, params: Params | None = None)
     if chi2 < 0:
         return None
     return float(chi2), float(out[0]), out[1:6].copy(), out[6:21].copy(), int(out[21]), int(out[22])
+
+
+def refit_hits(rows, y, z, geom: Geom | None = None, params: Params | None = None):
+    """R8 sector-track refit of a given cluster list (rows strictly ascending, holes allowed).
+    Returns (chi2, x, p[5], c[15], n) or None if the fit left the |sin phi| range."""
+    geom = geom or default_geom()
+    params = params or default_params()
+    rows = np.ascontiguousarray(rows, dtype=np.int32)
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    z = np.ascontiguousarray(z, dtype=np.float32)
+    out = np.zeros(24, dtype=np.float32)
+    chi2 = lib().orc_refit_hits(C.byref(geom), C.byref(params), _ptr(rows), _ptr(y), _ptr(z), len(rows), _ptr(out))
+    if chi2 < 0:
+        return None
+    return float(chi2), float(out[0]), out[1:6].copy(), out[6:21].copy(), int(out[21])
+
+
+def refit_tracks(clusters: np.ndarray, tracks: np.ndarray, cluster_ids: np.ndarray, geom=None, params=None):
+    """R8 for every track of a result: (fit[n_tracks] records x,p,c,chi2,n_clusters,ok) from the
+    tracks' cluster lists (original indices into ``clusters``)."""
+    dt = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"), ("n_clusters", "<u4"),
+                   ("flags", "<u4")])
+    out = np.zeros(len(tracks), dtype=dt)
+    for k, t in enumerate(tracks):
+        ids = cluster_ids[int(t["cluster_ofs"]): int(t["cluster_ofs"]) + int(t["n_clusters"])]
+        r = refit_hits(clusters["row"][ids], clusters["y"][ids], clusters["z"][ids], geom, params)
+        if r is None:
+            out[k]["flags"] = 1
+            continue
+        out[k]["chi2"], out[k]["x"], out[k]["p"], out[k]["c"], out[k]["n_clusters"] = r
+    return out

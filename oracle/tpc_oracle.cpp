@@ -815,6 +815,63 @@ float orc_fit_hits(const orc_geom* g, const orc_params* pp, const int32_t* rows,
   return tl.chi2;
 }
 
+// R8 sector-track refit ("a sector track refit at the beginning of the track merging
+// was added, guaranteeing reasonable initial parameters"; reading R8).  A pure Kalman fit
+// of a GIVEN cluster list (rows strictly ascending, holes allowed), no search and no chi2 cut:
+//   R8.1 init at the first cluster from the first two (dx = row distance * pitch), C = initial diagonal
+//   R8.2 outward: row by row to every further cluster (pure propagation on rows in between), update
+//   R8.3 turn at the last cluster as R5.4 (s,t,q after its update; y,z measured; C reset)
+//   R8.4 inward: back through the clusters to the first one, chi2 accumulated in this pass
+// out_state = x, p[5], c[15], n at the first cluster's row.  Returns chi2, or -1 if a propagation
+// or an update left the |sin phi| range (the fit failed; out_state untouched).
+float orc_refit_hits(const orc_geom* g, const orc_params* pp, const int32_t* rows, const float* y,
+                     const float* z, int n, float* out_state) {
+  orc_params P;
+  if (pp) P = *pp; else orc_default_params(&P);
+  const Tables T = make_tables(*g, P.grid_dy);
+  if (n < 2) return -1.0f;
+  const float vy = P.err_y * P.err_y, vz = P.err_z * P.err_z;
+  KFState<float> st;
+  auto reset_cov = [&]() {
+    for (int i = 0; i < 15; ++i) st.c[i] = 0.0f;
+    st.c[0] = vy; st.c[2] = vz; st.c[5] = P.init_var_sinphi; st.c[9] = P.init_var_tanl; st.c[14] = P.init_var_qpt;
+  };
+  {  // R8.1
+    const float dx = (float)(rows[1] - rows[0]) * T.dx_row;   // the pitch the propagation steps use
+    const float dy = y[1] - y[0];
+    const float dl = std::sqrt(dx * dx + dy * dy);
+    st.y = y[0]; st.z = z[0];
+    st.s = dy / dl;
+    st.t = (z[1] - z[0]) / dl;
+    st.q = 0.0f;
+    reset_cov();
+  }
+  float snap_s = st.s, snap_t = st.t, snap_q = st.q;
+  for (int i = 1; i < n; ++i) {  // R8.2
+    for (int r = rows[i - 1]; r < rows[i]; ++r)
+      if (!tpc_oracle::kf_propagate(st, T.dx_row, T.cfield, P.max_sinphi)) return -1.0f;
+    const KFGain<float> gn = tpc_oracle::kf_gain(st, vy, vz);
+    if (tpc_oracle::kf_update(st, gn, y[i], z[i], P.max_sinphi, P.max_qpt)) return -1.0f;
+    snap_s = st.s; snap_t = st.t; snap_q = st.q;
+  }
+  st.y = y[n - 1]; st.z = z[n - 1]; st.s = snap_s; st.t = snap_t; st.q = snap_q;  // R8.3
+  reset_cov();
+  float chi2 = 0.0f;
+  for (int i = n - 2; i >= 0; --i) {  // R8.4
+    for (int r = rows[i + 1]; r > rows[i]; --r)
+      if (!tpc_oracle::kf_propagate(st, -T.dx_row, T.cfield, P.max_sinphi)) return -1.0f;
+    const KFGain<float> gn = tpc_oracle::kf_gain(st, vy, vz);
+    const float c2 = tpc_oracle::kf_chi2(st, gn, y[i], z[i]);
+    if (tpc_oracle::kf_update(st, gn, y[i], z[i], P.max_sinphi, P.max_qpt)) return -1.0f;
+    chi2 = chi2 + c2;
+  }
+  out_state[0] = T.x[rows[0]];
+  out_state[1] = st.y; out_state[2] = st.z; out_state[3] = st.s; out_state[4] = st.t; out_state[5] = st.q;
+  for (int i = 0; i < 15; ++i) out_state[6 + i] = st.c[i];
+  out_state[21] = (float)n;
+  return chi2;
+}
+
 orc_result* orc_select_only(const orc_geom* g, const orc_params* pp, uint64_t n_clusters, int n_tracklets,
                             const int32_t* row_hit, const int32_t* n_hits, const float* chi2,
                             const uint32_t* seed_id) {

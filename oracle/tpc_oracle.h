@@ -125,6 +125,11 @@ double orc_update_d(double* state, double ym, double zm, double vy, double vz, d
  * out_state = 20 floats at rows[0]; returns chi2 of the down pass or -1 if the leg stopped. */
 float orc_fit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows, const float* y,
                    const float* z, int n, float* out_state);
+/* R8 sector-track refit: pure Kalman fit of a given cluster list (rows strictly ascending, holes
+ * allowed; outward pass, turn, inward pass; no search, no chi2 cut).  out_state = x, p[5], c[15], n
+ * (22 floats) at rows[0]; returns the chi2 of the inward pass or -1 if the fit left |sin phi|. */
+float orc_refit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows, const float* y,
+                     const float* z, int n, float* out_state);
 /* selector on hand-made tracklets: row_hit[n_tracklets][n_rows] (cluster ids or -1),
  * n_hits/chi2/seed_id per tracklet.  Results via orc_fetch_tracks. */
 orc_result* orc_select_only(const orc_geom* g, const orc_params* p, uint64_t n_clusters, int n_tracklets,

@@ -310,3 +310,65 @@ def test_noise_free_fit_recovers_generating_parameters():
         assert chi2 < 1e-3
         n_checked += 1
     assert n_checked > 100
+
+
+# ------------------------------------------------------------------ R8 sector-track refit
+def _track_hit_lists(cfg, min_hits, keep_holes):
+    clusters, labels, truth = dg.generate(cfg)
+    order = np.argsort(labels, kind="stable")
+    lab_s = labels[order]
+    starts = np.flatnonzero(np.r_[True, lab_s[1:] != lab_s[:-1]])
+    ends = np.r_[starts[1:], len(lab_s)]
+    for a, b in zip(starts, ends):
+        lab = lab_s[a]
+        if lab < 0 or lab % 8 != 0 or b - a < min_hits:
+            continue
+        idx = order[a:b]
+        rows = clusters["row"][idx].astype(np.int32)
+        o = np.argsort(rows, kind="stable")
+        rows, idx = rows[o], idx[o]
+        if len(np.unique(rows)) != len(rows):
+            continue
+        if not keep_holes and not (np.diff(rows) == 1).all():
+            continue
+        yield rows, clusters["y"][idx], clusters["z"][idx], truth[lab // 8]
+
+
+def test_refit_equals_the_follower_fit_on_hole_free_lists():
+    """On a cluster list without holes the refit (R8) performs the statements of the follower's
+    chain fit, turn and inward refit (R5.1, R5.2, R5.4, R5.5), which are pinned above: same bits."""
+    cfg = dg.preset("C1", tracks_per_event=400, noise_frac=0.0, seed=5, pt_lo=0.4, p_hit=1.0)
+    n = 0
+    for rows, y, z, _ in _track_hit_lists(cfg, 30, keep_holes=False):
+        a = oracle.fit_hits(rows, y, z)
+        b = oracle.refit_hits(rows, y, z)
+        if a is None or a[4] != len(rows) or a[5] != rows[0]:
+            continue            # the follower stopped early or picked something up: not the same hit list
+        assert b is not None
+        assert np.float32(a[0]).tobytes() == np.float32(b[0]).tobytes()
+        assert a[2].tobytes() == b[2].tobytes() and a[3].tobytes() == b[3].tobytes() and a[1] == b[1]
+        n += 1
+    assert n >= 100
+
+
+def test_refit_pulls_have_unit_width_with_holes():
+    """Lists with holes (hit probability 0.8): pulls of the refit parameters at the innermost cluster."""
+    cfg = dg.preset("C1", tracks_per_event=5000, noise_frac=0.0, seed=78, pt_lo=0.3, p_hit=0.8)
+    x_rows, _, _, _ = oracle.geom_tables()
+    alpha = math.radians(10.0)
+    pulls = []
+    for rows, y, z, tr in _track_hit_lists(cfg, 50, keep_holes=True):
+        fit = oracle.refit_hits(rows, y, z)
+        if fit is None:
+            continue
+        chi2, x, p, c, n = fit
+        assert x == x_rows[rows[0]] and n == len(rows)
+        want = _true_state_at(float(x), float(tr["phi0"]) - alpha, float(tr["pt"]), int(tr["charge"]), float(tr["tanl"]))
+        diag = np.array([c[0], c[2], c[5], c[9], c[14]], dtype=np.float64)
+        pulls.append((p.astype(np.float64) - want) / np.sqrt(diag))
+    pulls = np.array(pulls)
+    assert len(pulls) >= 1500, len(pulls)
+    mean, width = pulls.mean(axis=0), pulls.std(axis=0)
+    assert np.all(np.abs(mean[[0, 2, 4]]) <= 0.08), mean
+    assert np.all(np.abs(mean[[1, 3]]) <= 0.12), mean
+    assert np.all((width >= 0.93) & (width <= 1.12)), width
