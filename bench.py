@@ -332,6 +332,21 @@ def run_ours(args, rank, world, local_rank):
     stage_ms = trk.stage_ms()
     value = n_all * args.steps / (ms_total * 1e-3)
 
+    # ---- sector-track refit of the frame's tracks (first half; not part of `value`)
+    refit = None
+    if args.refit and not args.second_iteration:
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            B.tpc_refit_tracks(trk.ctx, stream.cuda_stream); B.tpc_get_refit(trk.ctx)      # warm-up
+            r0.record(stream)
+            for _ in range(args.steps):
+                B.tpc_refit_tracks(trk.ctx, stream.cuda_stream)
+            r1.record(stream)
+            B.tpc_get_refit(trk.ctx)
+        torch.cuda.synchronize()
+        ms = r0.elapsed_time(r1) / args.steps
+        refit = {"ms": ms, "tracks": int(v.n_tracks), "clusters_refitted_per_s": int(v.n_cluster_ids) / (ms * 1e-3)}
+
     if args.second_iteration:
         # reduced line: kernel times / roofline would describe the second pass only
         if rank == 0:
@@ -484,7 +499,7 @@ def run_ours(args, rank, world, local_rank):
         "roofline": roof, "stages_hbm": stages,
         "stage_ms": {k: round(x, 4) for k, x in stage_ms.items()},
         "kernels_ms_per_step": {k["name"]: round(k["ms_per_step"], 4) for k in per_kernel},
-        "cpu_baseline": cpu,
+        "cpu_baseline": cpu, "refit": refit,
     }
     print(json.dumps(line), flush=True)
     trk.close()
@@ -510,6 +525,7 @@ def main():
                     help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="equal chunks of whole sectors in the end-to-end leg (1 = one shot, 0 = ramped schedule)")
     ap.add_argument("--e2e-cuts", default="", help="sector boundaries of the chunks of the end-to-end leg (overrides --e2e-chunks)")
+    ap.add_argument("--refit", action="store_true", help="also time tpc_refit_tracks on the frame's tracks (reported beside the metric)")
     ap.add_argument("--second-iteration", action="store_true",
                     help="time tpc_sector_track_two_iterations (the path + a second seeding iteration) instead")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -297,6 +297,26 @@ int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                                     uint32_t flags);
 
+/* SECTOR-TRACK REFIT (section 3: "a sector track refit at the beginning of the track
+ * merging was added, guaranteeing reasonable initial parameters"; reading R8): a pure
+ * Kalman fit of every output track through ITS OWN cluster list (outward pass, turn, inward pass;
+ * no search, no chi2 cut), giving parameters that are valid at the track's innermost cluster also
+ * for the segments flagged TPC_TRACK_PARAMS_STALE.  Runs on the result of the last
+ * tpc_sector_track / tpc_sector_track_two_iterations of this context (its d_clusters must still be
+ * valid), in the mode (deterministic or fast) of that run; enqueued on cuda_stream. */
+typedef struct tpc_track_fit {
+  float x;               /* local x of the innermost cluster's row                          */
+  float p[5];            /* y, z, sin(phi), tan(lambda), q/pT there                          */
+  float c[15];           /* lower-triangular covariance                                      */
+  float chi2;            /* of the inward pass, ndf = 2*n_clusters - 5                       */
+  uint32_t n_clusters;
+  uint32_t flags;        /* bit 0: the fit left the |sin phi| range, record not valid        */
+} tpc_track_fit;         /* 96 bytes */
+int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream);
+/* Synchronises and returns the DEVICE array [n_tracks] written by tpc_refit_tracks (aliases the
+ * workspace, same lifetime as the track view). */
+int tpc_get_refit(tpc_ctx* ctx, const tpc_track_fit** d_fit);
+
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);
 

@@ -84,7 +84,7 @@ class DebugView(C.Structure):
 EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
            "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
-           "tpc_sector_track_two_iterations", "tpc_last_launch_count",
+           "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -121,6 +121,10 @@ def load_library():
     L.tpc_workspace_bytes_two_iterations.argtypes = [vp, C.c_uint64]
     L.tpc_sector_track_two_iterations.restype = C.c_int
     L.tpc_sector_track_two_iterations.argtypes = [vp, vp, C.c_uint64, vp, C.c_size_t, vp, C.c_uint32]
+    L.tpc_refit_tracks.restype = C.c_int
+    L.tpc_refit_tracks.argtypes = [vp, vp]
+    L.tpc_get_refit.restype = C.c_int
+    L.tpc_get_refit.argtypes = [vp, C.POINTER(C.c_void_p)]
     L.tpc_sector_track_host_chunks.restype = C.c_int
     L.tpc_sector_track_host_chunks.argtypes = [vp, vp, C.c_uint64, C.POINTER(C.c_uint64), C.c_int, vp, vp, C.c_size_t, vp,
                                                C.c_uint32, vp, C.c_uint64, vp, vp, C.c_uint64, vp]
@@ -238,6 +242,21 @@ def tpc_sector_track_two_iterations(ctx: int, d_clusters: int, n_clusters: int, 
                                     cuda_stream: int, flags: int) -> int:
     return load_library().tpc_sector_track_two_iterations(ctx, d_clusters, n_clusters, d_workspace, workspace_bytes,
                                                           cuda_stream, flags)
+
+
+TRACK_FIT_DTYPE = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"),
+                            ("n_clusters", "<u4"), ("flags", "<u4")])
+assert TRACK_FIT_DTYPE.itemsize == 96
+
+
+def tpc_refit_tracks(ctx: int, cuda_stream: int) -> int:
+    return load_library().tpc_refit_tracks(ctx, cuda_stream)
+
+
+def tpc_get_refit(ctx: int):
+    p = C.c_void_p()
+    rc = load_library().tpc_get_refit(ctx, C.byref(p))
+    return rc, p.value
 
 
 def tpc_last_launch_count(ctx: int) -> int:
@@ -361,6 +380,18 @@ class SectorTracker:
             raise TpcError(rc, "tpc_sector_track_two_iterations", tpc_last_cuda_error(self.ctx))
         self.n = n
         self._clusters = d_clusters
+
+    def refit(self, stream=None):
+        """Sector-track refit of the current result; returns the tpc_track_fit records."""
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc = tpc_refit_tracks(self.ctx, st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_refit_tracks", tpc_last_cuda_error(self.ctx))
+        rc, ptr = tpc_get_refit(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_refit", tpc_last_cuda_error(self.ctx))
+        rc, v = self.counts()
+        return self._to_numpy(ptr, v.n_tracks, TRACK_FIT_DTYPE)
 
     def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
         """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the

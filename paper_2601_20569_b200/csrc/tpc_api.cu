@@ -122,6 +122,7 @@ size_t carve(const tpc_ctx* c, uint64_t n, char* base, TpcBuffers* B) {
   b.tracks = (tpc_track*)take(sizeof(tpc_track) * (size_t)k.max_tracks);
   b.cluster_ids = (uint32_t*)take(4 * (size_t)k.max_ids);
   b.cluster_shared = (uint8_t*)take((size_t)k.max_ids);
+  b.track_fit = (tpc_track_fit*)take(sizeof(tpc_track_fit) * (size_t)k.max_tracks);
   if (B) *B = b;
   return off;
 }
@@ -662,6 +663,30 @@ int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters,
   ctx->launches = launches1 + ctx->launches + 5;
   ctx->ran = true;
   ctx->synced = true;
+  return TPC_OK;
+}
+
+int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream) {
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  rc = device_status(ctx);
+  if (rc == TPC_E_OVERFLOW) return rc;
+  const uint32_t n_tracks = ctx->h_cnt->n_tracks;
+  (void)cudaGetLastError();
+  const int l = (ctx->flags & TPC_DETERMINISTIC)
+                    ? tpc_det::run_refit(ctx->buf, &ctx->hconst, n_tracks, (cudaStream_t)cuda_stream, ctx->n_sm)
+                    : tpc_fast::run_refit(ctx->buf, &ctx->hconst, n_tracks, (cudaStream_t)cuda_stream, ctx->n_sm);
+  if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (refit)");
+  ctx->stream = (cudaStream_t)cuda_stream;
+  ctx->synced = false;
+  return TPC_OK;
+}
+
+int tpc_get_refit(tpc_ctx* ctx, const tpc_track_fit** d_fit) {
+  if (!d_fit) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  *d_fit = ctx->buf.track_fit;
   return TPC_OK;
 }
 

@@ -122,6 +122,7 @@ struct TpcBuffers {
   tpc_track* tracks;      // [max_tracks]
   uint32_t* cluster_ids;  // [max_ids]
   uint8_t* cluster_shared;// [max_ids]
+  tpc_track_fit* track_fit;// [max_tracks] sector-track refit (R8)
 };
 
 #define TPC_MAX_KERNELS 32
@@ -134,9 +135,11 @@ struct TpcStageEvents {
 };
 
 namespace tpc_det {
+int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
+int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 

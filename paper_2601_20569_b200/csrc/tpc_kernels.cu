@@ -2117,6 +2117,85 @@ __global__ void k_init(TpcBuffers B) {
   }
 }
 
+// ================================================================== R8 sector-track refit
+// "a sector track refit at the beginning of the track merging was added,
+// guaranteeing reasonable initial parameters".  One thread per output track: a pure Kalman fit
+// through the track's own cluster list (outward pass, turn, inward pass; no search, no chi2
+// cut) with the propagation / update statements of the follower.  The clusters are read from
+// the input frame through their original indices.
+__global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_constant__ FollowConst F, uint32_t n_tracks) {
+  for (uint32_t ti = blockIdx.x * blockDim.x + threadIdx.x; ti < n_tracks; ti += gridDim.x * blockDim.x) {
+    const tpc_track* __restrict__ t = B.tracks + ti;
+    const uint32_t* __restrict__ ids = B.cluster_ids + t->cluster_ofs;
+    const int n = t->n_clusters;
+    tpc_track_fit out;
+    out.x = 0.f; out.chi2 = 0.f; out.n_clusters = (uint32_t)n; out.flags = 1u;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) out.p[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) out.c[i] = 0.f;
+    auto rec = [&](int i, float& y, float& z, int& row) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + (ids[i] - B.id_base));
+      y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); row = (int)((raw.w >> 8) & 0xFF);
+    };
+    bool ok = n >= 2;
+    if (ok) {
+      KF k;
+      float y0, z0, y1, z1;
+      int r0, r1;
+      rec(0, y0, z0, r0);
+      rec(1, y1, z1, r1);
+      {  // R8.1
+        const float dx = (float)(r1 - r0) * F.dx;
+        const float dy = y1 - y0;
+        const float dl = sqrtf(dx * dx + dy * dy);
+        k.y = y0; k.z = z0;
+        k.s = dy / dl;
+        k.t = (z1 - z0) / dl;
+        k.q = 0.f;
+        kf_init_cov(k, F);
+      }
+      float snap_s = k.s, snap_t = k.t, snap_q = k.q;
+      float ym = y0, zm = z0;
+      int r = r0;
+      for (int i = 1; i < n && ok; ++i) {  // R8.2 outward
+        int ri;
+        rec(i, ym, zm, ri);
+        for (; r < ri && ok; ++r) ok = kf_propagate(k, F.dx, F);
+        if (!ok) break;
+        const Gain g = kf_gain(k, F);
+        if (kf_update(k, g, ym, zm, F)) ok = false;
+        snap_s = k.s; snap_t = k.t; snap_q = k.q;
+      }
+      if (ok) {  // R8.3 turn
+        k.y = ym; k.z = zm; k.s = snap_s; k.t = snap_t; k.q = snap_q;
+        kf_init_cov(k, F);
+      }
+      float chi2 = 0.f;
+      for (int i = n - 2; i >= 0 && ok; --i) {  // R8.4 inward
+        int ri;
+        rec(i, ym, zm, ri);
+        for (; r > ri && ok; --r) ok = kf_propagate(k, -F.dx, F);
+        if (!ok) break;
+        const Gain g = kf_gain(k, F);
+        const float c2 = kf_chi2(k, g, ym, zm);
+        if (kf_update(k, g, ym, zm, F)) ok = false;
+        chi2 = chi2 + c2;
+      }
+      if (ok) {
+        out.x = B.K->x[r0];
+        out.p[0] = k.y; out.p[1] = k.z; out.p[2] = k.s; out.p[3] = k.t; out.p[4] = k.q;
+        out.c[0] = k.c00; out.c[1] = k.c10; out.c[2] = k.c11; out.c[3] = k.c20; out.c[4] = k.c21; out.c[5] = k.c22;
+        out.c[6] = k.c30; out.c[7] = k.c31; out.c[8] = k.c32; out.c[9] = k.c33;
+        out.c[10] = k.c40; out.c[11] = k.c41; out.c[12] = k.c42; out.c[13] = k.c43; out.c[14] = k.c44;
+        out.chi2 = chi2;
+        out.flags = 0u;
+      }
+    }
+    B.track_fit[ti] = out;
+  }
+}
+
 // ================================================================== host: enqueue the path
 #define TPC_LAUNCH_CHECK(name)                                      \
   do {                                                              \
@@ -2143,6 +2222,13 @@ static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
   const uint64_t cap = (uint64_t)n_sm * ctas_per_sm;
   if (g > cap) g = cap;
   return g < 1 ? 1 : (int)g;
+}
+
+int run_refit(const TpcBuffers& B, const TpcConst* hK, uint32_t n_tracks, cudaStream_t st, int n_sm) {
+  if (n_tracks == 0) return 0;
+  const FollowConst F = follow_const(hK);
+  k_track_refit<<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit, 128)), 128, 0, st>>>(B, F, n_tracks);
+  return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

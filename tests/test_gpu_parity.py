@@ -375,3 +375,43 @@ def test_det_parity_second_seeding_iteration(B, name):
     assert n2 == o.second.n_tracks
     if name.startswith("C5"):
         assert n2 > 0
+
+
+@pytest.mark.parametrize("name", ["C1", "C4_reduced", "C5_two_iterations"])
+def test_det_parity_sector_track_refit(B, name):
+    """SURVEY.md 8(f) row 2, first half: sector-track refit of every output track
+    through its own cluster list; deterministic mode, bit-exact against oracle.refit_tracks."""
+    if name == "C1":
+        cl, _, _ = dg.generate(dg.preset("C1"))
+        pkw = {}
+    elif name == "C4_reduced":
+        cl, _, _ = dg.generate(dg.preset("C4", n_events=6, tracks_per_event=1500, t_window_us=120.0))
+        pkw = dict(grid_dz=8.0, max_bins=200_000_000)
+    else:
+        cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        d = trk.upload(cl)
+        if name == "C5_two_iterations":
+            trk.track_two_iterations(d, flags=1)
+        else:
+            trk.track(d, flags=1)
+        tracks, ids, shared, view = trk.tracks()
+        fit = trk.refit()
+    finally:
+        trk.close()
+    assert len(fit) == len(tracks) > 0
+    ref = oracle.refit_tracks(cl, tracks, ids, params=op)
+    assert (fit["flags"] == ref["flags"]).all()
+    ok = ref["flags"] == 0
+    assert ok.sum() >= 0.9 * len(ok)
+    assert (fit["n_clusters"] == tracks["n_clusters"]).all()
+    for f in ("x", "p", "c", "chi2"):
+        a = np.ascontiguousarray(fit[f][ok]).view(np.uint32)
+        b = np.ascontiguousarray(ref[f][ok]).view(np.uint32)
+        assert (a == b).all(), (f, int((a != b).sum()))
+    # segments whose parameters were stale now carry parameters at their own innermost row
+    x_rows, _, _, _ = oracle.geom_tables()
+    assert (fit["x"][ok] == x_rows[tracks["row_first"][ok]]).all()
