@@ -448,10 +448,13 @@ def run_ours(args, rank, world, local_rank):
                 "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": None,
                 "peak_source": "148 SM x 128 fp32 lanes x sm_max_mhz x (2 if FMA) — DESIGN.md"}
     roof["share_of_step"] = dom["ms_per_step"] / ksum if ksum else None
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # written from an ncu --set full capture
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")   # from an ncu --set full capture (profiles/traffic.md)
     if os.path.exists(traffic_file):
         try:
-            roof["traffic"] = json.load(open(traffic_file)).get(dom["name"])
+            for ln in open(traffic_file).read().splitlines()[1:]:
+                k, b = ln.split(",")
+                if k == dom["name"]:
+                    roof["traffic"] = float(b)
         except Exception:
             pass
     # north star: HBM fraction of the grid and neighbour stages
