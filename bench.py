@@ -381,7 +381,7 @@ def run_ours(args, rank, world, local_rank):
     if args.e2e_cuts and n:       # explicit sector boundaries, e.g. "0,2,6,12,20,28,34,36"
         cuts = [int(x) for x in args.e2e_cuts.split(",")]
         n_chunks = len(cuts) - 1
-    elif args.e2e_chunks == 0 and n:
+    elif args.e2e_chunks == 0 and n >= 20_000_000:   # (small frames go in one shot: a chunk costs a host synchronisation)
         # default: small chunks first and last (short pipeline fill and drain), large ones between
         # (measured on the C4 frame: 112.0 ms against 119.7 ms for six equal chunks)
         ns = int(sec.max()) + 1
