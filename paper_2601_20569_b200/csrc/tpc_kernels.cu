@@ -1851,6 +1851,20 @@ __global__ void __launch_bounds__(TPC_SEL_BLOCK) k_sel_masks(TpcBuffers B) {
     if (warp < W) s_tw[warp][lane] = key ? B.tl_mask[(size_t)(TPC_MASK_WORDS + warp) * hstride + sd] : 0u;
     for (int r = threadIdx.x; r < R; r += TPC_SEL_BLOCK) s_own[r] = 0u;
     __syncthreads();
+    // a tracklet whose tentative hits are too few for any segment (the bound of walk_tracklet;
+    // owned hits are a subset of the tentative ones) is not looked at: its owned mask is left
+    // empty, which the count pass rejects by the same bound
+    if (warp == 0) {
+      int n_tent = 0;
+      for (int w = 0; w < W; ++w) n_tent += __popc(s_tw[w][lane]);
+      const tpc_params& P = B.K->P;
+      const bool hopeless = P.shared_fixed_cap
+                                ? n_tent * 1000 + P.shared_permille * (int)(sd < n_seeds ? B.tracklets[sd].n_hits : 0) < P.min_hits_track * 1000
+                                : n_tent * 1000 < P.min_hits_track * (1000 - P.shared_permille);
+      if (hopeless)
+        for (int w = 0; w < W; ++w) s_tw[w][lane] = 0u;
+    }
+    __syncthreads();
     const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * (size_t)R;
     const bool vec = (R & 3) == 0;
     for (int rb = warp * TPC_SEL_UNROLL; rb < R; rb += (TPC_SEL_BLOCK / 32) * TPC_SEL_UNROLL) {
