@@ -1222,7 +1222,9 @@ __device__ __forceinline__ int32_t pick_cluster(const TpcBuffers& B, const TpcCo
 // finished claims the next one at once (chunks from a global counter).  Loads are software-
 // pipelined one row ahead.  The arithmetic per seed, and its order, are exactly those of
 // R5.1-R5.7, so neither the assignment of seeds to lanes nor the split changes a result.
+#ifndef TPC_FOLLOW_BLOCK
 #define TPC_FOLLOW_BLOCK 128
+#endif
 // idle lanes of a warp that trigger a refill from the queue: refilling in groups amortises the
 // claim and keeps groups of lanes on neighbouring seeds (measured: 1 -> 4 lanes, -3 ms per frame)
 #ifndef TPC_REFILL_UP
