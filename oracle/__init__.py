@@ -30,6 +30,9 @@ TRACK_DTYPE = np.dtype(
      ("seed_id", "<u4"), ("n_clusters", "<i4"), ("n_shared", "<i4"), ("sector", "<i4"),
      ("row_first", "<i4"), ("row_last", "<i4"), ("flags", "<i4"), ("n_hits_tracklet", "<i4"),
      ("segment", "<i4")])
+TRACE_DTYPE = np.dtype(
+    [("seed", "<i4"), ("row", "<i4"), ("dir", "<i4"), ("searched", "<i4"), ("y", "<f4"), ("z", "<f4"),
+     ("c00", "<f4"), ("c10", "<f4"), ("c11", "<f4"), ("chi2", "<f4"), ("picked_id", "<i4"), ("accepted", "<i4")])
 
 
 class Geom(C.Structure):
@@ -86,6 +89,10 @@ def lib():
         L.orc_free.argtypes = [vp]
         L.orc_sizes.argtypes = [vp, vp]
         L.orc_stage_seconds.argtypes = [vp, vp]
+        L.orc_set_trace.argtypes = [C.c_int]
+        L.orc_trace_size.restype = C.c_uint64
+        L.orc_trace_size.argtypes = [vp]
+        L.orc_fetch_trace.argtypes = [vp, vp]
         L.orc_fetch_grid.argtypes = [vp] * 4
         L.orc_fetch_links.argtypes = [vp] * 5
         L.orc_fetch_seeds.argtypes = [vp] * 2
@@ -157,6 +164,9 @@ class Result:
             self.tracklets = np.zeros(self.n_seeds, dtype=TRACKLET_DTYPE)
             self.row_hit = np.zeros((self.n_seeds, self.n_rows), dtype=np.int32)
             L.orc_fetch_tracklets(h, _ptr(self.tracklets), _ptr(self.row_hit))
+        if "trace" in want:
+            self.trace = np.zeros(int(L.orc_trace_size(h)), dtype=TRACE_DTYPE)
+            L.orc_fetch_trace(h, _ptr(self.trace))
         if "tracks" in want:
             self.tracks = np.zeros(self.n_tracks, dtype=TRACK_DTYPE)
             self.cluster_ids = np.zeros(self.n_cluster_ids, dtype=np.uint32)
@@ -173,8 +183,12 @@ def run(clusters: np.ndarray, geom: Geom | None = None, params: Params | None = 
     geom = geom or default_geom()
     params = params or default_params()
     L = lib()
-    h = L.orc_run(clusters.ctypes.data, len(clusters), C.byref(geom), C.byref(params),
-                  sector_lo, min(sector_hi, geom.n_sectors), n_threads)
+    L.orc_set_trace(1 if "trace" in want else 0)
+    try:
+        h = L.orc_run(clusters.ctypes.data, len(clusters), C.byref(geom), C.byref(params),
+                      sector_lo, min(sector_hi, geom.n_sectors), 1 if "trace" in want else n_threads)
+    finally:
+        L.orc_set_trace(0)
     if not h:
         raise ValueError("oracle: bad argument")
     try:

@@ -81,7 +81,10 @@ struct Sector {
   std::vector<uint8_t> shared;
   uint64_t n_ignored = 0, n_dropped = 0;
   double t_stage[5] = {0, 0, 0, 0, 0};
+  std::vector<orc_trace_rec> trace;    // road-search decisions (only when orc_set_trace(1))
 };
+
+int g_trace = 0;  // set by orc_set_trace before orc_run; read-only while sectors run
 
 inline int bin_coord(float v, float v0, float inv_d, int n) {
   int b = (int)std::floor((v - v0) * inv_d);
@@ -256,6 +259,8 @@ struct FollowCtx {
   const Tables& T;
   const orc_params& P;
   float vy, vz;
+  std::vector<orc_trace_rec>* trace = nullptr;  // observation only: never read by the algorithm
+  int32_t trace_seed = 0;
 };
 
 inline void init_cov(KFState<float>& st, const FollowCtx& X) {
@@ -301,10 +306,20 @@ inline void extrapolate(const FollowCtx& X, KFState<float>& st, int r_from, int 
   for (int r = r_from + dir; r >= 0 && r < X.T.n_rows; r += dir) {
     if (!tpc_oracle::kf_propagate(st, dx, X.T.cfield, P.max_sinphi)) break;
     bool got = false;
+    orc_trace_rec tr;
+    if (X.trace) {
+      tr.seed = X.trace_seed; tr.row = r; tr.dir = dir; tr.searched = 0;
+      tr.y = st.y; tr.z = st.z; tr.c00 = st.c[0]; tr.c10 = st.c[1]; tr.c11 = st.c[2];
+      tr.chi2 = 0; tr.picked_id = -1; tr.accepted = 0;
+    }
     if (std::fabs(st.y) <= X.T.ylim[r]) {
       const KFGain<float> g = tpc_oracle::kf_gain(st, X.vy, X.vz);
       float chi2 = 0;
       const int32_t c = pick_cluster(X, r, st, g, &chi2);
+      if (X.trace) {
+        tr.searched = 1; tr.chi2 = chi2; tr.picked_id = c < 0 ? -1 : (int32_t)X.S.ids[c];
+        tr.accepted = (c >= 0 && chi2 <= P.chi2_max_hit) ? 1 : 0;
+      }
       if (c >= 0 && chi2 <= P.chi2_max_hit) {
         const bool stop = tpc_oracle::kf_update(st, g, X.S.ys[c], X.S.zs[c], P.max_sinphi, P.max_qpt);
         hits[r] = c;
@@ -313,9 +328,11 @@ inline void extrapolate(const FollowCtx& X, KFState<float>& st, int r_from, int 
         on_hit(r);
         got = true;
         gap = 0;
+        if (X.trace) X.trace->push_back(tr);
         if (stop) break;
       }
     }
+    if (X.trace && !got) X.trace->push_back(tr);
     if (!got) {
       ++gap;
       if (gap > P.max_gap_follow) break;
@@ -435,12 +452,15 @@ void follow_seed(const FollowCtx& X, int32_t start, int seed_len, uint32_t seed_
 
 void follow_all(Sector& S, const Tables& T, const orc_params& P) {
   FollowCtx X{S, T, P, P.err_y * P.err_y, P.err_z * P.err_z};
+  if (g_trace) X.trace = &S.trace;
   const size_t ns = S.seeds.size();
   S.tracklets.resize(ns);
   S.row_hit.assign(ns * (size_t)T.n_rows, -1);
-  for (size_t k = 0; k < ns; ++k)
+  for (size_t k = 0; k < ns; ++k) {
+    X.trace_seed = (int32_t)k;
     follow_seed(X, S.seed_pos[k], S.seeds[k].len, S.seeds[k].start_id, S.tracklets[k],
                 &S.row_hit[k * (size_t)T.n_rows]);
+  }
 }
 
 // ------------------------------------------------------------------ R6 ambiguity solving
@@ -641,6 +661,26 @@ void orc_sizes(const orc_result* r, uint64_t out[10]) {
     out[6] += S.n_ignored;
     out[7] += S.n_dropped;
     for (const orc_tracklet& t : S.tracklets) out[9] += t.n_hits > 0;
+  }
+}
+
+void orc_set_trace(int on) { g_trace = on; }
+
+uint64_t orc_trace_size(const orc_result* r) {
+  uint64_t n = 0;
+  for (const Sector& S : r->sectors) n += S.trace.size();
+  return n;
+}
+
+void orc_fetch_trace(const orc_result* r, orc_trace_rec* out) {
+  size_t k = 0;
+  int32_t seed_base = 0;
+  for (const Sector& S : r->sectors) {
+    for (const orc_trace_rec& t : S.trace) {
+      out[k] = t;
+      out[k++].seed += seed_base;   // index into the concatenated seed / tracklet arrays
+    }
+    seed_base += (int32_t)S.seeds.size();
   }
 }
 

@@ -86,6 +86,15 @@ typedef struct orc_track {
   int32_t n_hits_tracklet, segment;
 } orc_track;
 
+/* One road search of the follower (R5.3 / R5.6), recorded for the pins only (orc_set_trace):
+ * the PREDICTED state on the row, whether the row was searched (|y| <= ylim_r), the best
+ * candidate found (original id, -1 none), its chi2 and whether it was accepted. */
+typedef struct orc_trace_rec {
+  int32_t seed, row, dir, searched;
+  float y, z, c00, c10, c11, chi2;
+  int32_t picked_id, accepted;
+} orc_trace_rec;
+
 typedef struct orc_result orc_result;
 
 void orc_default_params(orc_params* p);
@@ -100,6 +109,11 @@ void orc_free(orc_result* r);
  * out[5]=n_cluster_ids out[6]=n_ignored out[7]=n_dropped out[8]=n_bad (sector/row outside geometry)
  * out[9]=n_tracklets (n_hits>0) */
 void orc_sizes(const orc_result* r, uint64_t out[10]);
+/* road-search trace (pins only): orc_set_trace(1) before orc_run (single-threaded use), then
+ * orc_trace_size / orc_fetch_trace; the trace is observation only, no result depends on it */
+void orc_set_trace(int on);
+uint64_t orc_trace_size(const orc_result* r);
+void orc_fetch_trace(const orc_result* r, orc_trace_rec* out);
 /* stage wall times in seconds: grid, neighbours, cleanup+seeds, follower, selector */
 void orc_stage_seconds(const orc_result* r, double out[5]);
 /* copy-out; any pointer may be NULL.  Links are indexed by ORIGINAL cluster index and hold

@@ -9,7 +9,7 @@
 // up more clusters of the track" (section 2).  The paper gives no formula
 // (it defers to its ref. [7]); the track model below is DESIGN.md reading R5 (textbook
 // helix in a uniform solenoid field + linear Kalman update), written step by step in the
-// order of oracle/FORMULAS.md.  Rule D1: only + - * / sqrt, IEEE
+// order of DESIGN.md section 3 "Formulas".  Rule D1: only + - * / sqrt, IEEE
 // round-to-nearest, no FMA contraction (compile with -ffp-contract=off), no reassociation.
 //
 // Templated on the scalar type so the pins (tests/test_oracle_*.py) can run the very same
@@ -45,7 +45,7 @@ inline T o_abs(T v) { return v < T(0) ? -v : v; }
 // plane; z advances by tan(lambda) times the arc length.  `cfield` = signed curvature per
 // unit q/pT (R0: c = -0.00299792458*Bz, rounded once to the scalar type).
 // Returns false (state untouched) when |sin(phi)| would exceed max_sinphi: the leg ends.
-// FORMULAS.md section P.
+// DESIGN.md section 3, block P.
 template <class T>
 inline bool kf_propagate(KFState<T>& st, T dx, T cfield, T max_sinphi, KFJac<T>* jac_out = nullptr) {
   const T s = st.s, t = st.t, q = st.q;
@@ -124,7 +124,7 @@ inline bool kf_propagate(KFState<T>& st, T dx, T cfield, T max_sinphi, KFJac<T>*
 }
 
 // Innovation covariance inverse for a measurement (y,z) with V = diag(vy, vz).
-// FORMULAS.md section U.
+// DESIGN.md section 3, block U.
 template <class T>
 struct KFGain {
   T si00, si01, si11;
