@@ -25,8 +25,9 @@
  *  - Every function returns TPC_OK (0) or a negative tpc_error; nothing throws or aborts.
  *  - A context is not thread-safe; use one context per host thread / stream.
  *  - The library allocates device memory only inside tpc_geom_init (a few KB of tables
- *    and counters) and creates no streams.  All scratch and all outputs live in the
- *    caller's workspace.
+ *    and counters).  All scratch and all outputs live in the caller's workspace.  Kernels run
+ *    on the caller's stream; the library owns two copy streams, created in tpc_geom_init and
+ *    used by tpc_sector_track_host_chunks alone.
  */
 #ifndef TPC_TRACK_H
 #define TPC_TRACK_H
@@ -91,7 +92,7 @@ typedef struct tpc_params {
   float road_nsigma, road_min, road_max; /* search road (3.5, 0.3 cm, 2.0 cm)           */
   float chi2_max_hit;            /* 2-dof chi2 cut for pick-up (12)                     */
   int32_t max_gap_follow;        /* rows without hit before the follower stops (4)      */
-  int32_t min_hits_tracklet;     /* (10)                                                */
+  int32_t min_hits_tracklet;     /* (10) >= 3: ndf = 2*nHits - 5 of the weight must be > 0 */
   float sel_chi2_weight;         /* weight = nHits - w*chi2/ndf (2.0)                   */
   int32_t shared_permille;       /* allowed shared-cluster fraction, permille (100)     */
   int32_t max_gap_select;        /* rows; a larger hole splits the track (4)            */
@@ -275,7 +276,9 @@ int tpc_sector_track_host(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t 
  * tracks concatenated in chunk order; *out holds the summed counts, its d_* pointers are NULL.
  * d_staging (DEVICE) holds the whole frame; the workspace must be at least twice
  * tpc_workspace_bytes(ctx, largest chunk) (else TPC_E_WORKSPACE).  A sector found in two
- * chunks gives TPC_E_ARG. */
+ * chunks gives TPC_E_ARG.  After this call the context holds no whole-frame result:
+ * tpc_get_tracks, tpc_get_intermediates and tpc_refit_tracks return TPC_E_STATE until the
+ * next tpc_sector_track / tpc_sector_track_two_iterations. */
 int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, uint64_t n_clusters,
                                  const uint64_t* chunk_ofs, int n_chunks, void* d_staging,
                                  void* d_workspace, size_t workspace_bytes, void* cuda_stream,

@@ -158,11 +158,72 @@ def _overlap_pairs(tr, ids, otr, oids, un_g, un_o, n_clusters_total, frac=0.9):
     return np.asarray(pg, dtype=np.int64), np.asarray(po, dtype=np.int64)
 
 
-def compare_tracks_fast(g_tracks, g_ids, g_shared, o, rel=1e-3):
+def _z_floor(z_ref):
+    """What fp32 cannot represent at the frame's absolute z: the state's z is carried at time-frame
+    coordinates (|z| up to ~7500 cm, ulp 4.9e-4 cm) and every row step rounds it there; 4 ulp(z) is
+    the floor under which two fp32 evaluation orders cannot agree."""
+    return 4.0 * np.spacing(np.abs(np.asarray(z_ref)).astype(np.float32)).astype(np.float64)
+
+
+_SCALE = np.array([1.0, 1.0, 0.1, 0.1, 0.1])
+
+
+def param_relerr(pa, pb):
+    """|dp_i| / max(|p_i|, scale_i), scales (1 cm, 1 cm, 0.1, 0.1, 0.1 c/GeV); z: absolute error above
+    the fp32 floor at that z, against a scale of 1 cm (offset-free)."""
+    pa, pb = np.asarray(pa, dtype=np.float64), np.asarray(pb, dtype=np.float64)
+    denom = np.maximum(np.abs(pb), _SCALE)
+    denom[:, 1] = 1.0
+    err = np.abs(pa - pb)
+    err[:, 1] = np.maximum(0.0, err[:, 1] - _z_floor(pb[:, 1]))
+    return err / denom
+
+
+def compare_tracklets_fast(gi, o, rel=1e-3):
+    """Fast mode at the tracklet level (needs TPC_KEEP_INTERMEDIATES): tracklets paired by
+    (sector, seed id); where EVERY decision of the follower coincides (identical row_hit arrays in
+    original ids) the fitted parameters must agree to `rel` -- fast mode may differ from the oracle
+    through rounding only.  Returns statistics and the keys of the identical tracklets."""
+    tl, rh = canonical_tracklets(gi)
+    ot, orh = o.tracklets, o.row_hit
+    kg = (tl["sector"].astype(np.int64) << 32) | tl["seed_id"].astype(np.int64)
+    ko = (ot["sector"].astype(np.int64) << 32) | ot["seed_id"].astype(np.int64)
+    common, ig, io = np.intersect1d(kg, ko, return_indices=True)
+    out = {"n_gpu": len(tl), "n_oracle": len(ot), "n_paired": len(common)}
+    a, b = tl[ig], ot[io]
+    both = (a["n_hits"] > 0) & (b["n_hits"] > 0)
+    out["n_accept_diff"] = int(((a["n_hits"] > 0) != (b["n_hits"] > 0)).sum())
+    same = both & (rh[ig] == orh[io]).all(axis=1)
+    out["n_both_accepted"] = int(both.sum())
+    out["n_identical_hits"] = int(same.sum())
+    relerr = param_relerr(a["p"][same], b["p"][same]) if same.any() else np.zeros((0, 5))
+    out["n_param_bad"] = int((relerr > rel).any(axis=1).sum())
+    out["max_rel_per_param"] = [float(v) for v in relerr.max(axis=0)] if len(relerr) else []
+    # the worst cases in full (for the record): parameter, error, value, its own uncertainty, hits
+    diag = np.array([0, 2, 5, 9, 14])
+    worst = []
+    if len(relerr):
+        bb = b[same]
+        for k in np.argsort(-relerr.max(axis=1))[:8]:
+            i = int(relerr[k].argmax())
+            if relerr[k, i] <= rel:
+                break
+            worst.append({"param": i, "rel": float(relerr[k, i]), "value": float(bb["p"][k][i]),
+                          "sigma": float(np.sqrt(max(bb["c"][k][diag[i]], 0.0))), "n_hits": int(bb["n_hits"][k]),
+                          "sinphi": float(bb["p"][k][2]), "rows": [int(bb["row_first"][k]), int(bb["row_last"][k])]})
+    out["worst"] = worst
+    chi = np.abs(a["chi2"][same].astype(np.float64) - b["chi2"][same]) / np.maximum(np.abs(b["chi2"][same]), 1.0)
+    out["max_rel_chi2"] = float(chi.max()) if len(chi) else 0.0
+    return out, set(common[same].tolist())
+
+
+def compare_tracks_fast(g_tracks, g_ids, g_shared, o, rel=1e-3, identical_tracklets=None):
     """Fast-mode comparison (north star): tracks paired by (sector, seed id, segment), falling
     back to >= 90 % cluster overlap; on the key pairs |dp_i| <= rel*max(|p_i|, scale_i), scales
-    (1 cm, 1 cm, 0.1, 0.1, 0.1 c/GeV), z taken relative to the oracle track's z.  Returns a dict
-    of statistics (n_paired = key pairs + overlap pairs)."""
+    (1 cm, 1 cm, 0.1, 0.1, 0.1 c/GeV), z as in param_relerr.  n_param_bad counts key pairs with
+    IDENTICAL cluster lists (and, when identical_tracklets is given, whose tracklet took the same
+    decisions on every row) whose parameters differ by more than rel.  Returns a dict of
+    statistics (n_paired = key pairs + overlap pairs)."""
     def keyof(t):
         return (t["sector"].astype(np.int64) << 40) | (t["seed_id"].astype(np.int64) << 8) | t["segment"].astype(np.int64)
     tr, ids, sh = canonical_tracks(g_tracks, g_ids, g_shared)
@@ -175,21 +236,35 @@ def compare_tracks_fast(g_tracks, g_ids, g_shared, o, rel=1e-3):
     pg, po = _overlap_pairs(tr, ids, otr, oids, un_g, un_o, o.n_clusters)
     out["n_paired_overlap"] = len(pg)
     out["n_paired"] = len(common) + len(pg)
-    scale = np.array([1.0, 1.0, 0.1, 0.1, 0.1])
-
     def relerr_of(a, b):
-        pa, pb = a["p"].astype(np.float64), b["p"].astype(np.float64)
-        denom = np.maximum(np.abs(pb), scale)
-        denom[:, 1] = 1.0  # z: relative to the track's own z (offset-free), scale 1 cm
-        return np.abs(pa - pb) / denom
-    out.update(n_param_bad=0, n_list_diff=0, max_rel=0.0, n_param_bad_overlap=0, max_rel_overlap=0.0)
+        return param_relerr(a["p"], b["p"])
+    out.update(n_param_bad=0, n_list_diff=0, max_rel=0.0, n_param_bad_overlap=0, max_rel_overlap=0.0,
+               n_param_bad_any_list=0)
     if len(common):
         a, b = tr[ig], otr[io]
         relerr = relerr_of(a, b)
+        # identical cluster LISTS (ids and shared flags, not just their counts)
         same_list = (a["n_clusters"] == b["n_clusters"]) & (a["n_shared"] == b["n_shared"])
+        g_ofs = np.cumsum(tr["n_clusters"].astype(np.int64)) - tr["n_clusters"].astype(np.int64)
+        o_ofs = np.cumsum(otr["n_clusters"].astype(np.int64)) - otr["n_clusters"].astype(np.int64)
+        cand = np.flatnonzero(same_list)
+        if len(cand):
+            n_per = a["n_clusters"][cand].astype(np.int64)
+            within = np.arange(int(n_per.sum()), dtype=np.int64) - np.repeat(np.cumsum(n_per) - n_per, n_per)
+            gg = np.repeat(g_ofs[ig[cand]], n_per) + within
+            oo = np.repeat(o_ofs[io[cand]], n_per) + within
+            diff = (ids[gg] != oids[oo]) | (sh[gg] != osh[oo])
+            n_diff = np.add.reduceat(diff.astype(np.int64), np.cumsum(n_per) - n_per)
+            same_list[cand[n_diff > 0]] = False
         out["n_list_diff"] = int((~same_list).sum())
+        if identical_tracklets is not None:      # only tracks whose tracklet made the same decisions everywhere
+            tk = (a["sector"].astype(np.int64) << 32) | a["seed_id"].astype(np.int64)
+            same_list &= np.fromiter((int(k) in identical_tracklets for k in tk), dtype=bool, count=len(tk))
+            out["n_identical_tracklet_and_list"] = int(same_list.sum())
         out["n_param_bad"] = int(((relerr > rel).any(axis=1) & same_list).sum())
+        out["n_param_bad_any_list"] = int((relerr > rel).any(axis=1).sum())
         out["max_rel"] = float(relerr[same_list].max()) if same_list.any() else 0.0
+        out["max_rel_per_param"] = [float(v) for v in relerr[same_list].max(axis=0)] if same_list.any() else []
     if len(pg):
         a, b = tr[pg], otr[po]
         ok = (a["row_first"] == b["row_first"]) & (a["flags"] == 0) & (b["flags"] == 0)   # parameters at the same x

@@ -157,7 +157,8 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
   tpc_params P;
   if (params) P = *params; else tpc_default_params(&P);
   if (!(P.grid_dy > 0.f) || !(P.grid_dz > 0.f) || P.shared_permille < 0 || P.shared_permille > 500 ||
-      P.seed_min_len < 2 || P.seed_min_len > 255 || P.min_hits_track < 1 || P.min_hits_tracklet < 2 ||
+      P.seed_min_len < 2 || P.seed_min_len > 255 || P.min_hits_track < 1 ||
+      P.min_hits_tracklet < 3 ||   // ndf = 2*nHits - 5 of the selection weight (R6.1) must be positive
       !(P.err_y > 0.f) || !(P.err_z > 0.f) || !(P.max_sinphi > 0.f) || !(P.max_sinphi < 1.f) ||
       P.max_gap_follow < 0 || P.max_gap_select < 0)
     return TPC_E_ARG;
@@ -443,8 +444,9 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
     return set_cuda_err(ctx, e, "cudaMemsetAsync(sector_seen)");
   // the copy streams start after whatever the caller has enqueued on `st`
   if ((e = cudaEventRecord(ctx->ev_done[0], st)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaEventRecord");
-  cudaStreamWaitEvent(ctx->s_in, ctx->ev_done[0], 0);
-  cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[0], 0);
+  if ((e = cudaStreamWaitEvent(ctx->s_in, ctx->ev_done[0], 0)) != cudaSuccess ||
+      (e = cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[0], 0)) != cudaSuccess)
+    return set_cuda_err(ctx, e, "cudaStreamWaitEvent");
   auto copy_in = [&](int c) -> cudaError_t {
     const uint64_t o = chunk_ofs[c], nc = chunk_ofs[c + 1] - o;
     if (nc) {
@@ -456,11 +458,12 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
   };
   if ((e = copy_in(0)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(clusters)");
   uint64_t n_tracks = 0, n_ids = 0;
-  int rc_all = TPC_OK, launches = 0;
+  int launches = 0;
   for (int c = 0; c < n_chunks; ++c) {
     const uint64_t o = chunk_ofs[c], nc = chunk_ofs[c + 1] - o;
-    cudaStreamWaitEvent(st, ctx->ev_in[c & 1], 0);                    // chunk c is on the device
-    if (c >= 2) cudaStreamWaitEvent(st, ctx->ev_out[c & 1], 0);       // workspace c&1 has been read back
+    e = cudaStreamWaitEvent(st, ctx->ev_in[c & 1], 0);                // chunk c is on the device
+    if (e == cudaSuccess && c >= 2) e = cudaStreamWaitEvent(st, ctx->ev_out[c & 1], 0);   // workspace c&1 has been read back
+    if (e != cudaSuccess) { cudaDeviceSynchronize(); ctx->ran = false; return set_cuda_err(ctx, e, "cudaStreamWaitEvent"); }
     int rc = enqueue_track(ctx, (const tpc_cluster*)d_staging + o, nc, ws[c & 1], ws_one, cuda_stream, flags,
                            (uint32_t)o, (uint32_t)c + 1u);
     if (rc != TPC_OK) { cudaDeviceSynchronize(); return rc; }
@@ -472,16 +475,23 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
     rc = tpc_get_tracks(ctx, &v);                                     // syncs `st`: counts of chunk c
     if (rc != TPC_OK) { cudaDeviceSynchronize(); return rc; }
     if (n_tracks + v.n_tracks > cap_tracks || n_ids + v.n_cluster_ids > cap_ids) { cudaDeviceSynchronize(); return TPC_E_OVERFLOW; }
-    if (v.n_tracks) k_shift_tracks<<<(unsigned)((v.n_tracks + 255) / 256), 256, 0, st>>>((tpc_track*)v.d_tracks, (uint32_t)v.n_tracks, (uint32_t)n_ids);
-    cudaEventRecord(ctx->ev_done[c & 1], st);
-    cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c & 1], 0);
-    if (h_tracks && v.n_tracks)
-      cudaMemcpyAsync(h_tracks + n_tracks, v.d_tracks, v.n_tracks * sizeof(tpc_track), cudaMemcpyDeviceToHost, ctx->s_out);
-    if (h_cluster_ids && v.n_cluster_ids)
-      cudaMemcpyAsync(h_cluster_ids + n_ids, v.d_cluster_ids, v.n_cluster_ids * 4, cudaMemcpyDeviceToHost, ctx->s_out);
-    if (h_cluster_shared && v.n_cluster_ids)
-      cudaMemcpyAsync(h_cluster_shared + n_ids, v.d_cluster_shared, v.n_cluster_ids, cudaMemcpyDeviceToHost, ctx->s_out);
-    cudaEventRecord(ctx->ev_out[c & 1], ctx->s_out);
+    // every CUDA call of the hand-over is checked: a failure drains the streams and is reported,
+    // never a partly filled result with TPC_OK
+    e = cudaSuccess;
+    if (v.n_tracks) {
+      k_shift_tracks<<<(unsigned)((v.n_tracks + 255) / 256), 256, 0, st>>>((tpc_track*)v.d_tracks, (uint32_t)v.n_tracks, (uint32_t)n_ids);
+      e = cudaPeekAtLastError();
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_done[c & 1], st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_out, ctx->ev_done[c & 1], 0);
+    if (e == cudaSuccess && h_tracks && v.n_tracks)
+      e = cudaMemcpyAsync(h_tracks + n_tracks, v.d_tracks, v.n_tracks * sizeof(tpc_track), cudaMemcpyDeviceToHost, ctx->s_out);
+    if (e == cudaSuccess && h_cluster_ids && v.n_cluster_ids)
+      e = cudaMemcpyAsync(h_cluster_ids + n_ids, v.d_cluster_ids, v.n_cluster_ids * 4, cudaMemcpyDeviceToHost, ctx->s_out);
+    if (e == cudaSuccess && h_cluster_shared && v.n_cluster_ids)
+      e = cudaMemcpyAsync(h_cluster_shared + n_ids, v.d_cluster_shared, v.n_cluster_ids, cudaMemcpyDeviceToHost, ctx->s_out);
+    if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_out[c & 1], ctx->s_out);
+    if (e != cudaSuccess) { cudaDeviceSynchronize(); ctx->ran = false; return set_cuda_err(ctx, e, "chunk hand-over"); }
     n_tracks += v.n_tracks; n_ids += v.n_cluster_ids;
     out->n_ignored += v.n_ignored; out->n_dropped += v.n_dropped; out->n_seeds += v.n_seeds;
     out->n_tracklets += v.n_tracklets; out->n_bins += v.n_bins;
@@ -496,7 +506,10 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
   out->n_tracks = n_tracks;
   out->n_cluster_ids = n_ids;
   ctx->launches = launches;
-  return rc_all;
+  // the context's buffers describe the LAST chunk only: tpc_get_tracks / tpc_get_intermediates /
+  // tpc_refit_tracks after a chunked call return TPC_E_STATE instead of a partial answer
+  ctx->ran = false;
+  return TPC_OK;
 }
 
 // ---------------------------------------------------------------- second seeding iteration (R7)

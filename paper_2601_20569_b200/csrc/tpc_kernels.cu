@@ -577,11 +577,33 @@ __device__ __forceinline__ BinWindow make_window(const tpc_row_desc& d, const Tp
 #ifndef TPC_NF_SLAB
 #define TPC_NF_SLAB 1024   // clusters staged per neighbour row
 #endif
-#define TPC_NF_BINS (TPC_NF_SLAB - 1)   // bins staged per neighbour row (+1 end marker)
+#define TPC_NF_BINS 1020   // bins staged per neighbour row (+1 end marker, + alignment slack)
 #ifndef TPC_NF_MINBLOCKS
-#define TPC_NF_MINBLOCKS 6
+#define TPC_NF_MINBLOCKS 5
 #endif
 #define TPC_NF_LIST 12     // window members kept per thread and side
+
+// ---- 1-D TMA (cp.async.bulk) + mbarrier: the slabs are contiguous ranges of the sorted arrays
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  } while (!ok);
+}
+// bytes: a multiple of 16; src and dst 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
 
 // The search of one cluster directly on global memory.
 __device__ __forceinline__ void nf_generic(const TpcBuffers& B, const BinWindow& wu, const BinWindow& wd, float yi,
@@ -711,24 +733,29 @@ __device__ __forceinline__ void nf_down_pairs(const BinWindow& w, int bz_lo, uin
 }
 
 __global__ void __launch_bounds__(TPC_NF_TILE, TPC_NF_MINBLOCKS) k_neighbours(TpcBuffers B) {
-  __shared__ float2 s_yz[2][TPC_NF_SLAB];
-  __shared__ uint32_t s_bin[2][TPC_NF_BINS + 1];
-  __shared__ uint16_t s_list[1][TPC_NF_LIST * TPC_NF_TILE];   // up-window members per thread
-  __shared__ int s_red[4];
+  __shared__ __align__(16) float2 s_yz[2][TPC_NF_SLAB + 2];
+  __shared__ __align__(16) uint32_t s_bin[2][TPC_NF_BINS + 8];
+  __shared__ uint16_t s_list[TPC_NF_LIST * TPC_NF_TILE];                 // up-window members per thread
+  __shared__ __align__(8) unsigned long long s_mbar;
   const TpcConst* __restrict__ K = B.K;
   if (B.cnt->error & TPC_DEVERR_BINS) return;
   const uint32_t n_tiles = B.cnt->n_tiles;
   const int R = K->n_rows;
   const float wy = K->wy, wz = K->wz, max_d2 = K->P.nf_max_d2;
+  const float dzbin = K->P.grid_dz, inv_dz = K->inv_dz;
   const uint32_t* __restrict__ bin_start = B.bin_start;
   const float2* __restrict__ yz = B.yz;
   const uint32_t* __restrict__ orig = B.orig_id;
   const int tx = threadIdx.x;
+  if (tx == 0) mbar_init(&s_mbar, 1);
+  __syncthreads();
+  uint32_t parity = 0;
   for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const uint32_t sr = B.tile_sr[tile];
     const int r = (int)(sr % (uint32_t)R);
     const tpc_row_desc d = B.row_desc[sr];
-    const uint32_t local = (tile - B.tile_ofs[sr]) * TPC_NF_TILE + (uint32_t)tx;
+    const uint32_t tile_first = (tile - B.tile_ofs[sr]) * TPC_NF_TILE;
+    const uint32_t local = tile_first + (uint32_t)tx;
     const bool have = local < d.count;
     const uint32_t i = d.clu_ofs + local;
     tpc_row_desc du, dd;
@@ -750,50 +777,61 @@ __global__ void __launch_bounds__(TPC_NF_TILE, TPC_NF_MINBLOCKS) k_neighbours(Tp
       wu = make_window(du, K, (yi + ty) - wy, (yi + ty) + wy, zi - wz, zi + wz);
       wd = make_window(dd, K, (yi - ty) - wy, (yi - ty) + wy, zi - wz, zi + wz);
     }
-    // ---- the z-rows of bins this tile's windows touch on either side (block min / max)
-    __syncthreads();  // s_red, s_yz, s_bin, s_list of the previous tile are no longer read
-    if (tx == 0) { s_red[0] = 0x7fffffff; s_red[1] = -1; s_red[2] = 0x7fffffff; s_red[3] = -1; }
-    __syncthreads();
-    {
-      const int m0 = __reduce_min_sync(0xffffffffu, wu.bz0), m1 = __reduce_max_sync(0xffffffffu, wu.bz1);
-      const int m2 = __reduce_min_sync(0xffffffffu, wd.bz0), m3 = __reduce_max_sync(0xffffffffu, wd.bz1);
-      if ((tx & 31) == 0) {
-        atomicMin(&s_red[0], m0); atomicMax(&s_red[1], m1);
-        atomicMin(&s_red[2], m2); atomicMax(&s_red[3], m3);
-      }
-    }
-    __syncthreads();
-    const int ulo = s_red[0], uhi = s_red[1], dlo = s_red[2], dhi = s_red[3];
+    // ---- the z-rows of bins the tile's windows can touch on either side, WITHOUT a reduction:
+    // the tile is a run of the z-major sorted row, so all its clusters lie in the z-rows of bins
+    // between those of its first and last cluster (a thread whose window is not covered, which
+    // rounding could only cause at a bin edge, takes the per-thread search below)
+    const uint32_t tile_last = min(tile_first + TPC_NF_TILE, d.count) - 1u;
+    const int bzf = bin_coord(yz[d.clu_ofs + tile_first].y, d.z0, inv_dz, d.nz);
+    const int bzl = bin_coord(yz[d.clu_ofs + tile_last].y, d.z0, inv_dz, d.nz);
+    const float zmin = d.z0 + (float)bzf * dzbin, zmax = d.z0 + (float)(bzl + 1) * dzbin;
+    const float mzt = 2e-3f + 1e-6f * fmaxf(fabsf(zmin), fabsf(zmax));
+    const int ulo = bin_coord((zmin - wz) - mzt, du.z0, inv_dz, du.nz), uhi = bin_coord((zmax + wz) + mzt, du.z0, inv_dz, du.nz);
+    const int dlo = bin_coord((zmin - wz) - mzt, dd.z0, inv_dz, dd.nz), dhi = bin_coord((zmax + wz) + mzt, dd.z0, inv_dz, dd.nz);
     const uint32_t ub0 = du.bin_ofs + (uint32_t)ulo * (uint32_t)du.ny;
     const uint32_t unb = (uint32_t)(uhi - ulo + 1) * (uint32_t)du.ny;
     const uint32_t db0 = dd.bin_ofs + (uint32_t)dlo * (uint32_t)dd.ny;
     const uint32_t dnb = (uint32_t)(dhi - dlo + 1) * (uint32_t)dd.ny;
     const uint32_t cu0 = bin_start[ub0], cu1 = bin_start[ub0 + unb];
     const uint32_t cd0 = bin_start[db0], cd1 = bin_start[db0 + dnb];
+    // 16-byte alignment of the bulk copies: start of the bin slice rounded down to 4 entries, start
+    // of the cluster slab to 2; sizes rounded up (the arrays are padded)
+    const uint32_t ub0a = ub0 & ~3u, db0a = db0 & ~3u, cu0a = cu0 & ~1u, cd0a = cd0 & ~1u;
+    const uint32_t unb_c = (ub0 + unb + 1u - ub0a + 3u) & ~3u, dnb_c = (db0 + dnb + 1u - db0a + 3u) & ~3u;
+    const uint32_t ucl_c = (cu1 - cu0a + 1u) & ~1u, dcl_c = (cd1 - cd0a + 1u) & ~1u;
     int32_t bj = -1, bk = -1;
-    const bool staged = unb <= TPC_NF_BINS && dnb <= TPC_NF_BINS && cu1 - cu0 <= TPC_NF_SLAB &&
-                        cd1 - cd0 <= TPC_NF_SLAB;
-    if (!staged) {
-      if (have) nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);
-    } else {
-      for (uint32_t t = tx; t <= unb; t += TPC_NF_TILE) s_bin[0][t] = bin_start[ub0 + t];
-      for (uint32_t t = tx; t <= dnb; t += TPC_NF_TILE) s_bin[1][t] = bin_start[db0 + t];
-      for (uint32_t t = tx; t < cu1 - cu0; t += TPC_NF_TILE) s_yz[0][t] = yz[cu0 + t];
-      for (uint32_t t = tx; t < cd1 - cd0; t += TPC_NF_TILE) s_yz[1][t] = yz[cd0 + t];
-      __syncthreads();
-      if (have && (wu.bz1 - wu.bz0 > 2 || wd.bz1 - wd.bz0 > 2)) {
-        nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);     // bins much smaller than the window
-      } else if (have) {
-        const int nU = nf_collect<true>(wu, ulo, du.bin_ofs, cu0, s_bin[0], s_yz[0], &s_list[0][tx], yi, zi, ty, wy, wz);
+    const bool staged = unb_c <= TPC_NF_BINS + 8 && dnb_c <= TPC_NF_BINS + 8 && ucl_c <= TPC_NF_SLAB + 2 &&
+                        dcl_c <= TPC_NF_SLAB + 2;
+    bool slow = !staged;   // this thread searches on global memory (nf_generic)
+    if (staged) {
+      __syncthreads();     // every warp is done with the previous tile's slabs
+      if (tx == 0) {
+        mbar_expect_tx(&s_mbar, 4u * (unb_c + dnb_c) + 8u * (ucl_c + dcl_c));
+        bulk_g2s(s_bin[0], bin_start + ub0a, 4u * unb_c, &s_mbar);
+        bulk_g2s(s_bin[1], bin_start + db0a, 4u * dnb_c, &s_mbar);
+        if (ucl_c) bulk_g2s(s_yz[0], yz + cu0a, 8u * ucl_c, &s_mbar);
+        if (dcl_c) bulk_g2s(s_yz[1], yz + cd0a, 8u * dcl_c, &s_mbar);
+      }
+      // windows this tile's slabs do not cover, or taller than three z-rows of bins
+      const bool covered = have && wu.bz0 >= ulo && wu.bz1 <= uhi && wd.bz0 >= dlo && wd.bz1 <= dhi &&
+                           wu.bz1 - wu.bz0 <= 2 && wd.bz1 - wd.bz0 <= 2;
+      slow = have && !covered;
+      mbar_wait(&s_mbar, parity);
+      parity ^= 1u;
+      if (covered) {
+        const int nU = nf_collect<true>(wu, 0, ub0a, cu0a, s_bin[0], s_yz[0], &s_list[tx], yi, zi, ty, wy, wz);
         if (nU > TPC_NF_LIST) {
-          nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);   // rare: crowded window
+          slow = true;                                                   // rare: crowded window
         } else if (nU) {
-          nf_down_pairs(wd, dlo, dd.bin_ofs, cd0, s_bin[1], s_yz[1], s_yz[0], &s_list[0][tx], nU, yi, zi, ty, wy, wz,
-                        max_d2, orig, cu0, cd0, bj, bk);
-          if (bj >= 0) { bj += (int32_t)cu0; bk += (int32_t)cd0; }
+          nf_down_pairs(wd, 0, db0a, cd0a, s_bin[1], s_yz[1], s_yz[0], &s_list[tx], nU, yi, zi, ty, wy, wz,
+                        max_d2, orig, cu0a, cd0a, bj, bk);
+          if (bj >= 0) { bj += (int32_t)cu0a; bk += (int32_t)cd0a; }
         }
       }
+    } else {
+      slow = have;
     }
+    if (slow) nf_generic(B, wu, wd, yi, zi, ty, wy, wz, max_d2, bj, bk);
     if (have) { B.link_up[i] = bj; B.link_dn[i] = bk; }
   }
 }
@@ -1306,7 +1344,7 @@ __device__ __forceinline__ void follow_count_work(const TpcBuffers& B, int which
 // pending: the record is a hand-over to k_follow_down (n_hits is then the raw count).
 __device__ __forceinline__ void write_tracklet(const TpcBuffers& B, uint32_t sd, const float (*s_kin)[TPC_FOLLOW_BLOCK],
                                                int tx, float x, float chi2, int nh, int r_in, int r_out, uint32_t start,
-                                               uint32_t sector, int min_hits, bool pending) {
+                                               uint32_t sector, int min_hits, bool pending, uint32_t& n_tl) {
   tpc_tracklet t;
   t.x = x;
 #pragma unroll
@@ -1325,7 +1363,7 @@ __device__ __forceinline__ void write_tracklet(const TpcBuffers& B, uint32_t sd,
   t.pad_ = pending ? (uint16_t)TPC_TL_PENDING : (uint16_t)0;
   t.pad2_[0] = 0; t.pad2_[1] = 0;
   B.tracklets[sd] = t;
-  if (!pending && keep) atomicAdd(&B.cnt->n_tracklets, 1u);
+  if (!pending && keep) ++n_tl;   // summed per warp at the end of the kernel (no contended atomic here)
 }
 
 // resident CTAs per SM the register budgets are sized for (measured on the C4 frame: fewer,
@@ -1496,7 +1534,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) 
   const float2* __restrict__ yz = B.yz;
   const int lane = threadIdx.x & 31;
   const int tx = threadIdx.x;
-  uint32_t w_step = 0, w_upd = 0;
+  uint32_t w_step = 0, w_upd = 0, n_tl = 0;
   uint32_t chunk_next = 0, chunk_end = 0;
   bool exhausted = false;
 
@@ -1568,17 +1606,19 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_REFIT_MINBLOCKS) 
       }
       if (fin) {
         // (hits below r_in are outside [row_first,row_last] and thereby not part of the tracklet)
-        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, false);
+        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, false, n_tl);
         active = false;
       } else if (r == r0) {
         // the start row is reached (its hit is always present, so the saved state is the live one)
         const bool pending = r0 > 0;   // rows below to extrapolate into
-        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, pending);
+        write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sector, F.min_hits, pending, n_tl);
         active = false;
       }
     }
   }
   follow_count_work(B, 1, lane, w_step, w_upd, 0u);
+  n_tl = __reduce_add_sync(0xffffffffu, n_tl);
+  if (lane == 0 && n_tl) atomicAdd(&B.cnt->n_tracklets, n_tl);
 }
 
 // ---- R5.6-R5.7: inward extrapolation below the start row, output
@@ -1596,7 +1636,7 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_DOWN_MINBLOCKS) k
   const uint32_t* __restrict__ bin_start = B.bin_start;
   const int lane = threadIdx.x & 31;
   const int tx = threadIdx.x;
-  uint32_t w_step = 0, w_cand = 0, w_upd = 0;
+  uint32_t w_step = 0, w_cand = 0, w_upd = 0, n_tl = 0;
   uint32_t chunk_next = 0, chunk_end = 0;
   bool exhausted = false;
 
@@ -1684,12 +1724,14 @@ __global__ void __launch_bounds__(TPC_FOLLOW_BLOCK, TPC_FOLLOW_DOWN_MINBLOCKS) k
       }
       if (fin) {
         write_tracklet(B, sd, s_kin, tx, s_x[r_in], chi2, nh, r_in, r_out, start, sr_base / (uint32_t)F.R, F.min_hits,
-                       false);
+                       false, n_tl);
         active = false;
       }
     }
   }
   follow_count_work(B, 2, lane, w_step, w_upd, w_cand);
+  n_tl = __reduce_add_sync(0xffffffffu, n_tl);
+  if (lane == 0 && n_tl) atomicAdd(&B.cnt->n_tracklets, n_tl);
 }
 
 // ================================================================== K5 ambiguity solving
@@ -1793,6 +1835,10 @@ __global__ void __launch_bounds__(TPC_SEL_BLOCK) k_sel_owner(TpcBuffers B) {
     const unsigned long long key = s_key[lane];
     const int r0 = s_r0[lane], r1 = s_r1[lane];
     const int t0 = __reduce_min_sync(0xffffffffu, r0), t1 = __reduce_max_sync(0xffffffffu, r1);
+    // a tile without a single accepted tracklet (t0 = INT_MAX, t1 = -1: e.g. 32 consecutive short
+    // stubs) has no rows to visit and no masks to write; CTA-uniform, the next iteration's first
+    // barrier is the only one skipped ahead of
+    if (t1 < 0) continue;
     const int32_t* __restrict__ hits = B.row_hit + (size_t)sd * (size_t)R;
     const bool vec = (R & 3) == 0;
     // two row groups per iteration: eight independent hit -> owner chains in flight per lane
