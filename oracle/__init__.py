@@ -14,7 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "liboracle.so")
-_SRCS = [os.path.join(_HERE, f) for f in ("tpc_oracle.cpp", "tpc_oracle.h", "tpc_oracle_math.hpp")]
+_SRCS = [os.path.join(_HERE, f) for f in ("tpc_oracle.cpp", "tpc_merge_oracle.cpp", "tpc_oracle.h", "tpc_oracle_math.hpp")]
 
 CLUSTER_DTYPE = np.dtype(
     [("y", "<f4"), ("z", "<f4"), ("q", "<f4"), ("sector", "u1"), ("row", "u1"), ("flags", "<u2")])
@@ -69,7 +69,7 @@ def build(force: bool = False) -> str:
             and all(os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in _SRCS)):
         return _LIB
     cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC", "-pthread",
-           _SRCS[0], "-o", _LIB]
+           _SRCS[0], _SRCS[1], "-o", _LIB]
     subprocess.run(cmd, check=True)
     return _LIB
 
@@ -264,32 +264,41 @@ def fit_hits(rows, y, z, geom: Geom | None = None, params: Params | None = None)
     return float(chi2), float(out[0]), out[1:6].copy(), out[6:21].copy(), int(out[21]), int(out[22])
 
 
-def refit_hits(rows, y, z, geom: Geom | None = None, params: Params | None = None):
+FIT_DTYPE = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"), ("n_clusters", "<u4"),
+                      ("flags", "<u4"), ("x_out", "<f4"), ("p_out", "<f4", (5,)), ("c_out", "<f4", (15,)),
+                      ("pad_", "<u4", (3,))])
+
+
+def refit_hits(rows, y, z, geom: Geom | None = None, params: Params | None = None, both_ends: bool = False):
     """R8 sector-track refit of a given cluster list (rows strictly ascending, holes allowed).
-    Returns (chi2, x, p[5], c[15], n) or None if the fit left the |sin phi| range."""
+    Returns (chi2, x, p[5], c[15], n) or None if the fit left the |sin phi| range; with both_ends
+    also (x_out, p_out[5], c_out[15]), the state after the outward pass at the last cluster."""
     geom = geom or default_geom()
     params = params or default_params()
     rows = np.ascontiguousarray(rows, dtype=np.int32)
     y = np.ascontiguousarray(y, dtype=np.float32)
     z = np.ascontiguousarray(z, dtype=np.float32)
-    out = np.zeros(24, dtype=np.float32)
+    out = np.zeros(48, dtype=np.float32)
     chi2 = lib().orc_refit_hits(C.byref(geom), C.byref(params), _ptr(rows), _ptr(y), _ptr(z), len(rows), _ptr(out))
     if chi2 < 0:
         return None
-    return float(chi2), float(out[0]), out[1:6].copy(), out[6:21].copy(), int(out[21])
+    r = (float(chi2), float(out[0]), out[1:6].copy(), out[6:21].copy(), int(out[21]))
+    if both_ends:
+        r = r + (float(out[22]), out[23:28].copy(), out[28:43].copy())
+    return r
 
 
 def refit_tracks(clusters: np.ndarray, tracks: np.ndarray, cluster_ids: np.ndarray, geom=None, params=None):
-    """R8 for every track of a result: (fit[n_tracks] records x,p,c,chi2,n_clusters,ok) from the
-    tracks' cluster lists (original indices into ``clusters``)."""
-    dt = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"), ("n_clusters", "<u4"),
-                   ("flags", "<u4")])
-    out = np.zeros(len(tracks), dtype=dt)
+    """R8 for every track of a result: (fit[n_tracks] records, FIT_DTYPE) from the tracks' cluster
+    lists (original indices into ``clusters``)."""
+    out = np.zeros(len(tracks), dtype=FIT_DTYPE)
     for k, t in enumerate(tracks):
         ids = cluster_ids[int(t["cluster_ofs"]): int(t["cluster_ofs"]) + int(t["n_clusters"])]
-        r = refit_hits(clusters["row"][ids], clusters["y"][ids], clusters["z"][ids], geom, params)
+        r = refit_hits(clusters["row"][ids], clusters["y"][ids], clusters["z"][ids], geom, params, both_ends=True)
         if r is None:
             out[k]["flags"] = 1
+            out[k]["n_clusters"] = len(ids)
             continue
-        out[k]["chi2"], out[k]["x"], out[k]["p"], out[k]["c"], out[k]["n_clusters"] = r
+        (out[k]["chi2"], out[k]["x"], out[k]["p"], out[k]["c"], out[k]["n_clusters"],
+         out[k]["x_out"], out[k]["p_out"], out[k]["c_out"]) = r
     return out

@@ -862,7 +862,8 @@ float orc_fit_hits(const orc_geom* g, const orc_params* pp, const int32_t* rows,
 //   R8.2 outward: row by row to every further cluster (pure propagation on rows in between), update
 //   R8.3 turn at the last cluster as R5.4 (s,t,q after its update; y,z measured; C reset)
 //   R8.4 inward: back through the clusters to the first one, chi2 accumulated in this pass
-// out_state = x, p[5], c[15], n at the first cluster's row.  Returns chi2, or -1 if a propagation
+// out_state = x, p[5], c[15], n at the first cluster's row, then x_out, p_out[5], c_out[15]: the state
+// after the outward pass R8.2 at the last cluster (43 floats).  Returns chi2, or -1 if a propagation
 // or an update left the |sin phi| range (the fit failed; out_state untouched).
 float orc_refit_hits(const orc_geom* g, const orc_params* pp, const int32_t* rows, const float* y,
                      const float* z, int n, float* out_state) {
@@ -894,6 +895,8 @@ float orc_refit_hits(const orc_geom* g, const orc_params* pp, const int32_t* row
     if (tpc_oracle::kf_update(st, gn, y[i], z[i], P.max_sinphi, P.max_qpt)) return -1.0f;
     snap_s = st.s; snap_t = st.t; snap_q = st.q;
   }
+  // the OUTER end (used by the merging, R9): the state after the outward pass at the last cluster
+  const KFState<float> st_out = st;
   st.y = y[n - 1]; st.z = z[n - 1]; st.s = snap_s; st.t = snap_t; st.q = snap_q;  // R8.3
   reset_cov();
   float chi2 = 0.0f;
@@ -909,6 +912,9 @@ float orc_refit_hits(const orc_geom* g, const orc_params* pp, const int32_t* row
   out_state[1] = st.y; out_state[2] = st.z; out_state[3] = st.s; out_state[4] = st.t; out_state[5] = st.q;
   for (int i = 0; i < 15; ++i) out_state[6 + i] = st.c[i];
   out_state[21] = (float)n;
+  out_state[22] = T.x[rows[n - 1]];
+  out_state[23] = st_out.y; out_state[24] = st_out.z; out_state[25] = st_out.s; out_state[26] = st_out.t; out_state[27] = st_out.q;
+  for (int i = 0; i < 15; ++i) out_state[28 + i] = st_out.c[i];
   return chi2;
 }
 

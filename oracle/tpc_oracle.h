@@ -141,7 +141,8 @@ float orc_fit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows, 
                    const float* z, int n, float* out_state);
 /* R8 sector-track refit: pure Kalman fit of a given cluster list (rows strictly ascending, holes
  * allowed; outward pass, turn, inward pass; no search, no chi2 cut).  out_state = x, p[5], c[15], n
- * (22 floats) at rows[0]; returns the chi2 of the inward pass or -1 if the fit left |sin phi|. */
+ * at rows[0], then x_out, p_out[5], c_out[15] = the state after the outward pass at rows[n-1]
+ * (43 floats); returns the chi2 of the inward pass or -1 if the fit left |sin phi|. */
 float orc_refit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows, const float* y,
                      const float* z, int n, float* out_state);
 /* selector on hand-made tracklets: row_hit[n_tracklets][n_rows] (cluster ids or -1),
@@ -149,6 +150,36 @@ float orc_refit_hits(const orc_geom* g, const orc_params* p, const int32_t* rows
 orc_result* orc_select_only(const orc_geom* g, const orc_params* p, uint64_t n_clusters, int n_tracklets,
                             const int32_t* row_hit, const int32_t* n_hits, const float* chi2,
                             const uint32_t* seed_id);
+
+/* ---- R9 track merging (tpc_merge_oracle.cpp; section 2, section 3) ---- */
+typedef struct orc_merge_params {
+  int32_t gap_in_sector;     /* (30) stage 1: 1 <= row_first_b - row_last_a <= this                  */
+  int32_t gap_adjacent_back; /* (3)  stage 2: -this <= row_first_b - row_last_a                        */
+  int32_t gap_adjacent;      /* (10) stage 2:          row_first_b - row_last_a <= this                */
+  int32_t gap_ce;            /* (6)  stage 3: 1 <= row_first_b - row_last_a <= this                    */
+  float chi2_max;            /* (20) match cut on the 5-parameter chi2                                 */
+  float sys[5];              /* (0.3 cm, 0.3 cm, 0.02, 0.02, 0.2 c/GeV) added in quadrature per parameter */
+  float ce_sys_z;            /* (3 cm) replaces sys[1] across the central electrode                   */
+  float pre_dz;              /* (40 cm) pre-cut on the z of the two untransported end states           */
+  int32_t stages;            /* (7) bit 0: in sector, bit 1: adjacent sectors, bit 2: central electrode */
+} orc_merge_params;
+
+typedef struct orc_merge_track { /* one sector track as the merging sees it */
+  int32_t sector, row_first, row_last, valid; /* valid = 0: refit failed, takes no part */
+  uint32_t seed_id;
+  int32_t segment, iter;                       /* iter = 1 for tracks of the second seeding iteration */
+  float p_in[5], c_in[15];                     /* R8 state at the innermost cluster's row  */
+  float p_out[5], c_out[15];                   /* R8 state after the outward pass at the outermost cluster's row */
+} orc_merge_track;
+
+void orc_merge_default_params(orc_merge_params* m);
+/* next[k] / prev[k] = track linked behind / before track k (-1 none), link_chi2[k] = chi2 of the
+ * link k -> next[k] (may be NULL).  Returns the number of links or -1. */
+int orc_merge_links(const orc_geom* g, const orc_params* p, const orc_merge_params* m, const orc_merge_track* t,
+                    int32_t n, int32_t* next, int32_t* prev, float* link_chi2);
+/* rotation of a state (y,z,s,t,q,c[15]) at local *x into the neighbouring sector's frame
+ * (sign +1: the sector with the next higher azimuth); returns 0 if |sin phi| leaves the range */
+int orc_merge_rotate(const orc_geom* g, float* state20, float* x, int sign, float max_sinphi);
 
 #ifdef __cplusplus
 }
