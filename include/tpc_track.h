@@ -314,11 +314,72 @@ typedef struct tpc_track_fit {
   float chi2;            /* of the inward pass, ndf = 2*n_clusters - 5                       */
   uint32_t n_clusters;
   uint32_t flags;        /* bit 0: the fit left the |sin phi| range, record not valid        */
-} tpc_track_fit;         /* 96 bytes */
+  float x_out;           /* local x of the OUTERMOST cluster's row                           */
+  float p_out[5];        /* state there after the outward pass (the end the merging extends) */
+  float c_out[15];
+  uint32_t pad_[3];
+} tpc_track_fit;         /* 192 bytes */
 int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream);
 /* Synchronises and returns the DEVICE array [n_tracks] written by tpc_refit_tracks (aliases the
  * workspace, same lifetime as the track view). */
 int tpc_get_refit(tpc_ctx* ctx, const tpc_track_fit** d_fit);
+
+/* TRACK MERGING (section 2: "merges tracks first inside the TPC sectors, then between
+ * adjacent sectors of the TPC halves, and then across the central electrode"; section 3:
+ * on top of the sector-track refit; reading R9).  Three stages in that order; in each,
+ * the refit state at the OUTER end of a track a is transported to the innermost row of a track b
+ * (stage 1 and 3: row steps of the follower's propagation; stage 2: rotation by one sector step,
+ * then one propagation step) and compared with b's refit state there:
+ * chi2 = sum_i d_i^2 / (C_a'[ii] + C_b[ii] + sys_i^2); a and b are linked iff chi2 <= chi2_max and
+ * they are each other's best choice by (chi2, sector, iteration, seed id, segment).  Links form
+ * chains; a merged track = the cluster lists of its segments in chain order.  Only tracks with a
+ * valid refit and a free end take part; later stages see the ends the earlier ones left free. */
+typedef struct tpc_merge_params {
+  int32_t gap_in_sector;     /* (30) stage 1: 1 <= row_first_b - row_last_a <= this                */
+  int32_t gap_adjacent_back; /* (3)  stage 2: -this <= row_first_b - row_last_a                      */
+  int32_t gap_adjacent;      /* (10) stage 2:          row_first_b - row_last_a <= this              */
+  int32_t gap_ce;            /* (6)  stage 3: 1 <= row_first_b - row_last_a <= this                  */
+  float chi2_max;            /* (20)                                                                 */
+  float sys[5];              /* (0.3 cm, 0.3 cm, 0.02, 0.02, 0.2 c/GeV)                              */
+  float ce_sys_z;            /* (3 cm) replaces sys[1] across the central electrode, where z_b + z_a' is compared */
+  float pre_dy, pre_dz;      /* (8 cm, 8 cm) pre-cuts between the transported state and b's state    */
+  float pre_coarse_dz;       /* (40 cm) pre-cut on z between the two end states as they are          */
+  int32_t stages;            /* (7) bit 0: in sector, bit 1: adjacent sectors, bit 2: central electrode */
+} tpc_merge_params;          /* 60 bytes */
+
+typedef struct tpc_merged_track {
+  uint32_t head;             /* index (into the sector-track array) of the innermost segment        */
+  uint32_t n_segments, n_clusters, n_shared;
+  uint32_t cluster_ofs;      /* first entry in d_cluster_ids / d_cluster_shared of the merged view  */
+  uint32_t seg_ofs;          /* first entry in d_seg_index                                          */
+  int32_t row_first, row_last, sector_first, sector_last;
+} tpc_merged_track;          /* 40 bytes */
+
+typedef struct tpc_merged_view {
+  uint64_t n_tracks;                 /* sector tracks that went in                                  */
+  uint64_t n_merged;                 /* merged tracks (chains; unlinked tracks are chains of one)   */
+  uint64_t n_links;
+  uint64_t n_cluster_ids;
+  const tpc_merged_track* d_merged;  /* [n_merged], heads in the order of the sector-track array    */
+  const uint32_t* d_seg_index;       /* [n_tracks] sector-track indices, chain by chain             */
+  const uint32_t* d_cluster_ids;     /* [n_cluster_ids] original cluster indices, chain order       */
+  const uint8_t* d_cluster_shared;
+  const int32_t* d_next;             /* [n_tracks] track linked behind / before each track, -1 none */
+  const int32_t* d_prev;
+  const float* d_link_chi2;          /* [n_tracks] chi2 of the link to d_next                       */
+} tpc_merged_view;
+
+void tpc_merge_default_params(tpc_merge_params* out);
+/* Scratch + output size of tpc_merge_tracks for n_tracks sector tracks holding n_cluster_ids ids. */
+size_t tpc_merge_workspace_bytes(const tpc_ctx* ctx, uint64_t n_tracks, uint64_t n_cluster_ids);
+/* Merge the tracks of the last run; needs tpc_refit_tracks to have run on them (else TPC_E_STATE).
+ * d_merge_workspace: DEVICE, 256-byte aligned, caller owned, >= tpc_merge_workspace_bytes(ctx,
+ * n_tracks, n_cluster_ids of the track view).  params == NULL: defaults.  Enqueued on cuda_stream
+ * (synchronises it first to learn the track count), in the mode (deterministic / fast) of the run. */
+int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_merge_workspace,
+                     size_t workspace_bytes, void* cuda_stream);
+/* Synchronises and fills *out (HOST) with device pointers into the merge workspace. */
+int tpc_get_merged(tpc_ctx* ctx, tpc_merged_view* out);
 
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);

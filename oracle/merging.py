@@ -22,7 +22,7 @@ MERGED_DTYPE = np.dtype(
 class MergeParams(C.Structure):
     _fields_ = [("gap_in_sector", C.c_int32), ("gap_adjacent_back", C.c_int32), ("gap_adjacent", C.c_int32),
                 ("gap_ce", C.c_int32), ("chi2_max", C.c_float), ("sys", C.c_float * 5), ("ce_sys_z", C.c_float),
-                ("pre_dz", C.c_float), ("stages", C.c_int32)]
+                ("pre_dy", C.c_float), ("pre_dz", C.c_float), ("pre_coarse_dz", C.c_float), ("stages", C.c_int32)]
 
 
 def _lib():

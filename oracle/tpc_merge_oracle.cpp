@@ -24,8 +24,9 @@
 //     stage 3, across the central electrode:  sector_b = sector_a +- 18, 1 <= f_b - l_a <= gap_ce,
 //              row steps; z compared as z_b + z_a' (the two drift sides see z_true -+ v t, so the
 //              sum vanishes where the track crosses the electrode) with sys_z replaced by ce_sys_z.
-//   Pre-cuts (part of the definition; they also bound the search): |z_b - z_a| <= pre_dz on the
-//   untransported end states (stage 3: |z_b + z_a|).
+//   Pre-cuts (part of the definition; they also bound the search): coarse, on the two end states as
+//   they are, |z_b - z_a| <= pre_coarse_dz (stage 3: |z_b + z_a|); fine, on the TRANSPORTED state,
+//   |y_b - y_a'| <= pre_dy and |z_b - z_a'| <= pre_dz (stage 3: |z_b + z_a'|).
 //   Tracks whose refit failed take no part.  Every link raises row_first by >= min_hits_track - 1 -
 //   gap_adjacent_back > 0 rows, so the links form simple chains.
 #include <cmath>
@@ -113,9 +114,9 @@ inline Key key_of(const orc_merge_track& t) { return Key{t.sector, t.iter, t.see
 bool match(const Geo& G, const orc_params& P, const orc_merge_params& M, const orc_merge_track& a,
            const orc_merge_track& b, int stage, float* chi2_out) {
   const int gap = b.row_first - a.row_last;
-  // pre-cut on the untransported end states
-  const float dz_pre = stage == 3 ? b.p_in[1] + a.p_out[1] : b.p_in[1] - a.p_out[1];
-  if (!(tpc_oracle::o_abs(dz_pre) <= M.pre_dz)) return false;
+  // coarse pre-cut on the untransported end states
+  const float dz_coarse = stage == 3 ? b.p_in[1] + a.p_out[1] : b.p_in[1] - a.p_out[1];
+  if (!(tpc_oracle::o_abs(dz_coarse) <= M.pre_coarse_dz)) return false;
   KFState<float> st;
   load_state(st, a.p_out, a.c_out);
   if (stage == 2) {
@@ -129,6 +130,10 @@ bool match(const Geo& G, const orc_params& P, const orc_merge_params& M, const o
     for (int i = 0; i < gap; ++i)
       if (!tpc_oracle::kf_propagate(st, G.dx_row, G.cfield, P.max_sinphi)) return false;
   }
+  // fine pre-cuts on the transported state
+  const float dz_pre = stage == 3 ? b.p_in[1] + st.z : b.p_in[1] - st.z;
+  if (!(tpc_oracle::o_abs(dz_pre) <= M.pre_dz)) return false;
+  if (!(tpc_oracle::o_abs(b.p_in[0] - st.y) <= M.pre_dy)) return false;
   const float pa[5] = {st.y, st.z, st.s, st.t, st.q};
   const int diag[5] = {0, 2, 5, 9, 14};
   float chi2 = 0.0f;
@@ -165,7 +170,7 @@ void orc_merge_default_params(orc_merge_params* m) {
   m->chi2_max = 20.0f;
   m->sys[0] = 0.3f; m->sys[1] = 0.3f; m->sys[2] = 0.02f; m->sys[3] = 0.02f; m->sys[4] = 0.2f;
   m->ce_sys_z = 3.0f;
-  m->pre_dz = 40.0f;
+  m->pre_dy = 8.0f; m->pre_dz = 8.0f; m->pre_coarse_dz = 40.0f;
   m->stages = 7;
 }
 

@@ -160,7 +160,8 @@ typedef struct orc_merge_params {
   float chi2_max;            /* (20) match cut on the 5-parameter chi2                                 */
   float sys[5];              /* (0.3 cm, 0.3 cm, 0.02, 0.02, 0.2 c/GeV) added in quadrature per parameter */
   float ce_sys_z;            /* (3 cm) replaces sys[1] across the central electrode                   */
-  float pre_dz;              /* (40 cm) pre-cut on the z of the two untransported end states           */
+  float pre_dy, pre_dz;      /* (8 cm, 8 cm) pre-cuts on y and z between the transported state and b's     */
+  float pre_coarse_dz;       /* (40 cm) pre-cut on z between the two end states as they are               */
   int32_t stages;            /* (7) bit 0: in sector, bit 1: adjacent sectors, bit 2: central electrode */
 } orc_merge_params;
 

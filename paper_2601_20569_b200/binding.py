@@ -72,6 +72,25 @@ class TrackView(C.Structure):
                 ("grid_by_rows", C.c_uint64)]
 
 
+class MergeParams(C.Structure):
+    _fields_ = [("gap_in_sector", C.c_int32), ("gap_adjacent_back", C.c_int32), ("gap_adjacent", C.c_int32),
+                ("gap_ce", C.c_int32), ("chi2_max", C.c_float), ("sys", C.c_float * 5), ("ce_sys_z", C.c_float),
+                ("pre_dy", C.c_float), ("pre_dz", C.c_float), ("pre_coarse_dz", C.c_float), ("stages", C.c_int32)]
+
+
+class MergedView(C.Structure):
+    _fields_ = [("n_tracks", C.c_uint64), ("n_merged", C.c_uint64), ("n_links", C.c_uint64),
+                ("n_cluster_ids", C.c_uint64), ("d_merged", C.c_void_p), ("d_seg_index", C.c_void_p),
+                ("d_cluster_ids", C.c_void_p), ("d_cluster_shared", C.c_void_p), ("d_next", C.c_void_p),
+                ("d_prev", C.c_void_p), ("d_link_chi2", C.c_void_p)]
+
+
+MERGED_DTYPE = np.dtype(
+    [("head", "<u4"), ("n_segments", "<u4"), ("n_clusters", "<u4"), ("n_shared", "<u4"), ("cluster_ofs", "<u4"),
+     ("seg_ofs", "<u4"), ("row_first", "<i4"), ("row_last", "<i4"), ("sector_first", "<i4"), ("sector_last", "<i4")])
+assert MERGED_DTYPE.itemsize == 40 and C.sizeof(MergeParams) == 60
+
+
 class DebugView(C.Structure):
     _fields_ = [("n_clusters", C.c_uint64), ("n_sorted", C.c_uint64), ("n_rows_total", C.c_uint64),
                 ("n_bins", C.c_uint64), ("n_seeds", C.c_uint64), ("tracklet_stride", C.c_uint64),
@@ -84,7 +103,8 @@ class DebugView(C.Structure):
 EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_sector_track",
            "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
-           "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_last_launch_count",
+           "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_merge_default_params",
+           "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -131,6 +151,14 @@ def load_library():
     L.tpc_sector_track_host.restype = C.c_int
     L.tpc_sector_track_host.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_size_t, vp, C.c_uint32, vp, C.c_uint64,
                                         vp, vp, C.c_uint64, C.POINTER(TrackView)]
+    L.tpc_merge_default_params.restype = None
+    L.tpc_merge_default_params.argtypes = [C.POINTER(MergeParams)]
+    L.tpc_merge_workspace_bytes.restype = C.c_size_t
+    L.tpc_merge_workspace_bytes.argtypes = [vp, C.c_uint64, C.c_uint64]
+    L.tpc_merge_tracks.restype = C.c_int
+    L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), vp, C.c_size_t, vp]
+    L.tpc_get_merged.restype = C.c_int
+    L.tpc_get_merged.argtypes = [vp, C.POINTER(MergedView)]
     L.tpc_last_launch_count.restype = C.c_int
     L.tpc_last_launch_count.argtypes = [vp]
     L.tpc_destroy.restype = None
@@ -245,8 +273,9 @@ def tpc_sector_track_two_iterations(ctx: int, d_clusters: int, n_clusters: int, 
 
 
 TRACK_FIT_DTYPE = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"),
-                            ("n_clusters", "<u4"), ("flags", "<u4")])
-assert TRACK_FIT_DTYPE.itemsize == 96
+                            ("n_clusters", "<u4"), ("flags", "<u4"), ("x_out", "<f4"), ("p_out", "<f4", (5,)),
+                            ("c_out", "<f4", (15,)), ("pad_", "<u4", (3,))])
+assert TRACK_FIT_DTYPE.itemsize == 192
 
 
 def tpc_refit_tracks(ctx: int, cuda_stream: int) -> int:
@@ -257,6 +286,33 @@ def tpc_get_refit(ctx: int):
     p = C.c_void_p()
     rc = load_library().tpc_get_refit(ctx, C.byref(p))
     return rc, p.value
+
+
+def tpc_merge_default_params(**overrides) -> MergeParams:
+    m = MergeParams()
+    load_library().tpc_merge_default_params(C.byref(m))
+    for k, v in overrides.items():
+        if k == "sys":
+            for i in range(5):
+                m.sys[i] = v[i]
+        else:
+            setattr(m, k, v)
+    return m
+
+
+def tpc_merge_workspace_bytes(ctx: int, n_tracks: int, n_cluster_ids: int) -> int:
+    return int(load_library().tpc_merge_workspace_bytes(ctx, n_tracks, n_cluster_ids))
+
+
+def tpc_merge_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, cuda_stream: int) -> int:
+    return load_library().tpc_merge_tracks(ctx, C.byref(params) if params is not None else None, d_workspace,
+                                           workspace_bytes, cuda_stream)
+
+
+def tpc_get_merged(ctx: int):
+    v = MergedView()
+    rc = load_library().tpc_get_merged(ctx, C.byref(v))
+    return rc, v
 
 
 def tpc_last_launch_count(ctx: int) -> int:
@@ -392,6 +448,40 @@ class SectorTracker:
             raise TpcError(rc, "tpc_get_refit", tpc_last_cuda_error(self.ctx))
         rc, v = self.counts()
         return self._to_numpy(ptr, v.n_tracks, TRACK_FIT_DTYPE)
+
+    def merge(self, mparams: MergeParams | None = None, stream=None, fetch: bool = True):
+        """Track merging (reading R9) of the current result; tpc_refit_tracks must have
+        run on it (refit()).  Returns a dict of arrays (merged, seg_index, cluster_ids, cluster_shared,
+        next, prev, link_chi2) or, with fetch=False, the view."""
+        rc, v = self.counts()
+        need = tpc_merge_workspace_bytes(self.ctx, v.n_tracks, v.n_cluster_ids)
+        if getattr(self, "merge_ws", None) is None or self.merge_ws.numel() < need + 256:
+            self.merge_ws = None
+            self.merge_ws = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        ws_ptr = (self.merge_ws.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc = tpc_merge_tracks(self.ctx, mparams, ws_ptr, need, st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_merge_tracks", tpc_last_cuda_error(self.ctx))
+        if not fetch:
+            return None
+        rc, mv = tpc_get_merged(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_merged", tpc_last_cuda_error(self.ctx))
+
+        def arr(ptr, count, dtype):
+            dtype = np.dtype(dtype)
+            if count == 0:
+                return np.zeros(0, dtype=dtype)
+            off = ptr - self.merge_ws.data_ptr()
+            return self.merge_ws[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
+        nt = int(mv.n_tracks)
+        return dict(view=mv, merged=arr(mv.d_merged, int(mv.n_merged), MERGED_DTYPE),
+                    seg_index=arr(mv.d_seg_index, nt, np.uint32),
+                    cluster_ids=arr(mv.d_cluster_ids, int(mv.n_cluster_ids), np.uint32),
+                    cluster_shared=arr(mv.d_cluster_shared, int(mv.n_cluster_ids), np.uint8),
+                    next=arr(mv.d_next, nt, np.int32), prev=arr(mv.d_prev, nt, np.int32),
+                    link_chi2=arr(mv.d_link_chi2, nt, np.float32))
 
     def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
         """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the

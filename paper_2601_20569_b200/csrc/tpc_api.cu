@@ -2,6 +2,7 @@
 // Host code only; all arithmetic of the method runs in the kernels of tpc_kernels.cu.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -32,6 +33,10 @@ struct tpc_ctx {
   uint32_t flags = 0;
   int launches = 0;
   uint64_t n_bins_cap = 0;
+  bool refit_done = false;     // tpc_refit_tracks ran on the current result
+  bool merged = false;         // tpc_merge_tracks ran on the current result
+  TpcMergeBuffers mbuf;
+  uint32_t* h_mcnt = nullptr;  // pinned: merge counters
   char cuda_err[256] = {0};
 };
 
@@ -198,6 +203,7 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
       (e = cudaMalloc(&c->d_cnt, sizeof(TpcCounters))) != cudaSuccess ||
       (e = cudaMalloc(&c->d_row_stat, sizeof(TpcRowStat) * n_sr)) != cudaSuccess ||
       (e = cudaMallocHost(&c->h_cnt, sizeof(TpcCounters))) != cudaSuccess ||
+      (e = cudaMallocHost(&c->h_mcnt, 4 * sizeof(uint32_t))) != cudaSuccess ||
       (e = cudaMalloc(&c->d_sector_seen, sizeof(uint32_t) * (size_t)geom->n_sectors)) != cudaSuccess ||
       (e = cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking)) != cudaSuccess ||
       (e = cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking)) != cudaSuccess ||
@@ -258,6 +264,8 @@ static int enqueue_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n
   ctx->flags = flags;
   ctx->ran = false;
   ctx->synced = false;
+  ctx->refit_done = false;
+  ctx->merged = false;
   ctx->events.enabled = (flags & TPC_STAGE_TIMERS) != 0;
   (void)cudaGetLastError();
   const int launches = (flags & TPC_DETERMINISTIC)
@@ -676,6 +684,8 @@ int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters,
   ctx->launches = launches1 + ctx->launches + 5;
   ctx->ran = true;
   ctx->synced = true;
+  ctx->refit_done = false;
+  ctx->merged = false;
   return TPC_OK;
 }
 
@@ -692,6 +702,8 @@ int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream) {
   if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (refit)");
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->synced = false;
+  ctx->refit_done = true;
+  ctx->merged = false;
   return TPC_OK;
 }
 
@@ -700,6 +712,108 @@ int tpc_get_refit(tpc_ctx* ctx, const tpc_track_fit** d_fit) {
   int rc = sync_run(ctx);
   if (rc != TPC_OK) return rc;
   *d_fit = ctx->buf.track_fit;
+  return TPC_OK;
+}
+
+// ---------------------------------------------------------------- track merging (R9)
+namespace {
+size_t carve_merge(const tpc_ctx* c, uint64_t n_tracks, uint64_t n_ids, char* base, TpcMergeBuffers* M) {
+  const uint32_t n_cells = (uint32_t)c->geom.n_sectors * (uint32_t)c->geom.n_rows * 1024u;   // TPC_MG_ZB slabs
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  TpcMergeBuffers m;
+  std::memset(&m, 0, sizeof(m));
+  m.n_tracks = (uint32_t)n_tracks; m.n_ids = (uint32_t)n_ids; m.n_rows = (uint32_t)c->geom.n_rows; m.n_cells = n_cells;
+  const size_t nt = n_tracks + 1;
+  const size_t n_part = (std::max<size_t>(n_cells + 1, nt) + 1023) / 1024 + 2;
+  m.cell_start = (uint32_t*)take(4 * ((size_t)n_cells + 1));
+  m.cell_cursor = (uint32_t*)take(4 * (size_t)n_cells);
+  m.partials = (uint32_t*)take(4 * n_part);
+  m.ends = (float*)take(64 * nt);
+  m.next = (int32_t*)take(4 * nt); m.prev = (int32_t*)take(4 * nt); m.link_chi2 = (float*)take(4 * nt);
+  m.best_out = (int32_t*)take(4 * nt); m.best_out_chi = (uint32_t*)take(4 * nt); m.best_in_chi = (uint32_t*)take(4 * nt);
+  m.best_in_key = (unsigned long long*)take(8 * nt);
+  m.head_ofs = (uint32_t*)take(4 * nt); m.seg_ofs = (uint32_t*)take(4 * nt); m.clu_ofs = (uint32_t*)take(4 * nt);
+  m.seg_dst = (uint32_t*)take(4 * nt);
+  m.merged = (tpc_merged_track*)take(sizeof(tpc_merged_track) * nt);
+  m.seg_index = (uint32_t*)take(4 * nt);
+  m.ids = (uint32_t*)take(4 * ((size_t)n_ids + 1));
+  m.shared = (uint8_t*)take((size_t)n_ids + 1);
+  m.counters = (uint32_t*)take(16);
+  if (M) *M = m;
+  return off;
+}
+}  // namespace
+
+void tpc_merge_default_params(tpc_merge_params* m) {
+  std::memset(m, 0, sizeof(*m));
+  m->gap_in_sector = 30; m->gap_adjacent_back = 3; m->gap_adjacent = 10; m->gap_ce = 6;
+  m->chi2_max = 20.0f;
+  m->sys[0] = 0.3f; m->sys[1] = 0.3f; m->sys[2] = 0.02f; m->sys[3] = 0.02f; m->sys[4] = 0.2f;
+  m->ce_sys_z = 3.0f;
+  m->pre_dy = 8.0f; m->pre_dz = 8.0f; m->pre_coarse_dz = 40.0f;
+  m->stages = 7;
+}
+
+size_t tpc_merge_workspace_bytes(const tpc_ctx* ctx, uint64_t n_tracks, uint64_t n_cluster_ids) {
+  if (!ctx || n_tracks >= (1ull << 31) || n_cluster_ids >= (1ull << 32)) return 0;
+  return carve_merge(ctx, n_tracks, n_cluster_ids, nullptr, nullptr);
+}
+
+int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_ws, size_t ws_bytes, void* cuda_stream) {
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->refit_done) return TPC_E_STATE;
+  rc = device_status(ctx);
+  if (rc == TPC_E_OVERFLOW) return rc;
+  if (!d_ws || ((uintptr_t)d_ws & 255u)) return TPC_E_ARG;
+  tpc_merge_params P;
+  if (params) P = *params; else tpc_merge_default_params(&P);
+  if (!(P.pre_dz > 0.f) || !(P.pre_dy > 0.f) || !(P.chi2_max >= 0.f) || P.gap_in_sector < 0 || P.gap_adjacent < 0 ||
+      P.gap_adjacent_back < 0 || P.gap_ce < 0 || P.gap_adjacent_back > ctx->params.min_hits_track - 2)
+    return TPC_E_ARG;   // (the last: links must raise the first row, so chains cannot close)
+  const uint32_t n_tracks = ctx->h_cnt->n_tracks, n_ids = ctx->h_cnt->n_ids;
+  TpcMergeBuffers M;
+  const size_t need = carve_merge(ctx, n_tracks, n_ids, (char*)d_ws, &M);
+  if (ws_bytes < need) return TPC_E_WORKSPACE;
+  M.P = P;
+  M.inv_w = 1.0f / P.pre_dz;
+  const double a = 2.0 * (double)ctx->geom.sector_half_angle_deg * (3.14159265358979323846 / 180.0);
+  M.ca = (float)std::cos(a);
+  M.sa = (float)std::sin(a);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  (void)cudaGetLastError();
+  const int l = (ctx->flags & TPC_DETERMINISTIC) ? tpc_det::run_merge(ctx->buf, &ctx->hconst, M, st, ctx->n_sm)
+                                                 : tpc_fast::run_merge(ctx->buf, &ctx->hconst, M, st, ctx->n_sm);
+  if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (merge)");
+  cudaError_t e = cudaMemcpyAsync(ctx->h_mcnt, M.counters, 16, cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(merge counters)");
+  ctx->mbuf = M;
+  ctx->stream = st;
+  ctx->synced = false;
+  ctx->merged = true;
+  ctx->launches = l;
+  return TPC_OK;
+}
+
+int tpc_get_merged(tpc_ctx* ctx, tpc_merged_view* out) {
+  if (!out) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->merged) return TPC_E_STATE;
+  const TpcMergeBuffers& M = ctx->mbuf;
+  std::memset(out, 0, sizeof(*out));
+  out->n_tracks = M.n_tracks;
+  out->n_merged = M.n_tracks ? ctx->h_mcnt[0] : 0;
+  out->n_links = ctx->h_mcnt[1];
+  out->n_cluster_ids = M.n_tracks ? ctx->h_mcnt[2] : 0;
+  out->d_merged = M.merged; out->d_seg_index = M.seg_index;
+  out->d_cluster_ids = M.ids; out->d_cluster_shared = M.shared;
+  out->d_next = M.next; out->d_prev = M.prev; out->d_link_chi2 = M.link_chi2;
   return TPC_OK;
 }
 
@@ -715,6 +829,7 @@ void tpc_destroy(tpc_ctx* c) {
   if (c->d_cnt) cudaFree(c->d_cnt);
   if (c->d_row_stat) cudaFree(c->d_row_stat);
   if (c->h_cnt) cudaFreeHost(c->h_cnt);
+  if (c->h_mcnt) cudaFreeHost(c->h_mcnt);
   if (c->d_sector_seen) cudaFree(c->d_sector_seen);
   if (c->s_in) cudaStreamDestroy(c->s_in);
   if (c->s_out) cudaStreamDestroy(c->s_out);

@@ -125,6 +125,25 @@ struct TpcBuffers {
   tpc_track_fit* track_fit;// [max_tracks] sector-track refit (R8)
 };
 
+// Buffers of the track merging (R9), pointers into the caller's merge workspace.
+struct TpcMergeBuffers {
+  tpc_merge_params P;
+  uint32_t n_tracks, n_ids, n_rows, n_cells;
+  float inv_w;            // 1 / width of a z slab of the end grid (= 1 / pre_dz)
+  float ca, sa;           // cos / sin of one sector step (tables: double, rounded once)
+  uint32_t* cell_start;   // [n_cells+1] inner ends per (sector, first row, z slab) -> exclusive scan
+  uint32_t* cell_cursor;  // [n_cells]
+  uint32_t* partials;     // scan scratch
+  float* ends;            // [n_tracks][16] compact inner-end records in cell order
+  int32_t* next; int32_t* prev; float* link_chi2;                  // [n_tracks]
+  int32_t* best_out; uint32_t* best_out_chi; uint32_t* best_in_chi; unsigned long long* best_in_key;
+  uint32_t* head_ofs; uint32_t* seg_ofs; uint32_t* clu_ofs; uint32_t* seg_dst;   // [n_tracks]
+  tpc_merged_track* merged;  // [n_tracks]
+  uint32_t* seg_index;       // [n_tracks]
+  uint32_t* ids; uint8_t* shared;   // [n_ids]
+  uint32_t* counters;        // [4] n_merged, n_links, n_ids out, -
+};
+
 #define TPC_MAX_KERNELS 32
 struct TpcStageEvents {
   cudaEvent_t ev[TPC_N_STAGES];  // boundaries: start, after grid, nf, seeds, follower, selector
@@ -135,10 +154,12 @@ struct TpcStageEvents {
 };
 
 namespace tpc_det {
+int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
+int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }

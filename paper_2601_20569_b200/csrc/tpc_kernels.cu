@@ -2192,10 +2192,12 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
     const int n = t->n_clusters;
     tpc_track_fit out;
     out.x = 0.f; out.chi2 = 0.f; out.n_clusters = (uint32_t)n; out.flags = 1u;
+    out.x_out = 0.f; out.pad_[0] = out.pad_[1] = out.pad_[2] = 0u;
 #pragma unroll
-    for (int i = 0; i < 5; ++i) out.p[i] = 0.f;
+    for (int i = 0; i < 5; ++i) { out.p[i] = 0.f; out.p_out[i] = 0.f; }
 #pragma unroll
-    for (int i = 0; i < 15; ++i) out.c[i] = 0.f;
+    for (int i = 0; i < 15; ++i) { out.c[i] = 0.f; out.c_out[i] = 0.f; }
+    int r_last = 0;
     auto rec = [&](int i, float& y, float& z, int& row) {
       const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + (ids[i] - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); row = (int)((raw.w >> 8) & 0xFF);
@@ -2229,6 +2231,13 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
         if (kf_update(k, g, ym, zm, F)) ok = false;
         snap_s = k.s; snap_t = k.t; snap_q = k.q;
       }
+      if (ok) {  // the outer end (R9 extends it): the state after the outward pass at the last cluster
+        r_last = r;
+        out.p_out[0] = k.y; out.p_out[1] = k.z; out.p_out[2] = k.s; out.p_out[3] = k.t; out.p_out[4] = k.q;
+        out.c_out[0] = k.c00; out.c_out[1] = k.c10; out.c_out[2] = k.c11; out.c_out[3] = k.c20; out.c_out[4] = k.c21;
+        out.c_out[5] = k.c22; out.c_out[6] = k.c30; out.c_out[7] = k.c31; out.c_out[8] = k.c32; out.c_out[9] = k.c33;
+        out.c_out[10] = k.c40; out.c_out[11] = k.c41; out.c_out[12] = k.c42; out.c_out[13] = k.c43; out.c_out[14] = k.c44;
+      }
       if (ok) {  // R8.3 turn
         k.y = ym; k.z = zm; k.s = snap_s; k.t = snap_t; k.q = snap_q;
         kf_init_cov(k, F);
@@ -2251,10 +2260,279 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
         out.c[6] = k.c30; out.c[7] = k.c31; out.c[8] = k.c32; out.c[9] = k.c33;
         out.c[10] = k.c40; out.c[11] = k.c41; out.c[12] = k.c42; out.c[13] = k.c43; out.c[14] = k.c44;
         out.chi2 = chi2;
+        out.x_out = B.K->x[r_last];
         out.flags = 0u;
       }
     }
     B.track_fit[ti] = out;
+  }
+}
+
+// ================================================================== R9 track merging
+// PAPER.md:29 (section 2): "merges tracks first inside the TPC sectors, then between adjacent
+// sectors of the TPC halves, and then across the central electrode"; on top of the
+// sector-track refit.  DESIGN.md reading R9.  Layout of the work:
+//   k_merge_bin_*   the INNER ends of the tracks with a valid refit are binned by (sector, first row,
+//                   z slab of pre_dz) -- a counting sort that also lays down compact 64-byte records
+//                   (state, diagonal variances, tie-break key, track index) in cell order;
+//   k_merge_sweep   one thread per track a with a free outer end carries its outer state along the
+//                   stage's path (row steps / rotation + one step) and looks the candidates of every
+//                   row it reaches up in the cells around its own z.  Pass 1: own best partner and
+//                   atomicMin of chi2 on the partner's word; pass 2 (same sweep again): the tracks that
+//                   hold a partner's minimum chi2 settle exact ties by their 64-bit key;
+//   k_merge_link    mutual choice -> next / prev;
+//   k_merge_chain_* chains -> merged records, segment lists, concatenated cluster lists.
+#define TPC_MG_ZB 1024   // z slabs per (sector,row), periodic (a slab is pre_dz wide)
+
+__device__ __forceinline__ unsigned long long merge_key(const tpc_track& t) {
+  return ((unsigned long long)t.sector << 41) | ((unsigned long long)((t.flags >> 1) & 1u) << 40) |
+         ((unsigned long long)t.seed_id << 8) | (unsigned long long)t.segment;
+}
+__device__ __forceinline__ uint32_t merge_cell(const TpcMergeBuffers& M, uint32_t sector, uint32_t row, float z) {
+  const int zb = ((int)floorf(z * M.inv_w)) & (TPC_MG_ZB - 1);
+  return (sector * M.n_rows + row) * TPC_MG_ZB + (uint32_t)zb;
+}
+
+__global__ void __launch_bounds__(256) k_merge_init(TpcBuffers B, TpcMergeBuffers M) {
+  const uint32_t stride = gridDim.x * blockDim.x, i0 = blockIdx.x * blockDim.x + threadIdx.x;
+  for (uint32_t c = i0; c < M.n_cells + 1; c += stride) M.cell_start[c] = 0u;
+  for (uint32_t t = i0; t < M.n_tracks; t += stride) { M.next[t] = -1; M.prev[t] = -1; M.link_chi2[t] = 0.f; }
+  if (i0 < 4) M.counters[i0] = 0u;
+}
+__global__ void __launch_bounds__(256) k_merge_bin_count(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
+    const tpc_track_fit* f = B.track_fit + t;
+    if (f->flags) continue;
+    atomicAdd(&M.cell_start[merge_cell(M, B.tracks[t].sector, B.tracks[t].row_first, f->p[1])], 1u);
+  }
+}
+// exclusive scan of a[0..n) in blocks of 1024: local prefixes in place, block totals to partials
+__global__ void __launch_bounds__(1024) k_scan_blocks(uint32_t* a, uint32_t n, uint32_t* partials) {
+  __shared__ uint32_t sm[33];
+  const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
+  const uint32_t v = i < n ? a[i] : 0u;
+  uint32_t tot;
+  const uint32_t pre = block_excl_scan(v, &tot, sm);
+  if (i < n) a[i] = pre;
+  if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(1024) k_scan_top(uint32_t* partials, uint32_t n_blocks, uint32_t* total_out) {
+  __shared__ uint32_t sm[33];
+  uint32_t carry = 0;
+  for (uint32_t b0 = 0; b0 < n_blocks; b0 += 1024) {
+    const uint32_t b = b0 + threadIdx.x;
+    const uint32_t v = b < n_blocks ? partials[b] : 0u;
+    uint32_t tot;
+    const uint32_t pre = block_excl_scan(v, &tot, sm);
+    if (b < n_blocks) partials[b] = carry + pre;
+    carry += tot;
+  }
+  if (threadIdx.x == 0 && total_out) *total_out = carry;
+}
+__global__ void __launch_bounds__(1024) k_scan_add(uint32_t* a, uint32_t n, const uint32_t* partials, uint32_t* end_out) {
+  const uint32_t i = blockIdx.x * 1024u + threadIdx.x;
+  if (i < n) a[i] += partials[blockIdx.x];
+  (void)end_out;
+}
+__global__ void __launch_bounds__(256) k_merge_bin_fill(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
+    const tpc_track_fit* f = B.track_fit + t;
+    if (f->flags) continue;
+    const tpc_track tr = B.tracks[t];
+    const uint32_t cell = merge_cell(M, tr.sector, tr.row_first, f->p[1]);
+    const uint32_t pos = M.cell_start[cell] + atomicAdd(&M.cell_cursor[cell], 1u);
+    const unsigned long long key = merge_key(tr);
+    uint4* rec = reinterpret_cast<uint4*>(M.ends + (size_t)pos * 16);
+    rec[0] = make_uint4(__float_as_uint(f->p[0]), __float_as_uint(f->p[1]), __float_as_uint(f->p[2]), __float_as_uint(f->p[3]));
+    rec[1] = make_uint4(__float_as_uint(f->p[4]), __float_as_uint(f->c[0]), __float_as_uint(f->c[2]), __float_as_uint(f->c[5]));
+    rec[2] = make_uint4(__float_as_uint(f->c[9]), __float_as_uint(f->c[14]), (uint32_t)key, (uint32_t)(key >> 32));
+    rec[3] = make_uint4(t, 0u, 0u, 0u);
+  }
+}
+__global__ void __launch_bounds__(256) k_merge_stage_reset(TpcMergeBuffers M) {
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
+    M.best_out[t] = -1; M.best_out_chi[t] = 0xFFFFFFFFu; M.best_in_chi[t] = 0xFFFFFFFFu; M.best_in_key[t] = ~0ull;
+  }
+}
+
+// rotation of a state at local x into the neighbouring sector's frame (sa carries the sign): same
+// point, direction phi' = phi - alpha, parameters on the plane x' = const through the point;
+// first-order Jacobian dy'/dy = ca - sa*tan(phi'), dz'/dy = -sa*t/cos(phi'), ds'/ds = ca + sa*s/cos(phi)
+__device__ __forceinline__ bool merge_rotate(KF& k, float& x, float ca, float sa, float max_sinphi) {
+  const float s = k.s;
+  const float cphi = sqrtf(1.f - s * s);
+  const float s1 = s * ca - cphi * sa;
+  if (!(fabsf(s1) <= max_sinphi)) return false;
+  const float cphi1 = sqrtf(1.f - s1 * s1);
+  const float xn = x * ca + k.y * sa;
+  const float yn = k.y * ca - x * sa;
+  const float a = ca - sa * (s1 / cphi1);
+  const float b = -(sa * (k.t / cphi1));
+  const float r = ca + sa * (s / cphi);
+  const float c00 = k.c00, c10 = k.c10, c11 = k.c11, c20 = k.c20, c21 = k.c21, c22 = k.c22;
+  const float c30 = k.c30, c31 = k.c31, c32 = k.c32, c40 = k.c40, c41 = k.c41, c42 = k.c42;
+  k.c00 = (a * a) * c00;
+  k.c10 = a * (b * c00 + c10);
+  k.c11 = ((b * b) * c00 + (2.f * b) * c10) + c11;
+  k.c20 = (a * r) * c20;
+  k.c21 = r * (b * c20 + c21);
+  k.c22 = (r * r) * c22;
+  k.c30 = a * c30;
+  k.c31 = b * c30 + c31;
+  k.c32 = r * c32;
+  k.c40 = a * c40;
+  k.c41 = b * c40 + c41;
+  k.c42 = r * c42;
+  x = xn; k.y = yn; k.s = s1;
+  return true;
+}
+
+template <int STAGE, int PASS>
+__global__ void __launch_bounds__(128) k_merge_sweep(TpcBuffers B, TpcMergeBuffers M, const __grid_constant__ FollowConst F) {
+  const tpc_merge_params& P = M.P;
+  const int R = (int)M.n_rows;
+  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < M.n_tracks; a += gridDim.x * blockDim.x) {
+    if (M.next[a] >= 0) continue;                      // outer end already linked by an earlier stage
+    const tpc_track_fit* fa = B.track_fit + a;
+    if (fa->flags) continue;
+    const tpc_track ta = B.tracks[a];
+    const unsigned long long key_a = merge_key(ta);
+    const int la = ta.row_last;
+    const float za_out = fa->p_out[1];
+    KF k0;
+    k0.y = fa->p_out[0]; k0.z = fa->p_out[1]; k0.s = fa->p_out[2]; k0.t = fa->p_out[3]; k0.q = fa->p_out[4];
+    k0.c00 = fa->c_out[0]; k0.c10 = fa->c_out[1]; k0.c11 = fa->c_out[2]; k0.c20 = fa->c_out[3]; k0.c21 = fa->c_out[4];
+    k0.c22 = fa->c_out[5]; k0.c30 = fa->c_out[6]; k0.c31 = fa->c_out[7]; k0.c32 = fa->c_out[8]; k0.c33 = fa->c_out[9];
+    k0.c40 = fa->c_out[10]; k0.c41 = fa->c_out[11]; k0.c42 = fa->c_out[12]; k0.c43 = fa->c_out[13]; k0.c44 = fa->c_out[14];
+    int32_t best = -1;
+    float best_chi2 = 0.f;
+    unsigned long long best_key = 0ull;
+    // candidates on row `row` of sector `sb` for the transported state k
+    auto visit = [&](uint32_t sb, int row, const KF& k) {
+      const float zc = STAGE == 3 ? -k.z : k.z;
+      const int zb0 = (int)floorf(((zc - P.pre_dz) - 0.01f) * M.inv_w), zb1 = (int)floorf(((zc + P.pre_dz) + 0.01f) * M.inv_w);   // (margin: rounding never hides a candidate; the cuts below decide)
+      for (int zb = zb0; zb <= zb1; ++zb) {
+        const uint32_t cell = (sb * M.n_rows + (uint32_t)row) * TPC_MG_ZB + (uint32_t)(zb & (TPC_MG_ZB - 1));
+        const uint32_t e1 = M.cell_start[cell + 1];
+        for (uint32_t e = M.cell_start[cell]; e < e1; ++e) {
+          const uint4* rec = reinterpret_cast<const uint4*>(M.ends + (size_t)e * 16);
+          const uint4 r0 = rec[0];
+          const float yb = __uint_as_float(r0.x), zbv = __uint_as_float(r0.y);
+          // pre-cuts: coarse on the end states as they are, fine on the transported state
+          const float dzc = STAGE == 3 ? zbv + za_out : zbv - za_out;
+          if (!(fabsf(dzc) <= P.pre_coarse_dz)) continue;
+          const float dzf = STAGE == 3 ? zbv + k.z : zbv - k.z;
+          if (!(fabsf(dzf) <= P.pre_dz)) continue;
+          if (!(fabsf(yb - k.y) <= P.pre_dy)) continue;
+          const uint4 r1 = rec[1], r2 = rec[2];
+          const uint32_t b = rec[3].x;
+          if (b == a || M.prev[b] >= 0) continue;        // inner end already linked by an earlier stage
+          const float pb[5] = {yb, zbv, __uint_as_float(r0.z), __uint_as_float(r0.w), __uint_as_float(r1.x)};
+          const float vb[5] = {__uint_as_float(r1.y), __uint_as_float(r1.z), __uint_as_float(r1.w), __uint_as_float(r2.x),
+                               __uint_as_float(r2.y)};
+          const float pa[5] = {k.y, k.z, k.s, k.t, k.q};
+          const float va[5] = {k.c00, k.c11, k.c22, k.c33, k.c44};
+          float chi2 = 0.f;
+#pragma unroll
+          for (int i = 0; i < 5; ++i) {
+            float d = pb[i] - pa[i];
+            float sys = P.sys[i];
+            if (i == 1 && STAGE == 3) { d = pb[1] + pa[1]; sys = P.ce_sys_z; }
+            const float var = (va[i] + vb[i]) + sys * sys;
+            chi2 = chi2 + (d * d) / var;
+          }
+          if (!(chi2 <= P.chi2_max)) continue;
+          const unsigned long long key_b = ((unsigned long long)r2.w << 32) | r2.z;
+          if (PASS == 1) {
+            if (best < 0 || chi2 < best_chi2 || (chi2 == best_chi2 && key_b < best_key)) {
+              best = (int32_t)b; best_chi2 = chi2; best_key = key_b;
+            }
+            atomicMin(&M.best_in_chi[b], __float_as_uint(chi2));      // chi2 >= 0: bit order = value order
+          } else if (__float_as_uint(chi2) == M.best_in_chi[b]) {
+            atomicMin(&M.best_in_key[b], key_a);
+          }
+        }
+      }
+    };
+    if (STAGE == 2) {
+      const uint32_t side = ta.sector / 18u, s18 = ta.sector % 18u;
+      for (int dir = 0; dir < 2; ++dir) {
+        const uint32_t sb = side * 18u + (dir == 0 ? (s18 + 1u) % 18u : (s18 + 17u) % 18u);
+        if (sb >= B.n_sectors) continue;
+        KF kr = k0;
+        float xr = B.K->x[la];
+        if (!merge_rotate(kr, xr, M.ca, dir == 0 ? M.sa : -M.sa, F.max_sinphi)) continue;
+        const int r_lo = max(0, la - P.gap_adjacent_back), r_hi = min(R - 1, la + P.gap_adjacent);
+        for (int row = r_lo; row <= r_hi; ++row) {
+          KF k = kr;
+          if (!kf_propagate(k, B.K->x[row] - xr, F)) continue;
+          visit(sb, row, k);
+        }
+      }
+    } else {
+      const uint32_t sb = STAGE == 1 ? ta.sector : (ta.sector < 18u ? ta.sector + 18u : ta.sector - 18u);
+      if (sb < B.n_sectors) {
+        KF k = k0;
+        const int G = STAGE == 1 ? P.gap_in_sector : P.gap_ce;
+        for (int g = 1; g <= G && la + g < R; ++g) {
+          if (!kf_propagate(k, F.dx, F)) break;
+          visit(sb, la + g, k);
+        }
+      }
+    }
+    if (PASS == 1) { M.best_out[a] = best; M.best_out_chi[a] = __float_as_uint(best_chi2); }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_merge_link(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < M.n_tracks; a += gridDim.x * blockDim.x) {
+    const int32_t b = M.best_out[a];
+    if (b < 0) continue;
+    if (M.best_out_chi[a] == M.best_in_chi[b] && M.best_in_key[b] == merge_key(B.tracks[a])) {
+      M.next[a] = b; M.prev[b] = (int32_t)a;
+      M.link_chi2[a] = __uint_as_float(M.best_out_chi[a]);
+      atomicAdd(&M.counters[1], 1u);
+    }
+  }
+}
+
+// chains: per head the number of segments / clusters -> three scans -> records, lists
+__global__ void __launch_bounds__(256) k_merge_chain_count(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
+    uint32_t ns = 0, nc = 0;
+    if (M.prev[t] < 0) {
+      for (int32_t k = (int32_t)t; k >= 0; k = M.next[k]) { ++ns; nc += B.tracks[k].n_clusters; }
+    }
+    M.head_ofs[t] = ns ? 1u : 0u; M.seg_ofs[t] = ns; M.clu_ofs[t] = nc;
+  }
+}
+__global__ void __launch_bounds__(256) k_merge_chain_emit(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
+    if (M.prev[t] >= 0) continue;
+    tpc_merged_track m;
+    m.head = t; m.n_segments = 0; m.n_clusters = 0; m.n_shared = 0;
+    m.cluster_ofs = M.clu_ofs[t]; m.seg_ofs = M.seg_ofs[t];
+    m.row_first = B.tracks[t].row_first; m.sector_first = B.tracks[t].sector;
+    m.row_last = 0; m.sector_last = 0;
+    for (int32_t k = (int32_t)t; k >= 0; k = M.next[k]) {
+      const tpc_track tk = B.tracks[k];
+      M.seg_index[m.seg_ofs + m.n_segments] = (uint32_t)k;
+      M.seg_dst[k] = m.cluster_ofs + m.n_clusters;
+      ++m.n_segments; m.n_clusters += tk.n_clusters; m.n_shared += tk.n_shared;
+      m.row_last = tk.row_last; m.sector_last = tk.sector;
+    }
+    M.merged[M.head_ofs[t]] = m;
+  }
+}
+__global__ void __launch_bounds__(256) k_merge_copy_ids(TpcBuffers B, TpcMergeBuffers M) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+  for (uint32_t t = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < M.n_tracks; t += n_warps) {
+    const uint32_t src = B.tracks[t].cluster_ofs, n = B.tracks[t].n_clusters, dst = M.seg_dst[t];
+    for (uint32_t i = lane; i < n; i += 32) {
+      M.ids[dst + i] = B.cluster_ids[src + i];
+      M.shared[dst + i] = B.cluster_shared[src + i];
+    }
   }
 }
 
@@ -2291,6 +2569,48 @@ int run_refit(const TpcBuffers& B, const TpcConst* hK, uint32_t n_tracks, cudaSt
   const FollowConst F = follow_const(hK);
   k_track_refit<<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit, 128)), 128, 0, st>>>(B, F, n_tracks);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+static inline void scan_u32(uint32_t* a, uint32_t n, uint32_t* partials, uint32_t* total_out, cudaStream_t st) {
+  const uint32_t nb = (n + 1023u) / 1024u;
+  if (!nb) return;
+  k_scan_blocks<<<nb, 1024, 0, st>>>(a, n, partials);
+  k_scan_top<<<1, 1024, 0, st>>>(partials, nb, total_out);
+  k_scan_add<<<nb, 1024, 0, st>>>(a, n, partials, nullptr);
+}
+
+// Returns the number of kernels launched, or -1 on a launch error.
+int run_merge(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, cudaStream_t st, int n_sm) {
+  const FollowConst F = follow_const(hK);
+  int launches = 0;
+  const int g256 = grid_for((uint64_t)M.n_tracks + 1, 256, n_sm, 8);
+  k_merge_init<<<grid_for((uint64_t)M.n_cells + 1, 256, n_sm, 8), 256, 0, st>>>(B, M);
+  cudaMemsetAsync(M.cell_cursor, 0, 4 * (size_t)M.n_cells, st);
+  ++launches;
+  if (M.n_tracks) {
+    k_merge_bin_count<<<g256, 256, 0, st>>>(B, M);
+    scan_u32(M.cell_start, M.n_cells + 1, M.partials, nullptr, st);
+    k_merge_bin_fill<<<g256, 256, 0, st>>>(B, M);
+    launches += 5;
+    const int gs = grid_for(M.n_tracks, 128, n_sm, 8);
+    for (int stage = 1; stage <= 3; ++stage) {
+      if (!((M.P.stages >> (stage - 1)) & 1)) continue;
+      k_merge_stage_reset<<<g256, 256, 0, st>>>(M);
+      if (stage == 1) { k_merge_sweep<1, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<1, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      if (stage == 2) { k_merge_sweep<2, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<2, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      if (stage == 3) { k_merge_sweep<3, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<3, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      k_merge_link<<<g256, 256, 0, st>>>(B, M);
+      launches += 4;
+    }
+    k_merge_chain_count<<<g256, 256, 0, st>>>(B, M);
+    scan_u32(M.head_ofs, M.n_tracks, M.partials, &M.counters[0], st);
+    scan_u32(M.seg_ofs, M.n_tracks, M.partials, nullptr, st);
+    scan_u32(M.clu_ofs, M.n_tracks, M.partials, &M.counters[2], st);
+    k_merge_chain_emit<<<g256, 256, 0, st>>>(B, M);
+    k_merge_copy_ids<<<grid_for((uint64_t)M.n_tracks * 32, 256, n_sm, 8), 256, 0, st>>>(B, M);
+    launches += 12;
+  }
+  return cudaPeekAtLastError() == cudaSuccess ? launches : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

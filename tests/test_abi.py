@@ -26,6 +26,10 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.Params) == 120
     assert B.Params.max_bins.offset == 96 and B.Params.max_seeds.offset == 104
     assert ctypes.sizeof(B.TrackView) == 184 and ctypes.sizeof(B.DebugView) == 136
+    assert B.TRACK_FIT_DTYPE.itemsize == 192 and B.MERGED_DTYPE.itemsize == 40
+    assert ctypes.sizeof(B.MergeParams) == 60 and ctypes.sizeof(B.MergedView) == 88
+    m = B.tpc_merge_default_params()
+    assert m.gap_in_sector == 30 and abs(m.chi2_max - 20.0) < 1e-6 and m.stages == 7
 
 
 def test_host_only_calls_without_gpu():

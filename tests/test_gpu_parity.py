@@ -610,3 +610,138 @@ def test_det_parity_sector_track_refit(B, name):
     # segments whose parameters were stale now carry parameters at their own innermost row
     x_rows, _, _, _ = oracle.geom_tables()
     assert (fit["x"][ok] == x_rows[tracks["row_first"][ok]]).all()
+
+
+def _canonical_merged(tracks, merged, seg_index, ids, shared):
+    """Merged tracks keyed by their head's (iteration, sector, seed id, segment); per merged track the
+    segment keys in chain order and the concatenated cluster list."""
+    it = (tracks["flags"].astype(np.int64) >> 1) & 1
+    key = (it << 56) | (tracks["sector"].astype(np.int64) << 48) | (tracks["seed_id"].astype(np.int64) << 8) | tracks["segment"].astype(np.int64)
+    out = {}
+    for m in merged:
+        segs = seg_index[int(m["seg_ofs"]):int(m["seg_ofs"]) + int(m["n_segments"])]
+        o, n = int(m["cluster_ofs"]), int(m["n_clusters"])
+        out[int(key[int(m["head"])])] = (tuple(int(key[k]) for k in segs), ids[o:o + n].tobytes(), shared[o:o + n].tobytes(),
+                                         int(m["n_shared"]), int(m["row_first"]), int(m["row_last"]),
+                                         int(m["sector_first"]), int(m["sector_last"]))
+    return out
+
+
+@pytest.mark.parametrize("name", ["C2_full", "C3_reduced", "C4_reduced", "C5_two_iterations", "ce_crossing"])
+def test_det_parity_track_merging(B, name):
+    """sector-track refit with both end states, then the three
+    merging stages; deterministic mode, links / chains / cluster lists identical to oracle.merging."""
+    from oracle import merging
+    two = False
+    if name == "C2_full":
+        cl, lab, _ = dg.generate(dg.preset("C2"))
+        pkw = {}
+    elif name == "C3_reduced":
+        cl, lab, _ = dg.generate(dg.preset("C3", tracks_per_event=500))
+        pkw = {}
+    elif name == "C4_reduced":
+        cl, lab, _ = dg.generate(dg.preset("C4", n_events=6, tracks_per_event=1500, t_window_us=120.0))
+        pkw = dict(grid_dz=8.0, max_bins=200_000_000)
+    elif name == "C5_two_iterations":
+        cl, lab, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+        two = True
+    else:
+        x, _, _, _ = oracle.geom_tables()
+        xm = 0.5 * (float(x[61]) + float(x[62]))
+        recs = []
+        for k in range(40):                                   # 40 electrode-crossing tracks side by side in z-time
+            for r in range(20, 101):
+                zt = 0.5 * (xm - float(x[r]))
+                recs.append((3, r, -12.0 + 0.6 * k, zt - 30.0 - 7.0 * k) if r <= 61 else (21, r, -12.0 + 0.6 * k, zt + 30.0 + 7.0 * k))
+        cl = np.zeros(len(recs), dtype=oracle.CLUSTER_DTYPE)
+        a = np.array(recs)
+        order = np.lexsort((a[:, 1], a[:, 0]))
+        cl["sector"], cl["row"], cl["y"], cl["z"] = a[order, 0], a[order, 1], a[order, 2], a[order, 3]
+        pkw = {}
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        d = trk.upload(cl)
+        if two:
+            trk.track_two_iterations(d, flags=1)
+        else:
+            trk.track(d, flags=1)
+        tracks, ids, shared, view = trk.tracks()
+        fit = trk.refit()
+        g = trk.merge()
+    finally:
+        trk.close()
+    if two:
+        from oracle import second_iteration as si
+        o = si.run_two_iterations(cl, params=op, n_threads=NT)
+    else:
+        o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
+    assert len(tracks) == o.n_tracks
+    # the outer-end states of the refit, track by track (canonical order on both sides)
+    it = (tracks["flags"].astype(np.int64) >> 1) & 1
+    g_order = np.lexsort((tracks["segment"], tracks["seed_id"], tracks["sector"], it))
+    ito = (o.tracks["flags"].astype(np.int64) >> 1) & 1
+    o_order = np.lexsort((o.tracks["segment"], o.tracks["seed_id"], o.tracks["sector"], ito))
+    fg, fo = fit[g_order], m.fit[o_order]
+    assert (fg["flags"] == fo["flags"]).all()
+    ok = fo["flags"] == 0
+    for f in ("x", "p", "c", "chi2", "x_out", "p_out", "c_out"):
+        a_, b_ = np.ascontiguousarray(fg[f][ok]).view(np.uint32), np.ascontiguousarray(fo[f][ok]).view(np.uint32)
+        assert (a_ == b_).all(), (f, int((a_ != b_).sum()))
+    # links, chains, lists
+    assert int(g["view"].n_links) == int((m.next >= 0).sum())
+    assert len(g["merged"]) == len(m.merged)
+    cg = _canonical_merged(tracks, g["merged"], g["seg_index"], g["cluster_ids"], g["cluster_shared"])
+    co = _canonical_merged(o.tracks, m.merged, m.seg_index, m.cluster_ids, m.cluster_shared)
+    assert cg.keys() == co.keys()
+    bad = [k for k in cg if cg[k] != co[k]]
+    assert not bad, (len(bad), cg[bad[0]][0], co[bad[0]][0])
+    # link chi2 bit-exact (by head key of the link's inner track)
+    kg = {(int(it[k]), int(tracks["sector"][k]), int(tracks["seed_id"][k]), int(tracks["segment"][k])): np.float32(g["link_chi2"][k]).view(np.uint32)
+          for k in np.flatnonzero(g["next"] >= 0)}
+    ko = {(int(ito[k]), int(o.tracks["sector"][k]), int(o.tracks["seed_id"][k]), int(o.tracks["segment"][k])): np.float32(m.link_chi2[k]).view(np.uint32)
+          for k in np.flatnonzero(m.next >= 0)}
+    assert kg == ko
+    if name == "ce_crossing":
+        assert len(m.merged) == 40 and (m.merged["sector_last"] == 21).all()
+    elif name != "C5_two_iterations":
+        assert (m.next >= 0).sum() > 50
+        stages_seen = set()
+        for a_, b_ in zip(np.flatnonzero(m.next >= 0), m.next[m.next >= 0]):
+            stages_seen.add(1 if o.tracks["sector"][a_] == o.tracks["sector"][b_] else 2)
+        assert stages_seen == {1, 2}
+
+
+def test_fast_mode_track_merging_quality(B):
+    """Fast build: the merged result is close to the oracle's (links decided within rounding of the cut
+    may differ) and the clone rate falls as in the oracle."""
+    from oracle import merging
+    base = dg.preset("C4")
+    cl, lab, _ = dg.generate(dg.preset("C4", n_events=20, t_window_us=base.t_window_us * 20 / base.n_events))
+    import bench
+    pkw = dict(bench.WORKLOAD_PARAMS["C4"])
+    sel = cl["sector"] < 4
+    cl, lab = cl[sel], lab[sel]
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        trk.track(trk.upload(cl), flags=0)
+        tracks, ids, shared, view = trk.tracks()
+        trk.refit()
+        g = trk.merge()
+    finally:
+        trk.close()
+    o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
+    q0 = quality(tracks, ids, lab)
+    qg = track_quality(g["merged"]["n_clusters"], g["merged"]["cluster_ofs"], g["cluster_ids"], g["merged"]["sector_first"], lab)
+    qo = track_quality(m.merged["n_clusters"], m.merged["cluster_ofs"], m.cluster_ids, m.merged["sector_first"], lab)
+    report("merge_C4_20_events", {"links_gpu": int(g["view"].n_links), "links_oracle": int((m.next >= 0).sum()),
+                                  "clone_before": q0["clone_rate"], "clone_gpu": qg["clone_rate"], "clone_oracle": qo["clone_rate"],
+                                  "eff_before": q0["efficiency"], "eff_gpu": qg["efficiency"], "eff_oracle": qo["efficiency"],
+                                  "fake_before": q0["fake_rate"], "fake_gpu": qg["fake_rate"], "fake_oracle": qo["fake_rate"]})
+    assert abs(int(g["view"].n_links) - int((m.next >= 0).sum())) <= 0.01 * max(1, (m.next >= 0).sum())
+    assert abs(qg["clone_rate"] - qo["clone_rate"]) <= 0.002 and abs(qg["efficiency"] - qo["efficiency"]) <= 0.002
+    assert qg["clone_rate"] < q0["clone_rate"] - 0.01

@@ -225,7 +225,7 @@ def test_stage1_links_equal_a_plain_python_implementation():
                 gap = int(mt["row_first"][b]) - int(mt["row_last"][a])
                 if a == b or gap < 1 or gap > mp.gap_in_sector:
                     continue
-                if not abs(f32(mt["p_in"][b][1]) - f32(mt["p_out"][a][1])) <= mp.pre_dz:
+                if not abs(f32(mt["p_in"][b][1]) - f32(mt["p_out"][a][1])) <= mp.pre_coarse_dz:
                     continue
                 st = np.concatenate([mt["p_out"][a], mt["c_out"][a]]).astype(f32)
                 ok = True
@@ -234,6 +234,8 @@ def test_stage1_links_equal_a_plain_python_implementation():
                     if not ok:
                         break
                 if not ok:
+                    continue
+                if not (abs(f32(mt["p_in"][b][1] - st[1])) <= mp.pre_dz and abs(f32(mt["p_in"][b][0] - st[0])) <= mp.pre_dy):
                     continue
                 c2 = f32(0)
                 for i in range(5):
