@@ -332,20 +332,7 @@ def run_ours(args, rank, world, local_rank):
     stage_ms = trk.stage_ms()
     value = n_all * args.steps / (ms_total * 1e-3)
 
-    # ---- sector-track refit of the frame's tracks (first half; not part of `value`)
     refit = None
-    if args.refit and not args.second_iteration:
-        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        with torch.cuda.stream(stream):
-            B.tpc_refit_tracks(trk.ctx, stream.cuda_stream); B.tpc_get_refit(trk.ctx)      # warm-up
-            r0.record(stream)
-            for _ in range(args.steps):
-                B.tpc_refit_tracks(trk.ctx, stream.cuda_stream)
-            r1.record(stream)
-            B.tpc_get_refit(trk.ctx)
-        torch.cuda.synchronize()
-        ms = r0.elapsed_time(r1) / args.steps
-        refit = {"ms": ms, "tracks": int(v.n_tracks), "clusters_refitted_per_s": int(v.n_cluster_ids) / (ms * 1e-3)}
 
     if args.second_iteration:
         # reduced line: kernel times / roofline would describe the second pass only
@@ -477,12 +464,83 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N=1 only)
     cpu = None
+    cpu_all = None
+    cpu_o, cpu_lo, cpu_hi = None, 0, 0
     if world == 1 and not args.no_cpu_baseline:
         lo, hi, n_sample = oracle_sample(clusters, args.oracle_budget)
         dt, o = time_oracle(clusters, args.workload, lo, hi)
+        cpu_o, cpu_lo, cpu_hi = o, lo, hi
+        names = ("grid", "neighbours", "cleanup_seeds", "follower", "selector")
         cpu = {"value": n_sample / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
                "sample": f"sectors [{lo},{hi}) of the same {args.workload} frame: {n_sample} of {n} clusters, "
-                         "single thread"}
+                         "single thread",
+               "stage_seconds": {k: round(float(x), 3) for k, x in zip(names, o.stage_seconds)}}
+        # the same oracle with the sectors spread over all host cores (one sector per thread)
+        ncores = os.cpu_count() or 1
+        per_sector = np.bincount(clusters["sector"], minlength=36)
+        present = [s_ for s_ in range(len(per_sector)) if per_sector[s_]]
+        if len(present) > 1 and ncores > 1:
+            hi_all = present[min(ncores, len(present)) - 1] + 1
+            n_all_s = int(per_sector[present[0]:hi_all].sum())
+            n_thr = min(ncores, hi_all - present[0])
+            dta, _oa = time_oracle(clusters, args.workload, present[0], hi_all, n_threads=n_thr)
+            del _oa
+            cpu_all = {"value": n_all_s / dta, "unit": UNIT, "cores": n_thr, "host_cores": ncores, "kind": "oracle",
+                       "seconds": dta,
+                       "sample": f"sectors [{present[0]},{hi_all}) of the same frame on {n_thr} threads (one sector each): "
+                                 f"{n_all_s} of {n} clusters"}
+
+    # ---- further legs on the same resident frame (rank 0, N = 1; a few steps each; none is part of `value`)
+    extras = {}
+    parity_obj = None
+    if world == 1 and not args.no_extras:
+        ex_steps = max(1, min(args.steps, 3))
+
+        def timed(fn, sync):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                fn(); sync()
+                e0.record(stream)
+                for _ in range(ex_steps):
+                    fn()
+                e1.record(stream)
+                sync()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / ex_steps
+        # (1) the fast result of the sampled sectors against the oracle's (the parity sample of the headline build)
+        with torch.cuda.stream(stream):
+            trk.track(d_clusters, flags=flags & ~B.TPC_STAGE_TIMERS, stream=stream)
+            g_tracks, g_ids, g_shared, gv = trk.tracks()
+        if cpu is not None and args.mode == "fast":
+            from oracle import parity as op_
+            m = (g_tracks["sector"] >= cpu_lo) & (g_tracks["sector"] < cpu_hi)
+            stp = op_.compare_tracks_fast(g_tracks[m], g_ids, g_shared, cpu_o)
+            parity_obj = {"what": f"fast build vs oracle, tracks of sectors [{cpu_lo},{cpu_hi}) of this frame",
+                          **{k: stp[k] for k in ("n_gpu", "n_oracle", "n_paired_key", "n_paired_overlap", "n_list_diff",
+                                                 "n_param_bad", "max_rel")}}
+        # (2) sector-track refit + merging
+        ms_refit = timed(lambda: B.tpc_refit_tracks(trk.ctx, stream.cuda_stream), lambda: B.tpc_get_refit(trk.ctx))
+        extras["refit"] = {"ms": ms_refit, "tracks": int(gv.n_tracks), "clusters_refitted_per_s": int(gv.n_cluster_ids) / (ms_refit * 1e-3)}
+        refit = extras["refit"]
+        ms_merge = timed(lambda: trk.merge(stream=stream, fetch=False), lambda: B.tpc_get_merged(trk.ctx))
+        rc_m, mv = B.tpc_get_merged(trk.ctx)
+        extras["merge"] = {"ms": ms_merge, "links": int(mv.n_links), "merged_tracks": int(mv.n_merged),
+                           "note": "includes one stream synchronisation per call (track count to the host)"}
+        trk.merge_ws = None
+        # (3) deterministic mode on the same frame
+        if args.mode == "fast":
+            det_flags = (flags | B.TPC_DETERMINISTIC) & ~B.TPC_STAGE_TIMERS
+            ms_det = timed(lambda: trk.track(d_clusters, flags=det_flags, stream=stream), lambda: trk.counts())
+            extras["det"] = {"ms_per_step": ms_det, "clusters_per_s": n / (ms_det * 1e-3)}
+        # (4) the path + a second seeding iteration on the leftover clusters
+        try:
+            f2 = flags & ~B.TPC_STAGE_TIMERS
+            ms_two = timed(lambda: trk.track_two_iterations(d_clusters, flags=f2, stream=stream), lambda: trk.counts())
+            rc2, v2 = trk.counts()
+            extras["second_iteration"] = {"ms_per_step": ms_two, "n_tracks": int(v2.n_tracks),
+                                          "workspace_gb": B.tpc_workspace_bytes_two_iterations(trk.ctx, n) / 1e9}
+        except Exception as e:      # (the two-iteration workspace is more than twice the plain one)
+            extras["second_iteration"] = {"error": str(e)[:200]}
 
     idx = int(args.workload[1]) - 1
     line = {
@@ -502,7 +560,8 @@ def run_ours(args, rank, world, local_rank):
         "roofline": roof, "stages_hbm": stages,
         "stage_ms": {k: round(x, 4) for k, x in stage_ms.items()},
         "kernels_ms_per_step": {k["name"]: round(k["ms_per_step"], 4) for k in per_kernel},
-        "cpu_baseline": cpu, "refit": refit,
+        "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "refit": refit, "merge": extras.get("merge"),
+        "det": extras.get("det"), "second_iteration": extras.get("second_iteration"), "parity": parity_obj,
     }
     print(json.dumps(line), flush=True)
     trk.close()
@@ -528,7 +587,8 @@ def main():
                     help="clusters in the CPU oracle's bounded sample (~20 s single thread)")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="equal chunks of whole sectors in the end-to-end leg (1 = one shot, 0 = ramped schedule)")
     ap.add_argument("--e2e-cuts", default="", help="sector boundaries of the chunks of the end-to-end leg (overrides --e2e-chunks)")
-    ap.add_argument("--refit", action="store_true", help="also time tpc_refit_tracks on the frame's tracks (reported beside the metric)")
+    ap.add_argument("--refit", action="store_true", help="(kept for compatibility: the refit, merging, deterministic-mode and second-iteration legs run by default)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the refit / merging / det / second-iteration legs and the parity sample")
     ap.add_argument("--second-iteration", action="store_true",
                     help="time tpc_sector_track_two_iterations (the path + a second seeding iteration) instead")
     ap.add_argument("--no-cpu-baseline", action="store_true")
