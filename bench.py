@@ -246,6 +246,54 @@ def whole_job_value(n_local: float, ms_local: float, steps: int, world: int, dev
     return n_all * steps / (ms_total * 1e-3), ms_total
 
 
+# ------------------------------------------------------------------ ONE frame over N GPUs by sector
+def run_split_sectors(args, rank, world, local_rank, dev, barrier):
+    """SURVEY.md 8(e), first axis (`--split sectors` under torchrun): every rank tracks the sectors
+    s mod N == rank of the SAME frame (no collective inside the path), then one variable-length
+    gather brings tracks + cluster lists to rank 0 (paper_2601_20569_b200/multigpu.py).  Strong
+    scaling: value = the frame's clusters / (max over ranks of tracking + gather time)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2601_20569_b200 import binding as B, multigpu as mg
+    cfg, clusters, labels, gen_s = make_frame(args.workload, 0, args.events, args.tracks)   # the same frame on every rank
+    sub, delta = mg.split_by_sector(clusters, rank, world)
+    pkw = dict(WORKLOAD_PARAMS[args.workload])
+    trk = B.SectorTracker(params=B.tpc_default_params(**pkw), device=local_rank)
+    stream = torch.cuda.Stream(device=dev)
+    d_sub = trk.upload(sub)
+    flags = B.TPC_DETERMINISTIC if args.mode == "det" else 0
+
+    def step():
+        trk.track(d_sub, flags=flags, stream=stream)
+        tracks, ids, shared, v = trk.tracks()
+        tracks, ids = mg.rebase(tracks, ids, delta)
+        return mg.gather_to_root(tracks, ids, shared, rank, world, dev), v
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            step()
+    barrier()
+    t0 = time.perf_counter()
+    with torch.cuda.stream(stream):
+        for _ in range(args.steps):
+            res, v = step()
+    barrier()
+    ms_total = reduce_over_ranks((time.perf_counter() - t0) * 1e3, "max", world, dev)
+    launches = trk.launch_count() * args.steps
+    if rank == 0:
+        n = len(clusters)
+        print(json.dumps({
+            "metric": METRIC, "value": n * args.steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{args.workload}, one frame split by sector over {world} ranks + gather to rank 0",
+                       "n_clusters": n, "mode": args.mode, "n_tracks_gathered": int(len(res[0])),
+                       "timing": "host clock around tracking + result read-back + gather, max over ranks"},
+            "gpu_launches": launches}), flush=True)
+    trk.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
 # ------------------------------------------------------------------ the CUDA arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -272,6 +320,9 @@ def run_ours(args, rank, world, local_rank):
     def sum_over_ranks(x: float) -> float:
         return reduce_over_ranks(x, "sum", world, dev)
 
+    if args.split == "sectors" and world > 1:
+        run_split_sectors(args, rank, world, local_rank, dev, barrier)
+        return
     cfg, clusters, labels, gen_s = make_frame(args.workload, rank, args.events, args.tracks)
     n = len(clusters)
     flags = B.TPC_STAGE_TIMERS | (B.TPC_DETERMINISTIC if args.mode == "det" else 0)
@@ -592,6 +643,8 @@ def main():
     ap.add_argument("--second-iteration", action="store_true",
                     help="time tpc_sector_track_two_iterations (the path + a second seeding iteration) instead")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--split", default="frames", choices=("frames", "sectors"),
+                    help="N > 1: independent frames per rank (default, weak scaling) or ONE frame split by sector + gather")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -745,3 +745,30 @@ def test_fast_mode_track_merging_quality(B):
     assert abs(int(g["view"].n_links) - int((m.next >= 0).sum())) <= 0.01 * max(1, (m.next >= 0).sum())
     assert abs(qg["clone_rate"] - qo["clone_rate"]) <= 0.002 and abs(qg["efficiency"] - qo["efficiency"]) <= 0.002
     assert qg["clone_rate"] < q0["clone_rate"] - 0.01
+
+
+def test_sector_split_equals_whole_frame(B):
+    """SURVEY.md 8(e) first axis on one GPU: the sub-frames of 3 'ranks' (sectors s mod 3 == r)
+    tracked one after the other, rebased to frame indices and concatenated, equal the whole-frame
+    result and the oracle (the gather itself is covered under gloo, tests/test_multi_rank_gloo.py)."""
+    from paper_2601_20569_b200 import multigpu as mg
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=2000, seed=23))
+    parts = []
+    for r in range(3):
+        sub, delta = mg.split_by_sector(cl, r, 3)
+        tracks, ids, shared, view, _ = run_gpu(B, sub, None, 1)
+        tracks, ids = mg.rebase(tracks, ids, delta)
+        parts.append((tracks, ids, shared))
+    base = 0
+    tr_all = []
+    for tracks, ids, shared in parts:
+        t = tracks.copy()
+        t["cluster_ofs"] += np.uint32(base)
+        tr_all.append(t)
+        base += len(ids)
+    tracks = np.concatenate(tr_all)
+    ids = np.concatenate([p[1] for p in parts])
+    shared = np.concatenate([p[2] for p in parts])
+    o = oracle.run(cl, n_threads=NT, want=("tracks",))
+    assert parity.all_zero(parity.compare_tracks(tracks, ids, shared, o))
+    assert mg.gather_to_root(tracks, ids, shared, 0, 1)[0] is tracks
