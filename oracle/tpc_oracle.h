@@ -182,6 +182,25 @@ int orc_merge_links(const orc_geom* g, const orc_params* p, const orc_merge_para
  * (sign +1: the sector with the next higher azimuth); returns 0 if |sin phi| leaves the range */
 int orc_merge_rotate(const orc_geom* g, float* state20, float* x, int sign, float max_sinphi);
 
+/* ---- R10 three-iteration track fit with interpolation rejection (tpc_fit_oracle.cpp;
+ * PAPER.md:31,37 section 2, section 3) ---- */
+typedef struct orc_fit_params {
+  float fit_chi2_max;       /* (16) cut on the 2-dof chi2 of a cluster against the interpolation   */
+  int32_t fit_min_clusters; /* (10) fewer unmarked clusters: the fit fails                         */
+  float ce_var;             /* (1e4 cm^2) variance given to z when it is re-based at the electrode */
+} orc_fit_params;
+void orc_fit_default_params(orc_fit_params* f);
+/* IEEE binary16 round-to-nearest-even conversions ("reduced precision" of the stored predictions) */
+uint16_t orc_float_to_half(float f);
+float orc_half_to_float(uint16_t h);
+/* One track: n clusters in chain order (sector, row, y, z), start_stq = (sin phi, tan lambda, q/pT) at
+ * the outermost cluster.  out_state = x, p[5], c[15] at the innermost unmarked cluster's row;
+ * chi2_cluster[n] = interpolation chi2 of iteration 2; rejected[n] = 1 where marked; *n_used =
+ * unmarked clusters.  Returns the chi2 of iteration 3, or -1 if the fit failed. */
+float orc_fit_track(const orc_geom* g, const orc_params* p, const orc_fit_params* f, const int32_t* sector,
+                    const int32_t* row, const float* y, const float* z, int n, const float* start_stq,
+                    float* out_state, float* chi2_cluster, uint8_t* rejected, int32_t* n_used);
+
 #ifdef __cplusplus
 }
 #endif
