@@ -577,6 +577,13 @@ def run_ours(args, rank, world, local_rank):
         rc_m, mv = B.tpc_get_merged(trk.ctx)
         extras["merge"] = {"ms": ms_merge, "links": int(mv.n_links), "merged_tracks": int(mv.n_merged),
                            "note": "includes one stream synchronisation per call (track count to the host)"}
+        # (2b) the three-iteration track fit with interpolation rejection on the merged tracks (8(f) row 3)
+        ms_fit = timed(lambda: trk.fit(stream=stream, fetch=False), lambda: B.tpc_get_fit(trk.ctx))
+        fit3, _chi, rej3 = trk.fit(stream=stream)
+        extras["fit3"] = {"ms": ms_fit, "merged_tracks": int(len(fit3)), "failed": int((fit3["flags"] != 0).sum()),
+                          "clusters": int(len(rej3)), "clusters_rejected": int(rej3.sum())}
+        del fit3, _chi, rej3
+        trk.fit_ws = None
         trk.merge_ws = None
         # (3) deterministic mode on the same frame
         if args.mode == "fast":
@@ -611,7 +618,7 @@ def run_ours(args, rank, world, local_rank):
         "roofline": roof, "stages_hbm": stages,
         "stage_ms": {k: round(x, 4) for k, x in stage_ms.items()},
         "kernels_ms_per_step": {k["name"]: round(k["ms_per_step"], 4) for k in per_kernel},
-        "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "refit": refit, "merge": extras.get("merge"),
+        "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "refit": refit, "merge": extras.get("merge"), "fit3": extras.get("fit3"),
         "det": extras.get("det"), "second_iteration": extras.get("second_iteration"), "parity": parity_obj,
     }
     print(json.dumps(line), flush=True)

@@ -381,6 +381,41 @@ int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_merge
 /* Synchronises and fills *out (HOST) with device pointers into the merge workspace. */
 int tpc_get_merged(tpc_ctx* ctx, tpc_merged_view* out);
 
+/* THREE-ITERATION TRACK FIT with the Phase-I interpolation rejection (section 2: "three
+ * iterations, first inward, then outward, then inward"; position and covariance stored per pad row "in
+ * reduced precision", clusters cut "against the interpolation"; section 3: stored in the
+ * first iteration, interpolation and chi2 cut in the second, rejection in the third; DESIGN.md reading
+ * R10).  Runs on the merged tracks of tpc_merge_tracks (cluster lists in chain order; sector changes
+ * by the rotation of the merging, the central electrode by re-basing z).  Start parameters: the
+ * refit's outer state of the chain's last segment. */
+typedef struct tpc_fit_params {
+  float fit_chi2_max;        /* (16) cut on the 2-dof chi2 of a cluster against the interpolation     */
+  int32_t fit_min_clusters;  /* (10) fewer unmarked clusters: the fit fails                           */
+  float ce_var;              /* (1e4 cm^2) variance given to z when it is re-based at the electrode   */
+} tpc_fit_params;            /* 12 bytes */
+typedef struct tpc_track_fit3 {
+  float x;                   /* local x of the innermost unmarked cluster's row (its sector's frame)  */
+  float p[5], c[15];         /* final parameters and covariance there                                 */
+  float chi2;                /* of the third iteration                                                */
+  uint32_t n_clusters;       /* clusters of the merged track                                          */
+  uint32_t n_used;           /* of which unmarked                                                     */
+  uint32_t flags;            /* bit 0: the fit failed                                                 */
+} tpc_track_fit3;            /* 100 bytes */
+typedef struct tpc_fit_view {
+  uint64_t n_merged, n_cluster_ids;
+  const tpc_track_fit3* d_fit;     /* [n_merged], order of the merged view                            */
+  const float* d_chi2_cluster;     /* [n_cluster_ids] chi2 against the interpolation (iteration 2)    */
+  const uint8_t* d_rejected;       /* [n_cluster_ids] 1 = marked and left out of iteration 3          */
+} tpc_fit_view;
+void tpc_fit_default_params(tpc_fit_params* out);
+size_t tpc_fit_workspace_bytes(const tpc_ctx* ctx, uint64_t n_merged, uint64_t n_cluster_ids);
+/* Needs tpc_merge_tracks to have run (else TPC_E_STATE).  d_fit_workspace: DEVICE, 256-byte aligned,
+ * caller owned, >= tpc_fit_workspace_bytes(ctx, n_merged, n_cluster_ids of the merged view).
+ * Enqueued on cuda_stream (synchronises it first to learn the merged-track count). */
+int tpc_fit_tracks(tpc_ctx* ctx, const tpc_fit_params* params, void* d_fit_workspace, size_t workspace_bytes,
+                   void* cuda_stream);
+int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out);
+
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);
 

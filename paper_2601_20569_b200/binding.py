@@ -91,6 +91,20 @@ MERGED_DTYPE = np.dtype(
 assert MERGED_DTYPE.itemsize == 40 and C.sizeof(MergeParams) == 60
 
 
+class FitParams(C.Structure):
+    _fields_ = [("fit_chi2_max", C.c_float), ("fit_min_clusters", C.c_int32), ("ce_var", C.c_float)]
+
+
+class FitView(C.Structure):
+    _fields_ = [("n_merged", C.c_uint64), ("n_cluster_ids", C.c_uint64), ("d_fit", C.c_void_p),
+                ("d_chi2_cluster", C.c_void_p), ("d_rejected", C.c_void_p)]
+
+
+TRACK_FIT3_DTYPE = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,)), ("chi2", "<f4"),
+                             ("n_clusters", "<u4"), ("n_used", "<u4"), ("flags", "<u4")])
+assert TRACK_FIT3_DTYPE.itemsize == 100 and C.sizeof(FitParams) == 12
+
+
 class DebugView(C.Structure):
     _fields_ = [("n_clusters", C.c_uint64), ("n_sorted", C.c_uint64), ("n_rows_total", C.c_uint64),
                 ("n_bins", C.c_uint64), ("n_seeds", C.c_uint64), ("tracklet_stride", C.c_uint64),
@@ -104,7 +118,8 @@ EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_se
            "tpc_get_tracks", "tpc_get_intermediates", "tpc_get_stage_ms", "tpc_get_kernel_ms",
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
            "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_merge_default_params",
-           "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_last_launch_count",
+           "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_fit_default_params",
+           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -159,6 +174,14 @@ def load_library():
     L.tpc_merge_tracks.argtypes = [vp, C.POINTER(MergeParams), vp, C.c_size_t, vp]
     L.tpc_get_merged.restype = C.c_int
     L.tpc_get_merged.argtypes = [vp, C.POINTER(MergedView)]
+    L.tpc_fit_default_params.restype = None
+    L.tpc_fit_default_params.argtypes = [C.POINTER(FitParams)]
+    L.tpc_fit_workspace_bytes.restype = C.c_size_t
+    L.tpc_fit_workspace_bytes.argtypes = [vp, C.c_uint64, C.c_uint64]
+    L.tpc_fit_tracks.restype = C.c_int
+    L.tpc_fit_tracks.argtypes = [vp, C.POINTER(FitParams), vp, C.c_size_t, vp]
+    L.tpc_get_fit.restype = C.c_int
+    L.tpc_get_fit.argtypes = [vp, C.POINTER(FitView)]
     L.tpc_last_launch_count.restype = C.c_int
     L.tpc_last_launch_count.argtypes = [vp]
     L.tpc_destroy.restype = None
@@ -312,6 +335,29 @@ def tpc_merge_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, c
 def tpc_get_merged(ctx: int):
     v = MergedView()
     rc = load_library().tpc_get_merged(ctx, C.byref(v))
+    return rc, v
+
+
+def tpc_fit_default_params(**overrides) -> FitParams:
+    f = FitParams()
+    load_library().tpc_fit_default_params(C.byref(f))
+    for k, v in overrides.items():
+        setattr(f, k, v)
+    return f
+
+
+def tpc_fit_workspace_bytes(ctx: int, n_merged: int, n_cluster_ids: int) -> int:
+    return int(load_library().tpc_fit_workspace_bytes(ctx, n_merged, n_cluster_ids))
+
+
+def tpc_fit_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, cuda_stream: int) -> int:
+    return load_library().tpc_fit_tracks(ctx, C.byref(params) if params is not None else None, d_workspace,
+                                         workspace_bytes, cuda_stream)
+
+
+def tpc_get_fit(ctx: int):
+    v = FitView()
+    rc = load_library().tpc_get_fit(ctx, C.byref(v))
     return rc, v
 
 
@@ -482,6 +528,36 @@ class SectorTracker:
                     cluster_shared=arr(mv.d_cluster_shared, int(mv.n_cluster_ids), np.uint8),
                     next=arr(mv.d_next, nt, np.int32), prev=arr(mv.d_prev, nt, np.int32),
                     link_chi2=arr(mv.d_link_chi2, nt, np.float32))
+
+    def fit(self, fparams: FitParams | None = None, stream=None, fetch: bool = True):
+        """Three-iteration track fit with interpolation rejection (reading R10) of
+        the merged tracks; merge() must have run.  Returns (fit records, chi2_cluster, rejected)."""
+        rc, mv = tpc_get_merged(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_merged", tpc_last_cuda_error(self.ctx))
+        need = tpc_fit_workspace_bytes(self.ctx, int(mv.n_merged), int(mv.n_cluster_ids))
+        if getattr(self, "fit_ws", None) is None or self.fit_ws.numel() < need + 256:
+            self.fit_ws = None
+            self.fit_ws = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        ws_ptr = (self.fit_ws.data_ptr() + 255) // 256 * 256
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc = tpc_fit_tracks(self.ctx, fparams, ws_ptr, need, st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_fit_tracks", tpc_last_cuda_error(self.ctx))
+        if not fetch:
+            return None
+        rc, fv = tpc_get_fit(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_fit", tpc_last_cuda_error(self.ctx))
+
+        def arr(ptr, count, dtype):
+            dtype = np.dtype(dtype)
+            if count == 0:
+                return np.zeros(0, dtype=dtype)
+            off = ptr - self.fit_ws.data_ptr()
+            return self.fit_ws[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
+        return (arr(fv.d_fit, int(fv.n_merged), TRACK_FIT3_DTYPE), arr(fv.d_chi2_cluster, int(fv.n_cluster_ids), np.float32),
+                arr(fv.d_rejected, int(fv.n_cluster_ids), np.uint8))
 
     def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
         """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the

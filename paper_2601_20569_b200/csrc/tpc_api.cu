@@ -35,7 +35,10 @@ struct tpc_ctx {
   uint64_t n_bins_cap = 0;
   bool refit_done = false;     // tpc_refit_tracks ran on the current result
   bool merged = false;         // tpc_merge_tracks ran on the current result
+  bool fitted = false;         // tpc_fit_tracks ran on the current merged result
   TpcMergeBuffers mbuf;
+  TpcFitBuffers fbuf;
+  uint32_t fit_n_merged = 0, fit_n_ids = 0;
   uint32_t* h_mcnt = nullptr;  // pinned: merge counters
   char cuda_err[256] = {0};
 };
@@ -266,6 +269,7 @@ static int enqueue_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n
   ctx->synced = false;
   ctx->refit_done = false;
   ctx->merged = false;
+  ctx->fitted = false;
   ctx->events.enabled = (flags & TPC_STAGE_TIMERS) != 0;
   (void)cudaGetLastError();
   const int launches = (flags & TPC_DETERMINISTIC)
@@ -796,6 +800,7 @@ int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_ws, s
   ctx->stream = st;
   ctx->synced = false;
   ctx->merged = true;
+  ctx->fitted = false;
   ctx->launches = l;
   return TPC_OK;
 }
@@ -814,6 +819,80 @@ int tpc_get_merged(tpc_ctx* ctx, tpc_merged_view* out) {
   out->d_merged = M.merged; out->d_seg_index = M.seg_index;
   out->d_cluster_ids = M.ids; out->d_cluster_shared = M.shared;
   out->d_next = M.next; out->d_prev = M.prev; out->d_link_chi2 = M.link_chi2;
+  return TPC_OK;
+}
+
+// ---------------------------------------------------------------- three-iteration track fit (R10)
+namespace {
+size_t carve_fit(uint64_t n_merged, uint64_t n_ids, char* base, TpcFitBuffers* T) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  TpcFitBuffers t;
+  std::memset(&t, 0, sizeof(t));
+  t.stored = (uint4*)take(16 * (n_ids + 1));
+  t.chi2_cluster = (float*)take(4 * (n_ids + 1));
+  t.rejected = (uint8_t*)take(n_ids + 1);
+  t.fit = (tpc_track_fit3*)take(sizeof(tpc_track_fit3) * (n_merged + 1));
+  if (T) *T = t;
+  return off;
+}
+}  // namespace
+
+void tpc_fit_default_params(tpc_fit_params* f) {
+  f->fit_chi2_max = 16.0f;
+  f->fit_min_clusters = 10;
+  f->ce_var = 10000.0f;
+}
+
+size_t tpc_fit_workspace_bytes(const tpc_ctx* ctx, uint64_t n_merged, uint64_t n_cluster_ids) {
+  if (!ctx || n_merged >= (1ull << 31) || n_cluster_ids >= (1ull << 32)) return 0;
+  return carve_fit(n_merged, n_cluster_ids, nullptr, nullptr);
+}
+
+int tpc_fit_tracks(tpc_ctx* ctx, const tpc_fit_params* params, void* d_ws, size_t ws_bytes, void* cuda_stream) {
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->merged) return TPC_E_STATE;
+  if (!d_ws || ((uintptr_t)d_ws & 255u)) return TPC_E_ARG;
+  tpc_fit_params P;
+  if (params) P = *params; else tpc_fit_default_params(&P);
+  if (!(P.fit_chi2_max >= 0.f) || P.fit_min_clusters < 2 || !(P.ce_var > 0.f)) return TPC_E_ARG;
+  const uint32_t n_merged = ctx->mbuf.n_tracks ? ctx->h_mcnt[0] : 0u, n_ids = ctx->mbuf.n_tracks ? ctx->h_mcnt[2] : 0u;
+  TpcFitBuffers T;
+  const size_t need = carve_fit(n_merged, n_ids, (char*)d_ws, &T);
+  if (ws_bytes < need) return TPC_E_WORKSPACE;
+  T.P = P;
+  T.ca = ctx->mbuf.ca; T.sa = ctx->mbuf.sa;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  (void)cudaGetLastError();
+  const int l = (ctx->flags & TPC_DETERMINISTIC)
+                    ? tpc_det::run_fit3(ctx->buf, &ctx->hconst, ctx->mbuf, T, n_merged, st, ctx->n_sm)
+                    : tpc_fast::run_fit3(ctx->buf, &ctx->hconst, ctx->mbuf, T, n_merged, st, ctx->n_sm);
+  if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (fit)");
+  ctx->fbuf = T;
+  ctx->fit_n_merged = n_merged; ctx->fit_n_ids = n_ids;
+  ctx->stream = st;
+  ctx->synced = false;
+  ctx->fitted = true;
+  ctx->launches = l;
+  return TPC_OK;
+}
+
+int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out) {
+  if (!out) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->fitted) return TPC_E_STATE;
+  std::memset(out, 0, sizeof(*out));
+  out->n_merged = ctx->fit_n_merged;
+  out->n_cluster_ids = ctx->fit_n_ids;
+  out->d_fit = ctx->fbuf.fit;
+  out->d_chi2_cluster = ctx->fbuf.chi2_cluster;
+  out->d_rejected = ctx->fbuf.rejected;
   return TPC_OK;
 }
 

@@ -144,6 +144,16 @@ struct TpcMergeBuffers {
   uint32_t* counters;        // [4] n_merged, n_links, n_ids out, -
 };
 
+// Buffers of the three-iteration track fit (R10), pointers into the caller's fit workspace.
+struct TpcFitBuffers {
+  tpc_fit_params P;
+  float ca, sa;
+  uint4* stored;           // [n_ids] predictions of iteration 1: halves (ry, rz | c00, c10 | c11, -)
+  float* chi2_cluster;     // [n_ids]
+  uint8_t* rejected;       // [n_ids]
+  tpc_track_fit3* fit;     // [n_merged]
+};
+
 #define TPC_MAX_KERNELS 32
 struct TpcStageEvents {
   cudaEvent_t ev[TPC_N_STAGES];  // boundaries: start, after grid, nf, seeds, follower, selector
@@ -154,11 +164,13 @@ struct TpcStageEvents {
 };
 
 namespace tpc_det {
+int run_fit3(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcFitBuffers& T, uint32_t n_merged, cudaStream_t stream, int n_sm);
 int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
+int run_fit3(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcFitBuffers& T, uint32_t n_merged, cudaStream_t stream, int n_sm);
 int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);

@@ -13,6 +13,7 @@
 //                 for unordered input, histogram -> per-row scan -> scatter [-> in-bin sort]),
 //                 K2 neighbour finder,  K3 link cleanup + seeds,  K4 Kalman track follower
 //                 (outward / refit / inward kernels),  K5 ambiguity solving.
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -2536,6 +2537,176 @@ __global__ void __launch_bounds__(256) k_merge_copy_ids(TpcBuffers B, TpcMergeBu
   }
 }
 
+// ================================================================== R10 three-iteration track fit
+// PAPER.md:31,37 (section 2) and PAPER.md:57 (section 3, Phase I): three passes over the cluster list
+// of every merged track -- inward (the predicted position and its covariance are STORED at every
+// cluster, in half precision), outward (the prediction is interpolated with the stored one, the
+// cluster's chi2 against the interpolation is cut: marking only), inward again through the unmarked
+// clusters.  One thread per merged track; the stored predictions live in a 16-byte record per
+// cluster of the merged list.  DESIGN.md reading R10.
+__device__ __forceinline__ float fit_round_half(float v) { return __half2float(__float2half_rn(v)); }
+
+__device__ __forceinline__ bool fit_transport(KF& k, int sec0, int row0, int sec1, int row1, float zc,
+                                              const TpcConst* __restrict__ K, const FollowConst& F,
+                                              const TpcFitBuffers& T) {
+  if (sec0 == sec1 || sec0 - sec1 == 18 || sec1 - sec0 == 18) {
+    const int n = row1 > row0 ? row1 - row0 : row0 - row1;
+    const float dx = row1 > row0 ? F.dx : -F.dx;
+    for (int i = 0; i < n; ++i)
+      if (!kf_propagate(k, dx, F)) return false;
+    if (sec0 != sec1) {   // central electrode: z re-based on the measurement, its correlations dropped
+      k.z = zc;
+      k.c10 = 0.f; k.c21 = 0.f; k.c31 = 0.f; k.c41 = 0.f;
+      k.c11 = T.P.ce_var;
+    }
+    return true;
+  }
+  const float sgn = (sec1 % 18 == (sec0 % 18 + 1) % 18) ? 1.f : -1.f;
+  float x = K->x[row0];
+  if (!merge_rotate(k, x, T.ca, sgn * T.sa, F.max_sinphi)) return false;
+  return kf_propagate(k, K->x[row1] - x, F);
+}
+__device__ __forceinline__ void fit_turn(KF& k, float y, float z, const FollowConst& F) {
+  k.y = y; k.z = z;
+  kf_init_cov(k, F);
+}
+__device__ __forceinline__ float fit_chi2_2x2(float r0, float r1, float a, float b, float d, float vy, float vz) {
+  const float s00 = a + vy, s01 = b, s11 = d + vz;
+  const float det = s00 * s11 - s01 * s01;
+  const float inv = 1.f / det;
+  const float i00 = s11 * inv, i01 = -(s01 * inv), i11 = s00 * inv;
+  return ((r0 * r0) * i00 + (2.f * (r0 * r1)) * i01) + (r1 * r1) * i11;
+}
+
+__global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffers M, TpcFitBuffers T,
+                                                    const __grid_constant__ FollowConst F) {
+  const TpcConst* __restrict__ K = B.K;
+  const uint32_t n_merged = M.counters[0];
+  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < n_merged; mi += gridDim.x * blockDim.x) {
+    const tpc_merged_track m = M.merged[mi];
+    const uint32_t* __restrict__ ids = M.ids + m.cluster_ofs;
+    const int n = (int)m.n_clusters;
+    tpc_track_fit3 out;
+    out.x = 0.f; out.chi2 = 0.f; out.n_clusters = (uint32_t)n; out.n_used = 0u; out.flags = 1u;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) out.p[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) out.c[i] = 0.f;
+    float* __restrict__ chi_c = T.chi2_cluster + m.cluster_ofs;
+    uint8_t* __restrict__ rej = T.rejected + m.cluster_ofs;
+    uint4* __restrict__ store = T.stored + m.cluster_ofs;
+    for (int i = 0; i < n; ++i) { chi_c[i] = 0.f; rej[i] = 0; }
+    auto rec = [&](int i, float& y, float& z, int& sec, int& row) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + (ids[i] - B.id_base));
+      y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); sec = (int)(raw.w & 0xFF); row = (int)((raw.w >> 8) & 0xFF);
+    };
+    const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
+    const tpc_track_fit* ft = B.track_fit + tail;
+    bool ok = n >= 2 && ft->flags == 0u;
+    KF k;
+    k.y = k.z = 0.f;
+    k.s = ft->p_out[2]; k.t = ft->p_out[3]; k.q = ft->p_out[4];
+    kf_init_cov(k, F);
+    float yc, zc, yp, zp;
+    int sc, rc, sp, rp;
+    // ---- iteration 1: inward from c_{n-1}; predictions stored in half precision
+    if (ok) {
+      rec(n - 1, yp, zp, sp, rp);
+      fit_turn(k, yp, zp, F);
+      for (int i = n - 2; i >= 0 && ok; --i) {
+        rec(i, yc, zc, sc, rc);
+        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
+        const uint32_t h0 = (uint32_t)__half_as_ushort(__float2half_rn(k.y - yc)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.z - zc)) << 16);
+        const uint32_t h1 = (uint32_t)__half_as_ushort(__float2half_rn(k.c00)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.c10)) << 16);
+        const uint32_t h2 = (uint32_t)__half_as_ushort(__float2half_rn(k.c11));
+        store[i] = make_uint4(h0, h1, h2, 0u);
+        const Gain g = kf_gain(k, F);
+        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
+        sp = sc; rp = rc;
+      }
+    }
+    // ---- iteration 2: outward from c_0; interpolation, chi2 cut (marking only)
+    int used = 0;
+    if (ok) {
+      rec(0, yp, zp, sp, rp);
+      fit_turn(k, yp, zp, F);
+      {
+        const uint4 st = store[0];
+        const float s_ry = __half2float(__ushort_as_half((unsigned short)(st.x & 0xFFFFu))), s_rz = __half2float(__ushort_as_half((unsigned short)(st.x >> 16)));
+        const float a1 = __half2float(__ushort_as_half((unsigned short)(st.y & 0xFFFFu))), b1 = __half2float(__ushort_as_half((unsigned short)(st.y >> 16)));
+        const float d1 = __half2float(__ushort_as_half((unsigned short)(st.z & 0xFFFFu)));
+        const float chi2 = fit_chi2_2x2(s_ry, s_rz, a1, b1, d1, F.vy, F.vz);
+        chi_c[0] = chi2;
+        if (!(chi2 <= T.P.fit_chi2_max)) rej[0] = 1; else ++used;
+      }
+      for (int i = 1; i < n && ok; ++i) {
+        rec(i, yc, zc, sc, rc);
+        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
+        const float r2y = k.y - yc, r2z = k.z - zc;
+        const float a2 = k.c00, b2 = k.c10, d2 = k.c11;
+        float chi2;
+        if (i == n - 1) {
+          chi2 = fit_chi2_2x2(r2y, r2z, a2, b2, d2, F.vy, F.vz);
+        } else {
+          const uint4 st = store[i];
+          const float s_ry = __half2float(__ushort_as_half((unsigned short)(st.x & 0xFFFFu))), s_rz = __half2float(__ushort_as_half((unsigned short)(st.x >> 16)));
+          const float a1 = __half2float(__ushort_as_half((unsigned short)(st.y & 0xFFFFu))), b1 = __half2float(__ushort_as_half((unsigned short)(st.y >> 16)));
+          const float d1 = __half2float(__ushort_as_half((unsigned short)(st.z & 0xFFFFu)));
+          const float det1 = a1 * d1 - b1 * b1, det2 = a2 * d2 - b2 * b2;
+          const float n1 = 1.f / det1, n2 = 1.f / det2;
+          const float i1a = d1 * n1, i1b = -(b1 * n1), i1d = a1 * n1;
+          const float i2a = d2 * n2, i2b = -(b2 * n2), i2d = a2 * n2;
+          const float ia = i1a + i2a, ib = i1b + i2b, id = i1d + i2d;
+          const float detw = ia * id - ib * ib;
+          const float nw = 1.f / detw;
+          const float wa = id * nw, wb = -(ib * nw), wd = ia * nw;
+          const float hy = (i1a * s_ry + i1b * s_rz) + (i2a * r2y + i2b * r2z);
+          const float hz = (i1b * s_ry + i1d * s_rz) + (i2b * r2y + i2d * r2z);
+          const float ry = wa * hy + wb * hz, rz = wb * hy + wd * hz;
+          chi2 = fit_chi2_2x2(ry, rz, wa, wb, wd, F.vy, F.vz);
+        }
+        chi_c[i] = chi2;
+        if (!(chi2 <= T.P.fit_chi2_max)) rej[i] = 1; else ++used;
+        const Gain g = kf_gain(k, F);
+        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
+        sp = sc; rp = rc;
+      }
+    }
+    // ---- iteration 3: inward through the unmarked clusters
+    if (ok) {
+      out.n_used = (uint32_t)used;
+      if (used < T.P.fit_min_clusters || used < 2) ok = false;
+    }
+    if (ok) {
+      int last = n - 1;
+      while (rej[last]) --last;
+      rec(last, yp, zp, sp, rp);
+      fit_turn(k, yp, zp, F);
+      float chi2 = 0.f;
+      for (int i = last - 1; i >= 0 && ok; --i) {
+        if (rej[i]) continue;
+        rec(i, yc, zc, sc, rc);
+        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
+        const Gain g = kf_gain(k, F);
+        const float c2 = kf_chi2(k, g, yc, zc);
+        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
+        chi2 = chi2 + c2;
+        sp = sc; rp = rc;
+      }
+      if (ok) {
+        out.x = K->x[rp];
+        out.p[0] = k.y; out.p[1] = k.z; out.p[2] = k.s; out.p[3] = k.t; out.p[4] = k.q;
+        out.c[0] = k.c00; out.c[1] = k.c10; out.c[2] = k.c11; out.c[3] = k.c20; out.c[4] = k.c21; out.c[5] = k.c22;
+        out.c[6] = k.c30; out.c[7] = k.c31; out.c[8] = k.c32; out.c[9] = k.c33;
+        out.c[10] = k.c40; out.c[11] = k.c41; out.c[12] = k.c42; out.c[13] = k.c43; out.c[14] = k.c44;
+        out.chi2 = chi2;
+        out.flags = 0u;
+      }
+    }
+    T.fit[mi] = out;
+  }
+}
+
 // ================================================================== host: enqueue the path
 #define TPC_LAUNCH_CHECK(name)                                      \
   do {                                                              \
@@ -2611,6 +2782,14 @@ int run_merge(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M,
     launches += 12;
   }
   return cudaPeekAtLastError() == cudaSuccess ? launches : -1;
+}
+
+int run_fit3(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, const TpcFitBuffers& T, uint32_t n_merged,
+             cudaStream_t st, int n_sm) {
+  if (n_merged == 0) return 0;
+  const FollowConst F = follow_const(hK);
+  k_track_fit3<<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3, 128)), 128, 0, st>>>(B, M, T, F);
+  return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

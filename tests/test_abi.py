@@ -28,6 +28,9 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.TrackView) == 184 and ctypes.sizeof(B.DebugView) == 136
     assert B.TRACK_FIT_DTYPE.itemsize == 192 and B.MERGED_DTYPE.itemsize == 40
     assert ctypes.sizeof(B.MergeParams) == 60 and ctypes.sizeof(B.MergedView) == 88
+    assert B.TRACK_FIT3_DTYPE.itemsize == 100 and ctypes.sizeof(B.FitParams) == 12 and ctypes.sizeof(B.FitView) == 40
+    f = B.tpc_fit_default_params()
+    assert abs(f.fit_chi2_max - 16.0) < 1e-6 and f.fit_min_clusters == 10
     m = B.tpc_merge_default_params()
     assert m.gap_in_sector == 30 and abs(m.chi2_max - 20.0) < 1e-6 and m.stages == 7
 

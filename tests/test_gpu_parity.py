@@ -772,3 +772,85 @@ def test_sector_split_equals_whole_frame(B):
     o = oracle.run(cl, n_threads=NT, want=("tracks",))
     assert parity.all_zero(parity.compare_tracks(tracks, ids, shared, o))
     assert mg.gather_to_root(tracks, ids, shared, 0, 1)[0] is tracks
+
+
+@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
+def test_det_parity_three_iteration_fit(B, name):
+    """the three-iteration fit with interpolation rejection
+    on the merged tracks; deterministic mode: final parameters, chi2, per-cluster interpolation chi2
+    and rejection marks bit-exact against oracle.trackfit."""
+    from oracle import merging, trackfit
+    if name == "C2_full":
+        cl, lab, _ = dg.generate(dg.preset("C2"))
+        pkw = {}
+    elif name == "C4_reduced":
+        cl, lab, _ = dg.generate(dg.preset("C4", n_events=6, tracks_per_event=1500, t_window_us=120.0))
+        pkw = dict(grid_dz=8.0, max_bins=200_000_000)
+    elif name == "C5_dense":
+        cl, lab, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+    else:
+        x, _, _, _ = oracle.geom_tables()
+        xm = 0.5 * (float(x[61]) + float(x[62]))
+        rng = np.random.default_rng(4)
+        recs = []
+        for k in range(40):
+            for r in range(20, 101):
+                zt = 0.5 * (xm - float(x[r]))
+                yy, dz = -12.0 + 0.6 * k + rng.normal(0, 0.1), rng.normal(0, 0.1)
+                if r == 40 + k % 20:
+                    yy += 1.0                                  # one outlier per track
+                recs.append((3, r, yy, zt - 30.0 - 7.0 * k + dz) if r <= 61 else (21, r, yy, zt + 30.0 + 7.0 * k + dz))
+        cl = np.zeros(len(recs), dtype=oracle.CLUSTER_DTYPE)
+        a = np.array(recs)
+        order = np.lexsort((a[:, 1], a[:, 0]))
+        cl["sector"], cl["row"], cl["y"], cl["z"] = a[order, 0], a[order, 1], a[order, 2], a[order, 3]
+        pkw = {}
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        trk.track(trk.upload(cl), flags=1)
+        tracks, ids, shared, view = trk.tracks()
+        trk.refit()
+        g = trk.merge()
+        gfit, gchi, grej = trk.fit()
+    finally:
+        trk.close()
+    o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
+    ofit, ochi, orej = trackfit.fit_merged(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids, params=op)
+    assert len(gfit) == len(ofit) > 0
+    # canonical order of the merged tracks: by the head's key, on both sides
+    def order_of(tr, merged):
+        h = merged["head"].astype(np.int64)
+        return np.lexsort((tr["segment"][h], tr["seed_id"][h], tr["sector"][h]))
+    og, oo = order_of(tracks, g["merged"]), order_of(o.tracks, m.merged)
+    fg, fo = gfit[og], ofit[oo]
+    assert (fg["flags"] == fo["flags"]).all() and (fg["n_used"] == fo["n_used"]).all() and (fg["n_clusters"] == fo["n_clusters"]).all()
+    ok = fo["flags"] == 0
+    assert ok.sum() >= 0.9 * len(ok)
+    for f in ("x", "p", "c", "chi2"):
+        a_, b_ = np.ascontiguousarray(fg[f][ok]).view(np.uint32), np.ascontiguousarray(fo[f][ok]).view(np.uint32)
+        assert (a_ == b_).all(), (f, int((a_ != b_).sum()))
+    # per-cluster results, merged track by merged track
+    def per_cluster(merged, order, chi, rej):
+        ch, rj = [], []
+        for k in order:
+            o_, n_ = int(merged["cluster_ofs"][k]), int(merged["n_clusters"][k])
+            ch.append(chi[o_:o_ + n_]); rj.append(rej[o_:o_ + n_])
+        return np.concatenate(ch), np.concatenate(rj)
+    cg, rg = per_cluster(g["merged"], og, gchi, grej)
+    co, ro = per_cluster(m.merged, oo, ochi, orej)
+    assert (rg == ro).all()
+    okc = np.repeat(ok, fo["n_clusters"].astype(np.int64))
+    assert (cg[okc].view(np.uint32) == co[okc].view(np.uint32)).all()
+    if name == "ce_crossing":
+        # (the 1 cm outliers never enter a track: the follower's own chi2 cut refuses them; the fit
+        # runs through the electrode on all 40 tracks)
+        assert len(fo) == 40 and ok.all() and (fo["n_clusters"] >= 79).all()
+    elif name == "C4_reduced":
+        # the space-charge distortion the tracker is unaware of (PAPER.md:39) bends the inner rows away
+        # from the helix: ~9 % of the attached clusters fail the cut against the interpolation
+        assert 0.02 * len(ro) < ro.sum() < 0.2 * len(ro)
+    else:
+        assert 0 < ro.sum() < 0.02 * len(ro)
