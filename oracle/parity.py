@@ -199,6 +199,16 @@ def compare_tracklets_fast(gi, o, rel=1e-3):
     relerr = param_relerr(a["p"][same], b["p"][same]) if same.any() else np.zeros((0, 5))
     out["n_param_bad"] = int((relerr > rel).any(axis=1).sum())
     out["max_rel_per_param"] = [float(v) for v in relerr.max(axis=0)] if len(relerr) else []
+    # the same deviations in units of the parameter's own uncertainty (weakly constrained q/pT of
+    # short tracklets: rounding scales with sigma, not with the value)
+    if len(relerr):
+        sig = np.sqrt(np.maximum(b["c"][same][:, [0, 2, 5, 9, 14]].astype(np.float64), 1e-30))
+        err = np.abs(a["p"][same].astype(np.float64) - b["p"][same].astype(np.float64))
+        err[:, 1] = np.maximum(0.0, err[:, 1] - _z_floor(b["p"][same][:, 1]))
+        over = relerr > rel                      # only the entries beyond the relative bound
+        out["max_err_in_sigma"] = float((err / sig)[over].max()) if over.any() else 0.0
+    else:
+        out["max_err_in_sigma"] = 0.0
     # the worst cases in full (for the record): parameter, error, value, its own uncertainty, hits
     diag = np.array([0, 2, 5, 9, 14])
     worst = []
