@@ -146,9 +146,11 @@ typedef struct tpc_track_view {
   uint64_t n_follow_candidates;     /* ... and chi2 evaluations of road candidates       */
   uint64_t follow_work[3][3];       /* the same three counters per follower kernel:
                                        [outward | refit | inward][steps, updates, candidates] */
-  uint64_t grid_by_rows;            /* 1: the grid was built row by row in shared memory (every
-                                       row's records contiguous in the input and small enough),
-                                       0: by the generic histogram / scan / scatter kernels  */
+  uint64_t grid_by_rows;            /* 1: EVERY row's grid was built row by row in shared memory
+                                       (k_row_sort); 0: some rows took the generic kernels      */
+  uint64_t n_rows_generic;          /* rows built by the generic histogram / scan / scatter kernels:
+                                       rows whose input records are not contiguous, that hold
+                                       >= 65536 records, or whose tables exceed 224 KB          */
 } tpc_track_view;
 
 /* One row of the search grid. */

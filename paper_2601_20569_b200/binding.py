@@ -69,7 +69,7 @@ class TrackView(C.Structure):
                 ("n_tracklets", C.c_uint64), ("n_bins", C.c_uint64),
                 ("n_follow_steps", C.c_uint64), ("n_follow_updates", C.c_uint64),
                 ("n_follow_candidates", C.c_uint64), ("follow_work", (C.c_uint64 * 3) * 3),
-                ("grid_by_rows", C.c_uint64)]
+                ("grid_by_rows", C.c_uint64), ("n_rows_generic", C.c_uint64)]
 
 
 class MergeParams(C.Structure):

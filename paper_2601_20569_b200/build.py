@@ -11,8 +11,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-# TPCTRACK_LIB: load/build another file than the in-tree default (A/B builds of the kernels)
-LIB_PATH = os.environ.get("TPCTRACK_LIB") or os.path.join(CSRC, "libtpctrack.so")
+LIB_PATH = os.path.join(CSRC, "libtpctrack.so")
 
 _NVCC_BASE = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + INCLUDE, "-I" + CSRC]
@@ -28,16 +27,12 @@ def build_tpctrack(force: bool = False, verbose: bool = False) -> str:
     if not force and _newer(LIB_PATH, srcs):
         return LIB_PATH
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("TPCTRACK_NVCC_FLAGS", "").split()   # e.g. -DTPC_FOLLOW_MINBLOCKS=6
-    tag = "_" + str(abs(hash(LIB_PATH)) % 10**8) if os.environ.get("TPCTRACK_LIB") else ""
-    det_o, fast_o, api_o = (os.path.join(CSRC, f"tpc_{n}{tag}.o") for n in ("kernels_det", "kernels_fast", "api"))
+    det_o, fast_o, api_o = (os.path.join(CSRC, f"tpc_{n}.o") for n in ("kernels_det", "kernels_fast", "api"))
     cmds = [
         _NVCC_BASE + extra + ["-DTPC_DET=1", "--fmad=false", "-c", srcs[0], "-o", det_o],
         # fast build: FMA contraction, approximate division / square root (MUFU based), denormals
         # flushed: rounding-level differences only, which is all fast mode may differ by
-        _NVCC_BASE + extra + ["-DTPC_DET=0", "--fmad=true"]
-        + os.environ.get("TPCTRACK_FAST_FLAGS", "--use_fast_math").split()
-        + ["-c", srcs[0], "-o", fast_o],
+        _NVCC_BASE + extra + ["-DTPC_DET=0", "--fmad=true", "--use_fast_math", "-c", srcs[0], "-o", fast_o],
         _NVCC_BASE + ["-c", srcs[1], "-o", api_o],
         ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB_PATH, det_o, fast_o, api_o],
     ]

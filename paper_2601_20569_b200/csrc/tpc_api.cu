@@ -68,7 +68,9 @@ Capacities capacities(const tpc_ctx* c, uint64_t n) {
                        ((uint64_t)std::ceil(c->geom.z_max / P.grid_dz) + 2);
   if (bins > 0xFFFFFFF0ull) bins = 0xFFFFFFF0ull;
   k.max_bins = bins;
-  uint64_t seeds = P.max_seeds ? P.max_seeds : n / 8 + 4096;
+  // seeds per cluster measured on the five workloads: 1/19 (C2, C3, C4), 1/23 (C5); the default leaves
+  // a third of headroom (was n/8: 18 GB of row_hit for the C4 frame); beyond it: TPC_E_OVERFLOW, set max_seeds
+  uint64_t seeds = P.max_seeds ? P.max_seeds : n / 12 + 4096;
   seeds = align_up(seeds, 64);
   k.max_seeds = (uint32_t)seeds;
   const uint64_t ids = n * 1000 / (1000 - (uint64_t)P.shared_permille) + 64;
@@ -331,6 +333,7 @@ int tpc_get_tracks(tpc_ctx* ctx, tpc_track_view* out) {
     for (int b = 0; b < 3; ++b) out->follow_work[a][b] = c.follow_work[a][b];
   }
   out->grid_by_rows = c.grid_rows;
+  out->n_rows_generic = c.n_rows_generic;
   return rc;
 }
 
@@ -512,6 +515,7 @@ int tpc_sector_track_host_chunks(tpc_ctx* ctx, const tpc_cluster* h_clusters, ui
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) out->follow_work[a][b] += v.follow_work[a][b];
     out->grid_by_rows = (c == 0) ? v.grid_by_rows : (out->grid_by_rows & v.grid_by_rows);
+    out->n_rows_generic += v.n_rows_generic;
   }
   if ((e = cudaStreamSynchronize(ctx->s_out)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize(copy-out)");
   if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return set_cuda_err(ctx, e, "cudaStreamSynchronize");

@@ -39,6 +39,8 @@ struct TpcCounters {
   uint32_t n_bins, n_tiles, n_seeds, n_tracklets;
   uint32_t n_tracks, n_ids, error;
   uint32_t grid_rows;   // 1: every row's input records are contiguous and fit k_row_sort (the per-row grid build)
+  uint32_t n_rows_generic;   // rows built by the generic histogram / scan / scatter kernels instead
+  uint32_t pad2_;
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
   unsigned long long follow_work[3][3];  // [kernel up/refit/down][steps, updates, candidates]

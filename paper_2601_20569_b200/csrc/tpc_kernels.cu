@@ -212,10 +212,10 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
   uint32_t base_bin = 0, base_clu = 0, base_tile = 0;
   unsigned long long bins64 = 0;
   bool overflow = false;
-  bool by_rows = true;   // every row qualifies for the per-row grid build (k_row_sort)
+  uint32_t n_generic = 0;   // rows that do not qualify for the per-row grid build (k_row_sort)
   for (uint32_t s0 = 0; s0 < B.n_sr; s0 += blockDim.x) {
     const uint32_t sr = s0 + threadIdx.x;
-    uint32_t cnt = 0, nb = 0, nt = 0;
+    uint32_t cnt = 0, nb = 0, nt = 0, by_row = 1u;
     int nz = 0, ny = 0;
     float z0 = 0.f, y0 = 0.f;
     if (sr < B.n_sr) {
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
         // counters + permutation in the cluster's shared memory
         const TpcRowStat rs = B.row_stat[sr];
         const uint32_t bytes = 4u * ((nb + 1) / 2) + 2u * cnt;
-        if (rs.last - rs.first + 1u != rs.n_all || rs.n_all > 65535u || bytes > TPC_RS_SMEM_BYTES) by_rows = false;
+        if (rs.last - rs.first + 1u != rs.n_all || rs.n_all > 65535u || bytes > TPC_RS_SMEM_BYTES) { by_row = 0u; ++n_generic; }
       }
     }
     if (B.chunk_tag && sr < B.n_sr && B.row_stat[sr].n_all) {   // chunked frame: sectors must not straddle chunks
@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
       d.bin_ofs = base_bin + pb;
       d.clu_ofs = base_clu + pc;
       d.count = cnt;
-      d.pad_ = 0;
+      d.pad_ = by_row;   // 1: this row's grid is built by k_row_sort, 0: by the generic kernels
       B.row_desc[sr] = d;
       B.tile_ofs[sr] = base_tile + pt;
     }
@@ -263,9 +263,14 @@ __global__ void __launch_bounds__(1024) k_row_desc(TpcBuffers B) {
     base_bin += tot_b; base_clu += tot_c; base_tile += tot_t;
   }
   overflow = __syncthreads_or(overflow || bins64 > B.max_bins);
-  by_rows = __syncthreads_and(by_rows);
+  __shared__ uint32_t s_generic;
+  if (threadIdx.x == 0) s_generic = 0u;
+  __syncthreads();
+  if (n_generic) atomicAdd(&s_generic, n_generic);
+  __syncthreads();
   if (threadIdx.x == 0) {
-    B.cnt->grid_rows = (by_rows && !overflow) ? 1u : 0u;
+    B.cnt->n_rows_generic = s_generic;
+    B.cnt->grid_rows = (s_generic == 0u && !overflow) ? 1u : 0u;
     B.tile_ofs[B.n_sr] = base_tile;
     B.cnt->n_sorted = base_clu;
     B.cnt->n_tiles = base_tile;
@@ -289,13 +294,14 @@ __global__ void __launch_bounds__(128) k_tile_rows(TpcBuffers B) {
 __global__ void __launch_bounds__(256) k_zero_bins(TpcBuffers B) {
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n_sr * TPC_SEED_SLABS; i += gridDim.x * blockDim.x)
     B.item_cnt[i] = 0u;
-  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
-  const uint32_t n = B.cnt->n_bins + 1;
-  uint4* p4 = reinterpret_cast<uint4*>(B.bin_start);
-  const uint32_t n4 = n / 4;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += gridDim.x * blockDim.x)
-    p4[i] = make_uint4(0, 0, 0, 0);
-  if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) B.bin_start[n4 * 4 + threadIdx.x] = 0;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->n_rows_generic == 0u) return;
+  // the bin counters of the rows the generic kernels build (the others belong to k_row_sort)
+  for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
+    const tpc_row_desc d = B.row_desc[sr];
+    if (d.pad_ || d.count == 0) continue;
+    const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
+    for (uint32_t b = threadIdx.x; b < nb; b += blockDim.x) B.bin_start[d.bin_ofs + b] = 0u;
+  }
 }
 
 __device__ __forceinline__ uint32_t bin_of(const tpc_row_desc& d, const TpcConst* __restrict__ K, float y, float z) {
@@ -308,7 +314,7 @@ __device__ __forceinline__ uint32_t bin_of(const tpc_row_desc& d, const TpcConst
 // so the scatter needs no second atomic.
 __global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
-  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->n_rows_generic == 0u) return;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
     const uint4 raw = ld_stream16(B.clusters + i);
     int sr, row;
@@ -316,7 +322,7 @@ __global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
     uint32_t s = 0xFFFFFFFFu;
     if (classify(raw, K, sr, y, z, row) == 0) {
       const tpc_row_desc d = B.row_desc[sr];
-      s = atomicAdd(&B.bin_start[bin_of(d, K, y, z)], 1u);
+      if (!d.pad_) s = atomicAdd(&B.bin_start[bin_of(d, K, y, z)], 1u);   // (rows of k_row_sort are not ours)
     }
     B.slot[i] = s;
   }
@@ -327,9 +333,10 @@ __global__ void __launch_bounds__(256) k_bin_hist(TpcBuffers B) {
 // (north star: "a per-row bin index built by a warp-level scan").
 __global__ void __launch_bounds__(512) k_bin_scan(TpcBuffers B) {
   __shared__ uint32_t sm[33];
-  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->n_rows_generic == 0u) return;
   for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
     const tpc_row_desc d = B.row_desc[sr];
+    if (d.pad_) continue;
     const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
     uint32_t* p = B.bin_start + d.bin_ofs;
     uint32_t carry = d.clu_ofs;
@@ -357,7 +364,7 @@ __global__ void __launch_bounds__(512) k_bin_scan(TpcBuffers B) {
 // K1e: scatter into bin order: sorted (y,z) pairs + original index.
 __global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
   const TpcConst* __restrict__ K = B.K;
-  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->n_rows_generic == 0u) return;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < B.n; i += gridDim.x * blockDim.x) {
     const uint32_t s = B.slot[i];
     if (s == 0xFFFFFFFFu) continue;
@@ -381,21 +388,26 @@ __global__ void __launch_bounds__(256) k_scatter(TpcBuffers B) {
 // K1f (deterministic mode only): order the clusters of every bin by ascending original index,
 // so that the sorted order is a function of the input alone (stable sort).
 __global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
-  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->grid_rows) return;
-  const uint32_t nb = B.cnt->n_bins;
-  for (uint32_t b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
-    const uint32_t lo = B.bin_start[b], hi = B.bin_start[b + 1];
-    for (uint32_t i = lo + 1; i < hi; ++i) {  // insertion sort, bins hold a few clusters
-      const uint32_t id = B.orig_id[i];
-      const float2 v = B.yz[i];
-      uint32_t j = i;
-      while (j > lo && B.orig_id[j - 1] > id) {
-        B.orig_id[j] = B.orig_id[j - 1];
-        B.yz[j] = B.yz[j - 1];
-        --j;
+  if ((B.cnt->error & TPC_DEVERR_BINS) || B.cnt->n_rows_generic == 0u) return;
+  for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
+    const tpc_row_desc d = B.row_desc[sr];
+    if (d.pad_ || d.count == 0) continue;
+    const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
+    for (uint32_t bb = threadIdx.x; bb < nb; bb += blockDim.x) {
+      const uint32_t b = d.bin_ofs + bb;
+      const uint32_t lo = B.bin_start[b], hi = B.bin_start[b + 1];
+      for (uint32_t i = lo + 1; i < hi; ++i) {  // insertion sort, bins hold a few clusters
+        const uint32_t id = B.orig_id[i];
+        const float2 v = B.yz[i];
+        uint32_t j = i;
+        while (j > lo && B.orig_id[j - 1] > id) {
+          B.orig_id[j] = B.orig_id[j - 1];
+          B.yz[j] = B.yz[j - 1];
+          --j;
+        }
+        B.orig_id[j] = id;
+        B.yz[j] = v;
       }
-      B.orig_id[j] = id;
-      B.yz[j] = v;
     }
   }
 }
@@ -417,13 +429,13 @@ __global__ void __launch_bounds__(256) k_bin_sort(TpcBuffers B) {
 __global__ void __launch_bounds__(TPC_RS_THREADS, 1) k_row_sort(TpcBuffers B) {
   extern __shared__ uint32_t rs_mem[];   // [nbw] packed bin counters / cursors | inv (16-bit)
   __shared__ uint32_t sm[33];
-  if ((B.cnt->error & TPC_DEVERR_BINS) || !B.cnt->grid_rows) return;
+  if (B.cnt->error & TPC_DEVERR_BINS) return;
   if (blockIdx.x == 0 && threadIdx.x == 0) B.bin_start[B.cnt->n_bins] = B.cnt->n_sorted;
   const TpcConst* __restrict__ K = B.K;
   const uint32_t tid = threadIdx.x;
   for (uint32_t sr = blockIdx.x; sr < B.n_sr; sr += gridDim.x) {
     const tpc_row_desc d = B.row_desc[sr];
-    if (d.count == 0) continue;
+    if (d.count == 0 || !d.pad_) continue;                   // (rows that do not qualify go to the generic kernels)
     const uint32_t nb = (uint32_t)d.ny * (uint32_t)d.nz;
     const uint32_t nbw = (nb + 1) / 2;                       // counter words
     uint16_t* inv = reinterpret_cast<uint16_t*>(rs_mem + nbw);
@@ -2172,7 +2184,7 @@ __global__ void k_init(TpcBuffers B) {
     c.n_sorted = c.n_ignored = c.n_dropped = c.n_bad = 0;
     c.n_bins = c.n_tiles = c.n_seeds = c.n_tracklets = 0;
     c.n_tracks = c.n_ids = c.error = 0;
-    c.grid_rows = 0;
+    c.grid_rows = 0; c.n_rows_generic = 0;
     for (int a = 0; a < 3; ++a)
       for (int b = 0; b < 3; ++b) c.follow_work[a][b] = 0ull;
     c.follow_next[0] = c.follow_next[1] = c.follow_next[2] = 0u; c.pad_ = 0u;
@@ -2811,7 +2823,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   cudaFuncSetAttribute(k_row_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, TPC_RS_SMEM_BYTES);
   k_row_sort<<<min((uint32_t)n_sm, B.n_sr), TPC_RS_THREADS, TPC_RS_SMEM_BYTES, st>>>(B);
   TPC_LAUNCH_CHECK("k_row_sort");
-  k_zero_bins<<<grid_for(B.max_bins / 4 + 1, 256, n_sm, 8), 256, 0, st>>>(B);
+  k_zero_bins<<<grid_for((uint64_t)B.n_sr * 256, 256, n_sm, 8), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_zero_bins");
   k_bin_hist<<<grid_for(B.n, 256, n_sm, resident_ctas(k_bin_hist, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_bin_hist");
@@ -2820,7 +2832,7 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   k_scatter<<<grid_for(B.n, 256, n_sm, resident_ctas(k_scatter, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_scatter");
 #if TPC_DET
-  k_bin_sort<<<grid_for(B.max_bins, 256, n_sm, resident_ctas(k_bin_sort, 256)), 256, 0, st>>>(B);
+  k_bin_sort<<<grid_for((uint64_t)B.n_sr * 256, 256, n_sm, resident_ctas(k_bin_sort, 256)), 256, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_bin_sort");
 #endif
   if (timers) cudaEventRecord(E.ev[1], st);

@@ -25,7 +25,7 @@ def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.GeomDesc) == 40
     assert ctypes.sizeof(B.Params) == 120
     assert B.Params.max_bins.offset == 96 and B.Params.max_seeds.offset == 104
-    assert ctypes.sizeof(B.TrackView) == 184 and ctypes.sizeof(B.DebugView) == 136
+    assert ctypes.sizeof(B.TrackView) == 192 and ctypes.sizeof(B.DebugView) == 136
     assert B.TRACK_FIT_DTYPE.itemsize == 192 and B.MERGED_DTYPE.itemsize == 40
     assert ctypes.sizeof(B.MergeParams) == 60 and ctypes.sizeof(B.MergedView) == 88
     assert B.TRACK_FIT3_DTYPE.itemsize == 100 and ctypes.sizeof(B.FitParams) == 12 and ctypes.sizeof(B.FitView) == 40

@@ -115,6 +115,27 @@ def test_det_parity_shuffled_input_and_ragged_sizes(B):
     assert_det_parity(B, cl, grid_by_rows=0)      # generic histogram / scan / scatter path
 
 
+def test_det_parity_one_oversized_row_leaves_the_others_on_the_row_path(B):
+    """The choice between the per-row grid build (k_row_sort) and the generic kernels is made ROW BY
+    ROW: a frame with one row of 70 000 records (>= 65536: does not fit the 16-bit tables) sends that
+    row, and only that row, to the generic path; every stage stays bit-exact."""
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=700, seed=33))
+    rng = np.random.default_rng(2)
+    big = np.zeros(70_000, dtype=cl.dtype)
+    big["sector"], big["row"] = 4, 77
+    big["y"] = rng.uniform(-25, 25, len(big))
+    big["z"] = rng.uniform(0, 240, len(big))
+    cl = np.concatenate([cl, big])
+    cl = cl[np.lexsort((cl["row"], cl["sector"]))]          # clusteriser order
+    gp, op = params_pair(B)
+    tracks, ids, shared, view, gi = run_gpu(B, cl, gp, DET)
+    assert view.grid_by_rows == 0 and view.n_rows_generic == 1
+    o = oracle.run(cl, params=op, n_threads=NT)
+    for name, bad in (("grid", parity.compare_grid(gi, o)), ("links", parity.compare_links(gi, o, len(cl))),
+                      ("tracklets", parity.compare_tracklets(gi, o)), ("tracks", parity.compare_tracks(tracks, ids, shared, o))):
+        assert parity.all_zero(bad), (name, bad)
+
+
 def test_det_parity_other_bin_sizes(B):
     cl, _, _ = dg.generate(dg.preset("C1"))
     ref = oracle.run(cl)
