@@ -185,11 +185,11 @@ def oracle_sample(clusters: np.ndarray, budget_clusters: int):
     return lo, hi, tot
 
 
-def time_oracle(clusters, workload, lo, hi, n_threads=1):
+def time_oracle(clusters, workload, lo, hi, n_threads=1, want=("tracks",)):
     import oracle
     t0 = time.perf_counter()
     o = oracle.run(clusters, params=oracle_params(workload), sector_lo=lo, sector_hi=hi, n_threads=n_threads,
-                   want=("tracks",))
+                   want=want)
     return time.perf_counter() - t0, o
 
 
@@ -519,7 +519,7 @@ def run_ours(args, rank, world, local_rank):
     cpu_o, cpu_lo, cpu_hi = None, 0, 0
     if world == 1 and not args.no_cpu_baseline:
         lo, hi, n_sample = oracle_sample(clusters, args.oracle_budget)
-        dt, o = time_oracle(clusters, args.workload, lo, hi)
+        dt, o = time_oracle(clusters, args.workload, lo, hi, want=("seeds", "tracklets", "tracks"))
         cpu_o, cpu_lo, cpu_hi = o, lo, hi
         names = ("grid", "neighbours", "cleanup_seeds", "follower", "selector")
         cpu = {"value": n_sample / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
@@ -563,12 +563,26 @@ def run_ours(args, rank, world, local_rank):
             trk.track(d_clusters, flags=flags & ~B.TPC_STAGE_TIMERS, stream=stream)
             g_tracks, g_ids, g_shared, gv = trk.tracks()
         if cpu is not None and args.mode == "fast":
+            # tracklet level on the sampled sectors tracked alone with intermediates kept (where every
+            # decision of the follower coincides, parameters must agree), track level on the frame's run
             from oracle import parity as op_
+            sel = (clusters["sector"] >= cpu_lo) & (clusters["sector"] < cpu_hi)
+            base = int(np.flatnonzero(sel)[0])
+            t2 = B.SectorTracker(params=B.tpc_default_params(**pkw), device=local_rank)
+            t2.track(t2.upload(clusters[sel]), flags=B.TPC_KEEP_INTERMEDIATES)
+            gi = t2.intermediates()
+            t2.close()
+            gi["orig_id"] = gi["orig_id"] + np.uint32(base)
+            gi["tracklets"]["seed_id"] += np.uint32(base)
+            tls, identical = op_.compare_tracklets_fast(gi, cpu_o)
+            del gi
             m = (g_tracks["sector"] >= cpu_lo) & (g_tracks["sector"] < cpu_hi)
-            stp = op_.compare_tracks_fast(g_tracks[m], g_ids, g_shared, cpu_o)
-            parity_obj = {"what": f"fast build vs oracle, tracks of sectors [{cpu_lo},{cpu_hi}) of this frame",
-                          **{k: stp[k] for k in ("n_gpu", "n_oracle", "n_paired_key", "n_paired_overlap", "n_list_diff",
-                                                 "n_param_bad", "max_rel")}}
+            stp = op_.compare_tracks_fast(g_tracks[m], g_ids, g_shared, cpu_o, identical_tracklets=identical)
+            parity_obj = {"what": f"fast build vs oracle, sectors [{cpu_lo},{cpu_hi}) of this frame (DESIGN.md section 7)",
+                          "tracklets": {k: tls[k] for k in ("n_paired", "n_both_accepted", "n_identical_hits", "n_param_bad",
+                                                            "max_err_in_sigma", "max_rel_per_param")},
+                          "tracks": {k: stp[k] for k in ("n_gpu", "n_oracle", "n_paired_key", "n_paired_overlap",
+                                                         "n_list_diff", "n_param_bad")}}
         # (2) sector-track refit + merging
         ms_refit = timed(lambda: B.tpc_refit_tracks(trk.ctx, stream.cuda_stream), lambda: B.tpc_get_refit(trk.ctx))
         extras["refit"] = {"ms": ms_refit, "tracks": int(gv.n_tracks), "clusters_refitted_per_s": int(gv.n_cluster_ids) / (ms_refit * 1e-3)}
