@@ -20,7 +20,11 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form geometry, exact-helix
  * propagation, finite-difference Jacobian, Kalman update == weighted least squares,
  * unit-width pulls, brute-force neighbour search, grid invariants + brute-force window
- * queries, link/seed invariants, selector invariants and constructed cases.
+ * queries, link/seed invariants, selector invariants and constructed cases; the follower's road
+ * search by hand-computed cases on a radial straight track and a brute-force linear scan of every
+ * search (test_oracle_road_search.py); merging (test_oracle_merging.py) and the three-iteration fit
+ * (test_oracle_trackfit.py) by exact geometry, textbook least squares and hand-built cases.  Each
+ * group is mutation-checked.
  * Parity unpinned: absolute efficiency / clone / fake values (the paper's Fig. 2 is an
  * image that is not in PAPER.md and is ALICE MC); only sanity floors are tested.
  */
