@@ -14,8 +14,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "liboracle.so")
-_SRCS = [os.path.join(_HERE, f) for f in ("tpc_oracle.cpp", "tpc_merge_oracle.cpp", "tpc_fit_oracle.cpp", "tpc_oracle.h",
-                                          "tpc_oracle_math.hpp")]
+_SRCS = [os.path.join(_HERE, f) for f in ("tpc_oracle.cpp", "tpc_merge_oracle.cpp", "tpc_fit_oracle.cpp",
+                                          "tpc_rebuild_oracle.cpp", "tpc_oracle.h", "tpc_oracle_math.hpp")]
 
 CLUSTER_DTYPE = np.dtype(
     [("y", "<f4"), ("z", "<f4"), ("q", "<f4"), ("sector", "u1"), ("row", "u1"), ("flags", "<u2")])
@@ -70,7 +70,7 @@ def build(force: bool = False) -> str:
             and all(os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in _SRCS)):
         return _LIB
     cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-shared", "-fPIC", "-pthread",
-           _SRCS[0], _SRCS[1], _SRCS[2], "-o", _LIB]
+           _SRCS[0], _SRCS[1], _SRCS[2], _SRCS[3], "-o", _LIB]
     subprocess.run(cmd, check=True)
     return _LIB
 

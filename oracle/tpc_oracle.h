@@ -205,6 +205,32 @@ float orc_fit_track(const orc_geom* g, const orc_params* p, const orc_fit_params
                     const int32_t* row, const float* y, const float* z, int n, const float* start_stq,
                     float* out_state, float* chi2_cluster, uint8_t* rejected, int32_t* n_used);
 
+/* ---- R11 Phase-II track rebuild (tpc_rebuild_oracle.cpp; section 3) ---- */
+#define ORC_RB_NCAND 3 /* candidates kept per (track, path step) */
+typedef struct orc_rebuild_params {
+  float cand_chi2_max;   /* (16) a cluster is a candidate if its chi2 against the interpolation is below */
+  float final_chi2_max;  /* (16) plain cut of the third iteration                                       */
+  int32_t min_clusters;  /* (10) fewer used clusters: the fit fails                                     */
+  float ce_var;          /* (1e4 cm^2) as orc_fit_params                                                */
+} orc_rebuild_params;
+typedef struct orc_rb_segment { int32_t sector, row_first, row_last; } orc_rb_segment;
+void orc_rebuild_default_params(orc_rebuild_params* r);
+/* number of (sector,row) steps on the path of a chain of segments */
+int64_t orc_rebuild_path_len(const orc_rb_segment* seg, int32_t n_seg);
+/* Phase II for ALL merged tracks of a frame (the second ambiguity solving couples them).  Per merged
+ * track m: segments segs[seg_ofs[m]..seg_ofs[m+1]), original clusters cluster_ids[clu_ofs[m]..) in chain
+ * order, start (s,t,q), valid flag, a unique 64-bit id for exact ties, path steps [step_ofs[m],
+ * step_ofs[m+1]).  Outputs per step: up to ORC_RB_NCAND candidates (original ids, -1 none) with their
+ * chi2, the attached cluster (-1 none), shared / used flags; per track: x,p[5],c[15] (21 floats) at the
+ * innermost used cluster, chi2 of pass 3, attached / used counts, flags (1 = failed).
+ * Returns 0, -1 bad argument, -2 inconsistent offsets. */
+int orc_rebuild(const orc_geom* g, const orc_params* p, const orc_rebuild_params* r, const orc_cluster* clusters,
+                uint64_t n_clusters, int32_t n_merged, const int32_t* seg_ofs, const orc_rb_segment* segs,
+                const int64_t* clu_ofs, const uint32_t* cluster_ids, const float* start_stq, const uint8_t* valid,
+                const uint64_t* key_id, const int64_t* step_ofs, int32_t* cand_id, float* cand_chi2,
+                int32_t* attached, uint8_t* shared, uint8_t* used, float* fit, float* chi2, int32_t* n_attached,
+                int32_t* n_used, uint8_t* flags);
+
 #ifdef __cplusplus
 }
 #endif
