@@ -418,6 +418,44 @@ int tpc_fit_tracks(tpc_ctx* ctx, const tpc_fit_params* params, void* d_fit_works
                    void* cuda_stream);
 int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out);
 
+/* PHASE-II TRACK REBUILD (section 3: "the track is practically rebuilt during iterations 2
+ * and 3 of the fit ... the fast cluster search grid from the sector tracking is queried for all clusters
+ * compatible with the chi2 cut and all candidates together with their residuals are written to temporary
+ * storage ... a second ambiguity solving step ... tracks failing to get their best candidate attached are
+ * still eligible for the second candidate"; "a simple chi2 cut for final cluster rejection";
+ * DESIGN.md reading R11).  Runs on the merged tracks of tpc_merge_tracks; needs the tracking workspace
+ * of the run still intact (it queries its grid).  A merged track's PATH = the (sector,row) steps of its
+ * segments and of the holes between segments of one sector.  Results per path step: up to 3 candidates
+ * (original cluster ids) with their chi2 against the interpolation, the attached cluster after the
+ * second ambiguity solving (owned or shared), whether the third pass used it; per merged track the final
+ * parameters (tpc_track_fit3; n_clusters = attached, n_used = used). */
+typedef struct tpc_rebuild_params {
+  float cand_chi2_max;       /* (16) candidate cut against the interpolation (2 dof)                  */
+  float final_chi2_max;      /* (16) plain cut of the third pass                                      */
+  int32_t min_clusters;      /* (10) fewer used clusters: the fit fails                               */
+  float ce_var;              /* (1e4 cm^2) as tpc_fit_params                                          */
+} tpc_rebuild_params;        /* 16 bytes */
+typedef struct tpc_rebuild_view {
+  uint64_t n_merged, n_steps;
+  const uint32_t* d_step_ofs;      /* [n_merged+1] first path step of each merged track              */
+  const int32_t* d_cand_id;        /* [n_steps][3] original cluster ids, -1 none, best first         */
+  const float* d_cand_chi2;        /* [n_steps][3]                                                   */
+  const int32_t* d_attached;       /* [n_steps] original cluster id or -1                            */
+  const uint8_t* d_shared;         /* [n_steps] 1 = attached as shared                               */
+  const uint8_t* d_used;           /* [n_steps] 1 = passed the cut of the third pass                 */
+  const tpc_track_fit3* d_fit;     /* [n_merged]                                                     */
+} tpc_rebuild_view;
+void tpc_rebuild_default_params(tpc_rebuild_params* out);
+/* Computes the path lengths of the merged tracks (needs tpc_merge_tracks; synchronises cuda_stream) and
+ * returns their sum in *n_steps (HOST): the size tpc_rebuild_workspace_bytes needs. */
+int tpc_rebuild_prepare(tpc_ctx* ctx, void* cuda_stream, uint64_t* n_steps);
+size_t tpc_rebuild_workspace_bytes(const tpc_ctx* ctx, uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters);
+/* d_rebuild_workspace: DEVICE, 256-byte aligned, caller owned.  TPC_E_STATE unless tpc_rebuild_prepare ran
+ * on the current merged result. */
+int tpc_rebuild_tracks(tpc_ctx* ctx, const tpc_rebuild_params* params, void* d_rebuild_workspace,
+                       size_t workspace_bytes, void* cuda_stream);
+int tpc_get_rebuild(tpc_ctx* ctx, tpc_rebuild_view* out);
+
 /* Number of kernel launches the last tpc_sector_track enqueued. */
 int tpc_last_launch_count(const tpc_ctx* ctx);
 

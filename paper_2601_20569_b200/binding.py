@@ -105,6 +105,16 @@ TRACK_FIT3_DTYPE = np.dtype([("x", "<f4"), ("p", "<f4", (5,)), ("c", "<f4", (15,
 assert TRACK_FIT3_DTYPE.itemsize == 100 and C.sizeof(FitParams) == 12
 
 
+class RebuildParams(C.Structure):
+    _fields_ = [("cand_chi2_max", C.c_float), ("final_chi2_max", C.c_float), ("min_clusters", C.c_int32), ("ce_var", C.c_float)]
+
+
+class RebuildView(C.Structure):
+    _fields_ = [("n_merged", C.c_uint64), ("n_steps", C.c_uint64), ("d_step_ofs", C.c_void_p), ("d_cand_id", C.c_void_p),
+                ("d_cand_chi2", C.c_void_p), ("d_attached", C.c_void_p), ("d_shared", C.c_void_p), ("d_used", C.c_void_p),
+                ("d_fit", C.c_void_p)]
+
+
 class DebugView(C.Structure):
     _fields_ = [("n_clusters", C.c_uint64), ("n_sorted", C.c_uint64), ("n_rows_total", C.c_uint64),
                 ("n_bins", C.c_uint64), ("n_seeds", C.c_uint64), ("tracklet_stride", C.c_uint64),
@@ -119,7 +129,9 @@ EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_se
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
            "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_merge_default_params",
            "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_fit_default_params",
-           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_last_launch_count",
+           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_rebuild_default_params",
+           "tpc_rebuild_prepare", "tpc_rebuild_workspace_bytes", "tpc_rebuild_tracks", "tpc_get_rebuild",
+           "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
 
 _lib = None
@@ -182,6 +194,16 @@ def load_library():
     L.tpc_fit_tracks.argtypes = [vp, C.POINTER(FitParams), vp, C.c_size_t, vp]
     L.tpc_get_fit.restype = C.c_int
     L.tpc_get_fit.argtypes = [vp, C.POINTER(FitView)]
+    L.tpc_rebuild_default_params.restype = None
+    L.tpc_rebuild_default_params.argtypes = [C.POINTER(RebuildParams)]
+    L.tpc_rebuild_prepare.restype = C.c_int
+    L.tpc_rebuild_prepare.argtypes = [vp, vp, C.POINTER(C.c_uint64)]
+    L.tpc_rebuild_workspace_bytes.restype = C.c_size_t
+    L.tpc_rebuild_workspace_bytes.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint64]
+    L.tpc_rebuild_tracks.restype = C.c_int
+    L.tpc_rebuild_tracks.argtypes = [vp, C.POINTER(RebuildParams), vp, C.c_size_t, vp]
+    L.tpc_get_rebuild.restype = C.c_int
+    L.tpc_get_rebuild.argtypes = [vp, C.POINTER(RebuildView)]
     L.tpc_last_launch_count.restype = C.c_int
     L.tpc_last_launch_count.argtypes = [vp]
     L.tpc_destroy.restype = None
@@ -358,6 +380,35 @@ def tpc_fit_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, cud
 def tpc_get_fit(ctx: int):
     v = FitView()
     rc = load_library().tpc_get_fit(ctx, C.byref(v))
+    return rc, v
+
+
+def tpc_rebuild_default_params(**overrides) -> RebuildParams:
+    r = RebuildParams()
+    load_library().tpc_rebuild_default_params(C.byref(r))
+    for k, v in overrides.items():
+        setattr(r, k, v)
+    return r
+
+
+def tpc_rebuild_prepare(ctx: int, cuda_stream: int):
+    n = C.c_uint64(0)
+    rc = load_library().tpc_rebuild_prepare(ctx, cuda_stream, C.byref(n))
+    return rc, int(n.value)
+
+
+def tpc_rebuild_workspace_bytes(ctx: int, n_steps: int, n_merged: int, n_clusters: int) -> int:
+    return int(load_library().tpc_rebuild_workspace_bytes(ctx, n_steps, n_merged, n_clusters))
+
+
+def tpc_rebuild_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, cuda_stream: int) -> int:
+    return load_library().tpc_rebuild_tracks(ctx, C.byref(params) if params is not None else None, d_workspace,
+                                             workspace_bytes, cuda_stream)
+
+
+def tpc_get_rebuild(ctx: int):
+    v = RebuildView()
+    rc = load_library().tpc_get_rebuild(ctx, C.byref(v))
     return rc, v
 
 
@@ -558,6 +609,42 @@ class SectorTracker:
             return self.fit_ws[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
         return (arr(fv.d_fit, int(fv.n_merged), TRACK_FIT3_DTYPE), arr(fv.d_chi2_cluster, int(fv.n_cluster_ids), np.float32),
                 arr(fv.d_rejected, int(fv.n_cluster_ids), np.uint8))
+
+    def rebuild(self, rparams: RebuildParams | None = None, stream=None, fetch: bool = True):
+        """Phase-II track rebuild (reading R11) of the merged tracks; merge() must have
+        run and the tracking workspace must be intact.  Returns a dict of arrays."""
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        rc, n_steps = tpc_rebuild_prepare(self.ctx, st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_rebuild_prepare", tpc_last_cuda_error(self.ctx))
+        rc, mv = tpc_get_merged(self.ctx)
+        need = tpc_rebuild_workspace_bytes(self.ctx, n_steps, int(mv.n_merged), self.n)
+        if getattr(self, "rebuild_ws", None) is None or self.rebuild_ws.numel() < need + 256:
+            self.rebuild_ws = None
+            self.rebuild_ws = self.torch.empty(need + 256, dtype=self.torch.uint8, device=self.device)
+        ws_ptr = (self.rebuild_ws.data_ptr() + 255) // 256 * 256
+        rc = tpc_rebuild_tracks(self.ctx, rparams, ws_ptr, need, st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_rebuild_tracks", tpc_last_cuda_error(self.ctx))
+        if not fetch:
+            return None
+        rc, rv = tpc_get_rebuild(self.ctx)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_get_rebuild", tpc_last_cuda_error(self.ctx))
+
+        def arr(buf, ptr, count, dtype):
+            dtype = np.dtype(dtype)
+            if count == 0:
+                return np.zeros(0, dtype=dtype)
+            off = ptr - buf.data_ptr()
+            return buf[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
+        ns, nm = int(rv.n_steps), int(rv.n_merged)
+        w = self.rebuild_ws
+        return dict(view=rv, step_ofs=arr(self.merge_ws, rv.d_step_ofs, nm + 1, np.uint32),
+                    cand_id=arr(w, rv.d_cand_id, 3 * ns, np.int32).reshape(-1, 3),
+                    cand_chi2=arr(w, rv.d_cand_chi2, 3 * ns, np.float32).reshape(-1, 3),
+                    attached=arr(w, rv.d_attached, ns, np.int32), shared=arr(w, rv.d_shared, ns, np.uint8),
+                    used=arr(w, rv.d_used, ns, np.uint8), fit=arr(w, rv.d_fit, nm, TRACK_FIT3_DTYPE))
 
     def track_host(self, h_clusters, d_staging, h_tracks, h_ids, h_shared, flags: int = 0, stream=None):
         """End-to-end call with HOST buffers (torch CPU tensors, pinned for speed): copies the

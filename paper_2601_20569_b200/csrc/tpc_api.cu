@@ -36,6 +36,9 @@ struct tpc_ctx {
   bool refit_done = false;     // tpc_refit_tracks ran on the current result
   bool merged = false;         // tpc_merge_tracks ran on the current result
   bool fitted = false;         // tpc_fit_tracks ran on the current merged result
+  bool rb_prepared = false, rebuilt = false;   // tpc_rebuild_prepare / tpc_rebuild_tracks ran on it
+  uint64_t rb_n_steps = 0;
+  TpcRebuildBuffers rbuf;
   TpcMergeBuffers mbuf;
   TpcFitBuffers fbuf;
   uint32_t fit_n_merged = 0, fit_n_ids = 0;
@@ -272,6 +275,7 @@ static int enqueue_track(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n
   ctx->refit_done = false;
   ctx->merged = false;
   ctx->fitted = false;
+  ctx->rb_prepared = false; ctx->rebuilt = false;
   ctx->events.enabled = (flags & TPC_STAGE_TIMERS) != 0;
   (void)cudaGetLastError();
   const int launches = (flags & TPC_DETERMINISTIC)
@@ -752,6 +756,7 @@ size_t carve_merge(const tpc_ctx* c, uint64_t n_tracks, uint64_t n_ids, char* ba
   m.ids = (uint32_t*)take(4 * ((size_t)n_ids + 1));
   m.shared = (uint8_t*)take((size_t)n_ids + 1);
   m.counters = (uint32_t*)take(16);
+  m.path_ofs = (uint32_t*)take(4 * (nt + 1));
   if (M) *M = m;
   return off;
 }
@@ -805,6 +810,7 @@ int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_ws, s
   ctx->synced = false;
   ctx->merged = true;
   ctx->fitted = false;
+  ctx->rb_prepared = false; ctx->rebuilt = false;
   ctx->launches = l;
   return TPC_OK;
 }
@@ -897,6 +903,114 @@ int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out) {
   out->d_fit = ctx->fbuf.fit;
   out->d_chi2_cluster = ctx->fbuf.chi2_cluster;
   out->d_rejected = ctx->fbuf.rejected;
+  return TPC_OK;
+}
+
+// ---------------------------------------------------------------- Phase-II rebuild (R11)
+namespace {
+size_t carve_rebuild(uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters, char* base, TpcRebuildBuffers* R) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) -> char* {
+    char* p = base ? base + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  TpcRebuildBuffers r;
+  std::memset(&r, 0, sizeof(r));
+  const size_t ns = n_steps + 1, nm = n_merged + 1, nc = n_clusters + 1;
+  r.stored = (uint4*)take(16 * ns);
+  r.cand_id = (int32_t*)take(4 * 3 * ns);
+  r.cand_chi2 = (float*)take(4 * 3 * ns);
+  r.attached = (int32_t*)take(4 * ns);
+  r.shared = (uint8_t*)take(ns); r.used = (uint8_t*)take(ns); r.ptr = (uint8_t*)take(ns);
+  r.step_track = (uint32_t*)take(4 * ns);
+  r.Qkey = (uint32_t*)take(4 * nm);
+  r.alive = (uint8_t*)take(nm);
+  r.stq2 = (float*)take(12 * nm);
+  r.bestQ = (uint32_t*)take(4 * nc);
+  r.bestId = (unsigned long long*)take(8 * nc);
+  r.owner = (int32_t*)take(4 * nc);
+  r.fit = (tpc_track_fit3*)take(sizeof(tpc_track_fit3) * nm);
+  if (R) *R = r;
+  return off;
+}
+}  // namespace
+
+void tpc_rebuild_default_params(tpc_rebuild_params* r) {
+  r->cand_chi2_max = 16.0f;
+  r->final_chi2_max = 16.0f;
+  r->min_clusters = 10;
+  r->ce_var = 10000.0f;
+}
+
+int tpc_rebuild_prepare(tpc_ctx* ctx, void* cuda_stream, uint64_t* n_steps) {
+  if (!n_steps) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->merged) return TPC_E_STATE;
+  if (ctx->buf.id_base != 0u) return TPC_E_STATE;   // (whole-frame runs only: cluster ids index the frame)
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  *n_steps = 0;
+  if (ctx->mbuf.n_tracks) {
+    (void)cudaGetLastError();
+    const int l = (ctx->flags & TPC_DETERMINISTIC) ? tpc_det::run_rebuild_paths(ctx->buf, ctx->mbuf, st, ctx->n_sm)
+                                                   : tpc_fast::run_rebuild_paths(ctx->buf, ctx->mbuf, st, ctx->n_sm);
+    if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (rebuild paths)");
+    cudaError_t e = cudaMemcpyAsync(ctx->h_mcnt, ctx->mbuf.counters, 16, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return set_cuda_err(ctx, e, "rebuild paths");
+    *n_steps = ctx->h_mcnt[3];
+  }
+  ctx->rb_n_steps = *n_steps;
+  ctx->rb_prepared = true;
+  ctx->rebuilt = false;
+  return TPC_OK;
+}
+
+size_t tpc_rebuild_workspace_bytes(const tpc_ctx* ctx, uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters) {
+  if (!ctx || n_steps >= (1ull << 32) || n_merged >= (1ull << 31) || n_clusters >= (1ull << 31)) return 0;
+  return carve_rebuild(n_steps, n_merged, n_clusters, nullptr, nullptr);
+}
+
+int tpc_rebuild_tracks(tpc_ctx* ctx, const tpc_rebuild_params* params, void* d_ws, size_t ws_bytes, void* cuda_stream) {
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->merged || !ctx->rb_prepared) return TPC_E_STATE;
+  if (!d_ws || ((uintptr_t)d_ws & 255u)) return TPC_E_ARG;
+  tpc_rebuild_params P;
+  if (params) P = *params; else tpc_rebuild_default_params(&P);
+  if (!(P.cand_chi2_max >= 0.f) || !(P.final_chi2_max >= 0.f) || P.min_clusters < 2 || !(P.ce_var > 0.f)) return TPC_E_ARG;
+  const uint32_t n_merged = ctx->mbuf.n_tracks ? ctx->h_mcnt[0] : 0u;
+  TpcRebuildBuffers R;
+  const size_t need = carve_rebuild(ctx->rb_n_steps, n_merged, ctx->buf.n, (char*)d_ws, &R);
+  if (ws_bytes < need) return TPC_E_WORKSPACE;
+  R.P = P;
+  R.ca = ctx->mbuf.ca; R.sa = ctx->mbuf.sa;
+  R.n_merged = n_merged; R.n_steps = (uint32_t)ctx->rb_n_steps; R.n_clusters = ctx->buf.n;
+  R.step_ofs = ctx->mbuf.path_ofs;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  (void)cudaGetLastError();
+  const int l = (ctx->flags & TPC_DETERMINISTIC) ? tpc_det::run_rebuild(ctx->buf, &ctx->hconst, ctx->mbuf, R, st, ctx->n_sm)
+                                                 : tpc_fast::run_rebuild(ctx->buf, &ctx->hconst, ctx->mbuf, R, st, ctx->n_sm);
+  if (l < 0) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (rebuild)");
+  ctx->rbuf = R;
+  ctx->stream = st;
+  ctx->synced = false;
+  ctx->rebuilt = true;
+  ctx->launches = l;
+  return TPC_OK;
+}
+
+int tpc_get_rebuild(tpc_ctx* ctx, tpc_rebuild_view* out) {
+  if (!out) return TPC_E_ARG;
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  if (!ctx->rebuilt) return TPC_E_STATE;
+  const TpcRebuildBuffers& R = ctx->rbuf;
+  std::memset(out, 0, sizeof(*out));
+  out->n_merged = R.n_merged; out->n_steps = R.n_steps;
+  out->d_step_ofs = R.step_ofs; out->d_cand_id = R.cand_id; out->d_cand_chi2 = R.cand_chi2;
+  out->d_attached = R.attached; out->d_shared = R.shared; out->d_used = R.used; out->d_fit = R.fit;
   return TPC_OK;
 }
 

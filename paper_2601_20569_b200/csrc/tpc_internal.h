@@ -143,7 +143,8 @@ struct TpcMergeBuffers {
   tpc_merged_track* merged;  // [n_tracks]
   uint32_t* seg_index;       // [n_tracks]
   uint32_t* ids; uint8_t* shared;   // [n_ids]
-  uint32_t* counters;        // [4] n_merged, n_links, n_ids out, -
+  uint32_t* counters;        // [4] n_merged, n_links, n_ids out, n_steps (R11 paths)
+  uint32_t* path_ofs;        // [n_tracks+1] first path step of every merged track (R11), exclusive scan
 };
 
 // Buffers of the three-iteration track fit (R10), pointers into the caller's fit workspace.
@@ -156,6 +157,28 @@ struct TpcFitBuffers {
   tpc_track_fit3* fit;     // [n_merged]
 };
 
+// Buffers of the Phase-II rebuild (R11), pointers into the caller's rebuild workspace.
+#define TPC_RB_NCAND 3
+struct TpcRebuildBuffers {
+  tpc_rebuild_params P;
+  float ca, sa;
+  uint32_t n_merged, n_steps, n_clusters;
+  const uint32_t* step_ofs;    // [n_merged+1] (= merge workspace path_ofs)
+  uint4* stored;               // [n_steps] pass-1 prediction: y, z (fp32), halves C00|C10, C11
+  int32_t* cand_id;            // [n_steps][3] original cluster ids, -1 none
+  float* cand_chi2;            // [n_steps][3]
+  int32_t* attached;           // [n_steps]
+  uint8_t* shared; uint8_t* used; uint8_t* ptr;   // [n_steps]
+  uint32_t* step_track;        // [n_steps] merged track of the step
+  uint32_t* Qkey;              // [n_merged] orderable weight
+  uint8_t* alive;              // [n_merged]
+  float* stq2;                 // [n_merged][3] (s,t,q) after pass 2
+  uint32_t* bestQ;             // [n_clusters] per round
+  unsigned long long* bestId;  // [n_clusters] per round
+  int32_t* owner;              // [n_clusters] merged track that owns the cluster, -1 none
+  tpc_track_fit3* fit;         // [n_merged]
+};
+
 #define TPC_MAX_KERNELS 32
 struct TpcStageEvents {
   cudaEvent_t ev[TPC_N_STAGES];  // boundaries: start, after grid, nf, seeds, follower, selector
@@ -166,12 +189,16 @@ struct TpcStageEvents {
 };
 
 namespace tpc_det {
+int run_rebuild_paths(const TpcBuffers& B, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
+int run_rebuild(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcRebuildBuffers& Rb, cudaStream_t stream, int n_sm);
 int run_fit3(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcFitBuffers& T, uint32_t n_merged, cudaStream_t stream, int n_sm);
 int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);
 int run_pipeline(const TpcBuffers& B, const TpcConst* host_const, cudaStream_t stream, uint32_t flags, TpcStageEvents& E, int n_sm);
 }
 namespace tpc_fast {
+int run_rebuild_paths(const TpcBuffers& B, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
+int run_rebuild(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcRebuildBuffers& Rb, cudaStream_t stream, int n_sm);
 int run_fit3(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, const TpcFitBuffers& T, uint32_t n_merged, cudaStream_t stream, int n_sm);
 int run_merge(const TpcBuffers& B, const TpcConst* host_const, const TpcMergeBuffers& M, cudaStream_t stream, int n_sm);
 int run_refit(const TpcBuffers& B, const TpcConst* host_const, uint32_t n_tracks, cudaStream_t stream, int n_sm);

@@ -2558,9 +2558,9 @@ __global__ void __launch_bounds__(256) k_merge_copy_ids(TpcBuffers B, TpcMergeBu
 // cluster of the merged list.  DESIGN.md reading R10.
 __device__ __forceinline__ float fit_round_half(float v) { return __half2float(__float2half_rn(v)); }
 
-__device__ __forceinline__ bool fit_transport(KF& k, int sec0, int row0, int sec1, int row1, float zc,
-                                              const TpcConst* __restrict__ K, const FollowConst& F,
-                                              const TpcFitBuffers& T) {
+__device__ __forceinline__ bool link_transport(KF& k, int sec0, int row0, int sec1, int row1, float zc,
+                                               const TpcConst* __restrict__ K, const FollowConst& F, float ca, float sa,
+                                               float ce_var) {
   if (sec0 == sec1 || sec0 - sec1 == 18 || sec1 - sec0 == 18) {
     const int n = row1 > row0 ? row1 - row0 : row0 - row1;
     const float dx = row1 > row0 ? F.dx : -F.dx;
@@ -2569,14 +2569,19 @@ __device__ __forceinline__ bool fit_transport(KF& k, int sec0, int row0, int sec
     if (sec0 != sec1) {   // central electrode: z re-based on the measurement, its correlations dropped
       k.z = zc;
       k.c10 = 0.f; k.c21 = 0.f; k.c31 = 0.f; k.c41 = 0.f;
-      k.c11 = T.P.ce_var;
+      k.c11 = ce_var;
     }
     return true;
   }
   const float sgn = (sec1 % 18 == (sec0 % 18 + 1) % 18) ? 1.f : -1.f;
   float x = K->x[row0];
-  if (!merge_rotate(k, x, T.ca, sgn * T.sa, F.max_sinphi)) return false;
+  if (!merge_rotate(k, x, ca, sgn * sa, F.max_sinphi)) return false;
   return kf_propagate(k, K->x[row1] - x, F);
+}
+__device__ __forceinline__ bool fit_transport(KF& k, int sec0, int row0, int sec1, int row1, float zc,
+                                              const TpcConst* __restrict__ K, const FollowConst& F,
+                                              const TpcFitBuffers& T) {
+  return link_transport(k, sec0, row0, sec1, row1, zc, K, F, T.ca, T.sa, T.P.ce_var);
 }
 __device__ __forceinline__ void fit_turn(KF& k, float y, float z, const FollowConst& F) {
   k.y = y; k.z = z;
@@ -2719,6 +2724,376 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
   }
 }
 
+// ================================================================== R11 Phase-II track rebuild
+// PAPER.md:59,65 (section 3, Phase II); reading R11.  Kernels:
+//   k_rb_path_len   length of every merged track's path of (sector,row) steps (-> scan -> step offsets)
+//   k_rb_pass12     thread per merged track: pass 1 inward through the original clusters (prediction
+//                   stored at every step), pass 2 outward (interpolation, candidates of the step's row
+//                   from the search grid of the sector tracking, best three kept, update with the best)
+//   k_rb_round_*    thread per step: three proposal rounds of the second ambiguity solving (32-bit
+//                   atomicMax of the weight, 64-bit atomicMin of the id among its holders, resolve, commit)
+//   k_rb_pass3      thread per merged track: shared attachment from the outermost step inward, pass 3
+//                   inward with the plain chi2 cut
+// Iterator over the steps of a merged track, forward (outward) or backward; it also tells which
+// original cluster of the merged list, if any, sits on the step.
+struct RbPath {
+  const uint32_t* segs; const tpc_track* tracks; const uint32_t* ids; const tpc_cluster* cl;
+  int n_seg, n_ids;
+  uint32_t id_base;
+  int g, row, ci, hole_end;
+  bool hole;
+  int sec, f, l;                       // current segment
+  int c_sec, c_row; float c_y, c_z; uint32_t c_id; bool c_ok;   // the next original cluster in walking order
+  __device__ __forceinline__ void load_seg() { const tpc_track t = tracks[segs[g]]; sec = t.sector; f = t.row_first; l = t.row_last; }
+  __device__ __forceinline__ void load_cluster() {
+    c_ok = ci >= 0 && ci < n_ids;
+    if (c_ok) {
+      c_id = ids[ci];
+      const uint4 raw = *reinterpret_cast<const uint4*>(cl + (c_id - id_base));
+      c_y = __uint_as_float(raw.x); c_z = __uint_as_float(raw.y); c_sec = (int)(raw.w & 0xFF); c_row = (int)((raw.w >> 8) & 0xFF);
+    }
+  }
+  __device__ __forceinline__ void begin_fwd() { g = 0; load_seg(); row = f; hole = false; ci = 0; load_cluster(); }
+  __device__ __forceinline__ void begin_bwd() { g = n_seg - 1; load_seg(); row = l; hole = false; ci = n_ids - 1; load_cluster(); }
+  // the original cluster on the current step: true + (id, y, z); the cursor moves on by dir
+  __device__ __forceinline__ bool take_orig(int dir, int32_t& id, float& y, float& z) {
+    if (hole || !c_ok || c_sec != sec || c_row != row) return false;
+    id = (int32_t)c_id; y = c_y; z = c_z;
+    ci += dir;
+    load_cluster();
+    return true;
+  }
+  __device__ __forceinline__ bool next_fwd() {
+    if (!hole) {
+      if (row < l) { ++row; return true; }
+      if (g + 1 >= n_seg) return false;
+      const tpc_track tn = tracks[segs[g + 1]];
+      if ((int)tn.sector == sec && (int)tn.row_first > l + 1) { hole = true; row = l + 1; hole_end = tn.row_first; return true; }
+      ++g; load_seg(); row = f;
+      return true;
+    }
+    if (row + 1 < hole_end) { ++row; return true; }
+    hole = false; ++g; load_seg(); row = f;
+    return true;
+  }
+  __device__ __forceinline__ bool next_bwd() {
+    if (!hole) {
+      if (row > f) { --row; return true; }
+      if (g == 0) return false;
+      const tpc_track tp = tracks[segs[g - 1]];
+      if ((int)tp.sector == sec && f > (int)tp.row_last + 1) { hole = true; row = f - 1; hole_end = tp.row_last; return true; }
+      --g; load_seg(); row = l;
+      return true;
+    }
+    if (row - 1 > hole_end) { --row; return true; }
+    hole = false; --g; load_seg(); row = l;
+    return true;
+  }
+};
+__device__ __forceinline__ RbPath rb_path(const TpcBuffers& B, const TpcMergeBuffers& M, const tpc_merged_track& m) {
+  RbPath P;
+  P.segs = M.seg_index + m.seg_ofs; P.tracks = B.tracks; P.ids = M.ids + m.cluster_ofs; P.cl = B.clusters;
+  P.n_seg = (int)m.n_segments; P.n_ids = (int)m.n_clusters; P.id_base = B.id_base;
+  P.hole = false; P.hole_end = 0; P.c_ok = false;
+  return P;
+}
+
+__global__ void __launch_bounds__(256) k_rb_path_len(TpcBuffers B, TpcMergeBuffers M) {
+  const uint32_t n_merged = M.counters[0];
+  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < M.n_tracks + 1; mi += gridDim.x * blockDim.x) {
+    uint32_t n = 0;
+    if (mi < n_merged) {
+      const tpc_merged_track m = M.merged[mi];
+      const uint32_t* segs = M.seg_index + m.seg_ofs;
+      for (uint32_t g = 0; g < m.n_segments; ++g) {
+        const tpc_track t = B.tracks[segs[g]];
+        n += (uint32_t)(t.row_last - t.row_first + 1);
+        if (g + 1 < m.n_segments) {
+          const tpc_track tn = B.tracks[segs[g + 1]];
+          if (tn.sector == t.sector && tn.row_first > t.row_last + 1) n += (uint32_t)(tn.row_first - t.row_last - 1);
+        }
+      }
+    }
+    M.path_ofs[mi] = n;
+  }
+}
+
+__device__ __forceinline__ uint32_t rb_half2(float a, float b) {
+  return (uint32_t)__half_as_ushort(__float2half_rn(a)) | ((uint32_t)__half_as_ushort(__float2half_rn(b)) << 16);
+}
+__device__ __forceinline__ float rb_unhalf(uint32_t w, int hi) {
+  return __half2float(__ushort_as_half((unsigned short)(hi ? (w >> 16) : (w & 0xFFFFu))));
+}
+
+__global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb,
+                                                   const __grid_constant__ FollowConst F) {
+  const TpcConst* __restrict__ K = B.K;
+  const float w_sel = K->P.sel_chi2_weight;
+  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < Rb.n_merged; mi += gridDim.x * blockDim.x) {
+    const tpc_merged_track m = M.merged[mi];
+    const uint32_t s0 = Rb.step_ofs[mi];
+    const int n = (int)(Rb.step_ofs[mi + 1] - s0);
+    for (int k = 0; k < n; ++k) {
+      const uint32_t e = s0 + (uint32_t)k;
+#pragma unroll
+      for (int j = 0; j < TPC_RB_NCAND; ++j) { Rb.cand_id[(size_t)e * TPC_RB_NCAND + j] = -1; Rb.cand_chi2[(size_t)e * TPC_RB_NCAND + j] = 0.f; }
+      Rb.attached[e] = -1; Rb.shared[e] = 0; Rb.used[e] = 0; Rb.ptr[e] = 0; Rb.step_track[e] = mi;
+    }
+    Rb.alive[mi] = 0; Rb.Qkey[mi] = 0u;
+    const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
+    const tpc_track_fit* ft = B.track_fit + tail;
+    if (ft->flags != 0u || n < 2) continue;
+    RbPath P = rb_path(B, M, m);
+    KF k;
+    k.y = k.z = 0.f;
+    k.s = ft->p_out[2]; k.t = ft->p_out[3]; k.q = ft->p_out[4];
+    kf_init_cov(k, F);
+    int32_t oid; float oy, oz;
+    bool ok = true;
+    // ---- pass 1: inward through the original clusters; the prediction is stored at every step
+    P.begin_bwd();
+    if (!P.take_orig(-1, oid, oy, oz)) continue;       // (cannot happen: a segment's last row holds its last cluster)
+    fit_turn(k, oy, oz, F);
+    float chi1 = 0.f;
+    int n1 = 1, ps = P.sec, pr = P.row;
+    for (int kk = n - 2; kk >= 0 && ok; --kk) {
+      P.next_bwd();
+      const bool has = P.take_orig(-1, oid, oy, oz);
+      if (!link_transport(k, ps, pr, P.sec, P.row, has ? oz : 0.f, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
+      Rb.stored[s0 + (uint32_t)kk] = make_uint4(__float_as_uint(k.y), __float_as_uint(k.z), rb_half2(k.c00, k.c10), rb_half2(k.c11, 0.f));
+      if (has) {
+        const Gain g = kf_gain(k, F);
+        const float c2 = kf_chi2(k, g, oy, oz);
+        if (kf_update(k, g, oy, oz, F)) { ok = false; break; }
+        chi1 = chi1 + c2;
+        ++n1;
+      }
+      ps = P.sec; pr = P.row;
+    }
+    if (!ok) continue;
+    {
+      const int ndf = 2 * n1 - 5;
+      const float Q = (float)n1 - w_sel * (chi1 / (float)(ndf > 0 ? ndf : 1));
+      Rb.Qkey[mi] = f2key(Q);
+    }
+    // ---- pass 2: outward; interpolation, candidates from the search grid, update with the best
+    P.begin_fwd();
+    P.take_orig(+1, oid, oy, oz);
+    fit_turn(k, oy, oz, F);
+    ps = P.sec; pr = P.row;
+    for (int kk = 0; kk < n && ok; ++kk) {
+      if (kk > 0) {
+        P.next_fwd();
+        const bool has = P.take_orig(+1, oid, oy, oz);
+        if (!link_transport(k, ps, pr, P.sec, P.row, has ? oz : 0.f, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
+      }
+      float py, pz, wa, wb, wd;
+      const uint4 st = Rb.stored[s0 + (uint32_t)kk];
+      if (kk == 0) {
+        py = __uint_as_float(st.x); pz = __uint_as_float(st.y); wa = rb_unhalf(st.z, 0); wb = rb_unhalf(st.z, 1); wd = rb_unhalf(st.w, 0);
+      } else if (kk == n - 1) {
+        py = k.y; pz = k.z; wa = k.c00; wb = k.c10; wd = k.c11;
+      } else {
+        const float r1y = __uint_as_float(st.x) - k.y, r1z = __uint_as_float(st.y) - k.z;
+        const float a1 = rb_unhalf(st.z, 0), b1 = rb_unhalf(st.z, 1), d1 = rb_unhalf(st.w, 0), a2 = k.c00, b2 = k.c10, d2 = k.c11;
+        const float det1 = a1 * d1 - b1 * b1, det2 = a2 * d2 - b2 * b2;
+        const float n1i = 1.f / det1, n2i = 1.f / det2;
+        const float i1a = d1 * n1i, i1b = -(b1 * n1i), i1d = a1 * n1i;
+        const float i2a = d2 * n2i, i2b = -(b2 * n2i), i2d = a2 * n2i;
+        const float ia = i1a + i2a, ib = i1b + i2b, id = i1d + i2d;
+        const float detw = ia * id - ib * ib;
+        const float nw = 1.f / detw;
+        wa = id * nw; wb = -(ib * nw); wd = ia * nw;
+        const float hy = i1a * r1y + i1b * r1z, hz = i1b * r1y + i1d * r1z;
+        py = k.y + (wa * hy + wb * hz);
+        pz = k.z + (wb * hy + wd * hz);
+      }
+      const float ry = clampf(F.road_nsigma * sqrtf(wa + F.vy), F.road_min, F.road_max);
+      const float rz = clampf(F.road_nsigma * sqrtf(wd + F.vz), F.road_min, F.road_max);
+      // ---- all clusters of the step's (sector,row) inside the road and the chi2 cut: best three by (chi2, id)
+      int32_t bid[TPC_RB_NCAND];
+      float bchi[TPC_RB_NCAND];
+      float by0 = 0.f, bz0 = 0.f;
+      int nb = 0;
+      const uint32_t sr = (uint32_t)P.sec * (uint32_t)F.R + (uint32_t)P.row;
+      const tpc_row_desc d = ld_row_desc(B.row_desc + sr);
+      if (d.count) {
+        const BinWindow w = make_window(d, K, py - ry, py + ry, pz - rz, pz + rz);
+        for (int bz = w.bz0; bz <= w.bz1; ++bz) {
+          const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
+          const uint32_t c1 = B.bin_start[b + w.by_span];
+          for (uint32_t c = B.bin_start[b]; c < c1; ++c) {
+            const float2 mm = B.yz[c];
+            if (!(fabsf(mm.x - py) <= ry && fabsf(mm.y - pz) <= rz)) continue;
+            const float c2 = fit_chi2_2x2(mm.x - py, mm.y - pz, wa, wb, wd, F.vy, F.vz);
+            if (!(c2 <= Rb.P.cand_chi2_max)) continue;
+            const int32_t id = (int32_t)B.orig_id[c];
+            int pos = nb;
+            while (pos > 0 && (c2 < bchi[pos - 1] || (c2 == bchi[pos - 1] && id < bid[pos - 1]))) --pos;
+            if (pos >= TPC_RB_NCAND) continue;
+            const int last = nb < TPC_RB_NCAND ? nb : TPC_RB_NCAND - 1;
+            for (int j = last; j > pos; --j) { bid[j] = bid[j - 1]; bchi[j] = bchi[j - 1]; }
+            bid[pos] = id; bchi[pos] = c2;
+            if (pos == 0) { by0 = mm.x; bz0 = mm.y; }
+            if (nb < TPC_RB_NCAND) ++nb;
+          }
+        }
+      }
+      const size_t so = (size_t)(s0 + (uint32_t)kk) * TPC_RB_NCAND;
+      for (int j = 0; j < nb; ++j) { Rb.cand_id[so + j] = bid[j]; Rb.cand_chi2[so + j] = bchi[j]; }
+      if (kk > 0 && nb > 0) {
+        const Gain g = kf_gain(k, F);
+        if (kf_update(k, g, by0, bz0, F)) { ok = false; break; }
+      }
+      ps = P.sec; pr = P.row;
+    }
+    if (!ok) {   // a track that failed holds no candidates
+      for (int kk = 0; kk < n; ++kk)
+#pragma unroll
+        for (int j = 0; j < TPC_RB_NCAND; ++j) { Rb.cand_id[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = -1; Rb.cand_chi2[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = 0.f; }
+      continue;
+    }
+    Rb.alive[mi] = 1;
+    Rb.stq2[3 * (size_t)mi] = k.s; Rb.stq2[3 * (size_t)mi + 1] = k.t; Rb.stq2[3 * (size_t)mi + 2] = k.q;
+  }
+}
+
+// ---- second ambiguity solving: the step's best candidate not yet owned (-1 none); the pointer only
+// moves past clusters owned in EARLIER rounds (owner is written by k_rb_round_commit alone)
+__device__ __forceinline__ int32_t rb_proposal(const TpcRebuildBuffers& Rb, uint32_t e) {
+  if (Rb.attached[e] >= 0) return -1;
+  int p = Rb.ptr[e];
+  int32_t out = -1;
+  while (p < TPC_RB_NCAND) {
+    const int32_t c = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
+    if (c < 0) break;
+    if (Rb.owner[c] < 0) { out = c; break; }
+    ++p;
+  }
+  Rb.ptr[e] = (uint8_t)p;
+  return out;
+}
+__global__ void __launch_bounds__(256) k_rb_round_init(TpcRebuildBuffers Rb, int first) {
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < Rb.n_clusters; c += stride) {
+    Rb.bestQ[c] = 0u; Rb.bestId[c] = ~0ull;
+    if (first) Rb.owner[c] = -1;
+  }
+}
+__global__ void __launch_bounds__(256) k_rb_round_q(TpcRebuildBuffers Rb) {
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
+    const uint32_t m = Rb.step_track[e];
+    if (!Rb.alive[m]) continue;
+    const int32_t c = rb_proposal(Rb, e);
+    if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
+  }
+}
+__global__ void __launch_bounds__(256) k_rb_round_id(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb) {
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
+    const uint32_t m = Rb.step_track[e];
+    if (!Rb.alive[m]) continue;
+    const int32_t c = rb_proposal(Rb, e);
+    if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], merge_key(B.tracks[M.merged[m].head]));
+  }
+}
+__global__ void __launch_bounds__(256) k_rb_round_resolve(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb) {
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
+    const uint32_t m = Rb.step_track[e];
+    if (!Rb.alive[m]) continue;
+    const int32_t c = rb_proposal(Rb, e);
+    if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == merge_key(B.tracks[M.merged[m].head])) Rb.attached[e] = c;
+  }
+}
+__global__ void __launch_bounds__(256) k_rb_round_commit(TpcRebuildBuffers Rb) {
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
+    const int32_t c = Rb.attached[e];
+    if (c >= 0) Rb.owner[c] = (int32_t)Rb.step_track[e];   // (one winner per cluster: no race)
+  }
+}
+
+__global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb,
+                                                  const __grid_constant__ FollowConst F) {
+  const TpcConst* __restrict__ K = B.K;
+  const int permille = K->P.shared_permille;
+  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < Rb.n_merged; mi += gridDim.x * blockDim.x) {
+    tpc_track_fit3 out;
+    out.x = 0.f; out.chi2 = 0.f; out.n_clusters = 0u; out.n_used = 0u; out.flags = 1u;
+#pragma unroll
+    for (int i = 0; i < 5; ++i) out.p[i] = 0.f;
+#pragma unroll
+    for (int i = 0; i < 15; ++i) out.c[i] = 0.f;
+    if (!Rb.alive[mi]) { Rb.fit[mi] = out; continue; }
+    const tpc_merged_track m = M.merged[mi];
+    const uint32_t s0 = Rb.step_ofs[mi];
+    const int n = (int)(Rb.step_ofs[mi + 1] - s0);
+    // ---- shared attachment from the outermost step inward (the rule of R6.3)
+    int n_acc = 0, n_sh = 0, last = -1;
+    for (int kk = n - 1; kk >= 0; --kk) {
+      const uint32_t e = s0 + (uint32_t)kk;
+      if (Rb.attached[e] >= 0) { ++n_acc; if (last < 0) last = kk; continue; }
+      const int32_t c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
+      if (c < 0) continue;
+      if ((long long)(n_sh + 1) * 1000 <= (long long)permille * (n_acc + 1)) {
+        Rb.attached[e] = c; Rb.shared[e] = 1; ++n_acc; ++n_sh;
+        if (last < 0) last = kk;
+      }
+    }
+    out.n_clusters = (uint32_t)n_acc;
+    if (last < 0) { Rb.fit[mi] = out; continue; }
+    // ---- pass 3: inward through the attached clusters, plain chi2 cut
+    auto cluster_yz = [&](int32_t id, float& y, float& z) {
+      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + ((uint32_t)id - B.id_base));
+      y = __uint_as_float(raw.x); z = __uint_as_float(raw.y);
+    };
+    RbPath P = rb_path(B, M, m);
+    P.begin_bwd();
+    int32_t oid; float oy, oz;
+    bool has = P.take_orig(-1, oid, oy, oz);
+    for (int kk = n - 1; kk > last; --kk) { P.next_bwd(); has = P.take_orig(-1, oid, oy, oz); }   // walk to the outermost attached step
+    KF k;
+    k.s = Rb.stq2[3 * (size_t)mi]; k.t = Rb.stq2[3 * (size_t)mi + 1]; k.q = Rb.stq2[3 * (size_t)mi + 2];
+    float ay, az;
+    cluster_yz(Rb.attached[s0 + (uint32_t)last], ay, az);
+    fit_turn(k, ay, az, F);
+    Rb.used[s0 + (uint32_t)last] = 1;
+    KF kin = k;
+    int nu = 1, row_in = P.row, ps = P.sec, pr = P.row;
+    float chi3 = 0.f;
+    bool ok = true;
+    for (int kk = last - 1; kk >= 0 && ok; --kk) {
+      P.next_bwd();
+      has = P.take_orig(-1, oid, oy, oz);
+      const int32_t ca = Rb.attached[s0 + (uint32_t)kk];
+      float zc = k.z;
+      if (ca >= 0) { cluster_yz(ca, ay, az); zc = az; }
+      else if (has) zc = oz;
+      if (!link_transport(k, ps, pr, P.sec, P.row, zc, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
+      ps = P.sec; pr = P.row;
+      if (ca < 0) continue;
+      const Gain g = kf_gain(k, F);
+      const float c2 = kf_chi2(k, g, ay, az);
+      if (!(c2 <= Rb.P.final_chi2_max)) continue;   // plain cut: the cluster is dropped, no update
+      if (kf_update(k, g, ay, az, F)) { ok = false; break; }
+      chi3 = chi3 + c2;
+      Rb.used[s0 + (uint32_t)kk] = 1;
+      ++nu;
+      kin = k;
+      row_in = P.row;
+    }
+    out.n_used = (uint32_t)nu;
+    if (ok && nu >= Rb.P.min_clusters) {
+      out.flags = 0u;
+      out.chi2 = chi3;
+      out.x = K->x[row_in];
+      out.p[0] = kin.y; out.p[1] = kin.z; out.p[2] = kin.s; out.p[3] = kin.t; out.p[4] = kin.q;
+      out.c[0] = kin.c00; out.c[1] = kin.c10; out.c[2] = kin.c11; out.c[3] = kin.c20; out.c[4] = kin.c21; out.c[5] = kin.c22;
+      out.c[6] = kin.c30; out.c[7] = kin.c31; out.c[8] = kin.c32; out.c[9] = kin.c33;
+      out.c[10] = kin.c40; out.c[11] = kin.c41; out.c[12] = kin.c42; out.c[13] = kin.c43; out.c[14] = kin.c44;
+    }
+    Rb.fit[mi] = out;
+  }
+}
+
 // ================================================================== host: enqueue the path
 #define TPC_LAUNCH_CHECK(name)                                      \
   do {                                                              \
@@ -2802,6 +3177,30 @@ int run_fit3(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, 
   const FollowConst F = follow_const(hK);
   k_track_fit3<<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3, 128)), 128, 0, st>>>(B, M, T, F);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int run_rebuild_paths(const TpcBuffers& B, const TpcMergeBuffers& M, cudaStream_t st, int n_sm) {
+  k_rb_path_len<<<grid_for((uint64_t)M.n_tracks + 1, 256, n_sm, 8), 256, 0, st>>>(B, M);
+  scan_u32(M.path_ofs, M.n_tracks + 1, M.partials, &M.counters[3], st);
+  return cudaPeekAtLastError() == cudaSuccess ? 4 : -1;
+}
+
+int run_rebuild(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, const TpcRebuildBuffers& Rb, cudaStream_t st,
+                int n_sm) {
+  if (Rb.n_merged == 0) return 0;
+  const FollowConst F = follow_const(hK);
+  const int gt = grid_for(Rb.n_merged, 128, n_sm, 8);
+  const int gs = grid_for((uint64_t)Rb.n_steps + 1, 256, n_sm, 8), gc = grid_for((uint64_t)Rb.n_clusters + 1, 256, n_sm, 8);
+  k_rb_pass12<<<gt, 128, 0, st>>>(B, M, Rb, F);
+  for (int round = 0; round < TPC_RB_NCAND; ++round) {
+    k_rb_round_init<<<gc, 256, 0, st>>>(Rb, round == 0);
+    k_rb_round_q<<<gs, 256, 0, st>>>(Rb);
+    k_rb_round_id<<<gs, 256, 0, st>>>(B, M, Rb);
+    k_rb_round_resolve<<<gs, 256, 0, st>>>(B, M, Rb);
+    k_rb_round_commit<<<gs, 256, 0, st>>>(Rb);
+  }
+  k_rb_pass3<<<gt, 128, 0, st>>>(B, M, Rb, F);
+  return cudaPeekAtLastError() == cudaSuccess ? 2 + 5 * TPC_RB_NCAND : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

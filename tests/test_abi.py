@@ -31,6 +31,8 @@ def test_struct_layouts_match_header():
     assert B.TRACK_FIT3_DTYPE.itemsize == 100 and ctypes.sizeof(B.FitParams) == 12 and ctypes.sizeof(B.FitView) == 40
     f = B.tpc_fit_default_params()
     assert abs(f.fit_chi2_max - 16.0) < 1e-6 and f.fit_min_clusters == 10
+    assert ctypes.sizeof(B.RebuildParams) == 16 and ctypes.sizeof(B.RebuildView) == 72
+    assert abs(B.tpc_rebuild_default_params().cand_chi2_max - 16.0) < 1e-6
     m = B.tpc_merge_default_params()
     assert m.gap_in_sector == 30 and abs(m.chi2_max - 20.0) < 1e-6 and m.stages == 7
 

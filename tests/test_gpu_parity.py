@@ -801,12 +801,8 @@ def test_sector_split_equals_whole_frame(B):
     assert mg.gather_to_root(tracks, ids, shared, 0, 1)[0] is tracks
 
 
-@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
-def test_det_parity_three_iteration_fit(B, name):
-    """SURVEY.md 8(f) row 3 (PAPER.md:31,37,57): the three-iteration fit with interpolation rejection
-    on the merged tracks; deterministic mode: final parameters, chi2, per-cluster interpolation chi2
-    and rejection marks bit-exact against oracle.trackfit."""
-    from oracle import merging, trackfit
+def merged_case_frame(name):
+    """Frames of the merged-track tests: (clusters, parameter overrides)."""
     if name == "C2_full":
         cl, lab, _ = dg.generate(dg.preset("C2"))
         pkw = {}
@@ -833,6 +829,16 @@ def test_det_parity_three_iteration_fit(B, name):
         order = np.lexsort((a[:, 1], a[:, 0]))
         cl["sector"], cl["row"], cl["y"], cl["z"] = a[order, 0], a[order, 1], a[order, 2], a[order, 3]
         pkw = {}
+    return cl, pkw
+
+
+@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
+def test_det_parity_three_iteration_fit(B, name):
+    """SURVEY.md 8(f) row 3 (PAPER.md:31,37,57): the three-iteration fit with interpolation rejection
+    on the merged tracks; deterministic mode: final parameters, chi2, per-cluster interpolation chi2
+    and rejection marks bit-exact against oracle.trackfit."""
+    from oracle import merging, trackfit
+    cl, pkw = merged_case_frame(name)
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
     try:
@@ -881,3 +887,60 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0.02 * len(ro) < ro.sum() < 0.2 * len(ro)
     else:
         assert 0 < ro.sum() < 0.02 * len(ro)
+
+
+@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
+def test_det_parity_phase2_rebuild(B, name):
+    """SURVEY.md 8(f) row 4 (PAPER.md:59,65; reading R11): the Phase-II rebuild of the merged tracks;
+    deterministic mode: per path step the three candidates (ids and chi2 bits), the attached cluster
+    after the second ambiguity solving, the shared and used marks, and per track the final fit, all
+    bit-exact against oracle.rebuild."""
+    from oracle import merging, rebuild
+    cl, pkw = merged_case_frame(name)
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        trk.track(trk.upload(cl), flags=1)
+        tracks, ids, shared, view = trk.tracks()
+        trk.refit()
+        g = trk.merge()
+        r = trk.rebuild()
+    finally:
+        trk.close()
+    o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
+    q = rebuild.rebuild(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids, params=op)
+    nm = len(m.merged)
+    assert len(g["merged"]) == nm > 0 and len(r["fit"]) == nm
+    def order_of(tr, merged):
+        h = merged["head"].astype(np.int64)
+        return np.lexsort((tr["segment"][h], tr["seed_id"][h], tr["sector"][h]))
+    og, oo = order_of(tracks, g["merged"]), order_of(o.tracks, m.merged)
+    gofs, oofs = r["step_ofs"].astype(np.int64), q.step_ofs.astype(np.int64)
+    glen, olen = np.diff(gofs)[og], np.diff(oofs)[oo]
+    assert (glen == olen).all() and int(gofs[-1]) == int(oofs[-1]) == len(r["attached"])
+    def steps(ofs, order, lens):
+        return np.concatenate([np.arange(ofs[k], ofs[k] + n) for k, n in zip(order, lens)]) if len(order) else np.zeros(0, np.int64)
+    sg, so = steps(gofs, og, glen), steps(oofs, oo, olen)
+    assert (r["cand_id"][sg] == q.cand_id[so]).all(), int((r["cand_id"][sg] != q.cand_id[so]).sum())
+    have = q.cand_id[so] >= 0
+    assert (r["cand_chi2"][sg][have].view(np.uint32) == q.cand_chi2[so][have].view(np.uint32)).all()
+    assert (r["attached"][sg] == q.attached[so]).all(), int((r["attached"][sg] != q.attached[so]).sum())
+    assert (r["shared"][sg] == q.shared[so]).all() and (r["used"][sg] == q.used[so]).all()
+    fg, fo = r["fit"][og], q.fit[oo]
+    assert (fg["flags"] == fo["flags"]).all() and (fg["n_used"] == fo["n_used"]).all()
+    assert (fg["n_clusters"] == fo["n_attached"]).all()
+    ok = fo["flags"] == 0
+    for f in ("x", "p", "c", "chi2"):
+        a_, b_ = np.ascontiguousarray(fg[f][ok]).view(np.uint32), np.ascontiguousarray(fo[f][ok]).view(np.uint32)
+        assert (a_ == b_).all(), (f, int((a_ != b_).sum()))
+    # what the rebuild is for: additional clusters in the holes and beyond the segment ends, and every
+    # cluster owned by at most one track
+    att = q.attached[so]
+    own = att[(att >= 0) & (q.shared[so] == 0)]
+    assert len(np.unique(own)) == len(own)
+    assert ok.sum() >= 0.8 * nm
+    if name == "ce_crossing":
+        assert nm == 40 and ok.all()
+    print(f"rebuild {name}: merged {nm} steps {len(so)} attached {(att >= 0).sum()} shared {int(q.shared.sum())} "
+          f"used {int(q.used.sum())} failed {int((~ok).sum())}")
