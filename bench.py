@@ -598,6 +598,27 @@ def run_ours(args, rank, world, local_rank):
                           "clusters": int(len(rej3)), "clusters_rejected": int(rej3.sum())}
         del fit3, _chi, rej3
         trk.fit_ws = None
+        # (2c) the Phase-II rebuild of the merged tracks (8(f) row 4, reading R11); the summary counts are
+        # taken on the device (the per-step arrays of a C4 frame are several GB)
+        try:
+            ms_rb = timed(lambda: trk.rebuild(stream=stream, fetch=False), lambda: B.tpc_get_rebuild(trk.ctx))
+            rc_r, rv = B.tpc_get_rebuild(trk.ctx)
+            ns_, w_ = int(rv.n_steps), trk.rebuild_ws
+
+            def dev(ptr, count, dt, size):
+                off = ptr - w_.data_ptr()
+                return w_[off:off + count * size].view(dt)
+            att_ = dev(rv.d_attached, ns_, torch.int32, 4)
+            fl_ = dev(rv.d_fit, int(rv.n_merged) * 25, torch.int32, 4).view(-1, 25)[:, 24]
+            extras["rebuild"] = {"ms": ms_rb, "merged_tracks": int(rv.n_merged), "path_steps": ns_,
+                                 "attached": int((att_ >= 0).sum()), "shared": int(dev(rv.d_shared, ns_, torch.uint8, 1).sum()),
+                                 "used": int(dev(rv.d_used, ns_, torch.uint8, 1).sum()), "failed": int((fl_ != 0).sum()),
+                                 "workspace_gb": w_.numel() / 1e9,
+                                 "note": "includes one stream synchronisation per call (path length to the host)"}
+            del att_, fl_, w_
+        except Exception as e:
+            extras["rebuild"] = {"error": str(e)[:200]}
+        trk.rebuild_ws = None
         trk.merge_ws = None
         # (3) deterministic mode on the same frame
         if args.mode == "fast":
@@ -633,6 +654,7 @@ def run_ours(args, rank, world, local_rank):
         "stage_ms": {k: round(x, 4) for k, x in stage_ms.items()},
         "kernels_ms_per_step": {k["name"]: round(k["ms_per_step"], 4) for k in per_kernel},
         "cpu_baseline": cpu, "cpu_baseline_all_cores": cpu_all, "refit": refit, "merge": extras.get("merge"), "fit3": extras.get("fit3"),
+        "rebuild": extras.get("rebuild"),
         "det": extras.get("det"), "second_iteration": extras.get("second_iteration"), "parity": parity_obj,
     }
     print(json.dumps(line), flush=True)

@@ -922,9 +922,11 @@ size_t carve_rebuild(uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters, c
   r.cand_id = (int32_t*)take(4 * 3 * ns);
   r.cand_chi2 = (float*)take(4 * 3 * ns);
   r.attached = (int32_t*)take(4 * ns);
-  r.shared = (uint8_t*)take(ns); r.used = (uint8_t*)take(ns); r.ptr = (uint8_t*)take(ns);
+  r.shared = (uint8_t*)take(ns); r.used = (uint8_t*)take(ns);
   r.step_track = (uint32_t*)take(4 * ns);
   r.Qkey = (uint32_t*)take(4 * nm);
+  r.tkey = (unsigned long long*)take(8 * nm);
+  r.list_n = (uint32_t*)take(16);
   r.alive = (uint8_t*)take(nm);
   r.stq2 = (float*)take(12 * nm);
   r.bestQ = (uint32_t*)take(4 * nc);

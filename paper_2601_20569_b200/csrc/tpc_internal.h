@@ -164,17 +164,20 @@ struct TpcRebuildBuffers {
   float ca, sa;
   uint32_t n_merged, n_steps, n_clusters;
   const uint32_t* step_ofs;    // [n_merged+1] (= merge workspace path_ofs)
-  uint4* stored;               // [n_steps] pass-1 prediction: y, z (fp32), halves C00|C10, C11
+  uint4* stored;               // [n_steps] pass-1 prediction: y, z (fp32), halves C00|C10, C11 | bit 16 of .w: the
+                               // step holds an original cluster; after pass 2 the region holds the loser lists
   int32_t* cand_id;            // [n_steps][3] original cluster ids, -1 none
   float* cand_chi2;            // [n_steps][3]
   int32_t* attached;           // [n_steps]
-  uint8_t* shared; uint8_t* used; uint8_t* ptr;   // [n_steps]
+  uint8_t* shared; uint8_t* used;   // [n_steps]
   uint32_t* step_track;        // [n_steps] merged track of the step
   uint32_t* Qkey;              // [n_merged] orderable weight
+  unsigned long long* tkey;    // [n_merged] 64-bit id of the track (that of its head segment)
   uint8_t* alive;              // [n_merged]
   float* stq2;                 // [n_merged][3] (s,t,q) after pass 2
-  uint32_t* bestQ;             // [n_clusters] per round
-  unsigned long long* bestId;  // [n_clusters] per round
+  uint32_t* list_n;            // [4] lengths of the loser lists of rounds 2, 3
+  uint32_t* bestQ;             // [n_clusters]
+  unsigned long long* bestId;  // [n_clusters]
   int32_t* owner;              // [n_clusters] merged track that owns the cluster, -1 none
   tpc_track_fit3* fit;         // [n_merged]
 };

@@ -2754,6 +2754,7 @@ struct RbPath {
     }
   }
   __device__ __forceinline__ void begin_fwd() { g = 0; load_seg(); row = f; hole = false; ci = 0; load_cluster(); }
+  __device__ __forceinline__ void begin_bwd_rows() { g = n_seg - 1; load_seg(); row = l; hole = false; ci = -1; c_ok = false; }
   __device__ __forceinline__ void begin_bwd() { g = n_seg - 1; load_seg(); row = l; hole = false; ci = n_ids - 1; load_cluster(); }
   // the original cluster on the current step: true + (id, y, z); the cursor moves on by dir
   __device__ __forceinline__ bool take_orig(int dir, int32_t& id, float& y, float& z) {
@@ -2818,6 +2819,15 @@ __global__ void __launch_bounds__(256) k_rb_path_len(TpcBuffers B, TpcMergeBuffe
   }
 }
 
+// warp per merged track: the track of every step
+__global__ void __launch_bounds__(256) k_rb_step_track(TpcRebuildBuffers Rb) {
+  const uint32_t lane = threadIdx.x & 31u, wpb = blockDim.x >> 5;
+  for (uint32_t mi = blockIdx.x * wpb + (threadIdx.x >> 5); mi < Rb.n_merged; mi += gridDim.x * wpb) {
+    const uint32_t s0 = Rb.step_ofs[mi], s1 = Rb.step_ofs[mi + 1];
+    for (uint32_t e = s0 + lane; e < s1; e += 32u) Rb.step_track[e] = mi;
+  }
+}
+
 __device__ __forceinline__ uint32_t rb_half2(float a, float b) {
   return (uint32_t)__half_as_ushort(__float2half_rn(a)) | ((uint32_t)__half_as_ushort(__float2half_rn(b)) << 16);
 }
@@ -2833,16 +2843,17 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
     const tpc_merged_track m = M.merged[mi];
     const uint32_t s0 = Rb.step_ofs[mi];
     const int n = (int)(Rb.step_ofs[mi + 1] - s0);
-    for (int k = 0; k < n; ++k) {
-      const uint32_t e = s0 + (uint32_t)k;
+    // a track that fails holds no candidates (pass 2 writes all three entries of every step it reaches)
+    auto no_candidates = [&]() {
+      for (int kk = 0; kk < n; ++kk)
 #pragma unroll
-      for (int j = 0; j < TPC_RB_NCAND; ++j) { Rb.cand_id[(size_t)e * TPC_RB_NCAND + j] = -1; Rb.cand_chi2[(size_t)e * TPC_RB_NCAND + j] = 0.f; }
-      Rb.attached[e] = -1; Rb.shared[e] = 0; Rb.used[e] = 0; Rb.ptr[e] = 0; Rb.step_track[e] = mi;
-    }
+        for (int j = 0; j < TPC_RB_NCAND; ++j) { Rb.cand_id[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = -1; Rb.cand_chi2[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = 0.f; }
+    };
     Rb.alive[mi] = 0; Rb.Qkey[mi] = 0u;
+    Rb.tkey[mi] = merge_key(B.tracks[m.head]);
     const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
     const tpc_track_fit* ft = B.track_fit + tail;
-    if (ft->flags != 0u || n < 2) continue;
+    if (ft->flags != 0u || n < 2) { no_candidates(); continue; }
     RbPath P = rb_path(B, M, m);
     KF k;
     k.y = k.z = 0.f;
@@ -2852,7 +2863,7 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
     bool ok = true;
     // ---- pass 1: inward through the original clusters; the prediction is stored at every step
     P.begin_bwd();
-    if (!P.take_orig(-1, oid, oy, oz)) continue;       // (cannot happen: a segment's last row holds its last cluster)
+    if (!P.take_orig(-1, oid, oy, oz)) { no_candidates(); continue; }   // (cannot happen: a segment's last row holds its last cluster)
     fit_turn(k, oy, oz, F);
     float chi1 = 0.f;
     int n1 = 1, ps = P.sec, pr = P.row;
@@ -2860,7 +2871,8 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
       P.next_bwd();
       const bool has = P.take_orig(-1, oid, oy, oz);
       if (!link_transport(k, ps, pr, P.sec, P.row, has ? oz : 0.f, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
-      Rb.stored[s0 + (uint32_t)kk] = make_uint4(__float_as_uint(k.y), __float_as_uint(k.z), rb_half2(k.c00, k.c10), rb_half2(k.c11, 0.f));
+      Rb.stored[s0 + (uint32_t)kk] = make_uint4(__float_as_uint(k.y), __float_as_uint(k.z), rb_half2(k.c00, k.c10),
+                                                rb_half2(k.c11, 0.f) | (has ? 0x10000u : 0u));
       if (has) {
         const Gain g = kf_gain(k, F);
         const float c2 = kf_chi2(k, g, oy, oz);
@@ -2870,25 +2882,33 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
       }
       ps = P.sec; pr = P.row;
     }
-    if (!ok) continue;
+    if (!ok) { no_candidates(); continue; }
     {
       const int ndf = 2 * n1 - 5;
       const float Q = (float)n1 - w_sel * (chi1 / (float)(ndf > 0 ? ndf : 1));
       Rb.Qkey[mi] = f2key(Q);
     }
-    // ---- pass 2: outward; interpolation, candidates from the search grid, update with the best
+    // ---- pass 2: outward; interpolation, candidates from the search grid, update with the best.  The
+    // stored record says whether the step holds an original cluster; the cluster itself is only read
+    // where the electrode is crossed (z re-based on it).
     P.begin_fwd();
-    P.take_orig(+1, oid, oy, oz);
-    fit_turn(k, oy, oz, F);
+    fit_turn(k, P.c_y, P.c_z, F);
+    int ci = 1;
     ps = P.sec; pr = P.row;
     for (int kk = 0; kk < n && ok; ++kk) {
+      const uint4 st = Rb.stored[s0 + (uint32_t)kk];
       if (kk > 0) {
         P.next_fwd();
-        const bool has = P.take_orig(+1, oid, oy, oz);
-        if (!link_transport(k, ps, pr, P.sec, P.row, has ? oz : 0.f, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
+        const bool has = (st.w >> 16) & 1u;
+        float zc = 0.f;
+        if (has) {
+          if (P.sec != ps) zc = B.clusters[P.ids[ci] - B.id_base].z;
+          ++ci;
+        }
+        if (!link_transport(k, ps, pr, P.sec, P.row, zc, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
       }
+      const uint32_t sr = (uint32_t)P.sec * (uint32_t)F.R + (uint32_t)P.row;
       float py, pz, wa, wb, wd;
-      const uint4 st = Rb.stored[s0 + (uint32_t)kk];
       if (kk == 0) {
         py = __uint_as_float(st.x); pz = __uint_as_float(st.y); wa = rb_unhalf(st.z, 0); wb = rb_unhalf(st.z, 1); wd = rb_unhalf(st.w, 0);
       } else if (kk == n - 1) {
@@ -2910,104 +2930,129 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
       }
       const float ry = clampf(F.road_nsigma * sqrtf(wa + F.vy), F.road_min, F.road_max);
       const float rz = clampf(F.road_nsigma * sqrtf(wd + F.vz), F.road_min, F.road_max);
-      // ---- all clusters of the step's (sector,row) inside the road and the chi2 cut: best three by (chi2, id)
-      int32_t bid[TPC_RB_NCAND];
-      float bchi[TPC_RB_NCAND];
+      // ---- all clusters of the step's (sector,row) inside the road and the chi2 cut: best three by
+      // (chi2, original id); kept by sorted position, the ids are read at the end (and on a chi2 tie)
+      static_assert(TPC_RB_NCAND == 3, "the insertion below is written out for three candidates");
+      uint32_t bpos[TPC_RB_NCAND] = {0u, 0u, 0u};
+      float bchi[TPC_RB_NCAND] = {INFINITY, INFINITY, INFINITY};   // (an empty entry sorts behind every candidate)
       float by0 = 0.f, bz0 = 0.f;
       int nb = 0;
-      const uint32_t sr = (uint32_t)P.sec * (uint32_t)F.R + (uint32_t)P.row;
       const tpc_row_desc d = ld_row_desc(B.row_desc + sr);
       if (d.count) {
         const BinWindow w = make_window(d, K, py - ry, py + ry, pz - rz, pz + rz);
+        uint32_t b = w.base + (uint32_t)w.bz0 * (uint32_t)w.ny;
+        uint32_t c = B.bin_start[b], c1 = B.bin_start[b + w.by_span];
         for (int bz = w.bz0; bz <= w.bz1; ++bz) {
-          const uint32_t b = w.base + (uint32_t)bz * (uint32_t)w.ny;
-          const uint32_t c1 = B.bin_start[b + w.by_span];
-          for (uint32_t c = B.bin_start[b]; c < c1; ++c) {
+          uint32_t cn = 0u, cn1 = 0u;
+          if (bz < w.bz1) { cn = B.bin_start[b + (uint32_t)w.ny]; cn1 = B.bin_start[b + (uint32_t)w.ny + w.by_span]; }   // next z-row: requested before this one is scanned
+          for (; c < c1; ++c) {
             const float2 mm = B.yz[c];
             if (!(fabsf(mm.x - py) <= ry && fabsf(mm.y - pz) <= rz)) continue;
             const float c2 = fit_chi2_2x2(mm.x - py, mm.y - pz, wa, wb, wd, F.vy, F.vz);
             if (!(c2 <= Rb.P.cand_chi2_max)) continue;
-            const int32_t id = (int32_t)B.orig_id[c];
-            int pos = nb;
-            while (pos > 0 && (c2 < bchi[pos - 1] || (c2 == bchi[pos - 1] && id < bid[pos - 1]))) --pos;
-            if (pos >= TPC_RB_NCAND) continue;
-            const int last = nb < TPC_RB_NCAND ? nb : TPC_RB_NCAND - 1;
-            for (int j = last; j > pos; --j) { bid[j] = bid[j - 1]; bchi[j] = bchi[j - 1]; }
-            bid[pos] = id; bchi[pos] = c2;
-            if (pos == 0) { by0 = mm.x; bz0 = mm.y; }
+            auto before = [&](int j) { return c2 < bchi[j] || (c2 == bchi[j] && B.orig_id[c] < B.orig_id[bpos[j]]); };
+            if (before(0)) {
+              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = bpos[0]; bchi[1] = bchi[0]; bpos[0] = c; bchi[0] = c2;
+              by0 = mm.x; bz0 = mm.y;
+            } else if (before(1)) {
+              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = c; bchi[1] = c2;
+            } else if (before(2)) {
+              bpos[2] = c; bchi[2] = c2;
+            } else {
+              continue;
+            }
             if (nb < TPC_RB_NCAND) ++nb;
           }
+          b += (uint32_t)w.ny; c = cn; c1 = cn1;
         }
       }
       const size_t so = (size_t)(s0 + (uint32_t)kk) * TPC_RB_NCAND;
-      for (int j = 0; j < nb; ++j) { Rb.cand_id[so + j] = bid[j]; Rb.cand_chi2[so + j] = bchi[j]; }
+#pragma unroll
+      for (int j = 0; j < TPC_RB_NCAND; ++j) {
+        const bool in = j < nb;
+        Rb.cand_id[so + j] = in ? (int32_t)B.orig_id[bpos[j]] : -1;
+        Rb.cand_chi2[so + j] = in ? bchi[j] : 0.f;
+      }
       if (kk > 0 && nb > 0) {
         const Gain g = kf_gain(k, F);
         if (kf_update(k, g, by0, bz0, F)) { ok = false; break; }
       }
       ps = P.sec; pr = P.row;
     }
-    if (!ok) {   // a track that failed holds no candidates
-      for (int kk = 0; kk < n; ++kk)
-#pragma unroll
-        for (int j = 0; j < TPC_RB_NCAND; ++j) { Rb.cand_id[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = -1; Rb.cand_chi2[(size_t)(s0 + kk) * TPC_RB_NCAND + j] = 0.f; }
-      continue;
-    }
+    if (!ok) { no_candidates(); continue; }
     Rb.alive[mi] = 1;
     Rb.stq2[3 * (size_t)mi] = k.s; Rb.stq2[3 * (size_t)mi + 1] = k.t; Rb.stq2[3 * (size_t)mi + 2] = k.q;
   }
 }
 
-// ---- second ambiguity solving: the step's best candidate not yet owned (-1 none); the pointer only
-// moves past clusters owned in EARLIER rounds (owner is written by k_rb_round_commit alone)
-__device__ __forceinline__ int32_t rb_proposal(const TpcRebuildBuffers& Rb, uint32_t e) {
-  if (Rb.attached[e] >= 0) return -1;
-  int p = Rb.ptr[e];
-  int32_t out = -1;
-  while (p < TPC_RB_NCAND) {
-    const int32_t c = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
-    if (c < 0) break;
-    if (Rb.owner[c] < 0) { out = c; break; }
-    ++p;
-  }
-  Rb.ptr[e] = (uint8_t)p;
-  return out;
+// ---- second ambiguity solving: three proposal rounds.  A cluster goes to the proposing
+// track of largest (Q, then least 64-bit id): atomicMax of the weight key, atomicMin of the id among the
+// holders of that weight, then the winner writes attached[] and owner[] (owner is only read by the NEXT
+// round's proposals).  Round 1: every step of every live track proposes its first candidate.  The
+// losers are appended to a list (order irrelevant: the atomics commute); rounds 2 and 3 run over the
+// lists.  bestQ / bestId need no reset between rounds: a cluster proposed in a later round has no owner,
+// so nobody proposed it before.
+__device__ __forceinline__ void rb_append(uint2* list, uint32_t* n, bool lose, uint32_t e) {
+  const uint32_t mask = __ballot_sync(0xFFFFFFFFu, lose);
+  if (!mask) return;
+  const uint32_t lane = threadIdx.x & 31u;
+  uint32_t base = 0u;
+  if (lane == (uint32_t)(__ffs(mask) - 1)) base = atomicAdd(n, (uint32_t)__popc(mask));
+  base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
+  if (lose) list[base + __popc(mask & ((1u << lane) - 1u))] = make_uint2(e, 0u);
 }
-__global__ void __launch_bounds__(256) k_rb_round_init(TpcRebuildBuffers Rb, int first) {
-  const uint32_t stride = gridDim.x * blockDim.x;
-  for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < Rb.n_clusters; c += stride) {
-    Rb.bestQ[c] = 0u; Rb.bestId[c] = ~0ull;
-    if (first) Rb.owner[c] = -1;
-  }
-}
-__global__ void __launch_bounds__(256) k_rb_round_q(TpcRebuildBuffers Rb) {
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
-    const uint32_t m = Rb.step_track[e];
-    if (!Rb.alive[m]) continue;
-    const int32_t c = rb_proposal(Rb, e);
-    if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
-  }
-}
-__global__ void __launch_bounds__(256) k_rb_round_id(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb) {
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
-    const uint32_t m = Rb.step_track[e];
-    if (!Rb.alive[m]) continue;
-    const int32_t c = rb_proposal(Rb, e);
-    if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], merge_key(B.tracks[M.merged[m].head]));
-  }
-}
-__global__ void __launch_bounds__(256) k_rb_round_resolve(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb) {
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
-    const uint32_t m = Rb.step_track[e];
-    if (!Rb.alive[m]) continue;
-    const int32_t c = rb_proposal(Rb, e);
-    if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == merge_key(B.tracks[M.merged[m].head])) Rb.attached[e] = c;
+template <int PHASE>   // 0: weight, 1: id, 2: resolve
+__global__ void __launch_bounds__(256) k_rb_round1(TpcRebuildBuffers Rb, uint2* losers, uint32_t* n_losers) {
+  const uint32_t n_pad = (Rb.n_steps + 31u) & ~31u;
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < n_pad; e += gridDim.x * blockDim.x) {
+    int32_t c = -1;
+    uint32_t m = 0u;
+    if (e < Rb.n_steps) {
+      m = Rb.step_track[e];
+      if (Rb.alive[m]) c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
+    }
+    if (PHASE == 0) {
+      if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
+    } else if (PHASE == 1) {
+      if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], Rb.tkey[m]);
+    } else {
+      const bool win = c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == Rb.tkey[m];
+      if (win) { Rb.attached[e] = c; Rb.owner[c] = (int32_t)m; }
+      rb_append(losers, n_losers, c >= 0 && !win, e);
+    }
   }
 }
-__global__ void __launch_bounds__(256) k_rb_round_commit(TpcRebuildBuffers Rb) {
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < Rb.n_steps; e += gridDim.x * blockDim.x) {
-    const int32_t c = Rb.attached[e];
-    if (c >= 0) Rb.owner[c] = (int32_t)Rb.step_track[e];   // (one winner per cluster: no race)
+template <int PHASE>
+__global__ void __launch_bounds__(256) k_rb_roundn(TpcRebuildBuffers Rb, uint2* list, const uint32_t* n_list, uint2* losers,
+                                                   uint32_t* n_losers) {
+  const uint32_t n = *n_list, n_pad = (n + 31u) & ~31u;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_pad; i += gridDim.x * blockDim.x) {
+    int32_t c = -1;
+    uint32_t e = 0u, m = 0u;
+    if (i < n) {
+      const uint2 it = list[i];
+      e = it.x;
+      m = Rb.step_track[e];
+      if (PHASE == 0) {   // the best candidate that has no owner yet (owners are final, so the search restarts at 0)
+        for (int p = 0; p < TPC_RB_NCAND; ++p) {
+          const int32_t cc = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
+          if (cc < 0) break;
+          if (Rb.owner[cc] < 0) { c = cc; break; }
+        }
+        list[i].y = (uint32_t)c;
+      } else {
+        c = (int32_t)it.y;
+      }
+    }
+    if (PHASE == 0) {
+      if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
+    } else if (PHASE == 1) {
+      if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], Rb.tkey[m]);
+    } else {
+      const bool win = c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == Rb.tkey[m];
+      if (win) { Rb.attached[e] = c; Rb.owner[c] = (int32_t)m; }
+      if (losers) rb_append(losers, n_losers, c >= 0 && !win, e);
+    }
   }
 }
 
@@ -3026,62 +3071,74 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
     const tpc_merged_track m = M.merged[mi];
     const uint32_t s0 = Rb.step_ofs[mi];
     const int n = (int)(Rb.step_ofs[mi + 1] - s0);
-    // ---- shared attachment from the outermost step inward (the rule of R6.3)
-    int n_acc = 0, n_sh = 0, last = -1;
-    for (int kk = n - 1; kk >= 0; --kk) {
-      const uint32_t e = s0 + (uint32_t)kk;
-      if (Rb.attached[e] >= 0) { ++n_acc; if (last < 0) last = kk; continue; }
-      const int32_t c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
-      if (c < 0) continue;
-      if ((long long)(n_sh + 1) * 1000 <= (long long)permille * (n_acc + 1)) {
-        Rb.attached[e] = c; Rb.shared[e] = 1; ++n_acc; ++n_sh;
-        if (last < 0) last = kk;
-      }
-    }
-    out.n_clusters = (uint32_t)n_acc;
-    if (last < 0) { Rb.fit[mi] = out; continue; }
-    // ---- pass 3: inward through the attached clusters, plain chi2 cut
     auto cluster_yz = [&](int32_t id, float& y, float& z) {
       const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + ((uint32_t)id - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y);
     };
+    // One walk from the outermost step inward does both: the shared attachment (the rule of R6.3: its
+    // decision at a step depends on the steps outside of it only) and, from the outermost attached step
+    // on, pass 3 with the plain chi2 cut.  After a failed transport / update the walk goes on for the
+    // attachment marks alone.
     RbPath P = rb_path(B, M, m);
-    P.begin_bwd();
-    int32_t oid; float oy, oz;
-    bool has = P.take_orig(-1, oid, oy, oz);
-    for (int kk = n - 1; kk > last; --kk) { P.next_bwd(); has = P.take_orig(-1, oid, oy, oz); }   // walk to the outermost attached step
-    KF k;
+    P.begin_bwd_rows();
+    KF k, kin;
     k.s = Rb.stq2[3 * (size_t)mi]; k.t = Rb.stq2[3 * (size_t)mi + 1]; k.q = Rb.stq2[3 * (size_t)mi + 2];
-    float ay, az;
-    cluster_yz(Rb.attached[s0 + (uint32_t)last], ay, az);
-    fit_turn(k, ay, az, F);
-    Rb.used[s0 + (uint32_t)last] = 1;
-    KF kin = k;
-    int nu = 1, row_in = P.row, ps = P.sec, pr = P.row;
+    k.y = k.z = 0.f;
+    kf_init_cov(k, F);
+    kin = k;
+    int n_acc = 0, n_sh = 0, nu = 0, row_in = 0, ps = 0, pr = 0;
     float chi3 = 0.f;
-    bool ok = true;
-    for (int kk = last - 1; kk >= 0 && ok; --kk) {
-      P.next_bwd();
-      has = P.take_orig(-1, oid, oy, oz);
-      const int32_t ca = Rb.attached[s0 + (uint32_t)kk];
+    bool ok = true, started = false;
+    for (int kk = n - 1; kk >= 0; --kk) {
+      if (kk < n - 1) P.next_bwd();
+      const uint32_t e = s0 + (uint32_t)kk;
+      int32_t ca = Rb.attached[e];
+      if (ca >= 0) {
+        ++n_acc;
+      } else {
+        const int32_t c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
+        if (c >= 0 && (long long)(n_sh + 1) * 1000 <= (long long)permille * (n_acc + 1)) {
+          Rb.attached[e] = c; Rb.shared[e] = 1; ++n_acc; ++n_sh;
+          ca = c;
+        }
+      }
+      if (!ok) continue;
+      float ay = 0.f, az = 0.f;
+      if (!started) {
+        if (ca < 0) continue;
+        cluster_yz(ca, ay, az);
+        fit_turn(k, ay, az, F);
+        Rb.used[e] = 1;
+        kin = k; nu = 1; row_in = P.row; ps = P.sec; pr = P.row;
+        started = true;
+        continue;
+      }
       float zc = k.z;
       if (ca >= 0) { cluster_yz(ca, ay, az); zc = az; }
-      else if (has) zc = oz;
-      if (!link_transport(k, ps, pr, P.sec, P.row, zc, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
+      else if (P.sec != ps && (P.sec - ps == 18 || ps - P.sec == 18)) {
+        // the electrode is crossed onto a step without an attached cluster: z is re-based on the
+        // step's original cluster if it has one (rare: the merged list is searched)
+        for (int i = 0; i < P.n_ids; ++i) {
+          const uint4 raw = *reinterpret_cast<const uint4*>(P.cl + (P.ids[i] - P.id_base));
+          if ((int)(raw.w & 0xFF) == P.sec && (int)((raw.w >> 8) & 0xFF) == P.row) { zc = __uint_as_float(raw.y); break; }
+        }
+      }
+      if (!link_transport(k, ps, pr, P.sec, P.row, zc, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; continue; }
       ps = P.sec; pr = P.row;
       if (ca < 0) continue;
       const Gain g = kf_gain(k, F);
       const float c2 = kf_chi2(k, g, ay, az);
       if (!(c2 <= Rb.P.final_chi2_max)) continue;   // plain cut: the cluster is dropped, no update
-      if (kf_update(k, g, ay, az, F)) { ok = false; break; }
+      if (kf_update(k, g, ay, az, F)) { ok = false; continue; }
       chi3 = chi3 + c2;
-      Rb.used[s0 + (uint32_t)kk] = 1;
+      Rb.used[e] = 1;
       ++nu;
       kin = k;
       row_in = P.row;
     }
+    out.n_clusters = (uint32_t)n_acc;
     out.n_used = (uint32_t)nu;
-    if (ok && nu >= Rb.P.min_clusters) {
+    if (started && ok && nu >= Rb.P.min_clusters) {
       out.flags = 0u;
       out.chi2 = chi3;
       out.x = K->x[row_in];
@@ -3189,18 +3246,33 @@ int run_rebuild(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& 
                 int n_sm) {
   if (Rb.n_merged == 0) return 0;
   const FollowConst F = follow_const(hK);
-  const int gt = grid_for(Rb.n_merged, 128, n_sm, 8);
-  const int gs = grid_for((uint64_t)Rb.n_steps + 1, 256, n_sm, 8), gc = grid_for((uint64_t)Rb.n_clusters + 1, 256, n_sm, 8);
-  k_rb_pass12<<<gt, 128, 0, st>>>(B, M, Rb, F);
-  for (int round = 0; round < TPC_RB_NCAND; ++round) {
-    k_rb_round_init<<<gc, 256, 0, st>>>(Rb, round == 0);
-    k_rb_round_q<<<gs, 256, 0, st>>>(Rb);
-    k_rb_round_id<<<gs, 256, 0, st>>>(B, M, Rb);
-    k_rb_round_resolve<<<gs, 256, 0, st>>>(B, M, Rb);
-    k_rb_round_commit<<<gs, 256, 0, st>>>(Rb);
-  }
-  k_rb_pass3<<<gt, 128, 0, st>>>(B, M, Rb, F);
-  return cudaPeekAtLastError() == cudaSuccess ? 2 + 5 * TPC_RB_NCAND : -1;
+  const int gw = grid_for((uint64_t)Rb.n_merged * 32, 256, n_sm, 8);
+  const int gs = grid_for((uint64_t)Rb.n_steps + 32, 256, n_sm, 8);
+  const size_t ns = Rb.n_steps, nc = Rb.n_clusters;
+  cudaMemsetAsync(Rb.list_n, 0, 16, st);
+  cudaMemsetAsync(Rb.attached, 0xFF, 4 * ns, st);
+  cudaMemsetAsync(Rb.shared, 0, ns, st);
+  cudaMemsetAsync(Rb.used, 0, ns, st);
+  cudaMemsetAsync(Rb.bestQ, 0, 4 * nc, st);
+  cudaMemsetAsync(Rb.bestId, 0xFF, 8 * nc, st);
+  cudaMemsetAsync(Rb.owner, 0xFF, 4 * nc, st);
+  k_rb_step_track<<<gw, 256, 0, st>>>(Rb);
+  k_rb_pass12<<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass12, 128)), 128, 0, st>>>(B, M, Rb, F);
+  // the stored predictions are dead now: their region holds the loser lists of rounds 2 and 3
+  uint2* list2 = reinterpret_cast<uint2*>(Rb.stored);
+  uint2* list3 = list2 + ns;
+  k_rb_round1<0><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr);
+  k_rb_round1<1><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr);
+  k_rb_round1<2><<<gs, 256, 0, st>>>(Rb, list2, Rb.list_n);
+  const int gl = grid_for((uint64_t)Rb.n_steps / 8 + 32, 256, n_sm, 8);
+  k_rb_roundn<0><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, nullptr, nullptr);
+  k_rb_roundn<1><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, nullptr, nullptr);
+  k_rb_roundn<2><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, list3, Rb.list_n + 1);
+  k_rb_roundn<0><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
+  k_rb_roundn<1><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
+  k_rb_roundn<2><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
+  k_rb_pass3<<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass3, 128)), 128, 0, st>>>(B, M, Rb, F);
+  return cudaPeekAtLastError() == cudaSuccess ? 12 : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

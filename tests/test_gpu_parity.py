@@ -944,3 +944,60 @@ def test_det_parity_phase2_rebuild(B, name):
         assert nm == 40 and ok.all()
     print(f"rebuild {name}: merged {nm} steps {len(so)} attached {(att >= 0).sum()} shared {int(q.shared.sum())} "
           f"used {int(q.used.sum())} failed {int((~ok).sum())}")
+
+
+def rebuilt_lists(step_ofs, attached, used, fit_flags):
+    """Cluster lists of the rebuilt tracks (used clusters of the tracks whose fit succeeded)."""
+    ofs = np.asarray(step_ofs, dtype=np.int64)
+    trk_of = np.repeat(np.arange(len(ofs) - 1), np.diff(ofs))
+    keep = (attached >= 0) & (used != 0) & (fit_flags[trk_of] == 0)
+    n = np.bincount(trk_of[keep], minlength=len(ofs) - 1).astype(np.int64)
+    o = np.zeros(len(n), dtype=np.int64)
+    o[1:] = np.cumsum(n)[:-1]
+    return n, o, attached[keep].astype(np.uint32)
+
+
+def test_fast_mode_phase2_rebuild_quality(B):
+    """Fast build of the rebuild against the oracle's on 4 sectors of a 20-event C4 frame: the same
+    number of path steps within 1 %, attached / used fractions within 0.5 %, efficiency, clone and fake
+    rates of the rebuilt tracks within 0.003, and more clusters per track than the merged tracks hold."""
+    from oracle import merging, rebuild
+    base = dg.preset("C4")
+    cl, lab, _ = dg.generate(dg.preset("C4", n_events=20, t_window_us=base.t_window_us * 20 / base.n_events))
+    import bench
+    pkw = dict(bench.WORKLOAD_PARAMS["C4"])
+    sel = cl["sector"] < 4
+    cl, lab = cl[sel], lab[sel]
+    gp, op = params_pair(B, **pkw)
+    trk = B.SectorTracker(params=gp)
+    try:
+        trk.track(trk.upload(cl), flags=0)
+        tracks, ids, shared, view = trk.tracks()
+        trk.refit()
+        g = trk.merge()
+        r = trk.rebuild()
+    finally:
+        trk.close()
+    o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
+    q = rebuild.rebuild(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids, params=op)
+    ng, og_, ig = rebuilt_lists(r["step_ofs"], r["attached"], r["used"], r["fit"]["flags"])
+    no, oo_, io = rebuilt_lists(q.step_ofs, q.attached, q.used, q.fit["flags"])
+    qg = track_quality(ng, og_, ig, g["merged"]["sector_first"], lab)
+    qo = track_quality(no, oo_, io, m.merged["sector_first"], lab)
+    qm = track_quality(m.merged["n_clusters"], m.merged["cluster_ofs"], m.cluster_ids, m.merged["sector_first"], lab)
+    sg, so = len(r["attached"]), len(q.attached)
+    stats = {"steps_gpu": sg, "steps_oracle": so, "attached_gpu": int((r["attached"] >= 0).sum()),
+             "attached_oracle": int((q.attached >= 0).sum()), "used_gpu": int(r["used"].sum()), "used_oracle": int(q.used.sum()),
+             "shared_gpu": int(r["shared"].sum()), "shared_oracle": int(q.shared.sum()),
+             "failed_gpu": int((r["fit"]["flags"] != 0).sum()), "failed_oracle": int((q.fit["flags"] != 0).sum()),
+             "clusters_merged_oracle": int(m.merged["n_clusters"].sum()),
+             "eff_gpu": qg["efficiency"], "eff_oracle": qo["efficiency"], "eff_merged": qm["efficiency"],
+             "clone_gpu": qg["clone_rate"], "clone_oracle": qo["clone_rate"], "clone_merged": qm["clone_rate"],
+             "fake_gpu": qg["fake_rate"], "fake_oracle": qo["fake_rate"], "fake_merged": qm["fake_rate"]}
+    report("rebuild_C4_20_events", stats)
+    assert abs(sg - so) <= 0.01 * so
+    assert abs(stats["attached_gpu"] / sg - stats["attached_oracle"] / so) <= 0.005
+    assert abs(stats["used_gpu"] / sg - stats["used_oracle"] / so) <= 0.005
+    for k in ("eff", "clone", "fake"):
+        assert abs(stats[k + "_gpu"] - stats[k + "_oracle"]) <= 0.003, k
