@@ -929,9 +929,8 @@ size_t carve_rebuild(uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters, c
   r.list_n = (uint32_t*)take(16);
   r.alive = (uint8_t*)take(nm);
   r.stq2 = (float*)take(12 * nm);
-  r.bestQ = (uint32_t*)take(4 * nc);
+  r.best = (unsigned long long*)take(8 * nc);
   r.bestId = (unsigned long long*)take(8 * nc);
-  r.owner = (int32_t*)take(4 * nc);
   r.fit = (tpc_track_fit3*)take(sizeof(tpc_track_fit3) * nm);
   if (R) *R = r;
   return off;
@@ -983,6 +982,7 @@ int tpc_rebuild_tracks(tpc_ctx* ctx, const tpc_rebuild_params* params, void* d_w
   if (params) P = *params; else tpc_rebuild_default_params(&P);
   if (!(P.cand_chi2_max >= 0.f) || !(P.final_chi2_max >= 0.f) || P.min_clusters < 2 || !(P.ce_var > 0.f)) return TPC_E_ARG;
   const uint32_t n_merged = ctx->mbuf.n_tracks ? ctx->h_mcnt[0] : 0u;
+  if (n_merged >= 0x3FFFFFFFu) return TPC_E_OVERFLOW;   // (the track index shares a word with the round tag)
   TpcRebuildBuffers R;
   const size_t need = carve_rebuild(ctx->rb_n_steps, n_merged, ctx->buf.n, (char*)d_ws, &R);
   if (ws_bytes < need) return TPC_E_WORKSPACE;

@@ -176,9 +176,8 @@ struct TpcRebuildBuffers {
   uint8_t* alive;              // [n_merged]
   float* stq2;                 // [n_merged][3] (s,t,q) after pass 2
   uint32_t* list_n;            // [4] lengths of the loser lists of rounds 2, 3
-  uint32_t* bestQ;             // [n_clusters]
-  unsigned long long* bestId;  // [n_clusters]
-  int32_t* owner;              // [n_clusters] merged track that owns the cluster, -1 none
+  unsigned long long* best;    // [n_clusters] Q key << 32 | round tag << 30 | (0x3FFFFFFF - merged track) of the best proposer; 0 none
+  unsigned long long* bestId;  // [n_clusters] least 64-bit track id among proposers of equal weight (ties only)
   tpc_track_fit3* fit;         // [n_merged]
 };
 

@@ -2986,72 +2986,106 @@ __global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers
 }
 
 // ---- second ambiguity solving: three proposal rounds.  A cluster goes to the proposing
-// track of largest (Q, then least 64-bit id): atomicMax of the weight key, atomicMin of the id among the
-// holders of that weight, then the winner writes attached[] and owner[] (owner is only read by the NEXT
-// round's proposals).  Round 1: every step of every live track proposes its first candidate.  The
-// losers are appended to a list (order irrelevant: the atomics commute); rounds 2 and 3 run over the
-// lists.  bestQ / bestId need no reset between rounds: a cluster proposed in a later round has no owner,
-// so nobody proposed it before.
-__device__ __forceinline__ void rb_append(uint2* list, uint32_t* n, bool lose, uint32_t e) {
+// track of largest (Q, then least 64-bit id).  One 64-bit word per cluster, best[c] = Q key << 32 |
+// round tag << 30 | (0x3FFFFFFF - merged track): an atomicMax gives the largest Q (and, provisionally, the
+// least track INDEX among equal Q); the winner is whoever finds its own word there.  Exactly equal
+// weights of two tracks are rare: such proposers are flagged in the loser list and a pair of small
+// kernels settles them by the 64-bit id (atomicMin into bestId, take-over from the provisional winner).
+// A cluster is owned iff its word carries the tag of an EARLIER round (ownership is final, so no word is
+// ever reset).  Round 1: every step of every live track proposes its first candidate; rounds 2 and 3
+// run over the loser lists (their order is irrelevant: the atomics commute).
+#define TPC_RB_M_MASK 0x3FFFFFFFu
+__device__ __forceinline__ unsigned long long rb_word(uint32_t qkey, int round, uint32_t m) {
+  return ((unsigned long long)qkey << 32) | (unsigned long long)(((uint32_t)(3 - round) << 30) | (TPC_RB_M_MASK - m));
+}
+__device__ __forceinline__ uint32_t rb_word_track(unsigned long long w) { return TPC_RB_M_MASK - ((uint32_t)w & TPC_RB_M_MASK); }
+__device__ __forceinline__ bool rb_owned_before(unsigned long long w, int round) {
+  return w != 0ull && (int)(((uint32_t)w >> 30) & 3u) > 3 - round;
+}
+__device__ __forceinline__ void rb_append(uint2* list, uint32_t* n, bool lose, uint32_t e, uint32_t flag) {
   const uint32_t mask = __ballot_sync(0xFFFFFFFFu, lose);
   if (!mask) return;
   const uint32_t lane = threadIdx.x & 31u;
   uint32_t base = 0u;
   if (lane == (uint32_t)(__ffs(mask) - 1)) base = atomicAdd(n, (uint32_t)__popc(mask));
   base = __shfl_sync(0xFFFFFFFFu, base, __ffs(mask) - 1);
-  if (lose) list[base + __popc(mask & ((1u << lane) - 1u))] = make_uint2(e, 0u);
+  if (lose) list[base + __popc(mask & ((1u << lane) - 1u))] = make_uint2(e, flag);
 }
-template <int PHASE>   // 0: weight, 1: id, 2: resolve
-__global__ void __launch_bounds__(256) k_rb_round1(TpcRebuildBuffers Rb, uint2* losers, uint32_t* n_losers) {
-  const uint32_t n_pad = (Rb.n_steps + 31u) & ~31u;
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < n_pad; e += gridDim.x * blockDim.x) {
-    int32_t c = -1;
-    uint32_t m = 0u;
-    if (e < Rb.n_steps) {
-      m = Rb.step_track[e];
-      if (Rb.alive[m]) c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
-    }
-    if (PHASE == 0) {
-      if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
-    } else if (PHASE == 1) {
-      if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], Rb.tkey[m]);
-    } else {
-      const bool win = c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == Rb.tkey[m];
-      if (win) { Rb.attached[e] = c; Rb.owner[c] = (int32_t)m; }
-      rb_append(losers, n_losers, c >= 0 && !win, e);
-    }
-  }
-}
-template <int PHASE>
-__global__ void __launch_bounds__(256) k_rb_roundn(TpcRebuildBuffers Rb, uint2* list, const uint32_t* n_list, uint2* losers,
-                                                   uint32_t* n_losers) {
-  const uint32_t n = *n_list, n_pad = (n + 31u) & ~31u;
+// PHASE 0: propose; PHASE 1: resolve.  ROUND 1 runs over all steps (list == nullptr), the others over `list`.
+template <int ROUND, int PHASE>
+__global__ void __launch_bounds__(256) k_rb_round(TpcRebuildBuffers Rb, uint2* list, const uint32_t* n_list, uint2* losers,
+                                                  uint32_t* n_losers) {
+  const uint32_t n = ROUND == 1 ? Rb.n_steps : *n_list, n_pad = (n + 31u) & ~31u;
   for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_pad; i += gridDim.x * blockDim.x) {
     int32_t c = -1;
     uint32_t e = 0u, m = 0u;
     if (i < n) {
-      const uint2 it = list[i];
-      e = it.x;
-      m = Rb.step_track[e];
-      if (PHASE == 0) {   // the best candidate that has no owner yet (owners are final, so the search restarts at 0)
-        for (int p = 0; p < TPC_RB_NCAND; ++p) {
-          const int32_t cc = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
-          if (cc < 0) break;
-          if (Rb.owner[cc] < 0) { c = cc; break; }
-        }
-        list[i].y = (uint32_t)c;
+      if (ROUND == 1) {
+        e = i;
+        m = Rb.step_track[e];
+        if (Rb.alive[m]) c = Rb.cand_id[(size_t)e * TPC_RB_NCAND];
       } else {
-        c = (int32_t)it.y;
+        const uint2 it = list[i];
+        e = it.x;
+        m = Rb.step_track[e];
+        if (PHASE == 0) {
+          // the best candidate without an owner (owners are final, so the search restarts at the first);
+          // a step that took a cluster over in the tie kernels is done
+          if (Rb.attached[e] < 0)
+            for (int p = 0; p < TPC_RB_NCAND; ++p) {
+              const int32_t cc = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
+              if (cc < 0) break;
+              if (!rb_owned_before(Rb.best[cc], ROUND)) { c = cc; break; }
+            }
+          list[i].y = (uint32_t)c;
+        } else {
+          c = (int32_t)it.y;
+        }
       }
     }
     if (PHASE == 0) {
-      if (c >= 0) atomicMax(&Rb.bestQ[c], Rb.Qkey[m]);
-    } else if (PHASE == 1) {
-      if (c >= 0 && Rb.Qkey[m] == Rb.bestQ[c]) atomicMin(&Rb.bestId[c], Rb.tkey[m]);
+      if (c >= 0) atomicMax(&Rb.best[c], rb_word(Rb.Qkey[m], ROUND, m));
     } else {
-      const bool win = c >= 0 && Rb.Qkey[m] == Rb.bestQ[c] && Rb.bestId[c] == Rb.tkey[m];
-      if (win) { Rb.attached[e] = c; Rb.owner[c] = (int32_t)m; }
-      if (losers) rb_append(losers, n_losers, c >= 0 && !win, e);
+      bool win = false, tie = false;
+      if (c >= 0) {
+        const unsigned long long w = Rb.best[c], mine = rb_word(Rb.Qkey[m], ROUND, m);
+        win = w == mine;
+        tie = !win && (uint32_t)(w >> 32) == (uint32_t)(mine >> 32);
+        if (win) Rb.attached[e] = c;
+      }
+      rb_append(losers, n_losers, c >= 0 && !win, e, tie ? 1u : 0u);
+    }
+  }
+}
+// the flagged entries of a loser list: equal weight as the provisional winner of cluster c
+template <int PHASE>
+__global__ void __launch_bounds__(256) k_rb_ties(TpcRebuildBuffers Rb, uint2* list, uint32_t* n_list, int round) {
+  const uint32_t n = *n_list;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const uint2 it = list[i];
+    if (it.y != 1u) continue;
+    const uint32_t e = it.x, m = Rb.step_track[e];
+    // (the step's proposal of this round: its first candidate that was not owned before)
+    int32_t c = -1;
+    for (int p = 0; p < TPC_RB_NCAND; ++p) {
+      const int32_t cc = Rb.cand_id[(size_t)e * TPC_RB_NCAND + p];
+      if (cc < 0) break;
+      if (!rb_owned_before(Rb.best[cc], round)) { c = cc; break; }
+    }
+    if (c < 0) continue;
+    if (PHASE == 0) {
+      atomicMin(&Rb.bestId[c], Rb.tkey[m]);
+      atomicMin(&Rb.bestId[c], Rb.tkey[rb_word_track(Rb.best[c])]);
+    } else if (Rb.bestId[c] == Rb.tkey[m]) {
+      const unsigned long long old = atomicExch(&Rb.best[c], rb_word(Rb.Qkey[m], round, m));
+      const uint32_t mw = rb_word_track(old);
+      Rb.attached[e] = c;
+      if (mw != m)
+        for (uint32_t e2 = Rb.step_ofs[mw]; e2 < Rb.step_ofs[mw + 1]; ++e2)
+          if (Rb.attached[e2] == c) {
+            Rb.attached[e2] = -1;
+            list[atomicAdd(n_list, 1u)] = make_uint2(e2, 0u);
+          }
     }
   }
 }
@@ -3253,26 +3287,29 @@ int run_rebuild(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& 
   cudaMemsetAsync(Rb.attached, 0xFF, 4 * ns, st);
   cudaMemsetAsync(Rb.shared, 0, ns, st);
   cudaMemsetAsync(Rb.used, 0, ns, st);
-  cudaMemsetAsync(Rb.bestQ, 0, 4 * nc, st);
+  cudaMemsetAsync(Rb.best, 0, 8 * nc, st);
   cudaMemsetAsync(Rb.bestId, 0xFF, 8 * nc, st);
-  cudaMemsetAsync(Rb.owner, 0xFF, 4 * nc, st);
   k_rb_step_track<<<gw, 256, 0, st>>>(Rb);
   k_rb_pass12<<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass12, 128)), 128, 0, st>>>(B, M, Rb, F);
-  // the stored predictions are dead now: their region holds the loser lists of rounds 2 and 3
+  // the stored predictions are dead now: their region holds the loser lists (round 3's goes where round 2's was)
   uint2* list2 = reinterpret_cast<uint2*>(Rb.stored);
   uint2* list3 = list2 + ns;
-  k_rb_round1<0><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr);
-  k_rb_round1<1><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr);
-  k_rb_round1<2><<<gs, 256, 0, st>>>(Rb, list2, Rb.list_n);
+  uint32_t* cnt = Rb.list_n;
   const int gl = grid_for((uint64_t)Rb.n_steps / 8 + 32, 256, n_sm, 8);
-  k_rb_roundn<0><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, nullptr, nullptr);
-  k_rb_roundn<1><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, nullptr, nullptr);
-  k_rb_roundn<2><<<gl, 256, 0, st>>>(Rb, list2, Rb.list_n, list3, Rb.list_n + 1);
-  k_rb_roundn<0><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
-  k_rb_roundn<1><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
-  k_rb_roundn<2><<<gl, 256, 0, st>>>(Rb, list3, Rb.list_n + 1, nullptr, nullptr);
+  k_rb_round<1, 0><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr, nullptr, nullptr);
+  k_rb_round<1, 1><<<gs, 256, 0, st>>>(Rb, nullptr, nullptr, list2, cnt);
+  k_rb_ties<0><<<gl, 256, 0, st>>>(Rb, list2, cnt, 1);
+  k_rb_ties<1><<<gl, 256, 0, st>>>(Rb, list2, cnt, 1);
+  k_rb_round<2, 0><<<gl, 256, 0, st>>>(Rb, list2, cnt, nullptr, nullptr);
+  k_rb_round<2, 1><<<gl, 256, 0, st>>>(Rb, list2, cnt, list3, cnt + 1);
+  k_rb_ties<0><<<gl, 256, 0, st>>>(Rb, list3, cnt + 1, 2);
+  k_rb_ties<1><<<gl, 256, 0, st>>>(Rb, list3, cnt + 1, 2);
+  k_rb_round<3, 0><<<gl, 256, 0, st>>>(Rb, list3, cnt + 1, nullptr, nullptr);
+  k_rb_round<3, 1><<<gl, 256, 0, st>>>(Rb, list3, cnt + 1, list2, cnt + 2);
+  k_rb_ties<0><<<gl, 256, 0, st>>>(Rb, list2, cnt + 2, 3);
+  k_rb_ties<1><<<gl, 256, 0, st>>>(Rb, list2, cnt + 2, 3);
   k_rb_pass3<<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass3, 128)), 128, 0, st>>>(B, M, Rb, F);
-  return cudaPeekAtLastError() == cudaSuccess ? 12 : -1;
+  return cudaPeekAtLastError() == cudaSuccess ? 15 : -1;
 }
 
 // Returns the number of kernels launched, or -1 on a launch error.

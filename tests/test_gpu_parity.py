@@ -889,14 +889,11 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0 < ro.sum() < 0.02 * len(ro)
 
 
-@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
-def test_det_parity_phase2_rebuild(B, name):
-    """SURVEY.md 8(f) row 4 (PAPER.md:59,65; reading R11): the Phase-II rebuild of the merged tracks;
-    deterministic mode: per path step the three candidates (ids and chi2 bits), the attached cluster
-    after the second ambiguity solving, the shared and used marks, and per track the final fit, all
-    bit-exact against oracle.rebuild."""
+def rebuild_det_parity(B, cl, pkw):
+    """Phase-II rebuild, deterministic mode, against oracle.rebuild: per path step the three candidates
+    (ids and chi2 bits), the attached cluster after the second ambiguity solving, the shared and used
+    marks, per track the final fit -- all bit-exact.  Returns both sides for further checks."""
     from oracle import merging, rebuild
-    cl, pkw = merged_case_frame(name)
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
     try:
@@ -934,16 +931,68 @@ def test_det_parity_phase2_rebuild(B, name):
     for f in ("x", "p", "c", "chi2"):
         a_, b_ = np.ascontiguousarray(fg[f][ok]).view(np.uint32), np.ascontiguousarray(fo[f][ok]).view(np.uint32)
         assert (a_ == b_).all(), (f, int((a_ != b_).sum()))
-    # what the rebuild is for: additional clusters in the holes and beyond the segment ends, and every
-    # cluster owned by at most one track
+    # every cluster owned by at most one track
     att = q.attached[so]
     own = att[(att >= 0) & (q.shared[so] == 0)]
     assert len(np.unique(own)) == len(own)
+    return dict(tracks=tracks, merged=g["merged"], r=r, q=q, m=m, o=o, ok=ok, so=so)
+
+
+@pytest.mark.parametrize("name", ["C2_full", "C4_reduced", "ce_crossing", "C5_dense"])
+def test_det_parity_phase2_rebuild(B, name):
+    """SURVEY.md 8(f) row 4 (reading R11): the Phase-II rebuild of the merged tracks,
+    deterministic mode, bit-exact against oracle.rebuild (see rebuild_det_parity)."""
+    cl, pkw = merged_case_frame(name)
+    x = rebuild_det_parity(B, cl, pkw)
+    q, ok, so, nm = x["q"], x["ok"], x["so"], len(x["m"].merged)
     assert ok.sum() >= 0.8 * nm
     if name == "ce_crossing":
         assert nm == 40 and ok.all()
+    att = q.attached[so]
     print(f"rebuild {name}: merged {nm} steps {len(so)} attached {(att >= 0).sum()} shared {int(q.shared.sum())} "
           f"used {int(q.used.sum())} failed {int((~ok).sum())}")
+
+
+def test_det_parity_phase2_rebuild_equal_weights(B):
+    """Two mirror-image tracks (y = +-0.25 cm, rows 20..80) compete for one cluster at y = 0 on row 50
+    with EXACTLY equal weights Q (the arithmetic is symmetric under y -> -y): the 64-bit track id
+    decides (reading R11).  The kernels settle a tie in a separate step that takes the cluster over
+    from a provisional winner (the least track index); input orders are varied so that id order and
+    track order disagree in at least one case, and the owner must change with the id order."""
+    def frame(a_first, mode):
+        recs = []
+        for r in range(20, 81):
+            if r == 50:
+                recs.append((0, r, 0.0, 100.0))
+                continue
+            pair = [(0, r, 0.25, 100.0), (0, r, -0.25, 100.0)]
+            recs += pair if a_first else pair[::-1]
+        a = np.array(recs)
+        if mode == "reversed":
+            a = a[::-1]
+        elif mode == "shuffled":
+            a = a[np.random.default_rng(5).permutation(len(a))]
+        cl = np.zeros(len(a), dtype=oracle.CLUSTER_DTYPE)
+        cl["sector"], cl["row"], cl["y"], cl["z"] = a[:, 0], a[:, 1], a[:, 2], a[:, 3]
+        return cl
+    owners, takeover = set(), 0
+    for mode in ("sorted", "reversed", "shuffled"):
+        for a_first in (True, False):
+            cl = frame(a_first, mode)
+            x = rebuild_det_parity(B, cl, dict(grid_dy=0.3))
+            r, tracks, merged = x["r"], x["tracks"], x["merged"]
+            assert len(merged) == 2
+            xid = int(np.flatnonzero(cl["row"] == 50)[0])
+            ofs = r["step_ofs"].astype(np.int64)
+            who = [k for k in range(2) if ((r["attached"][ofs[k]:ofs[k + 1]] == xid) & (r["shared"][ofs[k]:ofs[k + 1]] == 0)).any()]
+            assert len(who) == 1
+            h = merged["head"].astype(np.int64)
+            key = (tracks["sector"][h].astype(np.int64) << 41) | (tracks["seed_id"][h].astype(np.int64) << 8) | tracks["segment"][h]
+            assert key[who[0]] == key.min()                  # decided by the id: the weights are equal
+            takeover += int(who[0] == 1)                     # the owner is not the provisional winner (index 0)
+            owners.add(float(np.sign(cl["y"][tracks["seed_id"][h[who[0]]]])))   # (seed id = a cluster of the track)
+    assert owners == {1.0, -1.0}
+    assert takeover >= 1
 
 
 def rebuilt_lists(step_ofs, attached, used, fit_flags):
