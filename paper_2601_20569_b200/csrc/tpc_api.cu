@@ -847,6 +847,7 @@ size_t carve_fit(uint64_t n_merged, uint64_t n_ids, char* base, TpcFitBuffers* T
   t.chi2_cluster = (float*)take(4 * (n_ids + 1));
   t.rejected = (uint8_t*)take(n_ids + 1);
   t.fit = (tpc_track_fit3*)take(sizeof(tpc_track_fit3) * (n_merged + 1));
+  t.work = (uint32_t*)take(16);
   if (T) *T = t;
   return off;
 }
@@ -926,7 +927,7 @@ size_t carve_rebuild(uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters, c
   r.step_track = (uint32_t*)take(4 * ns);
   r.Qkey = (uint32_t*)take(4 * nm);
   r.tkey = (unsigned long long*)take(8 * nm);
-  r.list_n = (uint32_t*)take(16);
+  r.list_n = (uint32_t*)take(32);
   r.alive = (uint8_t*)take(nm);
   r.stq2 = (float*)take(12 * nm);
   r.best = (unsigned long long*)take(8 * nc);

@@ -155,6 +155,7 @@ struct TpcFitBuffers {
   float* chi2_cluster;     // [n_ids]
   uint8_t* rejected;       // [n_ids]
   tpc_track_fit3* fit;     // [n_merged]
+  uint32_t* work;          // [4] chunk counter
 };
 
 // Buffers of the Phase-II rebuild (R11), pointers into the caller's rebuild workspace.
@@ -175,7 +176,7 @@ struct TpcRebuildBuffers {
   unsigned long long* tkey;    // [n_merged] 64-bit id of the track (that of its head segment)
   uint8_t* alive;              // [n_merged]
   float* stq2;                 // [n_merged][3] (s,t,q) after pass 2
-  uint32_t* list_n;            // [4] lengths of the loser lists of rounds 2, 3
+  uint32_t* list_n;            // [8] lengths of the three loser lists; [4] chunk counter of pass 1+2
   unsigned long long* best;    // [n_clusters] Q key << 32 | round tag << 30 | (0x3FFFFFFF - merged track) of the best proposer; 0 none
   unsigned long long* bestId;  // [n_clusters] least 64-bit track id among proposers of equal weight (ties only)
   tpc_track_fit3* fit;         // [n_merged]

@@ -2595,11 +2595,65 @@ __device__ __forceinline__ float fit_chi2_2x2(float r0, float r1, float a, float
   return ((r0 * r0) * i00 + (2.f * (r0 * r1)) * i01) + (r1 * r1) * i11;
 }
 
+// ---- work distribution of the per-track kernels (fit, rebuild).  Tracks next to each other in merge order start in the
+// same region of the chamber (their grid lines and pages are shared: a global sort by length was
+// measured 35 % slower), but their path lengths differ by up to 10x, and a warp runs as long as its
+// longest track.  So: CTAs fetch chunks of TPC_RB_CHUNK consecutive tracks from a counter, sort the
+// chunk by path length in shared memory, and the warps fetch groups of 32 tracks of similar length.
+#define TPC_RB_CHUNK 512
+#ifndef TPC_RB_MINB
+#define TPC_RB_MINB 5
+#endif
+struct RbChunkShared { uint32_t key[TPC_RB_CHUNK]; uint32_t chunk, group; };
+// len(i): work of item i (any monotone measure)
+template <class LenFn>
+__device__ __forceinline__ bool rb_chunk_begin(uint32_t n_items, LenFn len_of, uint32_t* counter, RbChunkShared& S, uint32_t& base) {
+  __syncthreads();   // (everybody is done with the previous chunk's keys)
+  if (threadIdx.x == 0) { S.chunk = atomicAdd(counter, 1u); S.group = 0u; }
+  __syncthreads();
+  base = S.chunk * (uint32_t)TPC_RB_CHUNK;
+  if (base >= n_items) return false;
+  for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK; i += blockDim.x) {
+    const uint32_t mi = base + i;
+    uint32_t len = mi < n_items ? len_of(mi) : 0u;
+    if (len > 0x3FFFFFu) len = 0x3FFFFFu;
+    S.key[i] = (len << 9) | i;
+  }
+  __syncthreads();
+  for (uint32_t size = 2; size <= TPC_RB_CHUNK; size <<= 1)         // bitonic sort, descending
+    for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
+      for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK / 2; i += blockDim.x) {
+        const uint32_t lo = 2u * i - (i & (stride - 1u)), hi = lo + stride;
+        const uint32_t a = S.key[lo], b = S.key[hi];
+        const bool desc = (lo & size) == 0u;
+        if ((a < b) == desc) { S.key[lo] = b; S.key[hi] = a; }
+      }
+      __syncthreads();
+    }
+  return true;
+}
+// the warp's next group of 32 tracks of the chunk; false: none left
+__device__ __forceinline__ bool rb_group_next(uint32_t n_items, RbChunkShared& S, uint32_t base, uint32_t& mi, bool& valid) {
+  uint32_t g = 0u;
+  if ((threadIdx.x & 31u) == 0u) g = atomicAdd(&S.group, 1u);
+  g = __shfl_sync(0xFFFFFFFFu, g, 0);
+  if (g >= TPC_RB_CHUNK / 32) return false;
+  mi = base + (S.key[g * 32u + (threadIdx.x & 31u)] & (uint32_t)(TPC_RB_CHUNK - 1));
+  valid = mi < n_items;
+  return true;
+}
+
 __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffers M, TpcFitBuffers T,
                                                     const __grid_constant__ FollowConst F) {
   const TpcConst* __restrict__ K = B.K;
   const uint32_t n_merged = M.counters[0];
-  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < n_merged; mi += gridDim.x * blockDim.x) {
+  __shared__ RbChunkShared S;
+  uint32_t base, mi;
+  bool valid;
+  auto len_of = [&](uint32_t i) { return M.merged[i].n_clusters; };
+  while (rb_chunk_begin(n_merged, len_of, T.work, S, base))
+  while (rb_group_next(n_merged, S, base, mi, valid)) {
+    if (!valid) continue;
     const tpc_merged_track m = M.merged[mi];
     const uint32_t* __restrict__ ids = M.ids + m.cluster_ofs;
     const int n = (int)m.n_clusters;
@@ -2727,13 +2781,14 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
 // ================================================================== R11 Phase-II track rebuild
 // PAPER.md:59,65 (section 3, Phase II); reading R11.  Kernels:
 //   k_rb_path_len   length of every merged track's path of (sector,row) steps (-> scan -> step offsets)
+//   k_rb_step_track warp per merged track: the track index of every step
 //   k_rb_pass12     thread per merged track: pass 1 inward through the original clusters (prediction
 //                   stored at every step), pass 2 outward (interpolation, candidates of the step's row
 //                   from the search grid of the sector tracking, best three kept, update with the best)
-//   k_rb_round_*    thread per step: three proposal rounds of the second ambiguity solving (32-bit
-//                   atomicMax of the weight, 64-bit atomicMin of the id among its holders, resolve, commit)
-//   k_rb_pass3      thread per merged track: shared attachment from the outermost step inward, pass 3
-//                   inward with the plain chi2 cut
+//   k_rb_round      thread per step (round 1) / per loser-list entry (rounds 2, 3): propose (64-bit
+//                   atomicMax of weight | round | track) and resolve; k_rb_ties settles equal weights
+//   k_rb_pass3      thread per merged track: one inward walk = shared attachment + pass 3 with the
+//                   plain chi2 cut
 // Iterator over the steps of a merged track, forward (outward) or backward; it also tells which
 // original cluster of the merged list, if any, sits on the step.
 struct RbPath {
@@ -2835,11 +2890,17 @@ __device__ __forceinline__ float rb_unhalf(uint32_t w, int hi) {
   return __half2float(__ushort_as_half((unsigned short)(hi ? (w >> 16) : (w & 0xFFFFu))));
 }
 
-__global__ void __launch_bounds__(128) k_rb_pass12(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb,
+__global__ void __launch_bounds__(128, TPC_RB_MINB) k_rb_pass12(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb,
                                                    const __grid_constant__ FollowConst F) {
   const TpcConst* __restrict__ K = B.K;
   const float w_sel = K->P.sel_chi2_weight;
-  for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < Rb.n_merged; mi += gridDim.x * blockDim.x) {
+  __shared__ RbChunkShared S;
+  uint32_t base, mi;
+  bool valid;
+  auto len_of = [&](uint32_t i) { return Rb.step_ofs[i + 1] - Rb.step_ofs[i]; };
+  while (rb_chunk_begin(Rb.n_merged, len_of, Rb.list_n + 4, S, base))
+  while (rb_group_next(Rb.n_merged, S, base, mi, valid)) {
+    if (!valid) continue;
     const tpc_merged_track m = M.merged[mi];
     const uint32_t s0 = Rb.step_ofs[mi];
     const int n = (int)(Rb.step_ofs[mi + 1] - s0);
@@ -3094,6 +3155,7 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
                                                   const __grid_constant__ FollowConst F) {
   const TpcConst* __restrict__ K = B.K;
   const int permille = K->P.shared_permille;
+  // (plain order: the chunked distribution of pass 1+2 was measured 5 % slower here)
   for (uint32_t mi = blockIdx.x * blockDim.x + threadIdx.x; mi < Rb.n_merged; mi += gridDim.x * blockDim.x) {
     tpc_track_fit3 out;
     out.x = 0.f; out.chi2 = 0.f; out.n_clusters = 0u; out.n_used = 0u; out.flags = 1u;
@@ -3266,6 +3328,7 @@ int run_fit3(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, 
              cudaStream_t st, int n_sm) {
   if (n_merged == 0) return 0;
   const FollowConst F = follow_const(hK);
+  cudaMemsetAsync(T.work, 0, 16, st);
   k_track_fit3<<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3, 128)), 128, 0, st>>>(B, M, T, F);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
@@ -3283,7 +3346,7 @@ int run_rebuild(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& 
   const int gw = grid_for((uint64_t)Rb.n_merged * 32, 256, n_sm, 8);
   const int gs = grid_for((uint64_t)Rb.n_steps + 32, 256, n_sm, 8);
   const size_t ns = Rb.n_steps, nc = Rb.n_clusters;
-  cudaMemsetAsync(Rb.list_n, 0, 16, st);
+  cudaMemsetAsync(Rb.list_n, 0, 32, st);
   cudaMemsetAsync(Rb.attached, 0xFF, 4 * ns, st);
   cudaMemsetAsync(Rb.shared, 0, ns, st);
   cudaMemsetAsync(Rb.used, 0, ns, st);
