@@ -40,7 +40,7 @@ struct TpcCounters {
   uint32_t n_tracks, n_ids, error;
   uint32_t grid_rows;   // 1: every row's input records are contiguous and fit k_row_sort (the per-row grid build)
   uint32_t n_rows_generic;   // rows built by the generic histogram / scan / scatter kernels instead
-  uint32_t pad2_;
+  uint32_t refit_next;       // chunk counter of the sector-track refit
   // work counters of the follower (roofline numerators): propagation steps, Kalman updates,
   // chi2 evaluations of road candidates
   unsigned long long follow_work[3][3];  // [kernel up/refit/down][steps, updates, candidates]

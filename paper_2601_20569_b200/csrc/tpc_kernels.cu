@@ -2198,8 +2198,62 @@ __global__ void k_init(TpcBuffers B) {
 // through the track's own cluster list (outward pass, turn, inward pass; no search, no chi2
 // cut) with the propagation / update statements of the follower.  The clusters are read from
 // the input frame through their original indices.
+// ---- work distribution of the per-track kernels (fit, rebuild).  Tracks next to each other in merge order start in the
+// same region of the chamber (their grid lines and pages are shared: a global sort by length was
+// measured 35 % slower), but their path lengths differ by up to 10x, and a warp runs as long as its
+// longest track.  So: CTAs fetch chunks of TPC_RB_CHUNK consecutive tracks from a counter, sort the
+// chunk by path length in shared memory, and the warps fetch groups of 32 tracks of similar length.
+#define TPC_RB_CHUNK 512
+#ifndef TPC_RB_MINB
+#define TPC_RB_MINB 5
+#endif
+struct RbChunkShared { uint32_t key[TPC_RB_CHUNK]; uint32_t chunk, group; };
+// len(i): work of item i (any monotone measure)
+template <class LenFn>
+__device__ __forceinline__ bool rb_chunk_begin(uint32_t n_items, LenFn len_of, uint32_t* counter, RbChunkShared& S, uint32_t& base) {
+  __syncthreads();   // (everybody is done with the previous chunk's keys)
+  if (threadIdx.x == 0) { S.chunk = atomicAdd(counter, 1u); S.group = 0u; }
+  __syncthreads();
+  base = S.chunk * (uint32_t)TPC_RB_CHUNK;
+  if (base >= n_items) return false;
+  for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK; i += blockDim.x) {
+    const uint32_t mi = base + i;
+    uint32_t len = mi < n_items ? len_of(mi) : 0u;
+    if (len > 0x3FFFFFu) len = 0x3FFFFFu;
+    S.key[i] = (len << 9) | i;
+  }
+  __syncthreads();
+  for (uint32_t size = 2; size <= TPC_RB_CHUNK; size <<= 1)         // bitonic sort, descending
+    for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
+      for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK / 2; i += blockDim.x) {
+        const uint32_t lo = 2u * i - (i & (stride - 1u)), hi = lo + stride;
+        const uint32_t a = S.key[lo], b = S.key[hi];
+        const bool desc = (lo & size) == 0u;
+        if ((a < b) == desc) { S.key[lo] = b; S.key[hi] = a; }
+      }
+      __syncthreads();
+    }
+  return true;
+}
+// the warp's next group of 32 tracks of the chunk; false: none left
+__device__ __forceinline__ bool rb_group_next(uint32_t n_items, RbChunkShared& S, uint32_t base, uint32_t& mi, bool& valid) {
+  uint32_t g = 0u;
+  if ((threadIdx.x & 31u) == 0u) g = atomicAdd(&S.group, 1u);
+  g = __shfl_sync(0xFFFFFFFFu, g, 0);
+  if (g >= TPC_RB_CHUNK / 32) return false;
+  mi = base + (S.key[g * 32u + (threadIdx.x & 31u)] & (uint32_t)(TPC_RB_CHUNK - 1));
+  valid = mi < n_items;
+  return true;
+}
+
 __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_constant__ FollowConst F, uint32_t n_tracks) {
-  for (uint32_t ti = blockIdx.x * blockDim.x + threadIdx.x; ti < n_tracks; ti += gridDim.x * blockDim.x) {
+  __shared__ RbChunkShared S;
+  uint32_t base, ti;
+  bool valid;
+  auto len_of = [&](uint32_t i) { return (uint32_t)B.tracks[i].n_clusters; };
+  while (rb_chunk_begin(n_tracks, len_of, &B.cnt->refit_next, S, base))
+  while (rb_group_next(n_tracks, S, base, ti, valid)) {
+    if (!valid) continue;
     const tpc_track* __restrict__ t = B.tracks + ti;
     const uint32_t* __restrict__ ids = B.cluster_ids + t->cluster_ofs;
     const int n = t->n_clusters;
@@ -2593,54 +2647,6 @@ __device__ __forceinline__ float fit_chi2_2x2(float r0, float r1, float a, float
   const float inv = 1.f / det;
   const float i00 = s11 * inv, i01 = -(s01 * inv), i11 = s00 * inv;
   return ((r0 * r0) * i00 + (2.f * (r0 * r1)) * i01) + (r1 * r1) * i11;
-}
-
-// ---- work distribution of the per-track kernels (fit, rebuild).  Tracks next to each other in merge order start in the
-// same region of the chamber (their grid lines and pages are shared: a global sort by length was
-// measured 35 % slower), but their path lengths differ by up to 10x, and a warp runs as long as its
-// longest track.  So: CTAs fetch chunks of TPC_RB_CHUNK consecutive tracks from a counter, sort the
-// chunk by path length in shared memory, and the warps fetch groups of 32 tracks of similar length.
-#define TPC_RB_CHUNK 512
-#ifndef TPC_RB_MINB
-#define TPC_RB_MINB 5
-#endif
-struct RbChunkShared { uint32_t key[TPC_RB_CHUNK]; uint32_t chunk, group; };
-// len(i): work of item i (any monotone measure)
-template <class LenFn>
-__device__ __forceinline__ bool rb_chunk_begin(uint32_t n_items, LenFn len_of, uint32_t* counter, RbChunkShared& S, uint32_t& base) {
-  __syncthreads();   // (everybody is done with the previous chunk's keys)
-  if (threadIdx.x == 0) { S.chunk = atomicAdd(counter, 1u); S.group = 0u; }
-  __syncthreads();
-  base = S.chunk * (uint32_t)TPC_RB_CHUNK;
-  if (base >= n_items) return false;
-  for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK; i += blockDim.x) {
-    const uint32_t mi = base + i;
-    uint32_t len = mi < n_items ? len_of(mi) : 0u;
-    if (len > 0x3FFFFFu) len = 0x3FFFFFu;
-    S.key[i] = (len << 9) | i;
-  }
-  __syncthreads();
-  for (uint32_t size = 2; size <= TPC_RB_CHUNK; size <<= 1)         // bitonic sort, descending
-    for (uint32_t stride = size >> 1; stride > 0; stride >>= 1) {
-      for (uint32_t i = threadIdx.x; i < TPC_RB_CHUNK / 2; i += blockDim.x) {
-        const uint32_t lo = 2u * i - (i & (stride - 1u)), hi = lo + stride;
-        const uint32_t a = S.key[lo], b = S.key[hi];
-        const bool desc = (lo & size) == 0u;
-        if ((a < b) == desc) { S.key[lo] = b; S.key[hi] = a; }
-      }
-      __syncthreads();
-    }
-  return true;
-}
-// the warp's next group of 32 tracks of the chunk; false: none left
-__device__ __forceinline__ bool rb_group_next(uint32_t n_items, RbChunkShared& S, uint32_t base, uint32_t& mi, bool& valid) {
-  uint32_t g = 0u;
-  if ((threadIdx.x & 31u) == 0u) g = atomicAdd(&S.group, 1u);
-  g = __shfl_sync(0xFFFFFFFFu, g, 0);
-  if (g >= TPC_RB_CHUNK / 32) return false;
-  mi = base + (S.key[g * 32u + (threadIdx.x & 31u)] & (uint32_t)(TPC_RB_CHUNK - 1));
-  valid = mi < n_items;
-  return true;
 }
 
 __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffers M, TpcFitBuffers T,
@@ -3278,6 +3284,7 @@ static inline int grid_for(uint64_t n, int block, int n_sm, int ctas_per_sm) {
 int run_refit(const TpcBuffers& B, const TpcConst* hK, uint32_t n_tracks, cudaStream_t st, int n_sm) {
   if (n_tracks == 0) return 0;
   const FollowConst F = follow_const(hK);
+  cudaMemsetAsync(&B.cnt->refit_next, 0, 4, st);
   k_track_refit<<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit, 128)), 128, 0, st>>>(B, F, n_tracks);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
