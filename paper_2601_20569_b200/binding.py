@@ -640,7 +640,7 @@ class SectorTracker:
             return buf[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
         ns, nm = int(rv.n_steps), int(rv.n_merged)
         w = self.rebuild_ws
-        return dict(view=rv, step_ofs=arr(self.merge_ws, rv.d_step_ofs, nm + 1, np.uint32),
+        return dict(view=rv, step_ofs=arr(self.merge_ws, rv.d_step_ofs, nm + 1, np.uint32) if nm else np.zeros(1, np.uint32),
                     cand_id=arr(w, rv.d_cand_id, 3 * ns, np.int32).reshape(-1, 3),
                     cand_chi2=arr(w, rv.d_cand_chi2, 3 * ns, np.float32).reshape(-1, 3),
                     attached=arr(w, rv.d_attached, ns, np.int32), shared=arr(w, rv.d_shared, ns, np.uint8),

@@ -697,7 +697,7 @@ int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters,
   ctx->ran = true;
   ctx->synced = true;
   ctx->refit_done = false;
-  ctx->merged = false;
+  ctx->merged = false; ctx->fitted = false; ctx->rb_prepared = false; ctx->rebuilt = false;
   return TPC_OK;
 }
 
@@ -715,7 +715,7 @@ int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream) {
   ctx->stream = (cudaStream_t)cuda_stream;
   ctx->synced = false;
   ctx->refit_done = true;
-  ctx->merged = false;
+  ctx->merged = false; ctx->fitted = false; ctx->rb_prepared = false; ctx->rebuilt = false;
   return TPC_OK;
 }
 

@@ -995,6 +995,72 @@ def test_det_parity_phase2_rebuild_equal_weights(B):
     assert takeover >= 1
 
 
+def test_merged_track_legs_edge_cases_and_call_order(B):
+    """Refit / merging / fit / rebuild on frames without tracks (empty input; stubs whose tracklets are
+    all rejected) give empty results, as the oracle does; calls out of order, short or misaligned
+    workspaces and invalid parameters are refused with the documented codes; a new refit invalidates
+    what was derived from the previous one."""
+    import torch
+    from oracle import merging, rebuild, trackfit
+    for cl in (np.zeros(0, dtype=B.CLUSTER_DTYPE), stub_frame(n_stubs=60)):
+        trk = B.SectorTracker()
+        try:
+            trk.track(trk.upload(cl), flags=DET)
+            tracks, ids, shared, view = trk.tracks()
+            assert view.n_tracks == 0
+            trk.refit()
+            g = trk.merge()
+            fit, chi, rej = trk.fit()
+            r = trk.rebuild()
+        finally:
+            trk.close()
+        assert len(g["merged"]) == 0 and len(fit) == 0 and len(chi) == 0 and len(rej) == 0
+        assert len(r["fit"]) == 0 and len(r["attached"]) == 0 and r["cand_id"].shape == (0, 3)
+        if len(cl):
+            o = oracle.run(cl, n_threads=NT, want=("tracks",))
+            m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared)
+            q = rebuild.rebuild(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids)
+            assert len(o.tracks) == 0 and len(m.merged) == 0 and len(q.attached) == 0
+    cl, _, _ = dg.generate(dg.preset("C1"))
+    trk = B.SectorTracker()
+    st = torch.cuda.current_stream().cuda_stream
+    try:
+        trk.track(trk.upload(cl), flags=DET)
+        trk.counts()
+        ws = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+        # merging needs the refit, fit and rebuild need the merging, the rebuild needs its prepare call
+        assert B.tpc_merge_tracks(trk.ctx, None, ws.data_ptr(), ws.numel(), st) == B.TPC_E_STATE
+        trk.refit()
+        assert B.tpc_fit_tracks(trk.ctx, None, ws.data_ptr(), ws.numel(), st) == B.TPC_E_STATE
+        assert B.tpc_rebuild_prepare(trk.ctx, st)[0] == B.TPC_E_STATE
+        assert B.tpc_get_rebuild(trk.ctx)[0] == B.TPC_E_STATE
+        g = trk.merge()
+        assert len(g["merged"]) > 0
+        assert B.tpc_rebuild_tracks(trk.ctx, None, ws.data_ptr(), ws.numel(), st) == B.TPC_E_STATE
+        rc, n_steps = B.tpc_rebuild_prepare(trk.ctx, st)
+        assert rc == B.TPC_OK and n_steps > 0
+        need = B.tpc_rebuild_workspace_bytes(trk.ctx, n_steps, len(g["merged"]), len(cl))
+        big = torch.empty(need + 512, dtype=torch.uint8, device="cuda")
+        base = (big.data_ptr() + 255) // 256 * 256
+        assert B.tpc_rebuild_tracks(trk.ctx, None, base, need - 1, st) == B.TPC_E_WORKSPACE
+        assert B.tpc_rebuild_tracks(trk.ctx, None, base + 8, need, st) == B.TPC_E_ARG
+        assert B.tpc_rebuild_tracks(trk.ctx, None, 0, need, st) == B.TPC_E_ARG
+        assert B.tpc_rebuild_tracks(trk.ctx, B.tpc_rebuild_default_params(min_clusters=1), base, need, st) == B.TPC_E_ARG
+        assert B.tpc_rebuild_tracks(trk.ctx, B.tpc_rebuild_default_params(cand_chi2_max=float("nan")), base, need, st) == B.TPC_E_ARG
+        assert B.tpc_rebuild_tracks(trk.ctx, None, base, need, st) == B.TPC_OK
+        rc, rv = B.tpc_get_rebuild(trk.ctx)
+        assert rc == B.TPC_OK and rv.n_steps == n_steps and rv.n_merged == len(g["merged"])
+        # a new refit: the merged result, the fit and the rebuild of the old one are gone
+        trk.fit()
+        trk.refit()
+        assert B.tpc_get_merged(trk.ctx)[0] == B.TPC_E_STATE
+        assert B.tpc_get_fit(trk.ctx)[0] == B.TPC_E_STATE
+        assert B.tpc_get_rebuild(trk.ctx)[0] == B.TPC_E_STATE
+        assert B.tpc_rebuild_prepare(trk.ctx, st)[0] == B.TPC_E_STATE
+    finally:
+        trk.close()
+
+
 def rebuilt_lists(step_ofs, attached, used, fit_flags):
     """Cluster lists of the rebuilt tracks (used clusters of the tracks whose fit succeeded)."""
     ofs = np.asarray(step_ofs, dtype=np.int64)
