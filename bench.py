@@ -279,6 +279,25 @@ def run_split_sectors(args, rank, world, local_rank, dev, barrier):
     barrier()
     ms_total = reduce_over_ranks((time.perf_counter() - t0) * 1e3, "max", world, dev)
     launches = trk.launch_count() * args.steps
+    root_leg = None
+    if rank == 0:
+        # what the gather is for: the root builds the search grid of the whole frame only, loads the
+        # gathered sector tracks (tpc_set_tracks) and runs refit + merging on them (timed apart)
+        root = B.SectorTracker(params=B.tpc_default_params(**pkw), device=local_rank)
+        d_all = root.upload(clusters)
+        with torch.cuda.stream(stream):
+            for it in range(2):
+                torch.cuda.synchronize()
+                t1 = time.perf_counter()
+                root.track(d_all, flags=flags | B.TPC_GRID_ONLY, stream=stream)
+                root.set_tracks(res[0], res[1], res[2], stream=stream)
+                assert B.tpc_refit_tracks(root.ctx, stream.cuda_stream) == B.TPC_OK
+                root.merge(stream=stream, fetch=False)
+                rc_m, mv = B.tpc_get_merged(root.ctx)
+                root_ms = (time.perf_counter() - t1) * 1e3
+        root_leg = {"ms": root_ms, "what": "grid of the whole frame + tpc_set_tracks (host arrays) + refit + merging on rank 0",
+                    "merged_tracks": int(mv.n_merged), "links": int(mv.n_links)}
+        root.close()
     if rank == 0:
         n = len(clusters)
         print(json.dumps({
@@ -288,10 +307,11 @@ def run_split_sectors(args, rank, world, local_rank, dev, barrier):
             "config": {"workload": f"{args.workload}, one frame split by sector over {world} ranks + gather to rank 0",
                        "n_clusters": n, "mode": args.mode, "n_tracks_gathered": int(len(res[0])),
                        "timing": "host clock around tracking + result read-back + gather, max over ranks"},
-            "gpu_launches": launches}), flush=True)
+            "root_merging": root_leg, "gpu_launches": launches}), flush=True)
     trk.close()
-    dist.barrier()
-    dist.destroy_process_group()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
 
 
 # ------------------------------------------------------------------ the CUDA arm
@@ -320,7 +340,7 @@ def run_ours(args, rank, world, local_rank):
     def sum_over_ranks(x: float) -> float:
         return reduce_over_ranks(x, "sum", world, dev)
 
-    if args.split == "sectors" and world > 1:
+    if args.split == "sectors":
         run_split_sectors(args, rank, world, local_rank, dev, barrier)
         return
     cfg, clusters, labels, gen_s = make_frame(args.workload, rank, args.events, args.tracks)

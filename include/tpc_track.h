@@ -208,6 +208,8 @@ typedef struct tpc_debug_view {
                                      stable grid order, scans instead of atomics         */
 #define TPC_KEEP_INTERMEDIATES 2u /* keep the buffers tpc_get_intermediates exposes      */
 #define TPC_STAGE_TIMERS 4u       /* record CUDA events per stage (tpc_get_stage_ms)     */
+#define TPC_GRID_ONLY 8u          /* build the search grid and stop: no seeds, no tracks; the tracks
+                                     then come from tpc_set_tracks (a frame tracked elsewhere)  */
 
 #define TPC_N_STAGES 6            /* grid, neighbours, cleanup+seeds, follower, selector, total */
 
@@ -301,6 +303,20 @@ size_t tpc_workspace_bytes_two_iterations(const tpc_ctx* ctx, uint64_t n_cluster
 int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters, uint64_t n_clusters,
                                     void* d_workspace, size_t workspace_bytes, void* cuda_stream,
                                     uint32_t flags);
+
+/* TRACKS FROM ELSEWHERE (first axis: one frame over several GPUs by sector;
+ * sector tracking is independent per sector, :29: merging is not): loads the sector
+ * tracks of the current frame -- tracked sector group by sector group on other contexts / ranks,
+ * rebased to frame cluster indices and concatenated in any order -- into this context, so that
+ * refit, merging, fit and rebuild run on them as on the context's own result.  Needs a finished
+ * tpc_sector_track of the WHOLE frame on this context (TPC_GRID_ONLY is enough: the rebuild queries
+ * the grid, refit and fit read the clusters), in the mode (deterministic or fast) the legs shall run in.
+ * h_tracks [n_tracks], h_cluster_ids / h_cluster_shared [n_cluster_ids]: HOST, copied before the call
+ * returns (synchronises cuda_stream).  TPC_E_OVERFLOW if they exceed the workspace's capacities
+ * (those of a frame of this size), TPC_E_ARG if a track names a sector / row outside the geometry, a
+ * cluster list outside [0, n_cluster_ids) or a cluster id outside the frame. */
+int tpc_set_tracks(tpc_ctx* ctx, const tpc_track* h_tracks, uint64_t n_tracks, const uint32_t* h_cluster_ids,
+                   const uint8_t* h_cluster_shared, uint64_t n_cluster_ids, void* cuda_stream);
 
 /* SECTOR-TRACK REFIT (section 3: "a sector track refit at the beginning of the track
  * merging was added, guaranteeing reasonable initial parameters"; reading R8): a pure

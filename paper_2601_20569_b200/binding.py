@@ -18,7 +18,7 @@ import numpy as np
 from .build import LIB_PATH
 
 TPC_OK, TPC_E_ARG, TPC_E_WORKSPACE, TPC_E_OVERFLOW, TPC_E_CUDA, TPC_E_STATE = 0, -1, -2, -3, -4, -5
-TPC_DETERMINISTIC, TPC_KEEP_INTERMEDIATES, TPC_STAGE_TIMERS = 1, 2, 4
+TPC_DETERMINISTIC, TPC_KEEP_INTERMEDIATES, TPC_STAGE_TIMERS, TPC_GRID_ONLY = 1, 2, 4, 8
 TPC_N_STAGES = 6
 STAGE_NAMES = ("grid", "neighbours", "cleanup_seeds", "follower", "selector", "total")
 
@@ -129,7 +129,7 @@ EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_se
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
            "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_merge_default_params",
            "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_fit_default_params",
-           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_rebuild_default_params",
+           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_rebuild_default_params", "tpc_set_tracks",
            "tpc_rebuild_prepare", "tpc_rebuild_workspace_bytes", "tpc_rebuild_tracks", "tpc_get_rebuild",
            "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
@@ -194,6 +194,8 @@ def load_library():
     L.tpc_fit_tracks.argtypes = [vp, C.POINTER(FitParams), vp, C.c_size_t, vp]
     L.tpc_get_fit.restype = C.c_int
     L.tpc_get_fit.argtypes = [vp, C.POINTER(FitView)]
+    L.tpc_set_tracks.restype = C.c_int
+    L.tpc_set_tracks.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_uint64, vp]
     L.tpc_rebuild_default_params.restype = None
     L.tpc_rebuild_default_params.argtypes = [C.POINTER(RebuildParams)]
     L.tpc_rebuild_prepare.restype = C.c_int
@@ -381,6 +383,11 @@ def tpc_get_fit(ctx: int):
     v = FitView()
     rc = load_library().tpc_get_fit(ctx, C.byref(v))
     return rc, v
+
+
+def tpc_set_tracks(ctx: int, h_tracks: int, n_tracks: int, h_cluster_ids: int, h_cluster_shared: int, n_cluster_ids: int,
+                   cuda_stream: int) -> int:
+    return load_library().tpc_set_tracks(ctx, h_tracks, n_tracks, h_cluster_ids, h_cluster_shared, n_cluster_ids, cuda_stream)
 
 
 def tpc_rebuild_default_params(**overrides) -> RebuildParams:
@@ -609,6 +616,19 @@ class SectorTracker:
             return self.fit_ws[off:off + count * dtype.itemsize].cpu().numpy().view(dtype).copy()
         return (arr(fv.d_fit, int(fv.n_merged), TRACK_FIT3_DTYPE), arr(fv.d_chi2_cluster, int(fv.n_cluster_ids), np.float32),
                 arr(fv.d_rejected, int(fv.n_cluster_ids), np.uint8))
+
+    def set_tracks(self, tracks, cluster_ids, cluster_shared, stream=None):
+        """Loads sector tracks of the current frame that were made elsewhere (tpc_set_tracks): numpy
+        arrays TRACK_DTYPE / uint32 / uint8 with frame cluster indices."""
+        st = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        t = np.ascontiguousarray(tracks, dtype=TRACK_DTYPE)
+        i = np.ascontiguousarray(cluster_ids, dtype=np.uint32)
+        s = np.ascontiguousarray(cluster_shared, dtype=np.uint8)
+        if len(i) != len(s):
+            raise ValueError("cluster_ids and cluster_shared differ in length")
+        rc = tpc_set_tracks(self.ctx, t.ctypes.data, len(t), i.ctypes.data, s.ctypes.data, len(i), st.cuda_stream)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpc_set_tracks", tpc_last_cuda_error(self.ctx))
 
     def rebuild(self, rparams: RebuildParams | None = None, stream=None, fetch: bool = True):
         """Phase-II track rebuild (reading R11) of the merged tracks; merge() must have

@@ -701,6 +701,41 @@ int tpc_sector_track_two_iterations(tpc_ctx* ctx, const tpc_cluster* d_clusters,
   return TPC_OK;
 }
 
+int tpc_set_tracks(tpc_ctx* ctx, const tpc_track* h_tracks, uint64_t n_tracks, const uint32_t* h_ids,
+                   const uint8_t* h_shared, uint64_t n_ids, void* cuda_stream) {
+  int rc = sync_run(ctx);
+  if (rc != TPC_OK) return rc;
+  rc = device_status(ctx);
+  if (rc != TPC_OK) return rc;
+  if ((n_tracks && !h_tracks) || (n_ids && (!h_ids || !h_shared))) return TPC_E_ARG;
+  const TpcBuffers& B = ctx->buf;
+  if (B.id_base != 0u) return TPC_E_STATE;   // (the context holds one chunk of a chunked host call)
+  if (n_tracks > B.max_tracks || n_ids > B.max_ids) return TPC_E_OVERFLOW;
+  for (uint64_t i = 0; i < n_tracks; ++i) {
+    const tpc_track& t = h_tracks[i];
+    if ((int)t.sector >= ctx->geom.n_sectors || t.row_first > t.row_last || (int)t.row_last >= ctx->geom.n_rows ||
+        (uint64_t)t.cluster_ofs + t.n_clusters > n_ids)
+      return TPC_E_ARG;
+  }
+  for (uint64_t i = 0; i < n_ids; ++i)
+    if (h_ids[i] >= B.n) return TPC_E_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaSuccess;
+  if (n_tracks) e = cudaMemcpyAsync(B.tracks, h_tracks, sizeof(tpc_track) * n_tracks, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && n_ids) e = cudaMemcpyAsync(B.cluster_ids, h_ids, 4 * n_ids, cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess && n_ids) e = cudaMemcpyAsync(B.cluster_shared, h_shared, n_ids, cudaMemcpyHostToDevice, st);
+  ctx->h_cnt->n_tracks = (uint32_t)n_tracks;
+  ctx->h_cnt->n_ids = (uint32_t)n_ids;
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(&ctx->d_cnt->n_tracks, &ctx->h_cnt->n_tracks, 2 * sizeof(uint32_t), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return set_cuda_err(ctx, e, "cudaMemcpyAsync(tracks)");
+  ctx->stream = st;
+  ctx->refit_done = false;
+  ctx->merged = false; ctx->fitted = false; ctx->rb_prepared = false; ctx->rebuilt = false;
+  return TPC_OK;
+}
+
 int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream) {
   int rc = sync_run(ctx);
   if (rc != TPC_OK) return rc;

@@ -3414,6 +3414,11 @@ int run_pipeline(const TpcBuffers& B, const TpcConst* hK, cudaStream_t st, uint3
   TPC_LAUNCH_CHECK("k_bin_sort");
 #endif
   if (timers) cudaEventRecord(E.ev[1], st);
+  if (flags & TPC_GRID_ONLY) {   // the tracks come from tpc_set_tracks
+    if (timers) for (int i = 2; i <= 5; ++i) cudaEventRecord(E.ev[i], st);
+    E.n_kernels = launches < TPC_MAX_KERNELS ? launches : TPC_MAX_KERNELS;
+    return launches;
+  }
   // ---- K2 neighbour finder
   k_neighbours<<<grid_for((uint64_t)(B.n / TPC_NF_TILE + B.n_sr) * TPC_NF_TILE, TPC_NF_TILE, n_sm, resident_ctas(k_neighbours, TPC_NF_TILE)), TPC_NF_TILE, 0, st>>>(B);
   TPC_LAUNCH_CHECK("k_neighbours");

@@ -889,7 +889,7 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0 < ro.sum() < 0.02 * len(ro)
 
 
-def rebuild_det_parity(B, cl, pkw):
+def rebuild_det_parity(B, cl, pkw, tracking=None):
     """Phase-II rebuild, deterministic mode, against oracle.rebuild: per path step the three candidates
     (ids and chi2 bits), the attached cluster after the second ambiguity solving, the shared and used
     marks, per track the final fit -- all bit-exact.  Returns both sides for further checks."""
@@ -897,7 +897,10 @@ def rebuild_det_parity(B, cl, pkw):
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
     try:
-        trk.track(trk.upload(cl), flags=1)
+        if tracking is None:
+            trk.track(trk.upload(cl), flags=1)
+        else:
+            tracking(trk, gp)          # (leaves the frame's sector tracks in trk by other means)
         tracks, ids, shared, view = trk.tracks()
         trk.refit()
         g = trk.merge()
@@ -993,6 +996,59 @@ def test_det_parity_phase2_rebuild_equal_weights(B):
             owners.add(float(np.sign(cl["y"][tracks["seed_id"][h[who[0]]]])))   # (seed id = a cluster of the track)
     assert owners == {1.0, -1.0}
     assert takeover >= 1
+
+
+def test_sector_split_then_merging_and_rebuild_on_the_root(B):
+    """SURVEY.md 8(e) first axis composed with 8(f): the frame is tracked in 3 sector groups ('ranks',
+    one after the other on this GPU), the results are rebased and concatenated as the gather does,
+    and the root -- which builds only the search grid of the whole frame (TPC_GRID_ONLY) -- loads them
+    with tpc_set_tracks and runs refit, merging (incl. across sector edges and the electrode) and the
+    Phase-II rebuild: bit-exact against the oracle's whole-frame chain in deterministic mode.  Also:
+    the argument checks of tpc_set_tracks."""
+    from paper_2601_20569_b200 import multigpu as mg
+    cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=3000, seed=29))
+
+    def tracking(trk, gp):
+        parts, base = [], 0
+        for r in range(3):
+            sub, delta = mg.split_by_sector(cl, r, 3)
+            t2 = B.SectorTracker(params=gp)
+            try:
+                t2.track(t2.upload(sub), flags=DET)
+                tracks, ids, shared, view = t2.tracks()
+            finally:
+                t2.close()
+            tracks, ids = mg.rebase(tracks, ids, delta)
+            tracks["cluster_ofs"] += np.uint32(base)
+            base += len(ids)
+            parts.append((tracks, ids, shared))
+        tracks = np.concatenate([p[0] for p in parts])
+        ids = np.concatenate([p[1] for p in parts])
+        shared = np.concatenate([p[2] for p in parts])
+        trk.track(trk.upload(cl), flags=DET | B.TPC_GRID_ONLY)
+        rc, v = trk.counts()
+        assert v.n_tracks == 0 and v.n_seeds == 0
+        # refused: a cluster list beyond the id array, a cluster id beyond the frame, a row beyond the geometry
+        bad = tracks.copy(); bad["cluster_ofs"][-1] = len(ids)
+        with pytest.raises(B.TpcError):
+            trk.set_tracks(bad, ids, shared)
+        bad_ids = ids.copy(); bad_ids[0] = len(cl)
+        with pytest.raises(B.TpcError):
+            trk.set_tracks(tracks, bad_ids, shared)
+        bad = tracks.copy(); bad["row_last"][0] = 152
+        with pytest.raises(B.TpcError):
+            trk.set_tracks(bad, ids, shared)
+        trk.set_tracks(tracks, ids, shared)
+        rc, v = trk.counts()
+        assert v.n_tracks == len(tracks) and v.n_cluster_ids == len(ids)
+
+    x = rebuild_det_parity(B, cl, {}, tracking=tracking)
+    m = x["m"]
+    # the frame does have merges across sector groups: links between tracks of different sectors
+    nxt = m.next
+    a = np.flatnonzero(nxt >= 0)
+    assert (x["o"].tracks["sector"][a] != x["o"].tracks["sector"][nxt[a]]).sum() > 10
+    assert x["ok"].sum() > 0.9 * len(m.merged)
 
 
 def test_merged_track_legs_edge_cases_and_call_order(B):
