@@ -784,6 +784,7 @@ size_t carve_merge(const tpc_ctx* c, uint64_t n_tracks, uint64_t n_ids, char* ba
   m.next = (int32_t*)take(4 * nt); m.prev = (int32_t*)take(4 * nt); m.link_chi2 = (float*)take(4 * nt);
   m.best_out = (int32_t*)take(4 * nt); m.best_out_chi = (uint32_t*)take(4 * nt); m.best_in_chi = (uint32_t*)take(4 * nt);
   m.best_in_key = (unsigned long long*)take(8 * nt);
+  m.cand = (uint2*)take(8 * (size_t)TPC_MG_CAND * nt); m.cand_cnt = (uint32_t*)take(4 * nt);
   m.head_ofs = (uint32_t*)take(4 * nt); m.seg_ofs = (uint32_t*)take(4 * nt); m.clu_ofs = (uint32_t*)take(4 * nt);
   m.seg_dst = (uint32_t*)take(4 * nt);
   m.merged = (tpc_merged_track*)take(sizeof(tpc_merged_track) * nt);

@@ -128,6 +128,7 @@ struct TpcBuffers {
 };
 
 // Buffers of the track merging (R9), pointers into the caller's merge workspace.
+#define TPC_MG_CAND 4
 struct TpcMergeBuffers {
   tpc_merge_params P;
   uint32_t n_tracks, n_ids, n_rows, n_cells;
@@ -139,6 +140,7 @@ struct TpcMergeBuffers {
   float* ends;            // [n_tracks][16] compact inner-end records in cell order
   int32_t* next; int32_t* prev; float* link_chi2;                  // [n_tracks]
   int32_t* best_out; uint32_t* best_out_chi; uint32_t* best_in_chi; unsigned long long* best_in_key;
+  uint2* cand; uint32_t* cand_cnt;   // [n_tracks][TPC_MG_CAND] accepted candidates (partner, chi2 bits) of the stage's pass 1; their number
   uint32_t* head_ofs; uint32_t* seg_ofs; uint32_t* clu_ofs; uint32_t* seg_dst;   // [n_tracks]
   tpc_merged_track* merged;  // [n_tracks]
   uint32_t* seg_index;       // [n_tracks]

@@ -2419,6 +2419,7 @@ __global__ void __launch_bounds__(256) k_merge_bin_fill(TpcBuffers B, TpcMergeBu
 __global__ void __launch_bounds__(256) k_merge_stage_reset(TpcMergeBuffers M) {
   for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < M.n_tracks; t += gridDim.x * blockDim.x) {
     M.best_out[t] = -1; M.best_out_chi[t] = 0xFFFFFFFFu; M.best_in_chi[t] = 0xFFFFFFFFu; M.best_in_key[t] = ~0ull;
+    M.cand_cnt[t] = 0u;
   }
 }
 
@@ -2460,6 +2461,8 @@ __global__ void __launch_bounds__(128) k_merge_sweep(TpcBuffers B, TpcMergeBuffe
   const int R = (int)M.n_rows;
   for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < M.n_tracks; a += gridDim.x * blockDim.x) {
     if (M.next[a] >= 0) continue;                      // outer end already linked by an earlier stage
+    if (PASS == 2 && M.cand_cnt[a] <= TPC_MG_CAND) continue;   // settled from the cached candidates (k_merge_resolve)
+    uint32_t n_cand = 0u;
     const tpc_track_fit* fa = B.track_fit + a;
     if (fa->flags) continue;
     const tpc_track ta = B.tracks[a];
@@ -2515,6 +2518,8 @@ __global__ void __launch_bounds__(128) k_merge_sweep(TpcBuffers B, TpcMergeBuffe
               best = (int32_t)b; best_chi2 = chi2; best_key = key_b;
             }
             atomicMin(&M.best_in_chi[b], __float_as_uint(chi2));      // chi2 >= 0: bit order = value order
+            if (n_cand < TPC_MG_CAND) M.cand[(size_t)a * TPC_MG_CAND + n_cand] = make_uint2(b, __float_as_uint(chi2));
+            ++n_cand;
           } else if (__float_as_uint(chi2) == M.best_in_chi[b]) {
             atomicMin(&M.best_in_key[b], key_a);
           }
@@ -2547,7 +2552,23 @@ __global__ void __launch_bounds__(128) k_merge_sweep(TpcBuffers B, TpcMergeBuffe
         }
       }
     }
-    if (PASS == 1) { M.best_out[a] = best; M.best_out_chi[a] = __float_as_uint(best_chi2); }
+    if (PASS == 1) { M.best_out[a] = best; M.best_out_chi[a] = __float_as_uint(best_chi2); M.cand_cnt[a] = n_cand; }
+  }
+}
+
+// Pass 2 for the tracks whose accepted candidates fit the cache (nearly all): among the holders of a
+// partner's minimum chi2 the least 64-bit id wins.  The others repeat the sweep (k_merge_sweep<., 2>).
+// (The cached chi2 bits are pass 1's own, so the comparison with the minimum cannot miss by a rounding
+// difference between two compilations of the sweep, which the fast build's repeated sweep could.)
+__global__ void __launch_bounds__(256) k_merge_resolve(TpcBuffers B, TpcMergeBuffers M) {
+  for (uint32_t a = blockIdx.x * blockDim.x + threadIdx.x; a < M.n_tracks; a += gridDim.x * blockDim.x) {
+    const uint32_t n = M.cand_cnt[a];
+    if (n == 0u || n > TPC_MG_CAND) continue;
+    const unsigned long long key_a = merge_key(B.tracks[a]);
+    for (uint32_t i = 0; i < n; ++i) {
+      const uint2 c = M.cand[(size_t)a * TPC_MG_CAND + i];
+      if (c.y == M.best_in_chi[c.x]) atomicMin(&M.best_in_key[c.x], key_a);
+    }
   }
 }
 
@@ -3314,11 +3335,11 @@ int run_merge(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M,
     for (int stage = 1; stage <= 3; ++stage) {
       if (!((M.P.stages >> (stage - 1)) & 1)) continue;
       k_merge_stage_reset<<<g256, 256, 0, st>>>(M);
-      if (stage == 1) { k_merge_sweep<1, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<1, 2><<<gs, 128, 0, st>>>(B, M, F); }
-      if (stage == 2) { k_merge_sweep<2, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<2, 2><<<gs, 128, 0, st>>>(B, M, F); }
-      if (stage == 3) { k_merge_sweep<3, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_sweep<3, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      if (stage == 1) { k_merge_sweep<1, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_resolve<<<g256, 256, 0, st>>>(B, M); k_merge_sweep<1, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      if (stage == 2) { k_merge_sweep<2, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_resolve<<<g256, 256, 0, st>>>(B, M); k_merge_sweep<2, 2><<<gs, 128, 0, st>>>(B, M, F); }
+      if (stage == 3) { k_merge_sweep<3, 1><<<gs, 128, 0, st>>>(B, M, F); k_merge_resolve<<<g256, 256, 0, st>>>(B, M); k_merge_sweep<3, 2><<<gs, 128, 0, st>>>(B, M, F); }
       k_merge_link<<<g256, 256, 0, st>>>(B, M);
-      launches += 4;
+      launches += 5;
     }
     k_merge_chain_count<<<g256, 256, 0, st>>>(B, M);
     scan_u32(M.head_ofs, M.n_tracks, M.partials, &M.counters[0], st);
