@@ -49,7 +49,8 @@ typedef enum tpc_error {
   TPC_E_OVERFLOW = -3,  /* a capacity bound was hit on the device (bin index, tracks);
                            results are invalid, never silently truncated               */
   TPC_E_CUDA = -4,      /* a CUDA runtime call failed; see tpc_last_cuda_error()         */
-  TPC_E_STATE = -5      /* call order violated (e.g. tpc_get_tracks before a run)       */
+  TPC_E_STATE = -5,     /* call order violated (e.g. tpc_get_tracks before a run)       */
+  TPC_E_LIMIT = -6      /* a size beyond the fixed maximum of tpc_fit_tracks_noalloc; nothing run */
 } tpc_error;
 
 /* ------------------------------------------------------------------ input */
@@ -433,6 +434,37 @@ size_t tpc_fit_workspace_bytes(const tpc_ctx* ctx, uint64_t n_merged, uint64_t n
 int tpc_fit_tracks(tpc_ctx* ctx, const tpc_fit_params* params, void* d_fit_workspace, size_t workspace_bytes,
                    void* cuda_stream);
 int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out);
+
+/* THE FIT WITHOUT ANY ALLOCATION AND WITHOUT A WORKSPACE (for callers that cannot call cudaMalloc: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  The same three-iteration fit
+ * as tpc_fit_tracks (reading R10; the same kernel, the same results), but the
+ * caller passes every input and output as a DEVICE pointer and the kernel's scratch -- the predictions
+ * stored in iteration 1, 16 bytes per cluster id, plus a 256-byte header (merged-track count, work
+ * counter) -- lives in ONE array inside the library: 256 + 16 * TPC_FIT_NOALLOC_MAX_IDS bytes (16 MiB)
+ * that every GPU which loads the library holds until the process exits.  Its device address is resolved
+ * once per device in tpc_geom_init (set-up; cudaGetSymbolAddress with that device current); this call
+ * performs no cudaMalloc / cudaFree and calls no allocating routine, and does not synchronise.
+ *   ctx            geometry, parameters and the device of tpc_geom_init (which must be the current device,
+ *                  else TPC_E_STATE); the context's own run state is neither needed nor touched
+ *   d_clusters     [n_clusters] the frame; d_refit [n_tracks] the sector-track refit records (tpc_get_refit)
+ *   d_merged       [n_merged] merged tracks; d_seg_index [n_tracks], d_cluster_ids [n_cluster_ids] as in
+ *                  the merged view; the caller guarantees that their offsets and indices stay inside
+ *                  these arrays: device contents are not checked
+ *   d_fit_out      [n_merged], d_chi2_out / d_rejected_out [n_cluster_ids]: written by the call
+ *   flags          TPC_DETERMINISTIC or 0: the build to run
+ * Errors: TPC_E_LIMIT if n_cluster_ids > TPC_FIT_NOALLOC_MAX_IDS (text in tpc_last_cuda_error; nothing
+ * is launched); TPC_E_ARG for null / misaligned pointers or invalid
+ * parameters; TPC_E_CUDA if the set-up could not resolve the array or a launch failed.
+ * EVERY call on a device shares the one array, which keeps the previous call's contents: the call itself
+ * resets what must start at zero (the header); the stored predictions are written before they are read.
+ * Two calls that overlap on the GPU (different streams, or the same data from two host threads) RACE on
+ * it: serialise them (one stream, or an event between them). */
+#define TPC_FIT_NOALLOC_MAX_IDS (1u << 20)
+int tpc_fit_tracks_noalloc(tpc_ctx* ctx, const tpc_fit_params* params, const tpc_cluster* d_clusters,
+                           uint64_t n_clusters, const tpc_track_fit* d_refit, uint64_t n_tracks,
+                           const tpc_merged_track* d_merged, uint64_t n_merged, const uint32_t* d_seg_index,
+                           const uint32_t* d_cluster_ids, uint64_t n_cluster_ids, tpc_track_fit3* d_fit_out,
+                           float* d_chi2_out, uint8_t* d_rejected_out, uint32_t flags, void* cuda_stream);
 
 /* PHASE-II TRACK REBUILD (section 3: "the track is practically rebuilt during iterations 2
  * and 3 of the fit ... the fast cluster search grid from the sector tracking is queried for all clusters

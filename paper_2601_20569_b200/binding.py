@@ -129,7 +129,7 @@ EXPORTS = ("tpc_default_params", "tpc_geom_init", "tpc_workspace_bytes", "tpc_se
            "tpc_sector_track_host", "tpc_sector_track_host_chunks", "tpc_workspace_bytes_two_iterations",
            "tpc_sector_track_two_iterations", "tpc_refit_tracks", "tpc_get_refit", "tpc_merge_default_params",
            "tpc_merge_workspace_bytes", "tpc_merge_tracks", "tpc_get_merged", "tpc_fit_default_params",
-           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_rebuild_default_params", "tpc_set_tracks",
+           "tpc_fit_workspace_bytes", "tpc_fit_tracks", "tpc_get_fit", "tpc_fit_tracks_noalloc", "tpc_rebuild_default_params", "tpc_set_tracks",
            "tpc_rebuild_prepare", "tpc_rebuild_workspace_bytes", "tpc_rebuild_tracks", "tpc_get_rebuild",
            "tpc_last_launch_count",
            "tpc_destroy", "tpc_strerror", "tpc_last_cuda_error")
@@ -194,6 +194,9 @@ def load_library():
     L.tpc_fit_tracks.argtypes = [vp, C.POINTER(FitParams), vp, C.c_size_t, vp]
     L.tpc_get_fit.restype = C.c_int
     L.tpc_get_fit.argtypes = [vp, C.POINTER(FitView)]
+    L.tpc_fit_tracks_noalloc.restype = C.c_int
+    L.tpc_fit_tracks_noalloc.argtypes = [vp, C.POINTER(FitParams), vp, C.c_uint64, vp, C.c_uint64, vp, C.c_uint64, vp, vp,
+                                         C.c_uint64, vp, vp, vp, C.c_uint32, vp]
     L.tpc_set_tracks.restype = C.c_int
     L.tpc_set_tracks.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_uint64, vp]
     L.tpc_rebuild_default_params.restype = None
@@ -377,6 +380,20 @@ def tpc_fit_workspace_bytes(ctx: int, n_merged: int, n_cluster_ids: int) -> int:
 def tpc_fit_tracks(ctx: int, params, d_workspace: int, workspace_bytes: int, cuda_stream: int) -> int:
     return load_library().tpc_fit_tracks(ctx, C.byref(params) if params is not None else None, d_workspace,
                                          workspace_bytes, cuda_stream)
+
+
+TPC_E_LIMIT = -6
+TPC_FIT_NOALLOC_MAX_IDS = 1 << 20
+
+
+def tpc_fit_tracks_noalloc(ctx: int, params, d_clusters: int, n_clusters: int, d_refit: int, n_tracks: int, d_merged: int,
+                           n_merged: int, d_seg_index: int, d_cluster_ids: int, n_cluster_ids: int, d_fit_out: int,
+                           d_chi2_out: int, d_rejected_out: int, flags: int, cuda_stream: int) -> int:
+    """The three-iteration fit with every input / output passed as a device pointer and the scratch inside
+    the library (no workspace, no allocation; at most TPC_FIT_NOALLOC_MAX_IDS cluster ids)."""
+    return load_library().tpc_fit_tracks_noalloc(ctx, C.byref(params) if params is not None else None, d_clusters, n_clusters,
+                                                 d_refit, n_tracks, d_merged, n_merged, d_seg_index, d_cluster_ids,
+                                                 n_cluster_ids, d_fit_out, d_chi2_out, d_rejected_out, flags, cuda_stream)
 
 
 def tpc_get_fit(ctx: int):

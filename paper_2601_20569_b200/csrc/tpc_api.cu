@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "tpc_internal.h"
@@ -43,12 +44,55 @@ struct tpc_ctx {
   TpcFitBuffers fbuf;
   uint32_t fit_n_merged = 0, fit_n_ids = 0;
   uint32_t* h_mcnt = nullptr;  // pinned: merge counters
+  void* noalloc_scratch = nullptr;   // device address of g_fit_noalloc_scratch on this context's device (set-up)
+  char noalloc_err[128] = {0};       // why it could not be resolved
   char cuda_err[256] = {0};
 };
+
+// ---- scratch of tpc_fit_tracks_noalloc: ONE array inside the library, held by every GPU that loads it.
+// Layout: [0,16) counters (word 0: merged-track count), [16,32) work counter of the kernel, [256, ...) the
+// predictions stored in iteration 1 (16 bytes per cluster id).  In HOST code the name below is a
+// stand-in, not a device address: the address comes from cudaGetSymbolAddress, once per device, at
+// set-up (noalloc_setup, called by tpc_geom_init with that device current).
+#define TPC_FIT_NOALLOC_HDR 256
+static __device__ __align__(256) unsigned char g_fit_noalloc_scratch[TPC_FIT_NOALLOC_HDR + 16ull * TPC_FIT_NOALLOC_MAX_IDS];
+
+// (device code of this file names the array directly)
+__global__ void k_fit_noalloc_header(uint32_t n_merged) {
+  uint32_t* h = reinterpret_cast<uint32_t*>(g_fit_noalloc_scratch);
+  if (threadIdx.x < 8) h[threadIdx.x] = threadIdx.x == 0 ? n_merged : 0u;
+}
 
 namespace {
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+#define TPC_NOALLOC_MAX_DEVICES 64
+std::mutex g_noalloc_mutex;
+void* g_noalloc_ptr[TPC_NOALLOC_MAX_DEVICES] = {nullptr};
+bool g_noalloc_done[TPC_NOALLOC_MAX_DEVICES] = {false};
+cudaError_t g_noalloc_rc[TPC_NOALLOC_MAX_DEVICES] = {cudaSuccess};
+
+// Once per device, with that device current.  Never fatal for the caller: a failure is reported by
+// tpc_fit_tracks_noalloc alone.
+void noalloc_setup(tpc_ctx* c) {
+  c->noalloc_scratch = nullptr;
+  if (c->device < 0 || c->device >= TPC_NOALLOC_MAX_DEVICES) {
+    std::snprintf(c->noalloc_err, sizeof(c->noalloc_err), "device ordinal %d beyond %d", c->device, TPC_NOALLOC_MAX_DEVICES);
+    return;
+  }
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_done[c->device]) {
+    void* p = nullptr;
+    g_noalloc_rc[c->device] = cudaGetSymbolAddress(&p, g_fit_noalloc_scratch);
+    g_noalloc_ptr[c->device] = g_noalloc_rc[c->device] == cudaSuccess ? p : nullptr;
+    g_noalloc_done[c->device] = true;
+    if (g_noalloc_rc[c->device] != cudaSuccess) (void)cudaGetLastError();
+  }
+  c->noalloc_scratch = g_noalloc_ptr[c->device];
+  if (!c->noalloc_scratch)
+    std::snprintf(c->noalloc_err, sizeof(c->noalloc_err), "cudaGetSymbolAddress: %s", cudaGetErrorString(g_noalloc_rc[c->device]));
+}
 
 int set_cuda_err(tpc_ctx* c, cudaError_t e, const char* what) {
   if (c) std::snprintf(c->cuda_err, sizeof(c->cuda_err), "%s: %s", what, cudaGetErrorString(e));
@@ -220,6 +264,7 @@ int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx**
     tpc_destroy(c);
     return TPC_E_CUDA;
   }
+  noalloc_setup(c);   // (address of the library's static scratch on this device; see tpc_fit_tracks_noalloc)
   c->events.enabled = false;
   c->events.n_kernels = 0;
   for (int i = 0; i < TPC_N_STAGES; ++i) c->events.ev[i] = nullptr;
@@ -943,6 +988,72 @@ int tpc_get_fit(tpc_ctx* ctx, tpc_fit_view* out) {
   return TPC_OK;
 }
 
+int tpc_fit_tracks_noalloc(tpc_ctx* ctx, const tpc_fit_params* params, const tpc_cluster* d_clusters, uint64_t n_clusters,
+                           const tpc_track_fit* d_refit, uint64_t n_tracks, const tpc_merged_track* d_merged,
+                           uint64_t n_merged, const uint32_t* d_seg_index, const uint32_t* d_cluster_ids,
+                           uint64_t n_cluster_ids, tpc_track_fit3* d_fit_out, float* d_chi2_out, uint8_t* d_rejected_out,
+                           uint32_t flags, void* cuda_stream) {
+  if (!ctx) return TPC_E_ARG;
+  if (n_cluster_ids > TPC_FIT_NOALLOC_MAX_IDS) {
+    std::snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
+                  "tpc_fit_tracks_noalloc: %llu cluster ids exceed TPC_FIT_NOALLOC_MAX_IDS = %u (the library's static scratch); "
+                  "use tpc_fit_tracks with a workspace", (unsigned long long)n_cluster_ids, (unsigned)TPC_FIT_NOALLOC_MAX_IDS);
+    return TPC_E_LIMIT;
+  }
+  if (n_merged > n_cluster_ids || n_merged > n_tracks || n_clusters >= (1ull << 30) || n_tracks >= (1ull << 30)) return TPC_E_ARG;
+  if (n_merged && (!d_clusters || !d_refit || !d_merged || !d_seg_index || !d_cluster_ids || !d_fit_out || !d_chi2_out ||
+                   !d_rejected_out))
+    return TPC_E_ARG;
+  if (((uintptr_t)d_clusters & 15u) || ((uintptr_t)d_refit & 3u) || ((uintptr_t)d_merged & 3u) || ((uintptr_t)d_seg_index & 3u) ||
+      ((uintptr_t)d_cluster_ids & 3u) || ((uintptr_t)d_fit_out & 3u) || ((uintptr_t)d_chi2_out & 3u))
+    return TPC_E_ARG;
+  if (flags & ~TPC_DETERMINISTIC) return TPC_E_ARG;
+  tpc_fit_params P;
+  if (params) P = *params; else tpc_fit_default_params(&P);
+  if (!(P.fit_chi2_max >= 0.f) || P.fit_min_clusters < 2 || !(P.ce_var > 0.f)) return TPC_E_ARG;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device) return TPC_E_STATE;   // (the address belongs to ctx's device)
+  if (!ctx->noalloc_scratch) {
+    std::snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "tpc_fit_tracks_noalloc: static scratch not resolved at set-up: %s",
+                  ctx->noalloc_err);
+    return TPC_E_CUDA;
+  }
+  if (n_merged == 0) return TPC_OK;
+  char* scratch = (char*)ctx->noalloc_scratch;
+  TpcBuffers B;
+  std::memset(&B, 0, sizeof(B));
+  B.K = ctx->d_const;
+  B.clusters = d_clusters;
+  B.n = (uint32_t)n_clusters;
+  B.id_base = 0u;
+  B.track_fit = const_cast<tpc_track_fit*>(d_refit);          // (read only by the fit)
+  TpcMergeBuffers M;
+  std::memset(&M, 0, sizeof(M));
+  M.n_tracks = (uint32_t)n_tracks;
+  M.counters = reinterpret_cast<uint32_t*>(scratch);
+  M.merged = const_cast<tpc_merged_track*>(d_merged);
+  M.seg_index = const_cast<uint32_t*>(d_seg_index);
+  M.ids = const_cast<uint32_t*>(d_cluster_ids);
+  TpcFitBuffers T;
+  std::memset(&T, 0, sizeof(T));
+  T.P = P;
+  const double a = 2.0 * (double)ctx->geom.sector_half_angle_deg * (3.14159265358979323846 / 180.0);
+  T.ca = (float)std::cos(a);
+  T.sa = (float)std::sin(a);
+  T.work = reinterpret_cast<uint32_t*>(scratch + 16);
+  T.stored = reinterpret_cast<uint4*>(scratch + TPC_FIT_NOALLOC_HDR);
+  T.chi2_cluster = d_chi2_out;
+  T.rejected = d_rejected_out;
+  T.fit = d_fit_out;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  (void)cudaGetLastError();
+  k_fit_noalloc_header<<<1, 32, 0, st>>>((uint32_t)n_merged);   // what must start at zero, and the count the kernel reads
+  const int l = (flags & TPC_DETERMINISTIC) ? tpc_det::run_fit3(B, &ctx->hconst, M, T, (uint32_t)n_merged, st, ctx->n_sm)
+                                            : tpc_fast::run_fit3(B, &ctx->hconst, M, T, (uint32_t)n_merged, st, ctx->n_sm);
+  if (l < 0 || cudaPeekAtLastError() != cudaSuccess) return set_cuda_err(ctx, cudaGetLastError(), "kernel launch (fit, no allocation)");
+  return TPC_OK;
+}
+
 // ---------------------------------------------------------------- Phase-II rebuild (R11)
 namespace {
 size_t carve_rebuild(uint64_t n_steps, uint64_t n_merged, uint64_t n_clusters, char* base, TpcRebuildBuffers* R) {
@@ -1085,6 +1196,7 @@ const char* tpc_strerror(int err) {
     case TPC_E_OVERFLOW: return "device capacity exceeded (bins, seeds or tracks); results invalid";
     case TPC_E_CUDA: return "CUDA runtime error";
     case TPC_E_STATE: return "call order violated";
+    case TPC_E_LIMIT: return "size beyond the fixed maximum of the no-allocation entry point";
     default: return "unknown error";
   }
 }
