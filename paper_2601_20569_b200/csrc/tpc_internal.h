@@ -66,7 +66,9 @@ struct TpcRowStat {
 #define TPC_RS_THREADS 1024
 #define TPC_RS_SMEM_BYTES (224 * 1024)   // dynamic shared memory per CTA
 #ifndef TPC_RS_BATCH
-#define TPC_RS_BATCH 4                   // records requested together per thread
+#ifndef TPC_RS_BATCH
+#define TPC_RS_BATCH 4                   // records requested together per thread (C4: 3.08 ms; 6: 3.16, 8: 3.12)
+#endif
 #endif
 
 // Seeds are handed to the follower / selector ordered by (sector, z-slab, row): tracklets that
