@@ -105,7 +105,12 @@ typedef struct tpc_params {
   uint32_t shared_fixed_cap;     /* 0: shared clusters by the running fraction counted from the outermost
                                     row (Phase I); 1: fixed cap shared_permille*nHits/1000
                                     per segment (the rule before Phase I; A/B variant)             */
-  uint32_t reserved[2];
+  uint32_t max_ids;              /* capacity of the tracks' cluster lists; 0 = default n/(1 - shared_permille/1000) + 64,
+                                    the exact bound of the running-fraction rule.  With shared_fixed_cap = 1 a
+                                    cluster may be shared by every clone of its track (the cap counts per
+                                    tracklet), so no bound follows from n: TPC_E_OVERFLOW then asks for a
+                                    larger value here (the oracle's count, or a few times n)            */
+  uint32_t reserved;
 } tpc_params;
 
 /* ------------------------------------------------------------------ output */

@@ -59,7 +59,7 @@ class Params(C.Structure):
                 ("shared_permille", C.c_int32), ("max_gap_select", C.c_int32), ("min_hits_track", C.c_int32),
                 ("grid_dy", C.c_float), ("grid_dz", C.c_float),
                 ("max_bins", C.c_uint64), ("max_seeds", C.c_uint32), ("shared_fixed_cap", C.c_uint32),
-                ("reserved", C.c_uint32 * 2)]
+                ("max_ids", C.c_uint32), ("reserved", C.c_uint32)]
 
 
 class TrackView(C.Structure):

@@ -120,7 +120,7 @@ Capacities capacities(const tpc_ctx* c, uint64_t n) {
   uint64_t seeds = P.max_seeds ? P.max_seeds : n / 12 + 4096;
   seeds = align_up(seeds, 64);
   k.max_seeds = (uint32_t)seeds;
-  const uint64_t ids = n * 1000 / (1000 - (uint64_t)P.shared_permille) + 64;
+  const uint64_t ids = P.max_ids ? (uint64_t)P.max_ids : n * 1000 / (1000 - (uint64_t)P.shared_permille) + 64;
   k.max_ids = (uint32_t)(ids > 0xFFFFFFF0ull ? 0xFFFFFFF0ull : ids);
   k.max_tracks = (uint32_t)(k.max_ids / (uint32_t)(P.min_hits_track > 0 ? P.min_hits_track : 1) + 1);
   const uint64_t b1 = (n + 1023) / 1024 + 2, b2 = 2 * ((seeds + 255) / 256 + 2);
@@ -202,6 +202,7 @@ void tpc_default_params(tpc_params* p) {
   p->shared_permille = 100; p->max_gap_select = 4; p->min_hits_track = 20;
   p->grid_dy = 2.0f; p->grid_dz = 2.0f;
   p->max_bins = 0; p->max_seeds = 0;
+  p->max_ids = 0; p->reserved = 0;
 }
 
 int tpc_geom_init(const tpc_geom_desc* geom, const tpc_params* params, tpc_ctx** out) {

@@ -29,7 +29,7 @@ def B():
 
 
 def params_pair(B, **kw):
-    okw = {k: v for k, v in kw.items() if k not in ("max_bins", "max_seeds")}   # capacities: library only
+    okw = {k: v for k, v in kw.items() if k not in ("max_bins", "max_seeds", "max_ids")}   # capacities: library only
     return B.tpc_default_params(**kw), oracle.default_params(**okw)
 
 
@@ -889,7 +889,7 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0 < ro.sum() < 0.02 * len(ro)
 
 
-def rebuild_det_parity(B, cl, pkw, tracking=None):
+def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False):
     """Phase-II rebuild, deterministic mode, against oracle.rebuild: per path step the three candidates
     (ids and chi2 bits), the attached cluster after the second ambiguity solving, the shared and used
     marks, per track the final fit -- all bit-exact.  Returns both sides for further checks."""
@@ -911,6 +911,9 @@ def rebuild_det_parity(B, cl, pkw, tracking=None):
     m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
     q = rebuild.rebuild(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids, params=op)
     nm = len(m.merged)
+    if allow_empty and nm == 0:
+        assert len(g["merged"]) == 0 and len(r["fit"]) == 0
+        return None
     assert len(g["merged"]) == nm > 0 and len(r["fit"]) == nm
     def order_of(tr, merged):
         h = merged["head"].astype(np.int64)
@@ -1115,6 +1118,64 @@ def test_merged_track_legs_edge_cases_and_call_order(B):
         assert B.tpc_rebuild_prepare(trk.ctx, st)[0] == B.TPC_E_STATE
     finally:
         trk.close()
+
+
+def random_case(it):
+    """Frame and tracker parameters drawn from a seeded generator: workload kind, multiplicity, noise, hit
+    efficiency, smearing, loopers, drift window; bin sizes, cuts, gap and length limits, selector variant;
+    30 % of the frames with their records shuffled (the generic grid path)."""
+    rng = np.random.default_rng(1000 + it)
+    kind = str(rng.choice(["C2", "C3", "C4", "C5", "C1"]))
+    ov = dict(seed=int(rng.integers(1, 1 << 30)), noise_frac=float(rng.uniform(0, 0.4)), p_hit=float(rng.uniform(0.6, 1.0)),
+              smear_y=float(rng.uniform(0.05, 0.2)), smear_z=float(rng.uniform(0.05, 0.2)), looper_frac=float(rng.uniform(0, 0.1)))
+    if kind in ("C2", "C3", "C4"):
+        ov["n_events"] = int(rng.integers(1, 5))
+        ov["tracks_per_event"] = int(rng.integers(20, 1500))
+        if kind != "C2":
+            ov["t_window_us"] = float(rng.uniform(10, 300))
+    elif kind == "C5":
+        ov["tracks_per_event"] = int(rng.integers(200, 6000))
+    else:
+        ov["tracks_per_event"] = int(rng.integers(1, 400))
+        ov["single_sector"] = int(rng.integers(0, 36))
+    cl, _, _ = dg.generate(dg.preset(kind, **ov))
+    pkw = dict(grid_dy=float(rng.uniform(1.5, 5)), grid_dz=float(rng.uniform(1.5, 8)), err_y=float(rng.uniform(0.08, 0.2)),
+               err_z=float(rng.uniform(0.08, 0.2)), nf_max_d2=float(rng.uniform(0.3, 2.0)), seed_min_len=int(rng.integers(3, 7)),
+               road_nsigma=float(rng.uniform(2.5, 5)), chi2_max_hit=float(rng.uniform(6, 20)), max_gap_follow=int(rng.integers(2, 7)),
+               min_hits_tracklet=int(rng.integers(6, 16)), sel_chi2_weight=float(rng.uniform(0, 4)),
+               shared_permille=int(rng.integers(0, 300)), max_gap_select=int(rng.integers(2, 7)),
+               min_hits_track=int(rng.integers(10, 30)), shared_fixed_cap=int(rng.integers(0, 2)), max_bins=400_000_000)
+    if rng.random() < 0.3:
+        cl = cl[rng.permutation(len(cl))]
+    return kind, cl, pkw
+
+
+@pytest.mark.parametrize("block", [0, 1, 2, 3])
+def test_det_parity_randomised_frames_and_parameters(B, block):
+    """A seeded sweep off the beaten track of the five configs: 10 random frames x random parameters per
+    block, each through the whole chain in deterministic mode -- grid, links, tracklets, tracks, then
+    merging and the Phase-II rebuild -- bit-exact against the oracle.  With the fixed-cap selector
+    variant the default capacity of the cluster lists does not hold (a cluster is shared by every clone
+    of its track): the library must say TPC_E_OVERFLOW, and pass with max_ids raised."""
+    n_overflow = 0
+    for it in range(10 * block, 10 * block + 10):
+        kind, cl, pkw = random_case(it)
+        if pkw["shared_fixed_cap"]:
+            trk = B.SectorTracker(params=B.tpc_default_params(**pkw))
+            try:
+                trk.track(trk.upload(cl), flags=1)
+                rc, v = trk.counts(check=False)
+            finally:
+                trk.close()
+            assert rc in (B.TPC_OK, B.TPC_E_OVERFLOW)
+            if rc == B.TPC_E_OVERFLOW:
+                assert v.n_tracks == 0 and v.n_cluster_ids == 0      # (never a truncated result)
+                n_overflow += 1
+            pkw["max_ids"] = 40 * len(cl) + 64
+        assert_det_parity(B, cl, **pkw)
+        rebuild_det_parity(B, cl, pkw, allow_empty=True)
+    if True:
+        print("randomised block", block, "overflow reports", n_overflow)
 
 
 def rebuilt_lists(step_ofs, attached, used, fit_flags):
