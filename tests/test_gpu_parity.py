@@ -1178,6 +1178,45 @@ def test_det_parity_randomised_frames_and_parameters(B, block):
         print("randomised block", block, "overflow reports", n_overflow)
 
 
+def test_fast_mode_randomised_statistics(B):
+    """The fast build against the oracle over the first 100 random cases (random_case), aggregated: where the
+    follower's decisions coincide the parameters agree to 1e-3 (budget 5e-4 of the tracklets, each within
+    half its own sigma), no accept / reject decision differs, every oracle tracklet has its partner; track
+    lists differ in < 1e-3 of the tracks with the default (running-fraction) sharing rule.  The fixed-cap
+    variant keeps a capped remainder of every losing clone as a track of its own, and which of two clones
+    with the same hits loses is decided by weights that differ in the last bits: its list differences are
+    reported and bounded at 3 %."""
+    tot = dict(n_paired=0, n_oracle=0, n_both_accepted=0, n_identical_hits=0, n_param_bad=0, n_accept_diff=0)
+    split = {0: [0, 0, 0], 1: [0, 0, 0]}
+    worst = 0.0
+    for it in range(100):
+        kind, cl, pkw = random_case(it)
+        if pkw["shared_fixed_cap"]:
+            pkw["max_ids"] = 40 * len(cl) + 64
+        gp, op = params_pair(B, **pkw)
+        tracks, ids, shared, view, gi = run_gpu(B, cl, gp, FAST)
+        o = oracle.run(cl, params=op, n_threads=NT, want=("seeds", "tracklets", "tracks"))
+        assert view.n_seeds == o.n_seeds
+        if o.n_seeds == 0:
+            continue
+        tl, identical = parity.compare_tracklets_fast(gi, o)
+        st = parity.compare_tracks_fast(tracks, ids, shared, o, identical_tracklets=identical)
+        for k in tot:
+            tot[k] += int(tl[k])
+        worst = max(worst, float(tl["max_err_in_sigma"]))
+        v = split[int(pkw["shared_fixed_cap"])]
+        v[0] += int(st["n_paired"]); v[1] += int(st["n_list_diff"]); v[2] += int(st["n_param_bad"])
+        assert st["n_paired"] >= 0.99 * st["n_oracle"] - 2, (it, st)
+    report("random_100_cases", {**tot, "max_err_in_sigma": worst, "tracks_running_rule": split[0][0],
+                                "list_diff_running_rule": split[0][1], "tracks_fixed_cap": split[1][0],
+                                "list_diff_fixed_cap": split[1][1], "track_param_bad": split[0][2] + split[1][2]})
+    assert tot["n_paired"] == tot["n_oracle"] > 500_000 and tot["n_accept_diff"] == 0
+    assert tot["n_identical_hits"] >= 0.999 * tot["n_both_accepted"]
+    assert tot["n_param_bad"] <= 5e-4 * tot["n_identical_hits"] and worst <= 0.5
+    assert split[0][1] <= 1e-3 * split[0][0] and split[1][1] <= 0.03 * split[1][0]
+    assert split[0][2] + split[1][2] <= 5e-4 * (split[0][0] + split[1][0])
+
+
 def rebuilt_lists(step_ofs, attached, used, fit_flags):
     """Cluster lists of the rebuilt tracks (used clusters of the tracks whose fit succeeded)."""
     ofs = np.asarray(step_ofs, dtype=np.int64)
