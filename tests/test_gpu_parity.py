@@ -889,7 +889,7 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0 < ro.sum() < 0.02 * len(ro)
 
 
-def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False):
+def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False, two_iterations=False):
     """Phase-II rebuild, deterministic mode, against oracle.rebuild: per path step the three candidates
     (ids and chi2 bits), the attached cluster after the second ambiguity solving, the shared and used
     marks, per track the final fit -- all bit-exact.  Returns both sides for further checks."""
@@ -897,7 +897,9 @@ def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False):
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
     try:
-        if tracking is None:
+        if two_iterations:
+            trk.track_two_iterations(trk.upload(cl), flags=1)
+        elif tracking is None:
             trk.track(trk.upload(cl), flags=1)
         else:
             tracking(trk, gp)          # (leaves the frame's sector tracks in trk by other means)
@@ -907,7 +909,11 @@ def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False):
         r = trk.rebuild()
     finally:
         trk.close()
-    o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
+    if two_iterations:
+        from oracle import second_iteration as si
+        o = si.run_two_iterations(cl, params=op, n_threads=NT)
+    else:
+        o = oracle.run(cl, params=op, n_threads=NT, want=("tracks",))
     m = merging.merge(cl, o.tracks, o.cluster_ids, o.cluster_shared, params=op)
     q = rebuild.rebuild(cl, o.tracks, m.fit, m.merged, m.seg_index, m.cluster_ids, params=op)
     nm = len(m.merged)
@@ -917,7 +923,7 @@ def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False):
     assert len(g["merged"]) == nm > 0 and len(r["fit"]) == nm
     def order_of(tr, merged):
         h = merged["head"].astype(np.int64)
-        return np.lexsort((tr["segment"][h], tr["seed_id"][h], tr["sector"][h]))
+        return np.lexsort((tr["segment"][h], tr["seed_id"][h], tr["sector"][h], (tr["flags"][h].astype(np.int64) >> 1) & 1))
     og, oo = order_of(tracks, g["merged"]), order_of(o.tracks, m.merged)
     gofs, oofs = r["step_ofs"].astype(np.int64), q.step_ofs.astype(np.int64)
     glen, olen = np.diff(gofs)[og], np.diff(oofs)[oo]
@@ -957,6 +963,22 @@ def test_det_parity_phase2_rebuild(B, name):
     att = q.attached[so]
     print(f"rebuild {name}: merged {nm} steps {len(so)} attached {(att >= 0).sum()} shared {int(q.shared.sum())} "
           f"used {int(q.used.sum())} failed {int((~ok).sum())}")
+
+
+@pytest.mark.parametrize("name", ["C5_dense", "C2_reduced"])
+def test_det_parity_phase2_rebuild_after_two_iterations(B, name):
+    """The legs compose with the second seeding iteration (8(f) rows 1, 2, 4): tracks of both iterations,
+    merged, then rebuilt -- the rebuild queries the grid of the FIRST iteration's workspace (the whole
+    frame) with the ids of the combined result; bit-exact against the oracle's chain."""
+    if name == "C5_dense":
+        cl, _, _ = dg.generate(dg.preset("C5", tracks_per_event=8000))
+        pkw = dict(err_y=0.15, err_z=0.15, nf_max_d2=1.6)
+    else:
+        cl, _, _ = dg.generate(dg.preset("C2", tracks_per_event=3000, seed=41))
+        pkw = {}
+    x = rebuild_det_parity(B, cl, pkw, two_iterations=True)
+    it2 = ((x["tracks"]["flags"].astype(np.int64) >> 1) & 1).sum()
+    assert it2 > (20 if name == "C5_dense" else 0) and x["ok"].sum() > 0.8 * len(x["m"].merged)
 
 
 def test_det_parity_phase2_rebuild_equal_weights(B):
