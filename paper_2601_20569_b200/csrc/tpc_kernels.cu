@@ -2198,6 +2198,21 @@ __global__ void k_init(TpcBuffers B) {
 // through the track's own cluster list (outward pass, turn, inward pass; no search, no chi2
 // cut) with the propagation / update statements of the follower.  The clusters are read from
 // the input frame through their original indices.
+// A cluster record gathered by original index is used once: the load bypasses L1 allocation
+// (TPC_GATHER_NA = 1) so that the lines of the per-thread streams (id lists, stored predictions) survive there.
+#ifndef TPC_GATHER_NA
+#define TPC_GATHER_NA 1
+#endif
+__device__ __forceinline__ uint4 ld_cluster_once(const tpc_cluster* p) {
+#if TPC_GATHER_NA
+  uint4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+#else
+  return *reinterpret_cast<const uint4*>(p);
+#endif
+}
+
 // ---- work distribution of the per-track kernels (fit, rebuild).  Tracks next to each other in merge order start in the
 // same region of the chamber (their grid lines and pages are shared: a global sort by length was
 // measured 35 % slower), but their path lengths differ by up to 10x, and a warp runs as long as its
@@ -2266,7 +2281,7 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
     for (int i = 0; i < 15; ++i) { out.c[i] = 0.f; out.c_out[i] = 0.f; }
     int r_last = 0;
     auto rec = [&](int i, float& y, float& z, int& row) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + (ids[i] - B.id_base));
+      const uint4 raw = ld_cluster_once(B.clusters + (ids[i] - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); row = (int)((raw.w >> 8) & 0xFF);
     };
     bool ok = n >= 2;
@@ -2695,7 +2710,7 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
     uint4* __restrict__ store = T.stored + m.cluster_ofs;
     for (int i = 0; i < n; ++i) { chi_c[i] = 0.f; rej[i] = 0; }
     auto rec = [&](int i, float& y, float& z, int& sec, int& row) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + (ids[i] - B.id_base));
+      const uint4 raw = ld_cluster_once(B.clusters + (ids[i] - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); sec = (int)(raw.w & 0xFF); row = (int)((raw.w >> 8) & 0xFF);
     };
     const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
@@ -2831,7 +2846,7 @@ struct RbPath {
     c_ok = ci >= 0 && ci < n_ids;
     if (c_ok) {
       c_id = ids[ci];
-      const uint4 raw = *reinterpret_cast<const uint4*>(cl + (c_id - id_base));
+      const uint4 raw = ld_cluster_once(cl + (c_id - id_base));
       c_y = __uint_as_float(raw.x); c_z = __uint_as_float(raw.y); c_sec = (int)(raw.w & 0xFF); c_row = (int)((raw.w >> 8) & 0xFF);
     }
   }
@@ -3195,7 +3210,7 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
     const uint32_t s0 = Rb.step_ofs[mi];
     const int n = (int)(Rb.step_ofs[mi + 1] - s0);
     auto cluster_yz = [&](int32_t id, float& y, float& z) {
-      const uint4 raw = *reinterpret_cast<const uint4*>(B.clusters + ((uint32_t)id - B.id_base));
+      const uint4 raw = ld_cluster_once(B.clusters + ((uint32_t)id - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y);
     };
     // One walk from the outermost step inward does both: the shared attachment (the rule of R6.3: its
