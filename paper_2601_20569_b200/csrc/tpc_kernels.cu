@@ -3048,23 +3048,35 @@ __global__ void __launch_bounds__(128, TPC_RB_MINB) k_rb_pass12(TpcBuffers B, Tp
         for (int bz = w.bz0; bz <= w.bz1; ++bz) {
           uint32_t cn = 0u, cn1 = 0u;
           if (bz < w.bz1) { cn = B.bin_start[b + (uint32_t)w.ny]; cn1 = B.bin_start[b + (uint32_t)w.ny + w.by_span]; }   // next z-row: requested before this one is scanned
-          for (; c < c1; ++c) {
-            const float2 mm = B.yz[c];
-            if (!(fabsf(mm.x - py) <= ry && fabsf(mm.y - pz) <= rz)) continue;
+          // (four clusters of the range requested together: one memory round trip per batch, not per cluster)
+          auto consider = [&](uint32_t cc, const float2 mm) {
+            if (!(fabsf(mm.x - py) <= ry && fabsf(mm.y - pz) <= rz)) return;
             const float c2 = fit_chi2_2x2(mm.x - py, mm.y - pz, wa, wb, wd, F.vy, F.vz);
-            if (!(c2 <= Rb.P.cand_chi2_max)) continue;
-            auto before = [&](int j) { return c2 < bchi[j] || (c2 == bchi[j] && B.orig_id[c] < B.orig_id[bpos[j]]); };
+            if (!(c2 <= Rb.P.cand_chi2_max)) return;
+            auto before = [&](int j) { return c2 < bchi[j] || (c2 == bchi[j] && B.orig_id[cc] < B.orig_id[bpos[j]]); };
             if (before(0)) {
-              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = bpos[0]; bchi[1] = bchi[0]; bpos[0] = c; bchi[0] = c2;
+              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = bpos[0]; bchi[1] = bchi[0]; bpos[0] = cc; bchi[0] = c2;
               by0 = mm.x; bz0 = mm.y;
             } else if (before(1)) {
-              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = c; bchi[1] = c2;
+              bpos[2] = bpos[1]; bchi[2] = bchi[1]; bpos[1] = cc; bchi[1] = c2;
             } else if (before(2)) {
-              bpos[2] = c; bchi[2] = c2;
+              bpos[2] = cc; bchi[2] = c2;
             } else {
-              continue;
+              return;
             }
             if (nb < TPC_RB_NCAND) ++nb;
+          };
+          for (; c < c1; c += 4) {
+            const bool h1 = c + 1 < c1, h2 = c + 2 < c1, h3 = c + 3 < c1;
+            const float2 m0 = B.yz[c];
+            float2 m1 = m0, m2 = m0, m3 = m0;
+            if (h1) m1 = B.yz[c + 1];
+            if (h2) m2 = B.yz[c + 2];
+            if (h3) m3 = B.yz[c + 3];
+            consider(c, m0);
+            if (h1) consider(c + 1, m1);
+            if (h2) consider(c + 2, m2);
+            if (h3) consider(c + 3, m3);
           }
           b += (uint32_t)w.ny; c = cn; c1 = cn1;
         }
