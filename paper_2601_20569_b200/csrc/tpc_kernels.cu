@@ -3221,8 +3221,16 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
     const tpc_merged_track m = M.merged[mi];
     const uint32_t s0 = Rb.step_ofs[mi];
     const int n = (int)(Rb.step_ofs[mi + 1] - s0);
+    // The record of the cluster a step owns is requested one step ahead (attached[] of the next step and its
+    // record travel while this step is computed); a cluster attached as shared during this walk is loaded
+    // on demand.
+    int32_t pre_id = n > 0 ? Rb.attached[s0 + (uint32_t)(n - 1)] : -1;
+    uint4 pre_raw = make_uint4(0u, 0u, 0u, 0u);
+    if (pre_id >= 0) pre_raw = ld_cluster_once(B.clusters + ((uint32_t)pre_id - B.id_base));
+    int32_t cur_id = -1;
+    uint4 cur_raw = pre_raw;
     auto cluster_yz = [&](int32_t id, float& y, float& z) {
-      const uint4 raw = ld_cluster_once(B.clusters + ((uint32_t)id - B.id_base));
+      const uint4 raw = id == cur_id ? cur_raw : ld_cluster_once(B.clusters + ((uint32_t)id - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y);
     };
     // One walk from the outermost step inward does both: the shared attachment (the rule of R6.3: its
@@ -3242,7 +3250,12 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
     for (int kk = n - 1; kk >= 0; --kk) {
       if (kk < n - 1) P.next_bwd();
       const uint32_t e = s0 + (uint32_t)kk;
-      int32_t ca = Rb.attached[e];
+      int32_t ca = pre_id;
+      cur_id = pre_id; cur_raw = pre_raw;
+      if (kk > 0) {
+        pre_id = Rb.attached[e - 1u];
+        if (pre_id >= 0) pre_raw = ld_cluster_once(B.clusters + ((uint32_t)pre_id - B.id_base));
+      }
       if (ca >= 0) {
         ++n_acc;
       } else {
