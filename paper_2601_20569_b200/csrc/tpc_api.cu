@@ -788,6 +788,17 @@ int tpc_refit_tracks(tpc_ctx* ctx, void* cuda_stream) {
   rc = device_status(ctx);
   if (rc == TPC_E_OVERFLOW) return rc;
   const uint32_t n_tracks = ctx->h_cnt->n_tracks;
+  // The compact copy of the tracks' clusters (tpc_internal.h) goes where the tracklets' row -> hit table
+  // was: dead after the selection, unless the caller asked to keep the intermediates.
+  ctx->buf.trk_yz = nullptr; ctx->buf.trk_sr = nullptr;
+  {
+    const size_t have = 4 * (size_t)ctx->geom.n_rows * ctx->buf.max_seeds;
+    const size_t yz_bytes = align_up(8 * (size_t)ctx->buf.max_ids, 256), sr_bytes = 2 * (size_t)ctx->buf.max_ids;
+    if (!(ctx->flags & TPC_KEEP_INTERMEDIATES) && ctx->buf.row_hit && yz_bytes + sr_bytes <= have) {
+      ctx->buf.trk_yz = reinterpret_cast<float2*>(ctx->buf.row_hit);
+      ctx->buf.trk_sr = reinterpret_cast<uint16_t*>(reinterpret_cast<char*>(ctx->buf.row_hit) + yz_bytes);
+    }
+  }
   (void)cudaGetLastError();
   const int l = (ctx->flags & TPC_DETERMINISTIC)
                     ? tpc_det::run_refit(ctx->buf, &ctx->hconst, n_tracks, (cudaStream_t)cuda_stream, ctx->n_sm)
@@ -837,6 +848,8 @@ size_t carve_merge(const tpc_ctx* c, uint64_t n_tracks, uint64_t n_ids, char* ba
   m.seg_index = (uint32_t*)take(4 * nt);
   m.ids = (uint32_t*)take(4 * ((size_t)n_ids + 1));
   m.shared = (uint8_t*)take((size_t)n_ids + 1);
+  m.yz = (float2*)take(8 * ((size_t)n_ids + 1));
+  m.sr = (uint16_t*)take(2 * ((size_t)n_ids + 1));
   m.counters = (uint32_t*)take(16);
   m.path_ofs = (uint32_t*)take(4 * (nt + 1));
   if (M) *M = m;
@@ -876,6 +889,7 @@ int tpc_merge_tracks(tpc_ctx* ctx, const tpc_merge_params* params, void* d_ws, s
   const size_t need = carve_merge(ctx, n_tracks, n_ids, (char*)d_ws, &M);
   if (ws_bytes < need) return TPC_E_WORKSPACE;
   M.P = P;
+  if (!ctx->buf.trk_yz) { M.yz = nullptr; M.sr = nullptr; }   // (no compact copy of the tracks' clusters: the fit gathers)
   M.inv_w = 1.0f / P.pre_dz;
   const double a = 2.0 * (double)ctx->geom.sector_half_angle_deg * (3.14159265358979323846 / 180.0);
   M.ca = (float)std::cos(a);

@@ -127,6 +127,10 @@ struct TpcBuffers {
   uint32_t* cluster_ids;  // [max_ids]
   uint8_t* cluster_shared;// [max_ids]
   tpc_track_fit* track_fit;// [max_tracks] sector-track refit (R8)
+  // compact copy of the tracks' clusters in the order of cluster_ids (written by the refit's outward pass;
+  // nullptr: the kernels gather the 16-byte records of the frame by original index instead)
+  float2* trk_yz;         // [max_ids] (y, z)
+  uint16_t* trk_sr;       // [max_ids] sector << 8 | row
 };
 
 // Buffers of the track merging (R9), pointers into the caller's merge workspace.
@@ -147,6 +151,7 @@ struct TpcMergeBuffers {
   tpc_merged_track* merged;  // [n_tracks]
   uint32_t* seg_index;       // [n_tracks]
   uint32_t* ids; uint8_t* shared;   // [n_ids]
+  float2* yz; uint16_t* sr;         // [n_ids] compact copy of the merged lists' clusters (nullptr: gather)
   uint32_t* counters;        // [4] n_merged, n_links, n_ids out, n_steps (R11 paths)
   uint32_t* path_ofs;        // [n_tracks+1] first path step of every merged track (R11), exclusive scan
 };

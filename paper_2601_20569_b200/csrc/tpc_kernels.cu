@@ -2261,6 +2261,7 @@ __device__ __forceinline__ bool rb_group_next(uint32_t n_items, RbChunkShared& S
   return true;
 }
 
+template <bool COMPACT>   // leave / use the compact copy of the tracks' clusters (B.trk_yz, B.trk_sr)
 __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_constant__ FollowConst F, uint32_t n_tracks) {
   __shared__ RbChunkShared S;
   uint32_t base, ti;
@@ -2280,9 +2281,24 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
 #pragma unroll
     for (int i = 0; i < 15; ++i) { out.c[i] = 0.f; out.c_out[i] = 0.f; }
     int r_last = 0;
-    auto rec = [&](int i, float& y, float& z, int& row) {
+    // The outward pass gathers the 16-byte records of the frame by original index (a 64-byte DRAM access
+    // each) and leaves a compact copy in list order (10 bytes per cluster); the inward pass, the merging's
+    // copy, the fit and the rebuild read that instead of gathering again.
+    // (COMPACT is a template parameter on purpose: a run-time choice of the source inside these loaders made
+    // the compiler lose the lock-step of the lanes in the fit -- 4x the instructions at 5 lanes each)
+    float2* __restrict__ cyz = COMPACT ? B.trk_yz + t->cluster_ofs : nullptr;
+    uint16_t* __restrict__ csr = COMPACT ? B.trk_sr + t->cluster_ofs : nullptr;
+    int n_copied = 0;
+    auto rec = [&](int i, float& y, float& z, int& row) {          // gather (+ copy)
       const uint4 raw = ld_cluster_once(B.clusters + (ids[i] - B.id_base));
       y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); row = (int)((raw.w >> 8) & 0xFF);
+      if (COMPACT) {
+        if (i >= n_copied) { cyz[i] = make_float2(y, z); csr[i] = (uint16_t)(((raw.w & 0xFFu) << 8) | ((raw.w >> 8) & 0xFFu)); n_copied = i + 1; }
+      }
+    };
+    auto rec_back = [&](int i, float& y, float& z, int& row) {     // from the compact copy if there is one
+      if (COMPACT) { const float2 v = cyz[i]; y = v.x; z = v.y; row = (int)(csr[i] & 0xFFu); }
+      else rec(i, y, z, row);
     };
     bool ok = n >= 2;
     if (ok) {
@@ -2327,7 +2343,7 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
       float chi2 = 0.f;
       for (int i = n - 2; i >= 0 && ok; --i) {  // R8.4 inward
         int ri;
-        rec(i, ym, zm, ri);
+        rec_back(i, ym, zm, ri);
         for (; r > ri && ok; --r) ok = kf_propagate(k, -F.dx, F);
         if (!ok) break;
         const Gain g = kf_gain(k, F);
@@ -2346,6 +2362,8 @@ __global__ void __launch_bounds__(128) k_track_refit(TpcBuffers B, const __grid_
         out.flags = 0u;
       }
     }
+    if (COMPACT)   // (a pass that stopped early: the copy is completed all the same, other kernels rely on it)
+      for (int i = n_copied; i < n; ++i) { float y, z; int row; rec(i, y, z, row); }
     B.track_fit[ti] = out;
   }
 }
@@ -2635,6 +2653,7 @@ __global__ void __launch_bounds__(256) k_merge_copy_ids(TpcBuffers B, TpcMergeBu
     for (uint32_t i = lane; i < n; i += 32) {
       M.ids[dst + i] = B.cluster_ids[src + i];
       M.shared[dst + i] = B.cluster_shared[src + i];
+      if (M.yz) { M.yz[dst + i] = B.trk_yz[src + i]; M.sr[dst + i] = B.trk_sr[src + i]; }
     }
   }
 }
@@ -2685,6 +2704,7 @@ __device__ __forceinline__ float fit_chi2_2x2(float r0, float r1, float a, float
   return ((r0 * r0) * i00 + (2.f * (r0 * r1)) * i01) + (r1 * r1) * i11;
 }
 
+template <bool COMPACT>   // clusters from the compact copy of the merged lists (M.yz, M.sr) / gathered from the frame
 __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffers M, TpcFitBuffers T,
                                                     const __grid_constant__ FollowConst F) {
   const TpcConst* __restrict__ K = B.K;
@@ -2709,9 +2729,16 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
     uint8_t* __restrict__ rej = T.rejected + m.cluster_ofs;
     uint4* __restrict__ store = T.stored + m.cluster_ofs;
     for (int i = 0; i < n; ++i) { chi_c[i] = 0.f; rej[i] = 0; }
+    const float2* __restrict__ cyz = M.yz + m.cluster_ofs;
+    const uint16_t* __restrict__ csr = M.sr + m.cluster_ofs;
     auto rec = [&](int i, float& y, float& z, int& sec, int& row) {
-      const uint4 raw = ld_cluster_once(B.clusters + (ids[i] - B.id_base));
-      y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); sec = (int)(raw.w & 0xFF); row = (int)((raw.w >> 8) & 0xFF);
+      if (COMPACT) {
+        const float2 v = cyz[i]; const uint32_t w = csr[i];
+        y = v.x; z = v.y; sec = (int)(w >> 8); row = (int)(w & 0xFFu);
+      } else {
+        const uint4 raw = ld_cluster_once(B.clusters + (ids[i] - B.id_base));
+        y = __uint_as_float(raw.x); z = __uint_as_float(raw.y); sec = (int)(raw.w & 0xFF); row = (int)((raw.w >> 8) & 0xFF);
+      }
     };
     const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
     const tpc_track_fit* ft = B.track_fit + tail;
@@ -2833,8 +2860,10 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
 //                   plain chi2 cut
 // Iterator over the steps of a merged track, forward (outward) or backward; it also tells which
 // original cluster of the merged list, if any, sits on the step.
+template <bool COMPACT>   // original clusters from the compact copy of the merged lists / gathered from the frame
 struct RbPath {
   const uint32_t* segs; const tpc_track* tracks; const uint32_t* ids; const tpc_cluster* cl;
+  const float2* cyz; const uint16_t* csr;
   int n_seg, n_ids;
   uint32_t id_base;
   int g, row, ci, hole_end;
@@ -2846,8 +2875,13 @@ struct RbPath {
     c_ok = ci >= 0 && ci < n_ids;
     if (c_ok) {
       c_id = ids[ci];
-      const uint4 raw = ld_cluster_once(cl + (c_id - id_base));
-      c_y = __uint_as_float(raw.x); c_z = __uint_as_float(raw.y); c_sec = (int)(raw.w & 0xFF); c_row = (int)((raw.w >> 8) & 0xFF);
+      if (COMPACT) {
+        const float2 v = cyz[ci]; const uint32_t w = csr[ci];
+        c_y = v.x; c_z = v.y; c_sec = (int)(w >> 8); c_row = (int)(w & 0xFFu);
+      } else {
+        const uint4 raw = ld_cluster_once(cl + (c_id - id_base));
+        c_y = __uint_as_float(raw.x); c_z = __uint_as_float(raw.y); c_sec = (int)(raw.w & 0xFF); c_row = (int)((raw.w >> 8) & 0xFF);
+      }
     }
   }
   __device__ __forceinline__ void begin_fwd() { g = 0; load_seg(); row = f; hole = false; ci = 0; load_cluster(); }
@@ -2888,8 +2922,10 @@ struct RbPath {
     return true;
   }
 };
-__device__ __forceinline__ RbPath rb_path(const TpcBuffers& B, const TpcMergeBuffers& M, const tpc_merged_track& m) {
-  RbPath P;
+template <bool COMPACT>
+__device__ __forceinline__ RbPath<COMPACT> rb_path(const TpcBuffers& B, const TpcMergeBuffers& M, const tpc_merged_track& m) {
+  RbPath<COMPACT> P;
+  P.cyz = COMPACT ? M.yz + m.cluster_ofs : nullptr; P.csr = COMPACT ? M.sr + m.cluster_ofs : nullptr;
   P.segs = M.seg_index + m.seg_ofs; P.tracks = B.tracks; P.ids = M.ids + m.cluster_ofs; P.cl = B.clusters;
   P.n_seg = (int)m.n_segments; P.n_ids = (int)m.n_clusters; P.id_base = B.id_base;
   P.hole = false; P.hole_end = 0; P.c_ok = false;
@@ -2932,6 +2968,7 @@ __device__ __forceinline__ float rb_unhalf(uint32_t w, int hi) {
   return __half2float(__ushort_as_half((unsigned short)(hi ? (w >> 16) : (w & 0xFFFFu))));
 }
 
+template <bool COMPACT>
 __global__ void __launch_bounds__(128, TPC_RB_MINB) k_rb_pass12(TpcBuffers B, TpcMergeBuffers M, TpcRebuildBuffers Rb,
                                                    const __grid_constant__ FollowConst F) {
   const TpcConst* __restrict__ K = B.K;
@@ -2957,7 +2994,7 @@ __global__ void __launch_bounds__(128, TPC_RB_MINB) k_rb_pass12(TpcBuffers B, Tp
     const uint32_t tail = M.seg_index[m.seg_ofs + m.n_segments - 1];
     const tpc_track_fit* ft = B.track_fit + tail;
     if (ft->flags != 0u || n < 2) { no_candidates(); continue; }
-    RbPath P = rb_path(B, M, m);
+    RbPath<COMPACT> P = rb_path<COMPACT>(B, M, m);
     KF k;
     k.y = k.z = 0.f;
     k.s = ft->p_out[2]; k.t = ft->p_out[3]; k.q = ft->p_out[4];
@@ -3005,7 +3042,7 @@ __global__ void __launch_bounds__(128, TPC_RB_MINB) k_rb_pass12(TpcBuffers B, Tp
         const bool has = (st.w >> 16) & 1u;
         float zc = 0.f;
         if (has) {
-          if (P.sec != ps) zc = B.clusters[P.ids[ci] - B.id_base].z;
+          if (P.sec != ps) zc = COMPACT ? P.cyz[ci].y : B.clusters[P.ids[ci] - B.id_base].z;
           ++ci;
         }
         if (!link_transport(k, ps, pr, P.sec, P.row, zc, K, F, Rb.ca, Rb.sa, Rb.P.ce_var)) { ok = false; break; }
@@ -3237,7 +3274,7 @@ __global__ void __launch_bounds__(128) k_rb_pass3(TpcBuffers B, TpcMergeBuffers 
     // decision at a step depends on the steps outside of it only) and, from the outermost attached step
     // on, pass 3 with the plain chi2 cut.  After a failed transport / update the walk goes on for the
     // attachment marks alone.
-    RbPath P = rb_path(B, M, m);
+    RbPath<false> P = rb_path<false>(B, M, m);
     P.begin_bwd_rows();
     KF k, kin;
     k.s = Rb.stq2[3 * (size_t)mi]; k.t = Rb.stq2[3 * (size_t)mi + 1]; k.q = Rb.stq2[3 * (size_t)mi + 2];
@@ -3346,7 +3383,8 @@ int run_refit(const TpcBuffers& B, const TpcConst* hK, uint32_t n_tracks, cudaSt
   if (n_tracks == 0) return 0;
   const FollowConst F = follow_const(hK);
   cudaMemsetAsync(&B.cnt->refit_next, 0, 4, st);
-  k_track_refit<<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit, 128)), 128, 0, st>>>(B, F, n_tracks);
+  if (B.trk_yz) k_track_refit<true><<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit<true>, 128)), 128, 0, st>>>(B, F, n_tracks);
+  else k_track_refit<false><<<grid_for(n_tracks, 128, n_sm, resident_ctas(k_track_refit<false>, 128)), 128, 0, st>>>(B, F, n_tracks);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -3397,7 +3435,8 @@ int run_fit3(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& M, 
   if (n_merged == 0) return 0;
   const FollowConst F = follow_const(hK);
   cudaMemsetAsync(T.work, 0, 16, st);
-  k_track_fit3<<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3, 128)), 128, 0, st>>>(B, M, T, F);
+  if (M.yz) k_track_fit3<true><<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3<true>, 128)), 128, 0, st>>>(B, M, T, F);
+  else k_track_fit3<false><<<grid_for(n_merged, 128, n_sm, resident_ctas(k_track_fit3<false>, 128)), 128, 0, st>>>(B, M, T, F);
   return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -3421,7 +3460,8 @@ int run_rebuild(const TpcBuffers& B, const TpcConst* hK, const TpcMergeBuffers& 
   cudaMemsetAsync(Rb.best, 0, 8 * nc, st);
   cudaMemsetAsync(Rb.bestId, 0xFF, 8 * nc, st);
   k_rb_step_track<<<gw, 256, 0, st>>>(Rb);
-  k_rb_pass12<<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass12, 128)), 128, 0, st>>>(B, M, Rb, F);
+  if (M.yz) k_rb_pass12<true><<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass12<true>, 128)), 128, 0, st>>>(B, M, Rb, F);
+  else k_rb_pass12<false><<<grid_for(Rb.n_merged, 128, n_sm, resident_ctas(k_rb_pass12<false>, 128)), 128, 0, st>>>(B, M, Rb, F);
   // the stored predictions are dead now: their region holds the loser lists (round 3's goes where round 2's was)
   uint2* list2 = reinterpret_cast<uint2*>(Rb.stored);
   uint2* list3 = list2 + ns;

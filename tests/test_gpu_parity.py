@@ -842,7 +842,7 @@ def test_det_parity_three_iteration_fit(B, name):
     gp, op = params_pair(B, **pkw)
     trk = B.SectorTracker(params=gp)
     try:
-        trk.track(trk.upload(cl), flags=1)
+        trk.track(trk.upload(cl), flags=DET if name == "C2_full" else 1)   # (DET keeps the intermediates: the legs gather)
         tracks, ids, shared, view = trk.tracks()
         trk.refit()
         g = trk.merge()
@@ -889,7 +889,7 @@ def test_det_parity_three_iteration_fit(B, name):
         assert 0 < ro.sum() < 0.02 * len(ro)
 
 
-def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False, two_iterations=False):
+def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False, two_iterations=False, track_flags=1):
     """Phase-II rebuild, deterministic mode, against oracle.rebuild: per path step the three candidates
     (ids and chi2 bits), the attached cluster after the second ambiguity solving, the shared and used
     marks, per track the final fit -- all bit-exact.  Returns both sides for further checks."""
@@ -900,7 +900,7 @@ def rebuild_det_parity(B, cl, pkw, tracking=None, allow_empty=False, two_iterati
         if two_iterations:
             trk.track_two_iterations(trk.upload(cl), flags=1)
         elif tracking is None:
-            trk.track(trk.upload(cl), flags=1)
+            trk.track(trk.upload(cl), flags=track_flags)
         else:
             tracking(trk, gp)          # (leaves the frame's sector tracks in trk by other means)
         tracks, ids, shared, view = trk.tracks()
@@ -955,7 +955,9 @@ def test_det_parity_phase2_rebuild(B, name):
     """SURVEY.md 8(f) row 4 (reading R11): the Phase-II rebuild of the merged tracks,
     deterministic mode, bit-exact against oracle.rebuild (see rebuild_det_parity)."""
     cl, pkw = merged_case_frame(name)
-    x = rebuild_det_parity(B, cl, pkw)
+    # (with the intermediates kept the refit leaves no compact copy of the clusters and every leg gathers
+    # them from the frame: the other instantiation of the per-track kernels)
+    x = rebuild_det_parity(B, cl, pkw, track_flags=DET if name == "C5_dense" else 1)
     q, ok, so, nm = x["q"], x["ok"], x["so"], len(x["m"].merged)
     assert ok.sum() >= 0.8 * nm
     if name == "ce_crossing":

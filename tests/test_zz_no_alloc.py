@@ -1,9 +1,10 @@
 """tpc_fit_tracks_noalloc: the three-iteration fit with its scratch in a static array inside the library
 (include/tpc_track.h).  Collected last on purpose (the file name): the suite runs with pytest -x.
 
-The new entry point runs the same kernel as tpc_fit_tracks on the same inputs, so its output must equal the
-existing path's bit for bit (both builds); checked on calls in a row on frames of different sizes, which
-share the one array (what a call leaves behind must not reach the next one).
+The new entry point runs the same fit as tpc_fit_tracks on the same inputs: its output must equal the existing
+path's bit for bit in the deterministic build and within the fast-mode tolerance in the fast build; checked on
+calls in a row on frames of different sizes, which share the one array (what a call leaves behind must not
+reach the next one).
 """
 import numpy as np
 import pytest
@@ -56,12 +57,29 @@ class Case:
             self.flags & B.TPC_DETERMINISTIC, st)
 
     def check(self):
+        """Deterministic build: bit for bit.  Fast build: the workspace path reads a compact copy of the clusters
+        and is another instantiation of the kernel than the one this entry point runs (it gathers from the
+        frame), so the two may differ in the last bits: the fast-mode tolerance of the other tests (1e-3
+        relative on parameters and chi2, decisions at a cut may flip for a handful of clusters)."""
         B = self.B
         self.torch.cuda.synchronize()
         fit = self.o_fit.cpu().numpy().view(B.TRACK_FIT3_DTYPE)
-        assert fit.tobytes() == self.fit.tobytes()
-        assert self.o_chi2.cpu().numpy().tobytes() == self.chi2.tobytes()
-        assert (self.o_rej.cpu().numpy() == self.rejected).all()
+        chi2, rej = self.o_chi2.cpu().numpy(), self.o_rej.cpu().numpy()
+        if self.flags & B.TPC_DETERMINISTIC:
+            assert fit.tobytes() == self.fit.tobytes()
+            assert chi2.tobytes() == self.chi2.tobytes()
+            assert (rej == self.rejected).all()
+            return
+        assert (rej != self.rejected).sum() <= 1e-4 * len(rej) + 2
+        assert np.allclose(chi2, self.chi2, rtol=1e-3, atol=1e-3)
+        same = (fit["flags"] == self.fit["flags"]) & (fit["n_used"] == self.fit["n_used"])
+        assert (~same).sum() <= 1e-3 * len(fit) + 2
+        ok = same & (fit["flags"] == 0)
+        scale = np.array([0.1, 0.1, 0.01, 0.01, 0.1], dtype=np.float64)
+        a, b = fit["p"][ok].astype(np.float64), self.fit["p"][ok].astype(np.float64)
+        bad = (np.abs(a - b) > 1e-3 * np.maximum(np.abs(b), scale)).any(axis=1)
+        assert bad.sum() <= 5e-4 * ok.sum() + 2, int(bad.sum())
+        assert np.allclose(fit["chi2"][ok], self.fit["chi2"][ok], rtol=2e-3, atol=1e-2)
 
     def scribble(self):
         self.o_fit.fill_(0x5A); self.o_chi2.fill_(-3.0); self.o_rej.fill_(0x5A)
