@@ -2715,6 +2715,7 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
   auto len_of = [&](uint32_t i) { return M.merged[i].n_clusters; };
   while (rb_chunk_begin(n_merged, len_of, T.work, S, base))
   while (rb_group_next(n_merged, S, base, mi, valid)) {
+    const unsigned vm = __ballot_sync(0xffffffffu, valid);   // the lanes of this group: their loops below run in lock-step
     if (!valid) continue;
     const tpc_merged_track m = M.merged[mi];
     const uint32_t* __restrict__ ids = M.ids + m.cluster_ofs;
@@ -2749,25 +2750,69 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
     kf_init_cov(k, F);
     float yc, zc, yp, zp;
     int sc, rc, sp, rp;
+    // Transport between consecutive clusters, ONE ROW STEP PER LOOP ITERATION (as the follower): the plan for
+    // the next cluster gives the number of row steps; an iteration propagates one step and, when none is left,
+    // processes the cluster.  A lane crossing a hole of three rows then costs its warp three cheap
+    // iterations, not three propagations inside every other lane's cluster step.  Arithmetic and its order
+    // per track are those of link_transport: the row steps, then (electrode) the z re-base; (adjacent sector)
+    // rotation and one step over the x distance, done when the plan is made.
+    int steps = 0;
+    float dxs = 0.f;
+    bool ce = false;
+    auto plan = [&](int s0, int r0, int s1, int r1) -> bool {
+      if (s0 == s1 || s0 - s1 == 18 || s1 - s0 == 18) {
+        steps = r1 > r0 ? r1 - r0 : r0 - r1;
+        dxs = r1 > r0 ? F.dx : -F.dx;
+        ce = s0 != s1;
+        return true;
+      }
+      steps = 0; ce = false;
+      const float sgn = (s1 % 18 == (s0 % 18 + 1) % 18) ? 1.f : -1.f;
+      float x = K->x[r0];
+      if (!merge_rotate(k, x, T.ca, sgn * T.sa, F.max_sinphi)) return false;
+      return kf_propagate(k, K->x[r1] - x, F);
+    };
+    auto arrive = [&](float z_cluster) {     // after the last row step: the electrode re-base
+      if (ce) {
+        k.z = z_cluster;
+        k.c10 = 0.f; k.c21 = 0.f; k.c31 = 0.f; k.c41 = 0.f;
+        k.c11 = T.P.ce_var;
+      }
+    };
     // ---- iteration 1: inward from c_{n-1}; predictions stored in half precision
-    if (ok) {
-      rec(n - 1, yp, zp, sp, rp);
-      fit_turn(k, yp, zp, F);
-      for (int i = n - 2; i >= 0 && ok; --i) {
-        rec(i, yc, zc, sc, rc);
-        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
-        const uint32_t h0 = (uint32_t)__half_as_ushort(__float2half_rn(k.y - yc)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.z - zc)) << 16);
-        const uint32_t h1 = (uint32_t)__half_as_ushort(__float2half_rn(k.c00)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.c10)) << 16);
-        const uint32_t h2 = (uint32_t)__half_as_ushort(__float2half_rn(k.c11));
-        store[i] = make_uint4(h0, h1, h2, 0u);
-        const Gain g = kf_gain(k, F);
-        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
-        sp = sc; rp = rc;
+    {
+      int i = -1;
+      if (ok) {
+        rec(n - 1, yp, zp, sp, rp);
+        fit_turn(k, yp, zp, F);
+        i = n - 2;
+        if (i >= 0) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+      }
+      // (the loop condition is a vote of the group's lanes: they meet at the top of every iteration)
+      for (bool act = ok && i >= 0; __any_sync(vm, act); act = ok && i >= 0) {
+        if (!act) continue;
+        if (steps > 0) { if (!kf_propagate(k, dxs, F)) ok = false; else --steps; }
+        if (ok && steps == 0) {
+          arrive(zc);
+          const uint32_t h0 = (uint32_t)__half_as_ushort(__float2half_rn(k.y - yc)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.z - zc)) << 16);
+          const uint32_t h1 = (uint32_t)__half_as_ushort(__float2half_rn(k.c00)) | ((uint32_t)__half_as_ushort(__float2half_rn(k.c10)) << 16);
+          const uint32_t h2 = (uint32_t)__half_as_ushort(__float2half_rn(k.c11));
+          store[i] = make_uint4(h0, h1, h2, 0u);
+          const Gain g = kf_gain(k, F);
+          if (kf_update(k, g, yc, zc, F)) ok = false;
+          else {
+            sp = sc; rp = rc;
+            --i;
+            if (i >= 0) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+          }
+        }
       }
     }
     // ---- iteration 2: outward from c_0; interpolation, chi2 cut (marking only)
     int used = 0;
-    if (ok) {
+    {
+      int i = n;
+      if (ok) {
       rec(0, yp, zp, sp, rp);
       fit_turn(k, yp, zp, F);
       {
@@ -2779,37 +2824,47 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
         chi_c[0] = chi2;
         if (!(chi2 <= T.P.fit_chi2_max)) rej[0] = 1; else ++used;
       }
-      for (int i = 1; i < n && ok; ++i) {
-        rec(i, yc, zc, sc, rc);
-        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
-        const float r2y = k.y - yc, r2z = k.z - zc;
-        const float a2 = k.c00, b2 = k.c10, d2 = k.c11;
-        float chi2;
-        if (i == n - 1) {
-          chi2 = fit_chi2_2x2(r2y, r2z, a2, b2, d2, F.vy, F.vz);
-        } else {
-          const uint4 st = store[i];
-          const float s_ry = __half2float(__ushort_as_half((unsigned short)(st.x & 0xFFFFu))), s_rz = __half2float(__ushort_as_half((unsigned short)(st.x >> 16)));
-          const float a1 = __half2float(__ushort_as_half((unsigned short)(st.y & 0xFFFFu))), b1 = __half2float(__ushort_as_half((unsigned short)(st.y >> 16)));
-          const float d1 = __half2float(__ushort_as_half((unsigned short)(st.z & 0xFFFFu)));
-          const float det1 = a1 * d1 - b1 * b1, det2 = a2 * d2 - b2 * b2;
-          const float n1 = 1.f / det1, n2 = 1.f / det2;
-          const float i1a = d1 * n1, i1b = -(b1 * n1), i1d = a1 * n1;
-          const float i2a = d2 * n2, i2b = -(b2 * n2), i2d = a2 * n2;
-          const float ia = i1a + i2a, ib = i1b + i2b, id = i1d + i2d;
-          const float detw = ia * id - ib * ib;
-          const float nw = 1.f / detw;
-          const float wa = id * nw, wb = -(ib * nw), wd = ia * nw;
-          const float hy = (i1a * s_ry + i1b * s_rz) + (i2a * r2y + i2b * r2z);
-          const float hz = (i1b * s_ry + i1d * s_rz) + (i2b * r2y + i2d * r2z);
-          const float ry = wa * hy + wb * hz, rz = wb * hy + wd * hz;
-          chi2 = fit_chi2_2x2(ry, rz, wa, wb, wd, F.vy, F.vz);
+      i = 1;
+      if (i < n) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+      }
+      for (bool act = ok && i < n; __any_sync(vm, act); act = ok && i < n) {
+        if (!act) continue;
+        if (steps > 0) { if (!kf_propagate(k, dxs, F)) ok = false; else --steps; }
+        if (ok && steps == 0) {
+          arrive(zc);
+          const float r2y = k.y - yc, r2z = k.z - zc;
+          const float a2 = k.c00, b2 = k.c10, d2 = k.c11;
+          float chi2;
+          if (i == n - 1) {
+            chi2 = fit_chi2_2x2(r2y, r2z, a2, b2, d2, F.vy, F.vz);
+          } else {
+            const uint4 st = store[i];
+            const float s_ry = __half2float(__ushort_as_half((unsigned short)(st.x & 0xFFFFu))), s_rz = __half2float(__ushort_as_half((unsigned short)(st.x >> 16)));
+            const float a1 = __half2float(__ushort_as_half((unsigned short)(st.y & 0xFFFFu))), b1 = __half2float(__ushort_as_half((unsigned short)(st.y >> 16)));
+            const float d1 = __half2float(__ushort_as_half((unsigned short)(st.z & 0xFFFFu)));
+            const float det1 = a1 * d1 - b1 * b1, det2 = a2 * d2 - b2 * b2;
+            const float n1 = 1.f / det1, n2 = 1.f / det2;
+            const float i1a = d1 * n1, i1b = -(b1 * n1), i1d = a1 * n1;
+            const float i2a = d2 * n2, i2b = -(b2 * n2), i2d = a2 * n2;
+            const float ia = i1a + i2a, ib = i1b + i2b, id = i1d + i2d;
+            const float detw = ia * id - ib * ib;
+            const float nw = 1.f / detw;
+            const float wa = id * nw, wb = -(ib * nw), wd = ia * nw;
+            const float hy = (i1a * s_ry + i1b * s_rz) + (i2a * r2y + i2b * r2z);
+            const float hz = (i1b * s_ry + i1d * s_rz) + (i2b * r2y + i2d * r2z);
+            const float ry = wa * hy + wb * hz, rz = wb * hy + wd * hz;
+            chi2 = fit_chi2_2x2(ry, rz, wa, wb, wd, F.vy, F.vz);
+          }
+          chi_c[i] = chi2;
+          if (!(chi2 <= T.P.fit_chi2_max)) rej[i] = 1; else ++used;
+          const Gain g = kf_gain(k, F);
+          if (kf_update(k, g, yc, zc, F)) ok = false;
+          else {
+            sp = sc; rp = rc;
+            ++i;
+            if (i < n) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+          }
         }
-        chi_c[i] = chi2;
-        if (!(chi2 <= T.P.fit_chi2_max)) rej[i] = 1; else ++used;
-        const Gain g = kf_gain(k, F);
-        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
-        sp = sc; rp = rc;
       }
     }
     // ---- iteration 3: inward through the unmarked clusters
@@ -2817,21 +2872,34 @@ __global__ void __launch_bounds__(128) k_track_fit3(TpcBuffers B, TpcMergeBuffer
       out.n_used = (uint32_t)used;
       if (used < T.P.fit_min_clusters || used < 2) ok = false;
     }
-    if (ok) {
-      int last = n - 1;
-      while (rej[last]) --last;
-      rec(last, yp, zp, sp, rp);
-      fit_turn(k, yp, zp, F);
+    {
       float chi2 = 0.f;
-      for (int i = last - 1; i >= 0 && ok; --i) {
-        if (rej[i]) continue;
-        rec(i, yc, zc, sc, rc);
-        if (!fit_transport(k, sp, rp, sc, rc, zc, K, F, T)) { ok = false; break; }
-        const Gain g = kf_gain(k, F);
-        const float c2 = kf_chi2(k, g, yc, zc);
-        if (kf_update(k, g, yc, zc, F)) { ok = false; break; }
-        chi2 = chi2 + c2;
-        sp = sc; rp = rc;
+      int i = -1;
+      if (ok) {
+        int last = n - 1;
+        while (rej[last]) --last;
+        rec(last, yp, zp, sp, rp);
+        fit_turn(k, yp, zp, F);
+        i = last - 1;
+        while (i >= 0 && rej[i]) --i;
+        if (i >= 0) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+      }
+      for (bool act = ok && i >= 0; __any_sync(vm, act); act = ok && i >= 0) {
+        if (!act) continue;
+        if (steps > 0) { if (!kf_propagate(k, dxs, F)) ok = false; else --steps; }
+        if (ok && steps == 0) {
+          arrive(zc);
+          const Gain g = kf_gain(k, F);
+          const float c2 = kf_chi2(k, g, yc, zc);
+          if (kf_update(k, g, yc, zc, F)) ok = false;
+          else {
+            chi2 = chi2 + c2;
+            sp = sc; rp = rc;
+            --i;
+            while (i >= 0 && rej[i]) --i;
+            if (i >= 0) { rec(i, yc, zc, sc, rc); if (!plan(sp, rp, sc, rc)) ok = false; }
+          }
+        }
       }
       if (ok) {
         out.x = K->x[rp];
